@@ -1,0 +1,489 @@
+/* ===========================================================================
+ * ORACLE — TEST INFRASTRUCTURE, NOT PRODUCT CODE.
+ *
+ * Plain, slow, obviously-correct CPU implementation of the DBIE hot path of
+ * Wang, Yan & Tan (arXiv 1306.1122; /root/reference/PAPER.md), written from
+ * the paper.  It shares no code, header, table or constant with the CUDA path
+ * (paper_1306_1122_b200/csrc, include/dbie.h) and is used only by tests/,
+ * __graft_entry__.smoke() and bench.py's cpu_baseline / --impl reference legs.
+ *
+ * What each function follows:
+ *   orc_eval            Eq. 6 discretised as the nodal sum of
+ *                       Eq. 16, midpoint rule (reading A-1).
+ *   orc_residual        Eq. 8, 9, Eq. 13 frozen-lambda forward
+ *                       differences with delta = 1e-3 px,
+ *                       Eq. 14 J = curl B.
+ *   orc_solve_nm        Downhill Simplex of Nelder & Mead with the
+ *                       stopping rule Eq. 10-12.
+ *   orc_solve_grid      BASELINE.json config 5 reading (">= 8 trial lambda per
+ *                       component per iteration"); NOT in the paper
+ *                       (reading O-4).
+ *   orc_nm_generic      the same Nelder-Mead driver on a caller-supplied
+ *                       objective, so tests can pin it against SciPy (pin S-1).
+ *
+ * Pins (tests/test_oracle_pins.py): K-1..K-10, S-1..S-4 of DESIGN.md.  The
+ * agreement with the paper's OWN numerical output (its element quadrature,
+ * thresholds, initial simplex) is "parity unpinned": the paper prints no
+ * worked example of Eq. 6.
+ *
+ * Arithmetic: IEEE double, libm sqrt/sin/cos, products formed in double, sums
+ * accumulated in long double (x87 80-bit) in pixel-index order k = 0..N-1.
+ * Build: gcc -O2 -ffp-contract=off -fopenmp (never -ffast-math).
+ * ======================================================================== */
+#include <math.h>
+#include <stdlib.h>
+#include <string.h>
+#ifdef _OPENMP
+#include <omp.h>
+#endif
+
+#define ORC_PI 3.14159265358979323846264338327950288
+
+typedef struct {
+    int nx, ny;                 /* boundary grid, pixel k = iy*nx + ix              */
+    double h, x0, y0;           /* pixel size; corner of pixel (0,0)                */
+    const double *bx, *by, *bz; /* N = nx*ny each                                   */
+} orc_boundary;
+
+typedef struct {
+    int method;                 /* 0 = NM, 1 = GRID (informational)                 */
+    double delta;               /* FD step as a fraction of h (1e-3)   */
+    double cell;                /* d in g_i as a fraction of h (reading A-6)        */
+    double w_g;                 /* Phi = f + w_g g (reading A-7)                    */
+    double eps_f, eps_g;        /* Eq. 12 thresholds (reading A-8)                  */
+    double lam0, step;          /* initial simplex, units 1/h (reading A-9)         */
+    double xtol, ftol;          /* simplex tolerances (xtol in 1/h)                 */
+    int maxiter;
+    int n_trial, n_level;       /* GRID: T, number of levels                        */
+    double lam_max;             /* GRID: window [0, lam_max/h]                      */
+    int use_eq12;               /* 1: Eq. 12 early exit enabled                     */
+} orc_opts;
+
+/* ---------------------------------------------------------------- O-1 ---- */
+/* B_p(i) = (z_i h^2 / 2 pi) * sum_k [theta sin theta + cos theta] / r^3 * B_p0[k],
+ * theta = |lambda_p| r,  r = sqrt((x_k-x_i)^2 + (y_k-y_i)^2 + z_i^2).   Eq. 6/16. */
+static void eval_point(const orc_boundary *b, double xi, double yi, double zi,
+                       const double lam[3], double B[3])
+{
+    long double s0 = 0.0L, s1 = 0.0L, s2 = 0.0L;
+    const double l0 = fabs(lam[0]), l1 = fabs(lam[1]), l2 = fabs(lam[2]);
+    if (!(zi > 0.0) || !isfinite(xi) || !isfinite(yi) || !isfinite(zi) ||
+        !isfinite(l0) || !isfinite(l1) || !isfinite(l2)) {
+        B[0] = B[1] = B[2] = NAN;
+        return;
+    }
+    for (int iy = 0; iy < b->ny; ++iy) {
+        const double yk = b->y0 + (iy + 0.5) * b->h;
+        const double dy = yk - yi;
+        for (int ix = 0; ix < b->nx; ++ix) {
+            const double xk = b->x0 + (ix + 0.5) * b->h;
+            const double dx = xk - xi;
+            const double r2 = dx * dx + dy * dy + zi * zi;
+            const double r = sqrt(r2);
+            const double r3 = r2 * r;
+            const long k = (long)iy * b->nx + ix;
+            double th, a;
+            th = l0 * r; a = (th * sin(th) + cos(th)) / r3; s0 += (long double)(a * b->bx[k]);
+            th = l1 * r; a = (th * sin(th) + cos(th)) / r3; s1 += (long double)(a * b->by[k]);
+            th = l2 * r; a = (th * sin(th) + cos(th)) / r3; s2 += (long double)(a * b->bz[k]);
+        }
+    }
+    const long double c = (long double)zi * (long double)b->h * (long double)b->h /
+                          (2.0L * (long double)ORC_PI);
+    B[0] = (double)(c * s0);
+    B[1] = (double)(c * s1);
+    B[2] = (double)(c * s2);
+}
+
+void orc_eval(const orc_boundary *b, long M, const double *x, const double *y,
+              const double *z, const double *lam /* 3*M, lam[p*M+i] */,
+              double *B /* 3*M */, int nthreads)
+{
+#ifdef _OPENMP
+    if (nthreads > 0) omp_set_num_threads(nthreads);
+#endif
+#pragma omp parallel for schedule(dynamic, 4)
+    for (long i = 0; i < M; ++i) {
+        double l[3] = { lam[i], lam[M + i], lam[2 * M + i] }, Bi[3];
+        eval_point(b, x[i], y[i], z[i], l, Bi);
+        B[i] = Bi[0]; B[M + i] = Bi[1]; B[2 * M + i] = Bi[2];
+    }
+}
+
+/* ---------------------------------------------------------------- O-2 ---- */
+/* out[0..2] = B(r_i); out[3] = f (Eq. 8); out[4] = g (Eq. 9); out[5..7] = J
+ * (Eq. 14); out[8] = div B.  Returns Phi = f + w_g g, or NaN for an invalid
+ * point (z <= 0, non-finite input, |B| = 0).                                  */
+static double residual_from_stencil(const double B0[3], const double Bx[3],
+                                    const double By[3], const double Bz[3],
+                                    double delta_abs, double d_abs, double w_g,
+                                    double out[9])
+{
+    double G[3][3]; /* G[p][j] = dB_p/dx_j, forward difference, Eq. 13 */
+    for (int p = 0; p < 3; ++p) {
+        G[p][0] = (Bx[p] - B0[p]) / delta_abs;
+        G[p][1] = (By[p] - B0[p]) / delta_abs;
+        G[p][2] = (Bz[p] - B0[p]) / delta_abs;
+    }
+    const double Jx = G[2][1] - G[1][2];
+    const double Jy = G[0][2] - G[2][0];
+    const double Jz = G[1][0] - G[0][1];
+    const double div = G[0][0] + G[1][1] + G[2][2];
+    const double nB = sqrt(B0[0] * B0[0] + B0[1] * B0[1] + B0[2] * B0[2]);
+    const double nJ = sqrt(Jx * Jx + Jy * Jy + Jz * Jz);
+    const double cx = Jy * B0[2] - Jz * B0[1];
+    const double cy = Jz * B0[0] - Jx * B0[2];
+    const double cz = Jx * B0[1] - Jy * B0[0];
+    const double nC = sqrt(cx * cx + cy * cy + cz * cz);
+    out[0] = B0[0]; out[1] = B0[1]; out[2] = B0[2];
+    out[5] = Jx; out[6] = Jy; out[7] = Jz; out[8] = div;
+    if (!(nB > 0.0) || !isfinite(nB)) {
+        out[3] = out[4] = NAN;
+        return NAN;
+    }
+    const double f = (nJ <= 1e-300) ? 0.0 : nC / (nJ * nB);
+    const double g = fabs(div) * (d_abs / 6.0) / nB;
+    out[3] = f; out[4] = g;
+    return f + w_g * g;
+}
+
+typedef struct {
+    const orc_boundary *b;
+    double xi, yi, zi;
+    double delta_abs, d_abs, w_g;
+    long nfev;
+} point_ctx;
+
+/* objective of the per-point search: lambda triple -> Phi; aux = (B, f, g, J, div) */
+static double point_objective(const double lam[3], void *user, double aux[9])
+{
+    point_ctx *c = (point_ctx *)user;
+    double B0[3], Bx[3], By[3], Bz[3];
+    c->nfev++;
+    /* Eq. 13: the same lambda triple at r_i and at its delta-neighbours */
+    eval_point(c->b, c->xi, c->yi, c->zi, lam, B0);
+    eval_point(c->b, c->xi + c->delta_abs, c->yi, c->zi, lam, Bx);
+    eval_point(c->b, c->xi, c->yi + c->delta_abs, c->zi, lam, By);
+    eval_point(c->b, c->xi, c->yi, c->zi + c->delta_abs, lam, Bz);
+    return residual_from_stencil(B0, Bx, By, Bz, c->delta_abs, c->d_abs, c->w_g, aux);
+}
+
+void orc_residual(const orc_boundary *b, const orc_opts *o, long M, const double *x,
+                  const double *y, const double *z, const double *lam /* 3*M */,
+                  double *out /* 9*M: out[q*M+i], q as in residual_from_stencil */,
+                  double *phi /* M */, int nthreads)
+{
+#ifdef _OPENMP
+    if (nthreads > 0) omp_set_num_threads(nthreads);
+#endif
+#pragma omp parallel for schedule(dynamic, 1)
+    for (long i = 0; i < M; ++i) {
+        point_ctx c = { b, x[i], y[i], z[i], o->delta * b->h, o->cell * b->h, o->w_g, 0 };
+        double l[3] = { lam[i], lam[M + i], lam[2 * M + i] }, aux[9];
+        phi[i] = point_objective(l, &c, aux);
+        for (int q = 0; q < 9; ++q) out[q * M + i] = aux[q];
+    }
+}
+
+/* ---------------------------------------------------------------- O-3 ---- */
+/* Nelder & Mead (1965) in the Lagarias et al. (1998) ordering, coefficients
+ * rho = 1, chi = 2, psi = 1/2, sigma = 1/2 (reading A-9).  The vertex formulas
+ * are written as (1+rho) xbar - rho x_worst etc. so that the sequence can be
+ * pinned against SciPy's non-adaptive Nelder-Mead bit for bit (pin S-1).      */
+typedef double (*orc_objective)(const double lam[3], void *user, double aux[9]);
+
+typedef struct {
+    double V[4][3], F[4], aux[4][9];
+    int iters, status, nfev;
+    double margin; /* smallest |a-b| over every comparison a<b taken (protocol P-4) */
+} nm_state;
+
+static double as_inf(double v) { return isnan(v) ? INFINITY : v; }
+
+static void note_margin(nm_state *s, double a, double b)
+{
+    double d = fabs(a - b);
+    if (isfinite(d) && d < s->margin) s->margin = d;
+}
+
+static void nm_sort(nm_state *s)
+{
+    /* stable insertion sort, ascending Phi; ties keep the earlier index first */
+    for (int i = 1; i < 4; ++i) {
+        double v[3], f = s->F[i], a[9];
+        memcpy(v, s->V[i], sizeof v); memcpy(a, s->aux[i], sizeof a);
+        int j = i - 1;
+        while (j >= 0 && s->F[j] > f) {
+            memcpy(s->V[j + 1], s->V[j], sizeof v);
+            memcpy(s->aux[j + 1], s->aux[j], sizeof a);
+            s->F[j + 1] = s->F[j];
+            --j;
+        }
+        memcpy(s->V[j + 1], v, sizeof v); memcpy(s->aux[j + 1], a, sizeof a);
+        s->F[j + 1] = f;
+    }
+    for (int i = 0; i < 4; ++i)
+        for (int j = i + 1; j < 4; ++j) note_margin(s, s->F[i], s->F[j]);
+}
+
+static void nm_replace_worst(nm_state *s, const double v[3], double f, const double a[9])
+{
+    memcpy(s->V[3], v, 3 * sizeof(double));
+    memcpy(s->aux[3], a, 9 * sizeof(double));
+    s->F[3] = f;
+}
+
+static void nm_minimise(orc_objective obj, void *user, const double V0[4][3],
+                        double xtol_abs, double ftol, int maxiter, int use_eq12,
+                        double eps_f, double eps_g, nm_state *s,
+                        double *trace /* (maxiter+1)*3 best vertex per iteration, or NULL */)
+{
+    s->iters = 0; s->nfev = 0; s->status = 2; s->margin = INFINITY;
+    for (int j = 0; j < 4; ++j) {
+        memcpy(s->V[j], V0[j], 3 * sizeof(double));
+        s->F[j] = as_inf(obj(s->V[j], user, s->aux[j]));
+        s->nfev++;
+    }
+    nm_sort(s);
+    if (trace) memcpy(trace, s->V[0], 3 * sizeof(double));
+    while (s->iters < maxiter) {
+        /* Eq. 12: f <= eps_f and g <= eps_g at the best vertex */
+        if (use_eq12) {
+            note_margin(s, s->aux[0][3], eps_f);
+            note_margin(s, s->aux[0][4], eps_g);
+            if (s->aux[0][3] <= eps_f && s->aux[0][4] <= eps_g) { s->status = 0; return; }
+        }
+        double dx = 0.0, df = 0.0;
+        for (int j = 1; j < 4; ++j) {
+            for (int p = 0; p < 3; ++p) dx = fmax(dx, fabs(s->V[j][p] - s->V[0][p]));
+            df = fmax(df, fabs(s->F[0] - s->F[j]));
+        }
+        note_margin(s, df, ftol);
+        if (dx <= xtol_abs && df <= ftol) { s->status = 1; return; }
+
+        double xbar[3], xr[3], xt[3], ar[9], at[9], fr, ft;
+        for (int p = 0; p < 3; ++p) xbar[p] = ((s->V[0][p] + s->V[1][p]) + s->V[2][p]) / 3.0;
+        for (int p = 0; p < 3; ++p) xr[p] = 2.0 * xbar[p] - 1.0 * s->V[3][p];
+        fr = as_inf(obj(xr, user, ar)); s->nfev++;
+        int shrink = 0;
+        note_margin(s, fr, s->F[0]);
+        if (fr < s->F[0]) {
+            for (int p = 0; p < 3; ++p) xt[p] = 3.0 * xbar[p] - 2.0 * s->V[3][p];
+            ft = as_inf(obj(xt, user, at)); s->nfev++;
+            note_margin(s, ft, fr);
+            if (ft < fr) nm_replace_worst(s, xt, ft, at);
+            else nm_replace_worst(s, xr, fr, ar);
+        } else {
+            note_margin(s, fr, s->F[2]);
+            if (fr < s->F[2]) {
+                nm_replace_worst(s, xr, fr, ar);
+            } else {
+                note_margin(s, fr, s->F[3]);
+                if (fr < s->F[3]) { /* outside contraction */
+                    for (int p = 0; p < 3; ++p) xt[p] = 1.5 * xbar[p] - 0.5 * s->V[3][p];
+                    ft = as_inf(obj(xt, user, at)); s->nfev++;
+                    note_margin(s, ft, fr);
+                    if (ft <= fr) nm_replace_worst(s, xt, ft, at);
+                    else shrink = 1;
+                } else {            /* inside contraction */
+                    for (int p = 0; p < 3; ++p) xt[p] = 0.5 * xbar[p] + 0.5 * s->V[3][p];
+                    ft = as_inf(obj(xt, user, at)); s->nfev++;
+                    note_margin(s, ft, s->F[3]);
+                    if (ft < s->F[3]) nm_replace_worst(s, xt, ft, at);
+                    else shrink = 1;
+                }
+                if (shrink) {
+                    for (int j = 1; j < 4; ++j) {
+                        for (int p = 0; p < 3; ++p)
+                            s->V[j][p] = s->V[0][p] + 0.5 * (s->V[j][p] - s->V[0][p]);
+                        s->F[j] = as_inf(obj(s->V[j], user, s->aux[j])); s->nfev++;
+                    }
+                }
+            }
+        }
+        nm_sort(s);
+        s->iters++;
+        if (trace) memcpy(trace + 3 * s->iters, s->V[0], 3 * sizeof(double));
+    }
+    s->status = 2;
+}
+
+/* generic driver for pin S-1 (objective supplied by the test) */
+typedef double (*orc_objective3)(const double lam[3]);
+static double generic_adapter(const double lam[3], void *user, double aux[9])
+{
+    for (int q = 0; q < 9; ++q) aux[q] = 0.0;
+    return ((orc_objective3)user)(lam);
+}
+void orc_nm_generic(orc_objective3 fn, const double *simplex /* 4*3 */, double xtol,
+                    double ftol, int maxiter, double *trace /* (maxiter+1)*3 */,
+                    double *final_simplex /* 12 */, double *final_f /* 4 */,
+                    int *iters, int *nfev, int *status)
+{
+    nm_state s;
+    double V0[4][3];
+    memcpy(V0, simplex, sizeof V0);
+    nm_minimise(generic_adapter, (void *)fn, V0, xtol, ftol, maxiter, 0, 0.0, 0.0, &s, trace);
+    memcpy(final_simplex, s.V, sizeof s.V);
+    memcpy(final_f, s.F, sizeof s.F);
+    *iters = s.iters; *nfev = s.nfev; *status = s.status;
+}
+
+void orc_solve_nm(const orc_boundary *b, const orc_opts *o, long M, const double *x,
+                  const double *y, const double *z,
+                  double *B /* 3*M */, double *lam /* 3*M, >= 0 */,
+                  double *resid /* 2*M: f, g */, int *iters, int *status,
+                  double *margin /* M or NULL */, int *nfev /* M or NULL */,
+                  double *phi /* M or NULL */, int nthreads)
+{
+#ifdef _OPENMP
+    if (nthreads > 0) omp_set_num_threads(nthreads);
+#endif
+#pragma omp parallel for schedule(dynamic, 1)
+    for (long i = 0; i < M; ++i) {
+        point_ctx c = { b, x[i], y[i], z[i], o->delta * b->h, o->cell * b->h, o->w_g, 0 };
+        nm_state s;
+        double V0[4][3];
+        const double l0 = o->lam0 / b->h, st = o->step / b->h;
+        for (int j = 0; j < 4; ++j)
+            for (int p = 0; p < 3; ++p) V0[j][p] = l0;
+        for (int j = 1; j < 4; ++j) V0[j][j - 1] = l0 + st;
+        int invalid = !(z[i] > 0.0) || !isfinite(x[i]) || !isfinite(y[i]) || !isfinite(z[i]);
+        if (!invalid) {
+            nm_minimise(point_objective, &c, V0, o->xtol / b->h, o->ftol, o->maxiter,
+                        o->use_eq12, o->eps_f, o->eps_g, &s, NULL);
+            if (!isfinite(s.F[0])) invalid = 1;
+        }
+        if (invalid) {
+            for (int p = 0; p < 3; ++p) { B[p * M + i] = NAN; lam[p * M + i] = NAN; }
+            resid[i] = resid[M + i] = NAN;
+            iters[i] = 0; status[i] = 3;
+            if (margin) margin[i] = 0.0;
+            if (nfev) nfev[i] = 0;
+            if (phi) phi[i] = NAN;
+            continue;
+        }
+        for (int p = 0; p < 3; ++p) {
+            B[p * M + i] = s.aux[0][p];
+            lam[p * M + i] = fabs(s.V[0][p]);
+        }
+        resid[i] = s.aux[0][3]; resid[M + i] = s.aux[0][4];
+        iters[i] = s.iters; status[i] = s.status;
+        if (margin) margin[i] = s.margin;
+        if (nfev) nfev[i] = s.nfev;
+        if (phi) phi[i] = s.F[0];
+    }
+}
+
+/* ---------------------------------------------------------------- O-4 ---- */
+/* GRID search: T trial values per component per level, using separability
+ * (B_p depends on lambda_p only).  BASELINE.json config 5 reading,
+ * not in the paper.                                                          */
+void orc_solve_grid(const orc_boundary *b, const orc_opts *o, long M, const double *x,
+                    const double *y, const double *z,
+                    double *B, double *lam, double *resid, int *iters, int *status,
+                    double *margin /* M or NULL */, double *phi /* M or NULL */,
+                    int nthreads)
+{
+    const int T = o->n_trial;
+#ifdef _OPENMP
+    if (nthreads > 0) omp_set_num_threads(nthreads);
+#endif
+#pragma omp parallel for schedule(dynamic, 1)
+    for (long i = 0; i < M; ++i) {
+        const double da = o->delta * b->h, dc = o->cell * b->h;
+        const double Lmax = o->lam_max / b->h;
+        /* S[t][s][p]: component p at stencil position s (0, +x, +y, +z) for trial t;
+         * slot T is the incumbent */
+        double (*S)[4][3] = malloc(sizeof(double[4][3]) * (T + 1));
+        double *lt = malloc(sizeof(double) * 3 * (T + 1)); /* lt[p*(T+1)+t] */
+        double lo[3] = { 0.0, 0.0, 0.0 }, W = Lmax;
+        double best_phi = INFINITY, best_aux[9], mrg = INFINITY;
+        int have_inc = 0, st = 2, lev = 0;
+        int invalid = !(z[i] > 0.0) || !isfinite(x[i]) || !isfinite(y[i]) || !isfinite(z[i]);
+        for (lev = 0; lev < o->n_level && !invalid; ++lev) {
+            for (int t = 0; t < T; ++t) {
+                double l[3];
+                for (int p = 0; p < 3; ++p) {
+                    l[p] = lo[p] + W * (double)t / (double)(T - 1);
+                    lt[p * (T + 1) + t] = l[p];
+                }
+                eval_point(b, x[i], y[i], z[i], l, S[t][0]);
+                eval_point(b, x[i] + da, y[i], z[i], l, S[t][1]);
+                eval_point(b, x[i], y[i] + da, z[i], l, S[t][2]);
+                eval_point(b, x[i], y[i], z[i] + da, l, S[t][3]);
+            }
+            const int C = have_inc ? T + 1 : T;
+            int bt[3] = { -1, -1, -1 };
+            double lev_best = INFINITY, lev_second = INFINITY, lev_aux[9];
+            for (int tx = 0; tx < C; ++tx)
+                for (int ty = 0; ty < C; ++ty)
+                    for (int tz = 0; tz < C; ++tz) {
+                        const int tt[3] = { tx, ty, tz };
+                        double P0[3], Px[3], Py[3], Pz[3], aux[9];
+                        for (int p = 0; p < 3; ++p) {
+                            P0[p] = S[tt[p]][0][p]; Px[p] = S[tt[p]][1][p];
+                            Py[p] = S[tt[p]][2][p]; Pz[p] = S[tt[p]][3][p];
+                        }
+                        double ph = as_inf(residual_from_stencil(P0, Px, Py, Pz, da, dc,
+                                                                 o->w_g, aux));
+                        if (ph < lev_best) { /* strict: ties keep the lexicographically first */
+                            lev_second = lev_best;
+                            lev_best = ph; bt[0] = tx; bt[1] = ty; bt[2] = tz;
+                            memcpy(lev_aux, aux, sizeof aux);
+                        } else if (ph < lev_second) lev_second = ph;
+                    }
+            if (bt[0] < 0) { invalid = 1; break; }
+            if (isfinite(lev_second - lev_best) && lev_second - lev_best < mrg)
+                mrg = lev_second - lev_best;
+            /* the argmin becomes the incumbent (slot T) */
+            double inc[4][3], il[3];
+            for (int p = 0; p < 3; ++p) {
+                for (int s = 0; s < 4; ++s) inc[s][p] = S[bt[p]][s][p];
+                il[p] = lt[p * (T + 1) + bt[p]];
+            }
+            memcpy(S[T], inc, sizeof inc);
+            for (int p = 0; p < 3; ++p) lt[p * (T + 1) + T] = il[p];
+            have_inc = 1;
+            best_phi = lev_best; memcpy(best_aux, lev_aux, sizeof lev_aux);
+            if (o->use_eq12 && best_aux[3] <= o->eps_f && best_aux[4] <= o->eps_g) {
+                st = 0; ++lev; break;
+            }
+            /* next window centred on the incumbent, clipped to [0, Lmax] */
+            const double Wn = 2.0 * W / (double)(T - 1);
+            for (int p = 0; p < 3; ++p) {
+                double l = il[p] - 0.5 * Wn;
+                if (l < 0.0) l = 0.0;
+                if (l + Wn > Lmax) l = Lmax - Wn;
+                lo[p] = l;
+            }
+            W = Wn;
+            st = 1;
+        }
+        if (invalid || !isfinite(best_phi)) {
+            for (int p = 0; p < 3; ++p) { B[p * M + i] = NAN; lam[p * M + i] = NAN; }
+            resid[i] = resid[M + i] = NAN; iters[i] = 0; status[i] = 3;
+            if (margin) margin[i] = 0.0;
+            if (phi) phi[i] = NAN;
+        } else {
+            for (int p = 0; p < 3; ++p) {
+                B[p * M + i] = best_aux[p];
+                lam[p * M + i] = fabs(lt[p * (T + 1) + T]);
+            }
+            resid[i] = best_aux[3]; resid[M + i] = best_aux[4];
+            iters[i] = lev; status[i] = st;
+            if (margin) margin[i] = mrg;
+            if (phi) phi[i] = best_phi;
+        }
+        free(S); free(lt);
+    }
+}
+
+int orc_max_threads(void)
+{
+#ifdef _OPENMP
+    return omp_get_max_threads();
+#else
+    return 1;
+#endif
+}

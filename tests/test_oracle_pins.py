@@ -1,0 +1,441 @@
+"""Pins for the CPU oracle (oracle/dbie_oracle.c) against what the paper and the
+mathematics fix — closed forms, invariants, library routines, brute force.
+None of these tests touches the CUDA path.  Pin names follow DESIGN.md section 3.
+"""
+import math
+import os
+
+import mpmath as mp
+import numpy as np
+import pytest
+from scipy import integrate, optimize
+
+import oracle
+from workloads import Workload, config1, dipole_field, random_boundary
+
+GOLDEN = os.path.join(os.path.dirname(__file__), "golden")
+
+
+def _wl(nx, ny, h, x0, y0, bx, by, bz, pts, lam=None):
+    pts = np.atleast_2d(np.asarray(pts, dtype=np.float64))
+    M = pts.shape[0]
+    lam = np.zeros((3, M)) if lam is None else np.asarray(lam, dtype=np.float64).reshape(3, M)
+    return Workload("t", nx, ny, h, x0, y0, np.asarray(bx, float).ravel(),
+                    np.asarray(by, float).ravel(), np.asarray(bz, float).ravel(),
+                    pts[:, 0].copy(), pts[:, 1].copy(), pts[:, 2].copy(), lam)
+
+
+def _read_table(name):
+    rows = []
+    with open(os.path.join(GOLDEN, name)) as fh:
+        for line in fh:
+            if line.strip() and not line.startswith("#"):
+                rows.append([float(t) for t in line.split()])
+    return np.array(rows)
+
+
+# -- K-1 ---------------------------------------------------------------------
+def test_k1_one_pixel_worked_example():
+    tab = _read_table("k1_one_pixel.txt")
+    for lam, want in tab:
+        w = _wl(1, 1, 1.0, -0.5, -0.5, [1.0], [1.0], [1.0], [[0.0, 0.0, 1.0]],
+                [[lam], [lam], [lam]])
+        B = oracle.eval(w)
+        assert np.allclose(B[:, 0], want, rtol=0, atol=1e-15)
+    # a wrong sign of the sin term, a dropped cos term or 4 pi instead of 2 pi fail here:
+    assert abs(tab[2, 1] - (math.sin(1.0) + math.cos(1.0)) / (2 * math.pi)) < 1e-15
+
+
+# -- K-2 ---------------------------------------------------------------------
+def test_k2_kernel_is_normal_derivative_of_reference_function():
+    """Eq. 6's kernel equals dY/dz at z=0 of Eq. 5, and the oracle's single-pixel
+    term equals h^2 times it (off-axis pixel, all three lambdas different)."""
+    mp.mp.dps = 90
+    rng = np.random.default_rng(7)
+    for _ in range(5):
+        xi_f, yi_f = rng.uniform(-3, 3, 2)
+        zi_f = rng.uniform(0.5, 4.0)
+        xs_f, ys_f = rng.uniform(-3, 3, 2)
+        lams = rng.uniform(0.05, 1.5, 3)
+        h = 0.25
+        xi, yi, zi, xs, ys = (mp.mpf(float(v)) for v in (xi_f, yi_f, zi_f, xs_f, ys_f))
+        want = []
+        for lam in lams:
+            lam = mp.mpf(float(lam))
+            def Y(z, lam=lam):
+                rho = mp.sqrt((xs - xi) ** 2 + (ys - yi) ** 2 + (z - zi) ** 2)
+                rhop = mp.sqrt((xs - xi) ** 2 + (ys - yi) ** 2 + (z + zi) ** 2)
+                return mp.cos(lam * rho) / (4 * mp.pi * rho) - mp.cos(lam * rhop) / (4 * mp.pi * rhop)
+            dY = mp.diff(Y, 0)
+            r = mp.sqrt((xs - xi) ** 2 + (ys - yi) ** 2 + zi ** 2)
+            k6 = zi * (lam * r * mp.sin(lam * r) + mp.cos(lam * r)) / (2 * mp.pi * r ** 3)
+            assert abs(dY - k6) < mp.mpf(10) ** -30 * abs(k6)
+            want.append(float(dY) * h * h)
+        b0 = np.array([1.7, -0.4, 2.2])
+        w = _wl(1, 1, h, xs_f - h / 2, ys_f - h / 2, [b0[0]], [b0[1]], [b0[2]],
+                [[xi_f, yi_f, zi_f]], lams.reshape(3, 1))
+        B = oracle.eval(w)[:, 0]
+        assert np.allclose(B, np.array(want) * b0, rtol=1e-13, atol=0)
+
+
+# -- K-3 ---------------------------------------------------------------------
+@pytest.mark.parametrize("lam", [0.0, 0.2, 1.0])
+def test_k3_radial_gaussian_vs_1d_quadrature(lam):
+    """Radially symmetric boundary under the point: the 2-D nodal sum equals
+    int_0^inf z n(lam r) r^-3 B0(s) s ds (the 2 pi cancels).  Pins normalisation,
+    r, and the whole kernel for lambda != 0 independently of any PDE argument."""
+    n, h, sig = 128, 1.0, 5.0
+    c = (np.arange(n) + 0.5) * h
+    Yg, Xg = np.meshgrid(c, c, indexing="ij")
+    xc = yc = 0.5 * n * h
+    b0 = np.exp(-((Xg - xc) ** 2 + (Yg - yc) ** 2) / (2 * sig * sig))
+    z = 5.0
+    w = _wl(n, n, h, 0.0, 0.0, b0, b0, b0, [[xc, yc, z]], [[lam]] * 3)
+    got = oracle.eval(w)[0, 0]
+
+    def integrand(s):
+        r = math.sqrt(s * s + z * z)
+        th = lam * r
+        return z * (th * math.sin(th) + math.cos(th)) / r ** 3 * math.exp(-s * s / (2 * sig * sig)) * s
+    want, _ = integrate.quad(integrand, 0.0, 60.0, epsabs=0.0, epsrel=1e-12, limit=400)
+    assert abs(got - want) <= 1e-10 * abs(want)
+
+
+# -- K-4 ---------------------------------------------------------------------
+def test_k4_uniform_disc_closed_form():
+    """B0 = 1 on a disc of radius S under the point:
+    integral = cos(lam z) - z cos(lam sqrt(z^2+S^2)) / sqrt(z^2+S^2)
+    because d/dr[-cos(lam r)/r] = n(lam r)/r^2.  Pixelised disc converges to it."""
+    lam, z = 0.03, 20.0
+    errs = []
+    for S in (50.0, 200.0):
+        n = int(2 * S) + 8
+        c = np.arange(n) + 0.5
+        Yg, Xg = np.meshgrid(c, c, indexing="ij")
+        xc = 0.5 * n
+        disc = (((Xg - xc) ** 2 + (Yg - xc) ** 2) <= S * S).astype(float)
+        w = _wl(n, n, 1.0, 0.0, 0.0, disc, disc, disc, [[xc, xc, z]], [[lam]] * 3)
+        got = oracle.eval(w)[2, 0]
+        R = math.sqrt(z * z + S * S)
+        want = math.cos(lam * z) - z * math.cos(lam * R) / R
+        errs.append(abs(got - want))
+    assert errs[1] <= 1e-3
+    # independent check of the antiderivative itself by adaptive quadrature
+    S = 50.0
+    q, _ = integrate.quad(lambda s: z * ((lam * math.hypot(s, z)) * math.sin(lam * math.hypot(s, z))
+                                         + math.cos(lam * math.hypot(s, z))) / math.hypot(s, z) ** 3 * s,
+                          0.0, S, epsabs=0.0, epsrel=1e-12)
+    R = math.hypot(z, S)
+    assert abs(q - (math.cos(lam * z) - z * math.cos(lam * R) / R)) < 1e-13
+
+
+# -- K-5 ---------------------------------------------------------------------
+def test_k5_lambda0_rectangle_solid_angle():
+    """lambda = 0: Poisson kernel z/(2 pi r^3); uniform rectangle -> Omega / 2 pi.
+    Midpoint-rule error at z = 2h is the aliasing term ~ 4 e^{-2 pi z/h} (reading A-2)."""
+    n, z = 1001, 2.0
+    ones = np.ones(n * n)
+    xc = 0.5 * n
+    w = _wl(n, n, 1.0, 0.0, 0.0, ones, ones, ones, [[xc, xc, z]])
+    got = oracle.eval(w)[2, 0]
+    a = b = 0.5 * n
+    omega = 4.0 * math.atan(a * b / (z * math.sqrt(a * a + b * b + z * z)))
+    want = omega / (2 * math.pi)
+    rel = abs(got - want) / want
+    predicted = 4.0 * math.exp(-2 * math.pi * z)       # 1.40e-5
+    assert abs(rel - predicted) < 0.05 * predicted
+    # higher up the aliasing term is ~1e-21; what remains is the Euler-Maclaurin edge
+    # term of the truncated window, O(h^2 z / R_edge^4) ~ 1e-8
+    w = _wl(n, n, 1.0, 0.0, 0.0, ones, ones, ones, [[xc, xc, 8.0]])
+    got = oracle.eval(w)[2, 0]
+    omega = 4.0 * math.atan(a * b / (8.0 * math.sqrt(a * a + b * b + 64.0)))
+    assert abs(got - omega / (2 * math.pi)) < 2e-8
+
+
+# -- K-6 ---------------------------------------------------------------------
+def _dipole_err(n, sel=None):
+    w = config1(n)
+    if sel is not None:
+        w = w.subset(sel)
+    B = oracle.eval(w)
+    ref = np.array(dipole_field(w.x, w.y, w.z))
+    return np.linalg.norm(B - ref, axis=0) / np.linalg.norm(ref, axis=0), w
+
+
+def test_k6_buried_dipole_profile_and_convergence():
+    err, w = _dipole_err(16)
+    prof = err.reshape(8, 64).max(axis=1)
+    tab = _read_table("k6_dipole_profile.txt")
+    assert np.all(np.abs(prof - tab[:, 1]) <= 0.10 * tab[:, 1] + 5e-4)
+    # widening the window about the dipole converges to the closed form
+    e64, w64 = _dipole_err(64)
+    assert e64[w64.z >= 2.0].max() <= 1.5e-3
+    sel = np.arange(512)[::7]            # 74 points spread over all heights
+    e256, w256 = _dipole_err(256, sel)
+    assert e256[w256.z >= 3.0].max() <= 6e-6
+    e1k, w1k = _dipole_err(1024, sel[::2])
+    assert e1k[w1k.z >= 4.0].max() <= 3e-8
+    assert e1k[w1k.z >= 4.0].max() < e256[w256.z >= 4.0].max() < e64[w64.z >= 4.0].max()
+
+
+# -- K-7 ---------------------------------------------------------------------
+def test_k7_helmholtz_invariant():
+    """For fixed lambda the nodal sum u satisfies laplace(u) + lambda^2 u = 0 in z>0
+    exactly (each term is -d/dz_i[cos(lam r)/r] h^2 B_k / 2 pi).  The 7-point Laplacian has
+    an O(d^2) truncation error, removed here by one Richardson step."""
+    w = random_boundary(12, 9, seed=1, npts=1)
+    lam = 0.37
+    p = np.array([5.3, 4.1, 2.6])
+
+    def lap(d):
+        offs = [np.zeros(3)] + [s * d * e for e in np.eye(3) for s in (1, -1)]
+        pts = np.array([p + o for o in offs])
+        ww = _wl(w.nx, w.ny, w.h, w.x0, w.y0, w.bx, w.by, w.bz, pts, np.full((3, 7), lam))
+        B = oracle.eval(ww)
+        return (B[:, 1:].sum(axis=1) - 6 * B[:, 0]) / (d * d), B[:, 0]
+
+    l1, u = lap(0.04)
+    l2, _ = lap(0.02)
+    scale = np.abs(lam * lam * u).max()
+    r1, r2 = l1 + lam * lam * u, l2 + lam * lam * u
+    assert np.allclose(r1, 4.0 * r2, rtol=2e-3)                 # pure O(d^2) truncation
+    assert np.all(np.abs((4 * l2 - l1) / 3 + lam * lam * u) <= 1e-6 * scale)
+    # with a wrong lambda in the invariant it fails by orders of magnitude
+    assert np.abs((4 * l2 - l1) / 3 + (1.1 * lam) ** 2 * u).max() > 1e-2 * scale
+
+
+# -- K-8 ---------------------------------------------------------------------
+def test_k8_symmetries():
+    w = random_boundary(10, 7, seed=2, h=0.5, x0=-1.0, y0=2.0, npts=9)
+    B = oracle.eval(w)
+    # even in lambda, bit for bit
+    assert np.array_equal(B, oracle.eval(w, lam=-w.lam))
+    # linear in B0
+    w2 = _wl(w.nx, w.ny, w.h, w.x0, w.y0, 2.5 * w.bx, -1.0 * w.by, 0.0 * w.bz,
+             np.stack([w.x, w.y, w.z], 1), w.lam)
+    B2 = oracle.eval(w2)
+    assert np.allclose(B2[0], 2.5 * B[0], rtol=1e-14)
+    assert np.allclose(B2[1], -B[1], rtol=1e-14)
+    assert np.all(B2[2] == 0.0)
+    # each component depends on its own lambda only (separability)
+    lam3 = w.lam.copy(); lam3[1] *= 1.7
+    B3 = oracle.eval(w, lam=lam3)
+    assert np.array_equal(B3[0], B[0]) and np.array_equal(B3[2], B[2])
+    assert not np.allclose(B3[1], B[1])
+    # shifting the frame (x0, y0 and the points together)
+    w4 = _wl(w.nx, w.ny, w.h, w.x0 + 3.0, w.y0 - 5.0, w.bx, w.by, w.bz,
+             np.stack([w.x + 3.0, w.y - 5.0, w.z], 1), w.lam)
+    assert np.allclose(oracle.eval(w4), B, rtol=1e-12)
+    # 90 degree rotation of grid and points: (x, y) -> (-y, x)
+    bx = w.bx.reshape(w.ny, w.nx); by = w.by.reshape(w.ny, w.nx); bz = w.bz.reshape(w.ny, w.nx)
+    rot = lambda a: np.ascontiguousarray(a.T[:, ::-1])    # new[iy'=ix, ix'=ny-1-iy]
+    w5 = _wl(w.ny, w.nx, w.h, -(w.y0 + w.ny * w.h), w.x0, rot(bx), rot(by), rot(bz),
+             np.stack([-w.y, w.x, w.z], 1), w.lam)
+    assert np.allclose(oracle.eval(w5), B, rtol=1e-12)
+    # scaling lengths by s and lambda by 1/s leaves B unchanged (units, reading A-11)
+    s = 3.0
+    w6 = _wl(w.nx, w.ny, w.h * s, w.x0 * s, w.y0 * s, w.bx, w.by, w.bz,
+             np.stack([w.x * s, w.y * s, w.z * s], 1), w.lam / s)
+    assert np.allclose(oracle.eval(w6), B, rtol=1e-12)
+
+
+# -- K-9 ---------------------------------------------------------------------
+def _analytic_grad(w, p, lam):
+    """dB_p/d(x_i,y_i,z_i) from d/dr[n(lam r)/r^3] = lam^2 cos(lam r)/r^2 - 3 n/r^4."""
+    xk = w.x0 + (np.arange(w.nx) + 0.5) * w.h
+    yk = w.y0 + (np.arange(w.ny) + 0.5) * w.h
+    Yk, Xk = np.meshgrid(yk, xk, indexing="ij")
+    dx, dy, z = (Xk - p[0]).ravel(), (Yk - p[1]).ravel(), p[2]
+    r = np.sqrt(dx * dx + dy * dy + z * z)
+    G = np.zeros((3, 3))
+    c = w.h ** 2 / (2 * math.pi)
+    for comp, b0 in enumerate((w.bx, w.by, w.bz)):
+        l = abs(lam[comp])
+        n = l * r * np.sin(l * r) + np.cos(l * r)
+        dk = l * l * np.cos(l * r) / r ** 2 - 3 * n / r ** 4     # d/dr of n/r^3
+        G[comp, 0] = c * np.sum(z * dk * (-dx / r) * b0)
+        G[comp, 1] = c * np.sum(z * dk * (-dy / r) * b0)
+        G[comp, 2] = c * np.sum((n / r ** 3 + z * dk * (z / r)) * b0)
+    return G
+
+
+def test_k9_forward_difference_stencil_vs_analytic_gradient():
+    w = random_boundary(14, 11, seed=3, npts=4, zmin=1.5, zmax=5.0)
+    errs = []
+    for delta in (1e-3, 2.5e-4):
+        res = oracle.residual(w, w.lam, oracle.Opts(delta=delta))
+        worst = 0.0
+        for i in range(w.M):
+            G = _analytic_grad(w, (w.x[i], w.y[i], w.z[i]), w.lam[:, i])
+            J = np.array([G[2, 1] - G[1, 2], G[0, 2] - G[2, 0], G[1, 0] - G[0, 1]])
+            div = np.trace(G)
+            scale = np.abs(G).max()
+            worst = max(worst, np.abs(res["J"][:, i] - J).max() / scale,
+                        abs(res["div"][i] - div) / scale)
+            B = res["B"][:, i]
+            f = np.linalg.norm(np.cross(J, B)) / (np.linalg.norm(J) * np.linalg.norm(B))
+            g = abs(div) * (w.h / 6.0) / np.linalg.norm(B)
+            assert abs(res["f"][i] - f) < 20 * delta
+            assert abs(res["g"][i] - g) < 20 * delta * max(g, 1e-3)
+            assert abs(res["phi"][i] - (res["f"][i] + res["g"][i])) < 1e-15
+        errs.append(worst)
+    assert errs[0] <= 5e-3                       # <= 5 delta / h
+    assert errs[1] < 0.4 * errs[0]               # -> 0 linearly in delta
+
+
+# -- K-10 --------------------------------------------------------------------
+def test_k10_oracle_rounding_vs_mpmath():
+    mp.mp.dps = 30
+    w = random_boundary(16, 16, seed=4, npts=10)
+    B = oracle.eval(w)
+    for i in range(w.M):
+        for comp, b0 in enumerate((w.bx, w.by, w.bz)):
+            l = abs(w.lam[comp, i])
+            tot = mp.mpf(0); mag = mp.mpf(0)
+            for iy in range(w.ny):
+                for ix in range(w.nx):
+                    xk = w.x0 + (ix + 0.5) * w.h
+                    yk = w.y0 + (iy + 0.5) * w.h
+                    r = mp.sqrt((mp.mpf(xk) - w.x[i]) ** 2 + (mp.mpf(yk) - w.y[i]) ** 2
+                                + mp.mpf(w.z[i]) ** 2)
+                    t = (l * r * mp.sin(l * r) + mp.cos(l * r)) / r ** 3 * mp.mpf(float(b0[iy * w.nx + ix]))
+                    tot += t; mag += abs(t)
+            c = mp.mpf(w.z[i]) * w.h ** 2 / (2 * mp.pi)
+            assert abs(mp.mpf(float(B[comp, i])) - c * tot) <= mp.mpf(1e-14) * c * mag
+
+
+# -- S-1 ---------------------------------------------------------------------
+def _rosen3(x):
+    return (100.0 * (x[1] - x[0] * x[0]) ** 2 + (1.0 - x[0]) ** 2
+            + 100.0 * (x[2] - x[1] * x[1]) ** 2 + (1.0 - x[1]) ** 2)
+
+
+def _quad3(x):
+    d0, d1, d2 = x[0] - 0.3, x[1] + 0.2, x[2] - 0.1
+    return 3.0 * d0 * d0 + 0.5 * d1 * d1 + 2.0 * d2 * d2 + 0.7 * d0 * d1 - 0.4 * d1 * d2
+
+
+def _abs3(x):   # non-smooth: forces contractions and shrinks
+    return abs(x[0] - 0.1) + 2.0 * abs(x[1] + 0.3) + abs(x[0] * x[2]) + abs(x[2] - 0.2)
+
+
+@pytest.mark.parametrize("fn,start,step", [(_rosen3, -1.2, 0.4), (_quad3, 0.05, 0.05),
+                                           (_abs3, 0.05, 0.05), (_rosen3, 0.05, 0.05)])
+def test_s1_nelder_mead_matches_scipy_iterate_by_iterate(fn, start, step):
+    sim = np.full((4, 3), start)
+    for j in range(3):
+        sim[j + 1, j] += step
+    maxiter = 150
+    xtol, ftol = 1e-7, 1e-9
+    mine = oracle.nm_generic(fn, sim, xtol, ftol, maxiter)
+    ref = optimize.minimize(fn, sim[0], method="Nelder-Mead",
+                            options={"initial_simplex": sim, "adaptive": False, "xatol": xtol,
+                                     "fatol": ftol, "maxiter": maxiter + 1, "maxfev": 10 ** 6,
+                                     "return_all": True})
+    allvecs = np.array(ref.allvecs)
+    # SciPy starts its counter at 1: nit = 1 + number of simplex updates performed
+    assert mine["iters"] == ref.nit - 1
+    assert mine["nfev"] == ref.nfev
+    assert mine["trace"].shape == allvecs.shape
+    # SciPy records allvecs[0] before its initial sort; compare the sorted sequence from 1 on
+    assert np.allclose(mine["trace"][1:], allvecs[1:], rtol=0, atol=1e-15)
+    assert fn(mine["trace"][0]) == min(fn(v) for v in sim)
+    assert np.allclose(mine["simplex"], ref.final_simplex[0], rtol=0, atol=1e-15)
+    assert np.allclose(mine["f"], ref.final_simplex[1], rtol=0, atol=1e-15)
+    assert mine["status"] == (1 if ref.status == 0 else 2)
+
+
+# -- S-4 ---------------------------------------------------------------------
+def _numpy_eval(w, p, lam):
+    xk = w.x0 + (np.arange(w.nx) + 0.5) * w.h
+    yk = w.y0 + (np.arange(w.ny) + 0.5) * w.h
+    Yk, Xk = np.meshgrid(yk, xk, indexing="ij")
+    r = np.sqrt((Xk - p[0]) ** 2 + (Yk - p[1]) ** 2 + p[2] ** 2).ravel()
+    out = []
+    for comp, b0 in enumerate((w.bx, w.by, w.bz)):
+        th = abs(lam[comp]) * r
+        out.append(p[2] * w.h ** 2 / (2 * np.pi) * np.sum((th * np.sin(th) + np.cos(th)) / r ** 3 * b0))
+    return np.array(out)
+
+
+def _numpy_phi(w, p, lam, delta=1e-3, cell=1.0, w_g=1.0):
+    d = delta * w.h
+    p = np.asarray(p, float)
+    B0 = _numpy_eval(w, p, lam)
+    G = np.stack([(_numpy_eval(w, p + d * e, lam) - B0) / d for e in np.eye(3)], axis=1)
+    J = np.array([G[2, 1] - G[1, 2], G[0, 2] - G[2, 0], G[1, 0] - G[0, 1]])
+    f = np.linalg.norm(np.cross(J, B0)) / (np.linalg.norm(J) * np.linalg.norm(B0))
+    g = abs(np.trace(G)) * (cell * w.h / 6.0) / np.linalg.norm(B0)
+    return f + w_g * g, f, g, B0
+
+
+def test_s4_brute_force_tiny_grid():
+    w = random_boundary(4, 4, seed=5, npts=2, zmin=1.0, zmax=3.0)
+    B = oracle.eval(w)
+    res = oracle.residual(w, w.lam)
+    for i in range(2):
+        p = (w.x[i], w.y[i], w.z[i])
+        assert np.allclose(B[:, i], _numpy_eval(w, p, w.lam[:, i]), rtol=1e-13)
+        phi, f, g, B0 = _numpy_phi(w, p, w.lam[:, i])
+        # forward differences amplify rounding by 1/delta
+        assert abs(res["f"][i] - f) < 1e-9 and abs(res["g"][i] - g) < 1e-9
+    # exhaustive lambda scan: the simplex result is no worse than the best scan node
+    # reachable from its start (local method: compare with scan restricted to the box it searched)
+    sol = oracle.solve_nm(w, oracle.Opts(use_eq12=0, maxiter=300))
+    for i in range(2):
+        p = (w.x[i], w.y[i], w.z[i])
+        phi_star = _numpy_phi(w, p, sol["lam"][:, i])[0]
+        assert abs(phi_star - sol["phi"][i]) < 1e-8
+        assert abs(sol["f"][i] + sol["g"][i] - sol["phi"][i]) < 1e-15
+        phi_start = _numpy_phi(w, p, np.full(3, 0.05 / w.h))[0]
+        assert sol["phi"][i] <= phi_start + 1e-12
+        # local optimality on a 21^3 scan of half-width 0.02/h around lambda*
+        best = np.inf
+        ax = np.linspace(-0.02, 0.02, 21) / w.h
+        for a in ax:
+            for b in ax:
+                for c in ax:
+                    best = min(best, _numpy_phi(w, p, sol["lam"][:, i] + np.array([a, b, c]))[0])
+        assert sol["phi"][i] <= best + 5e-5
+
+
+def test_solver_invalid_points_and_statuses():
+    w = random_boundary(6, 6, seed=6, npts=4)
+    z = w.z.copy(); z[1] = 0.0; z[2] = -1.0
+    x = w.x.copy(); x[3] = np.nan
+    sol = oracle.solve_nm(w, oracle.Opts(maxiter=5), x=x, z=z)
+    assert list(sol["status"][1:]) == [3, 3, 3]
+    assert np.all(np.isnan(sol["B"][:, 1:])) and np.all(np.isnan(sol["lam"][:, 1:]))
+    assert sol["status"][0] in (0, 1, 2) and np.all(np.isfinite(sol["B"][:, 0]))
+    assert sol["iters"][0] <= 5
+    B = oracle.eval(w, x=x, z=z)
+    assert np.all(np.isnan(B[:, 1:])) and np.all(np.isfinite(B[:, 0]))
+    # M = 0 is a no-op
+    assert oracle.eval(w, x=np.zeros(0), y=np.zeros(0), z=np.zeros(0), lam=np.zeros((3, 0))).shape == (3, 0)
+
+
+# -- O-4 (GRID) ---------------------------------------------------------------
+def test_grid_mode_brute_force_and_monotone():
+    w = random_boundary(5, 6, seed=8, npts=3, zmin=1.0, zmax=3.0)
+    T = 4
+    phis = []
+    for nl in (1, 2, 3, 5):
+        o = oracle.Opts(method=1, n_trial=T, n_level=nl, lam_max=0.4, use_eq12=0)
+        sol = oracle.solve_grid(w, o)
+        phis.append(sol["phi"].copy())
+        # returned residual is the residual at the returned lambda
+        res = oracle.residual(w, sol["lam"], o)
+        assert np.allclose(res["phi"], sol["phi"], rtol=0, atol=1e-9)
+        assert np.all(sol["iters"] == nl) and np.all(sol["status"] == 1)
+    phis = np.array(phis)
+    assert np.all(np.diff(phis, axis=0) <= 1e-15)      # incumbent never gets worse
+    # level 0 is the exhaustive argmin over the T^3 lattice on [0, lam_max/h]
+    ax = 0.4 / w.h * np.arange(T) / (T - 1)
+    for i in range(w.M):
+        best = np.inf
+        for a in ax:
+            for b in ax:
+                for c in ax:
+                    r = oracle.residual(w.subset([i]), np.array([[a], [b], [c]]))
+                    best = min(best, r["phi"][0])
+        assert abs(phis[0, i] - best) < 1e-9
