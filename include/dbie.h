@@ -1,0 +1,151 @@
+/* dbie.h — C ABI of libdbie_b200.so: the data-parallel hot path of the Direct Boundary
+ * Integral Equation (DBIE) method for nonlinear force-free coronal fields
+ * (Wang, Yan & Tan, arXiv 1306.1122; citations are PAPER.md:<line>).
+ *
+ * What the library computes
+ * -------------------------
+ *  Eq. 6 discretised as the nodal sum Eq. 16, for every
+ *  evaluation point i and Cartesian component p in {x,y,z}:
+ *
+ *      B_p(i) = (z_i h^2 / 2 pi) * sum_{k<N} [theta sin(theta) + cos(theta)] / r_ik^3 * B_p0[k],
+ *      r_ik   = sqrt((x_k-x_i)^2 + (y_k-y_i)^2 + z_i^2),  theta = |lambda_p(i)| r_ik,
+ *      (x_k, y_k) = (x0 + (ix+1/2) h, y0 + (iy+1/2) h),   k = iy*nx + ix,
+ *
+ *  and, in dbie_solve, the per-point search of the pseudo-force-free factors
+ *  (lambda_x, lambda_y, lambda_z) by the Downhill Simplex method
+ *  that minimises f_i (Eq. 8) and g_i (Eq. 9), with the frozen-lambda
+ *  first-order finite differences of Eq. 13 and J = curl B (Eq. 14,
+ *  PAPER.md:108-110).  The readings taken where the paper is silent (pixel centres, the scalar
+ *  objective, thresholds, the initial simplex, the GRID mode) are listed in DESIGN.md section 3.
+ *
+ * Conventions
+ * -----------
+ *  - Every array pointer is a CUDA DEVICE pointer unless the function name ends in _host,
+ *    in which case every array pointer is a HOST pointer (pageable or pinned).
+ *  - Arrays are structure-of-arrays, fp64 unless stated: a "3*M" array holds component p of
+ *    point i at [p*M + i].
+ *  - Lengths (x, y, z, h, 1/lambda) share one unit; B is in the units of the boundary data.
+ *  - Ownership: the context copies the boundary in dbie_create (the caller may free its arrays
+ *    when the call returns).  Inputs/outputs of eval/solve are caller-allocated and
+ *    caller-owned.  Scratch memory is owned by the context and grown lazily, so ONE context
+ *    must not be used from two streams or two host threads at the same time.
+ *  - Device-pointer entry points are asynchronous on the given stream (they only enqueue work;
+ *    growing the scratch may synchronise the device once).  _host entry points return after
+ *    the results are in the host arrays.
+ *  - Errors: no exceptions, no aborts, no printing.  Every entry point returns a dbie_status;
+ *    argument errors are detected before any launch.  Per-point problems (z_i <= 0 or a
+ *    non-finite coordinate/lambda) do not fail the call: that point's outputs are NaN (and
+ *    status 3 in dbie_solve).
+ *  - There is no CPU fallback: without a CUDA device every compute entry point returns
+ *    DBIE_ECUDA.
+ */
+#ifndef DBIE_H
+#define DBIE_H
+
+#ifdef __cplusplus
+extern "C" {
+#endif
+
+typedef struct dbie_ctx dbie_ctx; /* opaque; owns its device copy of the boundary */
+
+typedef enum {
+    DBIE_OK = 0,
+    DBIE_EINVAL = 1, /* null pointer, nx/ny < 1, h <= 0, M < 0, bad option            */
+    DBIE_ENOMEM = 2, /* device or host allocation failed                              */
+    DBIE_ECUDA = 3,  /* a CUDA call failed; see dbie_last_cuda_error                  */
+    DBIE_ESTATE = 4  /* the context lacks what the call needs (e.g. no fp32 copy)     */
+} dbie_status;
+
+/* dbie_create flags */
+#define DBIE_WITH_FP32 1u /* also keep an fp32 copy of the boundary for dbie_eval_f32 */
+
+/* Boundary staging (Eq. 3, Eq. 16).
+ * nx, ny: boundary grid, N = nx*ny, pixel k = iy*nx + ix (x fastest).
+ * h: pixel size.  (x0, y0): coordinate of the CORNER of pixel (0,0); its centre is
+ * (x0 + h/2, y0 + h/2, 0) (reading A-1).  bx, by, bz: N doubles each, device, read once.
+ * Outside the nx*ny window the field is zero (reading A-4).
+ * The call synchronises the device before returning. */
+dbie_status dbie_create(dbie_ctx** out, int nx, int ny, double h, double x0, double y0,
+                        const double* bx, const double* by, const double* bz, unsigned flags);
+/* Same with HOST boundary arrays. */
+dbie_status dbie_create_host(dbie_ctx** out, int nx, int ny, double h, double x0, double y0,
+                             const double* bx, const double* by, const double* bz,
+                             unsigned flags);
+void dbie_destroy(dbie_ctx* ctx);
+
+/* Eq. 6 / Eq. 16 at given lambda.
+ * x, y, z: M each, z > 0.  lam: 3*M, lam[p*M+i] = lambda_p(i); only |lambda| matters
+ * (the kernel is even in lambda, reading A-3).  B: out, 3*M.  M = 0 is a no-op. */
+dbie_status dbie_eval(dbie_ctx* ctx, long long M, const double* x, const double* y,
+                      const double* z, const double* lam, double* B, void* cuda_stream);
+dbie_status dbie_eval_host(dbie_ctx* ctx, long long M, const double* x, const double* y,
+                           const double* z, const double* lam, double* B);
+
+/* fp32-arithmetic variant of dbie_eval (BASELINE.json config 4; needs DBIE_WITH_FP32).
+ * Geometry, sincos and products in fp32; partial sums are carried in fp64. */
+dbie_status dbie_eval_f32(dbie_ctx* ctx, long long M, const float* x, const float* y,
+                          const float* z, const float* lam, float* B, void* cuda_stream);
+
+/* Options of dbie_solve.  Fill with dbie_solve_default_opts, then change fields. */
+typedef struct {
+    int method;       /* 0 = NM: Downhill Simplex; 1 = GRID (O-4)     */
+    double delta;     /* finite-difference step as a FRACTION of h; 1e-3        */
+    double cell;      /* d in g_i = |div B| (d/6) / |B|, fraction of h; 1.0 (reading A-6)     */
+    double w_g;       /* Phi = f + w_g g; 1.0 (reading A-7)                                   */
+    double eps_f;     /* Eq. 12 thresholds; 1e-3, 1e-4 (reading A-8)         */
+    double eps_g;
+    double lam0;      /* NM initial simplex: V0 = (lam0,lam0,lam0)/h, V_j = V0 + step/h e_j;  */
+    double step;      /*   0.05, 0.05 (reading A-9)                                           */
+    double xtol;      /* NM stop: max |V_j - V_0| <= xtol/h and max |Phi_j - Phi_0| <= ftol;  */
+    double ftol;      /*   1e-4, 1e-6                                                         */
+    int maxiter;      /* NM iteration cap; 200                                                */
+    int n_trial;      /* GRID: T trial lambda per component per level (>= 2); 8               */
+    int n_level;      /* GRID: number of refinement levels; 10                                */
+    double lam_max;   /* GRID: search window [0, lam_max/h]; 0.4                              */
+    int use_eq12;     /* 1: stop a point as soon as f <= eps_f and g <= eps_g (Eq. 12)        */
+} dbie_solve_opts;
+
+void dbie_solve_default_opts(dbie_solve_opts* opts);
+
+/* Per-point lambda optimisation.  The whole search
+ * runs on the device; no per-iteration data returns to the host.
+ * B: out 3*M, field at lambda*.  lam: out 3*M, lambda* >= 0 (reading A-3).
+ * resid: out 2*M, resid[i] = f_i (Eq. 8), resid[M+i] = g_i (Eq. 9) at lambda*.
+ * iters: out M (NM iterations / GRID levels done).  status: out M: 0 = Eq. 12 thresholds
+ * met, 1 = simplex tolerance (GRID: all levels done), 2 = maxiter, 3 = invalid point. */
+dbie_status dbie_solve(dbie_ctx* ctx, long long M, const double* x, const double* y,
+                       const double* z, const dbie_solve_opts* opts, double* B, double* lam,
+                       double* resid, int* iters, int* status, void* cuda_stream);
+dbie_status dbie_solve_host(dbie_ctx* ctx, long long M, const double* x, const double* y,
+                            const double* z, const dbie_solve_opts* opts, double* B,
+                            double* lam, double* resid, int* iters, int* status);
+
+/* Eq. 8, 9, 13, 14 at given lambda triples (one objective evaluation per point; the same
+ * code path the solver uses).  out: 9*M, rows B_x,B_y,B_z, f, g, J_x,J_y,J_z, div B.
+ * delta, cell, w_g are taken from opts (NULL = defaults).  phi: out M (may be NULL). */
+dbie_status dbie_residual(dbie_ctx* ctx, long long M, const double* x, const double* y,
+                          const double* z, const double* lam, const dbie_solve_opts* opts,
+                          double* out, double* phi, void* cuda_stream);
+
+/* Counters of the last eval/solve/residual call on this context (host values, valid after
+ * the stream has been synchronised): point-pixel interactions evaluated (one interaction =
+ * one (evaluation point, pixel) pair, all three components), kernel launches enqueued, and
+ * objective evaluations.  Any pointer may be NULL. */
+dbie_status dbie_last_counters(dbie_ctx* ctx, double* interactions, long long* launches,
+                               long long* objective_evals);
+
+/* Measured peak of the FP64 pipe: runs a register-only DFMA loop on every SM for about
+ * `millis` ms and returns DFMA instructions (per lane) per second.  Synchronises. */
+dbie_status dbie_probe_dfma_rate(double millis, double* dfma_per_s, double* ffma_per_s);
+
+const char* dbie_strerror(dbie_status s);
+/* CUDA error string of the last DBIE_ECUDA on this context (or of the last failure with
+ * no context when ctx is NULL).  Never NULL. */
+const char* dbie_last_cuda_error(const dbie_ctx* ctx);
+/* Library version string, e.g. "dbie-b200 0.1 (sm_100a)". */
+const char* dbie_version(void);
+
+#ifdef __cplusplus
+}
+#endif
+#endif /* DBIE_H */

@@ -1,0 +1,430 @@
+// dbie_api.cu — the C ABI of include/dbie.h: argument checks, context and scratch management,
+// and the launch sequences of eval / residual / solve.  No arithmetic of the method lives here.
+#include <cuda_runtime.h>
+#include <math.h>
+#include <stdio.h>
+#include <stdlib.h>
+#include <string.h>
+
+#include "dbie_internal.h"
+
+using namespace dbie;
+
+struct dbie_ctx {
+    int device, sm_count;
+    BoundaryView bd;
+    double4* rec;
+    double* yk;
+    float4* rec32;
+    float* yk32;
+    double* part;       size_t part_bytes;    // chunk partial sums
+    char* state;        size_t state_bytes;   // optimiser state
+    char* io;           size_t io_bytes;      // device staging of the _host entry points
+    unsigned* counters;                       // device: nact[2], pad[2], then nevals (u64) at +16 B
+    cudaStream_t own_stream;
+    double last_interactions;
+    long long last_launches, last_evals;
+    int evals_on_device;                      // last call was a solve: read nevals back on demand
+    char err[256];
+};
+
+static char g_err[256] = "no error";
+
+static dbie_status fail_cuda(dbie_ctx* c, cudaError_t e, const char* where) {
+    char* dst = c ? c->err : g_err;
+    snprintf(dst, 256, "%s: %s", where, cudaGetErrorString(e));
+    if (c) memcpy(g_err, c->err, 256);
+    (void)cudaGetLastError();
+    return e == cudaErrorMemoryAllocation ? DBIE_ENOMEM : DBIE_ECUDA;
+}
+#define CU(call)                                                   \
+    do {                                                           \
+        cudaError_t e_ = (call);                                   \
+        if (e_ != cudaSuccess) return fail_cuda(ctx, e_, #call);   \
+    } while (0)
+
+static dbie_status ensure(dbie_ctx* ctx, void** ptr, size_t* have, size_t need) {
+    if (need <= *have) return DBIE_OK;
+    if (*ptr) {
+        CU(cudaFree(*ptr));   // synchronises the device: nothing in flight uses the old buffer after this
+        *ptr = nullptr;
+        *have = 0;
+    }
+    CU(cudaMalloc(ptr, need));
+    *have = need;
+    return DBIE_OK;
+}
+
+extern "C" const char* dbie_strerror(dbie_status s) {
+    switch (s) {
+        case DBIE_OK: return "ok";
+        case DBIE_EINVAL: return "invalid argument";
+        case DBIE_ENOMEM: return "out of memory";
+        case DBIE_ECUDA: return "CUDA error (see dbie_last_cuda_error)";
+        case DBIE_ESTATE: return "context lacks what the call needs";
+    }
+    return "unknown status";
+}
+extern "C" const char* dbie_last_cuda_error(const dbie_ctx* ctx) { return ctx ? ctx->err : g_err; }
+extern "C" const char* dbie_version(void) { return "dbie-b200 0.1 (sm_100a)"; }
+
+extern "C" void dbie_solve_default_opts(dbie_solve_opts* o) {
+    if (!o) return;
+    memset(o, 0, sizeof *o);
+    o->method = 0;
+    o->delta = 1e-3;
+    o->cell = 1.0;
+    o->w_g = 1.0;
+    o->eps_f = 1e-3;
+    o->eps_g = 1e-4;
+    o->lam0 = 0.05;
+    o->step = 0.05;
+    o->xtol = 1e-4;
+    o->ftol = 1e-6;
+    o->maxiter = 200;
+    o->n_trial = 8;
+    o->n_level = 10;
+    o->lam_max = 0.4;
+    o->use_eq12 = 1;
+}
+
+static void setup_tiling(BoundaryView& b) {
+    if (b.nx <= kTilePx) {
+        b.tile_rows = kTilePx / b.nx;
+        if (b.tile_rows < 1) b.tile_rows = 1;
+        b.segs_per_row = 1;
+        b.seg_w = b.nx;
+        b.ntiles = (b.ny + b.tile_rows - 1) / b.tile_rows;
+    } else {
+        b.tile_rows = 1;
+        b.segs_per_row = (b.nx + kTilePx - 1) / kTilePx;
+        b.seg_w = (b.nx + b.segs_per_row - 1) / b.segs_per_row;
+        b.seg_w += b.seg_w & 1;
+        b.ntiles = b.ny * b.segs_per_row;
+    }
+    b.nchunks = b.ntiles < kMaxChunks ? b.ntiles : kMaxChunks;
+}
+
+extern "C" void dbie_destroy(dbie_ctx* ctx) {
+    if (!ctx) return;
+    cudaFree(ctx->rec);
+    cudaFree(ctx->yk);
+    cudaFree(ctx->rec32);
+    cudaFree(ctx->yk32);
+    cudaFree(ctx->part);
+    cudaFree(ctx->state);
+    cudaFree(ctx->io);
+    cudaFree(ctx->counters);
+    if (ctx->own_stream) cudaStreamDestroy(ctx->own_stream);
+    (void)cudaGetLastError();
+    free(ctx);
+}
+
+extern "C" dbie_status dbie_create(dbie_ctx** out, int nx, int ny, double h, double x0, double y0,
+                                   const double* bx, const double* by, const double* bz, unsigned flags) {
+    if (!out) return DBIE_EINVAL;
+    *out = nullptr;
+    if (nx < 1 || ny < 1 || !(h > 0.0) || !isfinite(h) || !isfinite(x0) || !isfinite(y0) || !bx || !by || !bz)
+        return DBIE_EINVAL;
+    if ((long long)nx * ny > (1LL << 30)) return DBIE_EINVAL;
+    dbie_ctx* ctx = (dbie_ctx*)calloc(1, sizeof(dbie_ctx));
+    if (!ctx) return DBIE_ENOMEM;
+    strcpy(ctx->err, "no error");
+    dbie_status st = DBIE_OK;
+    do {
+        cudaError_t e;
+        if ((e = cudaGetDevice(&ctx->device)) != cudaSuccess) { st = fail_cuda(ctx, e, "cudaGetDevice"); break; }
+        if ((e = cudaDeviceGetAttribute(&ctx->sm_count, cudaDevAttrMultiProcessorCount, ctx->device)) != cudaSuccess) {
+            st = fail_cuda(ctx, e, "cudaDeviceGetAttribute"); break;
+        }
+        BoundaryView& b = ctx->bd;
+        b.nx = nx; b.ny = ny; b.N = (long long)nx * ny;
+        b.h = h; b.x0 = x0; b.y0 = y0;
+        setup_tiling(b);
+        if ((e = cudaMalloc(&ctx->rec, sizeof(double4) * b.N)) != cudaSuccess) { st = fail_cuda(ctx, e, "cudaMalloc(rec)"); break; }
+        if ((e = cudaMalloc(&ctx->yk, sizeof(double) * ny)) != cudaSuccess) { st = fail_cuda(ctx, e, "cudaMalloc(yk)"); break; }
+        if (flags & DBIE_WITH_FP32) {
+            if ((e = cudaMalloc(&ctx->rec32, sizeof(float4) * b.N)) != cudaSuccess) { st = fail_cuda(ctx, e, "cudaMalloc(rec32)"); break; }
+            if ((e = cudaMalloc(&ctx->yk32, sizeof(float) * ny)) != cudaSuccess) { st = fail_cuda(ctx, e, "cudaMalloc(yk32)"); break; }
+        }
+        if ((e = cudaMalloc(&ctx->counters, 64)) != cudaSuccess) { st = fail_cuda(ctx, e, "cudaMalloc(counters)"); break; }
+        if ((e = cudaMemset(ctx->counters, 0, 64)) != cudaSuccess) { st = fail_cuda(ctx, e, "cudaMemset"); break; }
+        if ((e = cudaStreamCreateWithFlags(&ctx->own_stream, cudaStreamNonBlocking)) != cudaSuccess) { st = fail_cuda(ctx, e, "cudaStreamCreate"); break; }
+        if ((e = launch_stage_boundary(nx, ny, h, x0, y0, bx, by, bz, ctx->rec, ctx->yk, ctx->rec32, ctx->yk32, 0)) != cudaSuccess) {
+            st = fail_cuda(ctx, e, "stage_boundary"); break;
+        }
+        if ((e = cudaDeviceSynchronize()) != cudaSuccess) { st = fail_cuda(ctx, e, "stage_boundary(sync)"); break; }
+        b.rec = ctx->rec; b.yk = ctx->yk; b.rec32 = ctx->rec32; b.yk32 = ctx->yk32;
+    } while (0);
+    if (st != DBIE_OK) {
+        memcpy(g_err, ctx->err, 256);
+        dbie_destroy(ctx);
+        return st;
+    }
+    *out = ctx;
+    return DBIE_OK;
+}
+
+extern "C" dbie_status dbie_create_host(dbie_ctx** out, int nx, int ny, double h, double x0, double y0,
+                                        const double* bx, const double* by, const double* bz, unsigned flags) {
+    if (!out) return DBIE_EINVAL;
+    *out = nullptr;
+    if (nx < 1 || ny < 1 || !bx || !by || !bz) return DBIE_EINVAL;
+    dbie_ctx* ctx = nullptr;   // for CU()
+    const size_t n = (size_t)nx * ny;
+    double* d = nullptr;
+    CU(cudaMalloc(&d, 3 * n * sizeof(double)));
+    cudaError_t e = cudaMemcpy(d, bx, n * sizeof(double), cudaMemcpyHostToDevice);
+    if (e == cudaSuccess) e = cudaMemcpy(d + n, by, n * sizeof(double), cudaMemcpyHostToDevice);
+    if (e == cudaSuccess) e = cudaMemcpy(d + 2 * n, bz, n * sizeof(double), cudaMemcpyHostToDevice);
+    if (e != cudaSuccess) { cudaFree(d); return fail_cuda(nullptr, e, "cudaMemcpy(boundary)"); }
+    const dbie_status st = dbie_create(out, nx, ny, h, x0, y0, d, d + n, d + 2 * n, flags);
+    cudaFree(d);
+    return st;
+}
+
+// ------------------------------------------------------------------------------ eval ------
+static const long long kEvalBatch = 1LL << 21;
+static const long long kStencilBatch = 1LL << 22;
+
+extern "C" dbie_status dbie_eval(dbie_ctx* ctx, long long M, const double* x, const double* y, const double* z,
+                                 const double* lam, double* B, void* cuda_stream) {
+    if (!ctx || M < 0) return DBIE_EINVAL;
+    if (M == 0) return DBIE_OK;
+    if (!x || !y || !z || !lam || !B) return DBIE_EINVAL;
+    cudaStream_t st = (cudaStream_t)cuda_stream;
+    const long long cap = M < kEvalBatch ? M : kEvalBatch;
+    const dbie_status s = ensure(ctx, (void**)&ctx->part, &ctx->part_bytes,
+                                 (size_t)ctx->bd.nchunks * 3 * cap * sizeof(double));
+    if (s != DBIE_OK) return s;
+    long long launches = 0;
+    for (long long off = 0; off < M; off += cap) {
+        const long long cnt = (M - off < cap) ? (M - off) : cap;
+        InteractParams p;
+        memset(&p, 0, sizeof p);
+        p.bd = ctx->bd;
+        p.x = x; p.y = y; p.z = z; p.lam = lam; p.ldlam = M;
+        p.count = cnt; p.slot0 = off;
+        p.part = ctx->part; p.cap = cap;
+        CU(launch_interact_eval(p, ctx->sm_count, st));
+        CU(launch_eval_finalize(ctx->bd, off, cnt, M, z, lam, ctx->part, cap, B, st));
+        launches += 2;
+    }
+    ctx->last_interactions = (double)M * (double)ctx->bd.N;
+    ctx->last_launches = launches;
+    ctx->last_evals = 0;
+    ctx->evals_on_device = 0;
+    return DBIE_OK;
+}
+
+static dbie_status io_reserve(dbie_ctx* ctx, size_t bytes) { return ensure(ctx, (void**)&ctx->io, &ctx->io_bytes, bytes); }
+
+extern "C" dbie_status dbie_eval_host(dbie_ctx* ctx, long long M, const double* x, const double* y,
+                                      const double* z, const double* lam, double* B) {
+    if (!ctx || M < 0) return DBIE_EINVAL;
+    if (M == 0) return DBIE_OK;
+    if (!x || !y || !z || !lam || !B) return DBIE_EINVAL;
+    const size_t m = (size_t)M * sizeof(double);
+    dbie_status s = io_reserve(ctx, 9 * m);
+    if (s != DBIE_OK) return s;
+    double* d = (double*)ctx->io;   // x, y, z, lam[3], B[3]
+    cudaStream_t st = ctx->own_stream;
+    CU(cudaMemcpyAsync(d, x, m, cudaMemcpyHostToDevice, st));
+    CU(cudaMemcpyAsync(d + M, y, m, cudaMemcpyHostToDevice, st));
+    CU(cudaMemcpyAsync(d + 2 * M, z, m, cudaMemcpyHostToDevice, st));
+    CU(cudaMemcpyAsync(d + 3 * M, lam, 3 * m, cudaMemcpyHostToDevice, st));
+    s = dbie_eval(ctx, M, d, d + M, d + 2 * M, d + 3 * M, d + 6 * M, st);
+    if (s != DBIE_OK) return s;
+    CU(cudaMemcpyAsync(B, d + 6 * M, 3 * m, cudaMemcpyDeviceToHost, st));
+    CU(cudaStreamSynchronize(st));
+    return DBIE_OK;
+}
+
+extern "C" dbie_status dbie_eval_f32(dbie_ctx* ctx, long long M, const float* x, const float* y, const float* z,
+                                     const float* lam, float* B, void* cuda_stream) {
+    (void)x; (void)y; (void)z; (void)lam; (void)B; (void)cuda_stream;
+    if (!ctx || M < 0) return DBIE_EINVAL;
+    if (!ctx->rec32) return DBIE_ESTATE;
+    snprintf(ctx->err, 256, "dbie_eval_f32: fp32 kernel not built in this version");
+    return DBIE_ESTATE;
+}
+
+// ------------------------------------------------------------------------------ solve -----
+static dbie_status make_consts(const dbie_ctx* ctx, const dbie_solve_opts* o, NMConsts* k) {
+    dbie_solve_opts d;
+    if (!o) { dbie_solve_default_opts(&d); o = &d; }
+    const double h = ctx->bd.h;
+    if (!(o->delta > 0.0) || !(o->cell > 0.0) || !isfinite(o->w_g) || o->maxiter < 0 || !(o->xtol >= 0.0) ||
+        !(o->ftol >= 0.0) || !isfinite(o->lam0) || !isfinite(o->step) || o->step == 0.0)
+        return DBIE_EINVAL;
+    k->delta_abs = o->delta * h;
+    k->d_abs = o->cell * h;
+    k->w_g = o->w_g;
+    k->eps_f = o->eps_f;
+    k->eps_g = o->eps_g;
+    k->xtol_abs = o->xtol / h;
+    k->ftol = o->ftol;
+    k->lam0_abs = o->lam0 / h;
+    k->step_abs = o->step / h;
+    k->h2_over_2pi = h * h / (2.0 * 3.14159265358979323846);
+    k->maxiter = o->maxiter;
+    k->use_eq12 = o->use_eq12;
+    return DBIE_OK;
+}
+
+extern "C" dbie_status dbie_residual(dbie_ctx* ctx, long long M, const double* x, const double* y,
+                                     const double* z, const double* lam, const dbie_solve_opts* opts,
+                                     double* out, double* phi, void* cuda_stream) {
+    if (!ctx || M < 0) return DBIE_EINVAL;
+    if (M == 0) return DBIE_OK;
+    if (!x || !y || !z || !lam || !out) return DBIE_EINVAL;
+    NMConsts k;
+    dbie_status s = make_consts(ctx, opts, &k);
+    if (s != DBIE_OK) return s;
+    cudaStream_t st = (cudaStream_t)cuda_stream;
+    const long long cap = M < kStencilBatch ? M : kStencilBatch;
+    s = ensure(ctx, (void**)&ctx->part, &ctx->part_bytes, (size_t)ctx->bd.nchunks * 12 * cap * sizeof(double));
+    if (s != DBIE_OK) return s;
+    long long launches = 0;
+    for (long long off = 0; off < M; off += cap) {
+        const long long cnt = (M - off < cap) ? (M - off) : cap;
+        InteractParams p;
+        memset(&p, 0, sizeof p);
+        p.bd = ctx->bd;
+        p.x = x + off; p.y = y + off; p.z = z + off;
+        p.lam = lam + off; p.ldlam = M;
+        p.count = cnt;
+        p.delta_abs = k.delta_abs;
+        p.part = ctx->part; p.cap = cap;
+        CU(launch_interact_stencil(p, ctx->sm_count, st));
+        CU(launch_residual_finalize(ctx->bd, k, cnt, M, z + off, ctx->part, cap, out + off, phi ? phi + off : nullptr, st));
+        launches += 2;
+    }
+    ctx->last_interactions = (double)M * kStencil * (double)ctx->bd.N;
+    ctx->last_launches = launches;
+    ctx->last_evals = M;
+    ctx->evals_on_device = 0;
+    return DBIE_OK;
+}
+
+static size_t align256(size_t v) { return (v + 255) & ~(size_t)255; }
+
+extern "C" dbie_status dbie_solve(dbie_ctx* ctx, long long M, const double* x, const double* y, const double* z,
+                                  const dbie_solve_opts* opts, double* B, double* lam, double* resid, int* iters,
+                                  int* status, void* cuda_stream) {
+    if (!ctx || M < 0) return DBIE_EINVAL;
+    if (M == 0) return DBIE_OK;
+    if (!x || !y || !z || !B || !lam || !resid || !iters || !status) return DBIE_EINVAL;
+    if (M > 0x7fffffffLL) return DBIE_EINVAL;
+    NMConsts k;
+    dbie_status s = make_consts(ctx, opts, &k);
+    if (s != DBIE_OK) return s;
+    if (opts && opts->method != 0) {
+        snprintf(ctx->err, 256, "dbie_solve: method %d (GRID) not built in this version", opts->method);
+        return DBIE_EINVAL;
+    }
+    cudaStream_t st = (cudaStream_t)cuda_stream;
+    const long long cap = M < kStencilBatch ? M : kStencilBatch;
+    s = ensure(ctx, (void**)&ctx->part, &ctx->part_bytes, (size_t)ctx->bd.nchunks * 12 * cap * sizeof(double));
+    if (s != DBIE_OK) return s;
+    // state layout: 48 doubles + 4 ints per point
+    const size_t isz = align256((size_t)cap * sizeof(int));
+    s = ensure(ctx, (void**)&ctx->state, &ctx->state_bytes, 48 * (size_t)cap * sizeof(double) + 5 * 256 + 4 * isz);
+    if (s != DBIE_OK) return s;
+    SolveArrays a;
+    char* base = ctx->state;
+    // arrays are indexed [q*cap + i], so each block of q rows must be contiguous with stride cap
+    const size_t dstride = (size_t)cap * sizeof(double);
+    a.V = (double*)base;                 base += align256(12 * dstride);
+    a.F = (double*)base;                 base += align256(4 * dstride);
+    a.aux = (double*)base;               base += align256(20 * dstride);
+    a.pend = (double*)base;              base += align256(9 * dstride);
+    a.cand = (double*)base;              base += align256(3 * dstride);
+    a.phase = (int*)base;                base += isz;
+    a.iters = (int*)base;                base += isz;
+    a.act[0] = (int*)base;               base += isz;
+    a.act[1] = (int*)base;               base += isz;
+    a.nact = ctx->counters;
+    unsigned long long* nevals = (unsigned long long*)((char*)ctx->counters + 16);
+    CU(cudaMemsetAsync(ctx->counters, 0, 64, st));
+    const int maxpass = 4 + 5 * k.maxiter + 1;
+    long long launches = 0;
+    for (long long off = 0; off < M; off += cap) {
+        const long long cnt = (M - off < cap) ? (M - off) : cap;
+        CU(cudaMemsetAsync(ctx->counters, 0, 8, st));
+        CU(launch_solve_init(a, k, cnt, M, x + off, y + off, z + off, B + off, lam + off, resid + off,
+                             iters + off, status + off, st));
+        ++launches;
+        for (int pass = 0; pass < maxpass; ++pass) {
+            InteractParams p;
+            memset(&p, 0, sizeof p);
+            p.bd = ctx->bd;
+            p.x = x + off; p.y = y + off; p.z = z + off;
+            p.lam = a.cand; p.ldlam = cnt;
+            p.act = a.act[pass & 1];
+            p.count_ptr = &a.nact[pass & 1];
+            p.zero_ptr = &a.nact[(pass + 1) & 1];
+            p.delta_abs = k.delta_abs;
+            p.part = ctx->part; p.cap = cap;
+            CU(launch_interact_stencil(p, ctx->sm_count, st));
+            CU(launch_solve_step(a, k, ctx->bd, pass, cnt, M, z + off, ctx->part, cap, B + off, lam + off,
+                                 resid + off, iters + off, status + off, nevals, st));
+            launches += 2;
+        }
+    }
+    ctx->last_launches = launches;
+    ctx->evals_on_device = 1;
+    return DBIE_OK;
+}
+
+extern "C" dbie_status dbie_solve_host(dbie_ctx* ctx, long long M, const double* x, const double* y,
+                                       const double* z, const dbie_solve_opts* opts, double* B, double* lam,
+                                       double* resid, int* iters, int* status) {
+    if (!ctx || M < 0) return DBIE_EINVAL;
+    if (M == 0) return DBIE_OK;
+    if (!x || !y || !z || !B || !lam || !resid || !iters || !status) return DBIE_EINVAL;
+    const size_t m = (size_t)M * sizeof(double);
+    dbie_status s = io_reserve(ctx, 11 * m + 2 * align256((size_t)M * sizeof(int)) + 512);
+    if (s != DBIE_OK) return s;
+    double* d = (double*)ctx->io;   // x, y, z, B[3], lam[3], resid[2], iters, status
+    int* di = (int*)(ctx->io + align256(11 * m));
+    int* ds = (int*)((char*)di + align256((size_t)M * sizeof(int)));
+    cudaStream_t st = ctx->own_stream;
+    CU(cudaMemcpyAsync(d, x, m, cudaMemcpyHostToDevice, st));
+    CU(cudaMemcpyAsync(d + M, y, m, cudaMemcpyHostToDevice, st));
+    CU(cudaMemcpyAsync(d + 2 * M, z, m, cudaMemcpyHostToDevice, st));
+    s = dbie_solve(ctx, M, d, d + M, d + 2 * M, opts, d + 3 * M, d + 6 * M, d + 9 * M, di, ds, st);
+    if (s != DBIE_OK) return s;
+    CU(cudaMemcpyAsync(B, d + 3 * M, 3 * m, cudaMemcpyDeviceToHost, st));
+    CU(cudaMemcpyAsync(lam, d + 6 * M, 3 * m, cudaMemcpyDeviceToHost, st));
+    CU(cudaMemcpyAsync(resid, d + 9 * M, 2 * m, cudaMemcpyDeviceToHost, st));
+    CU(cudaMemcpyAsync(iters, di, (size_t)M * sizeof(int), cudaMemcpyDeviceToHost, st));
+    CU(cudaMemcpyAsync(status, ds, (size_t)M * sizeof(int), cudaMemcpyDeviceToHost, st));
+    CU(cudaStreamSynchronize(st));
+    return DBIE_OK;
+}
+
+extern "C" dbie_status dbie_last_counters(dbie_ctx* ctx, double* interactions, long long* launches,
+                                          long long* objective_evals) {
+    if (!ctx) return DBIE_EINVAL;
+    if (ctx->evals_on_device) {
+        unsigned long long n = 0;
+        CU(cudaMemcpy(&n, (char*)ctx->counters + 16, sizeof n, cudaMemcpyDeviceToHost));
+        ctx->last_evals = (long long)n;
+        ctx->last_interactions = (double)n * kStencil * (double)ctx->bd.N;
+    }
+    if (interactions) *interactions = ctx->last_interactions;
+    if (launches) *launches = ctx->last_launches;
+    if (objective_evals) *objective_evals = ctx->last_evals;
+    return DBIE_OK;
+}
+
+extern "C" dbie_status dbie_probe_dfma_rate(double millis, double* dfma_per_s, double* ffma_per_s) {
+    dbie_ctx* ctx = nullptr;
+    if (!(millis > 0.0)) return DBIE_EINVAL;
+    int dev = 0, sms = 0;
+    CU(cudaGetDevice(&dev));
+    CU(cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, dev));
+    CU(launch_probe(millis, sms, dfma_per_s, ffma_per_s));
+    return DBIE_OK;
+}

@@ -1,0 +1,370 @@
+// dbie_interact.cu — the M x N point-pixel interaction kernel.
+//
+//   B_p(i) = (z_i h^2/2pi) sum_k [theta sin theta + cos theta]/r^3 * B_p0[k],  theta = |lambda_p| r
+//   (Eq. 6, Eq. 16).
+//
+// Mapping (the inverse of the paper's, which strides the PIXELS of one point
+// over 80x128 threads): evaluation points are the parallel dimension, register-blocked R per
+// thread; the boundary is streamed through shared memory in 16 KB tiles by the TMA bulk-copy
+// engine (cp.async.bulk + mbarrier, double buffered) and every thread of the CTA reads the same
+// pixel record as a broadcast LDS.128 pair.  The bound is the FP64 pipe (76 FP64 instructions per
+// interaction); there are no tensor-core or HBM-bound steps.
+#include <cuda_runtime.h>
+#include <stdint.h>
+
+#include "dbie_internal.h"
+#include "dbie_math.cuh"
+
+namespace dbie {
+
+// ------------------------------------------------------------------ PTX wrappers ----------
+__device__ __forceinline__ uint32_t smem_u32(const void* p) {
+    return (uint32_t)__cvta_generic_to_shared(p);
+}
+__device__ __forceinline__ void mbar_init(uint64_t* bar, unsigned count) {
+    asm volatile("mbarrier.init.shared::cta.b64 [%0], %1;" ::"r"(smem_u32(bar)), "r"(count) : "memory");
+}
+__device__ __forceinline__ void mbar_fence_init() {
+    asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
+    asm volatile("fence.proxy.async.shared::cta;" ::: "memory");
+}
+__device__ __forceinline__ void mbar_expect_tx(uint64_t* bar, unsigned bytes) {
+    asm volatile("mbarrier.arrive.expect_tx.shared::cta.b64 _, [%0], %1;" ::"r"(smem_u32(bar)), "r"(bytes)
+                 : "memory");
+}
+// TMA bulk copy global -> shared, completion signalled on the mbarrier (SASS: UBLKCP)
+__device__ __forceinline__ void bulk_g2s(void* dst, const void* src, unsigned bytes, uint64_t* bar) {
+    asm volatile(
+        "cp.async.bulk.shared::cluster.global.mbarrier::complete_tx::bytes [%0], [%1], %2, [%3];" ::"r"(
+            smem_u32(dst)),
+        "l"(src), "r"(bytes), "r"(smem_u32(bar))
+        : "memory");
+}
+__device__ __forceinline__ bool mbar_try_wait(uint64_t* bar, unsigned parity) {
+    uint32_t ok;
+    asm volatile(
+        "{\n\t.reg .pred p;\n\t"
+        "mbarrier.try_wait.parity.shared::cta.b64 p, [%1], %2;\n\t"
+        "selp.u32 %0, 1, 0, p;\n\t}"
+        : "=r"(ok)
+        : "r"(smem_u32(bar)), "r"(parity)
+        : "memory");
+    return ok != 0;
+}
+__device__ __forceinline__ void mbar_wait(uint64_t* bar, unsigned parity) {
+    while (!mbar_try_wait(bar, parity)) {
+    }
+}
+
+// ------------------------------------------------------------------ boundary staging ------
+// A1: rec[k] = {x_k, Bx0, By0, Bz0}; x_k = x0 + (ix + 1/2) h, multiply and add rounded separately.
+__global__ void stage_boundary_kernel(int nx, int ny, double h, double x0, double y0,
+                                      const double* __restrict__ bx, const double* __restrict__ by,
+                                      const double* __restrict__ bz, double4* __restrict__ rec,
+                                      double* __restrict__ yk, float4* __restrict__ rec32,
+                                      float* __restrict__ yk32) {
+    const long long N = (long long)nx * ny;
+    for (long long k = blockIdx.x * (long long)blockDim.x + threadIdx.x; k < N;
+         k += (long long)gridDim.x * blockDim.x) {
+        const int ix = (int)(k % nx);
+        const double xk = __dadd_rn(x0, __dmul_rn((double)ix + 0.5, h));
+        rec[k] = make_double4(xk, bx[k], by[k], bz[k]);
+        if (rec32) rec32[k] = make_float4((float)xk, (float)bx[k], (float)by[k], (float)bz[k]);
+        if (k < ny) {
+            const double y = __dadd_rn(y0, __dmul_rn((double)k + 0.5, h));
+            yk[k] = y;
+            if (yk32) yk32[k] = (float)y;
+        }
+    }
+}
+
+cudaError_t launch_stage_boundary(int nx, int ny, double h, double x0, double y0, const double* bx,
+                                  const double* by, const double* bz, double4* rec, double* yk,
+                                  float4* rec32, float* yk32, cudaStream_t st) {
+    const long long N = (long long)nx * ny;
+    int grid = (int)((N + 255) / 256);
+    if (grid > 4096) grid = 4096;
+    stage_boundary_kernel<<<grid, 256, 0, st>>>(nx, ny, h, x0, y0, bx, by, bz, rec, yk, rec32, yk32);
+    return cudaGetLastError();
+}
+
+// ------------------------------------------------------------------ interaction kernel ----
+enum { MODE_EVAL = 0, MODE_STENCIL = 1 };
+
+template <int MODE, int R, int THREADS, int MINB>
+__global__ void __launch_bounds__(THREADS, MINB) interact_kernel(const __grid_constant__ InteractParams p) {
+    constexpr int Q = (MODE == MODE_EVAL) ? 3 : 3 * R;        // sums per slot
+    constexpr int SPB = (MODE == MODE_EVAL) ? THREADS * R : THREADS;  // slots per work block
+    constexpr int NL = (MODE == MODE_EVAL) ? R : 1;            // lambda triples per thread
+    static_assert(MODE == MODE_EVAL || R == kStencil, "stencil mode evaluates 4 positions");
+
+    __shared__ alignas(128) double4 tile[2][kTilePx];
+    __shared__ alignas(8) uint64_t full[2];
+
+    const int tid = threadIdx.x;
+    if (tid == 0) {
+        mbar_init(&full[0], 1);
+        mbar_init(&full[1], 1);
+        mbar_fence_init();
+    }
+    __syncthreads();
+
+    if (p.zero_ptr && blockIdx.x == 0 && tid == 0) *p.zero_ptr = 0u;  // next pass's list counter
+    const long long count = p.count_ptr ? (long long)(*p.count_ptr) : p.count;
+    const long long nblk = (count + SPB - 1) / SPB;
+    if (nblk == 0) return;
+    const BoundaryView& bd = p.bd;
+    const int NCH = bd.nchunks;
+    int nsplit = 1;
+    if (nblk < p.target_items) {
+        nsplit = (int)((p.target_items + nblk - 1) / nblk);
+        if (nsplit > NCH) nsplit = NCH;
+    }
+    const long long nwork = nblk * nsplit;
+
+    unsigned it = 0;  // tiles consumed by this CTA so far: stage = it & 1, parity = (it >> 1) & 1
+    for (long long w = blockIdx.x; w < nwork; w += gridDim.x) {
+        const long long blk = w / nsplit;
+        const int sp = (int)(w % nsplit);
+        const int c0 = (int)(((long long)sp * NCH) / nsplit);
+        const int c1 = (int)(((long long)(sp + 1) * NCH) / nsplit);
+
+        // ---- per-thread evaluation points
+        double xi[R], yi[R], z2[R], lam[NL][3];
+        long long slot[NL];
+        if (MODE == MODE_EVAL) {
+#pragma unroll
+            for (int r = 0; r < R; ++r) {
+                slot[r] = blk * SPB + tid + (long long)r * THREADS;
+                const long long id = p.slot0 + (slot[r] < count ? slot[r] : count - 1);
+                xi[r] = p.x[id];
+                yi[r] = p.y[id];
+                const double z = p.z[id];
+                z2[r] = z * z;
+#pragma unroll
+                for (int c = 0; c < 3; ++c) lam[r][c] = fabs(p.lam[c * p.ldlam + id]);
+            }
+        } else {
+            slot[0] = blk * SPB + tid;
+            const long long j = slot[0] < count ? slot[0] : count - 1;
+            const long long id = p.act ? (long long)p.act[j] : j;
+            const double x = p.x[id], y = p.y[id], z = p.z[id];
+            const double zd = __dadd_rn(z, p.delta_abs);
+#pragma unroll
+            for (int r = 0; r < R; ++r) {
+                xi[r] = (r == 1) ? __dadd_rn(x, p.delta_abs) : x;
+                yi[r] = (r == 2) ? __dadd_rn(y, p.delta_abs) : y;
+                z2[r] = (r == 3) ? zd * zd : z * z;
+            }
+#pragma unroll
+            for (int c = 0; c < 3; ++c) lam[0][c] = fabs(p.lam[c * p.ldlam + id]);
+        }
+
+        double acc[R][3];
+#pragma unroll
+        for (int r = 0; r < R; ++r) acc[r][0] = acc[r][1] = acc[r][2] = 0.0;
+
+        const int t0 = chunk_first_tile(bd, c0), t1 = chunk_first_tile(bd, c1);
+        int c = c0;
+        int t_chunk_end = chunk_first_tile(bd, c + 1);
+        if (tid == 0) {
+            const TileDesc d = tile_desc(bd, t0);
+            mbar_expect_tx(&full[it & 1], (unsigned)d.npx * 32u);
+            bulk_g2s(&tile[it & 1][0], bd.rec + d.px0, (unsigned)d.npx * 32u, &full[it & 1]);
+        }
+        for (int t = t0; t < t1; ++t, ++it) {
+            if (tid == 0 && t + 1 < t1) {  // prefetch the next tile into the other stage
+                const TileDesc dn = tile_desc(bd, t + 1);
+                const unsigned sn = (it + 1) & 1;
+                mbar_expect_tx(&full[sn], (unsigned)dn.npx * 32u);
+                bulk_g2s(&tile[sn][0], bd.rec + dn.px0, (unsigned)dn.npx * 32u, &full[sn]);
+            }
+            const TileDesc d = tile_desc(bd, t);
+            mbar_wait(&full[it & 1], (it >> 1) & 1);
+            const double4* __restrict__ rp = &tile[it & 1][0];
+            for (int row = 0; row < d.nrows; ++row) {
+                const double yk = __ldg(bd.yk + d.row0 + row);
+                double cc[R];
+#pragma unroll
+                for (int r = 0; r < R; ++r) {
+                    const double dy = yk - yi[r];
+                    cc[r] = fma(dy, dy, z2[r]);
+                }
+#pragma unroll 1
+                for (int j = 0; j < d.ncols; ++j) {
+                    const double4 px = rp[j];  // {x_k, Bx0, By0, Bz0}: two broadcast LDS.128
+#pragma unroll
+                    for (int r = 0; r < R; ++r) {
+                        const double dx = px.x - xi[r];
+                        const double r2 = fma(dx, dx, cc[r]);
+                        const double y = rsqrt_full(r2);   // 1/r
+                        const double rr = r2 * y;          // r
+                        const double w = (y * y) * y;      // 1/r^3
+                        const int l = (NL == 1) ? 0 : r;
+                        acc[r][0] = fma(kernel_n(lam[l][0] * rr), w * px.y, acc[r][0]);
+                        acc[r][1] = fma(kernel_n(lam[l][1] * rr), w * px.z, acc[r][1]);
+                        acc[r][2] = fma(kernel_n(lam[l][2] * rr), w * px.w, acc[r][2]);
+                    }
+                }
+                rp += d.ncols;
+            }
+            if (t + 1 == t_chunk_end) {  // A4: one partial sum per chunk, added in chunk order later
+                if (MODE == MODE_EVAL) {
+#pragma unroll
+                    for (int r = 0; r < R; ++r)
+                        if (slot[r] < count) {
+#pragma unroll
+                            for (int q = 0; q < 3; ++q)
+                                p.part[((long long)c * Q + q) * p.cap + slot[r]] = acc[r][q];
+                        }
+                } else if (slot[0] < count) {
+#pragma unroll
+                    for (int r = 0; r < R; ++r)
+#pragma unroll
+                        for (int q = 0; q < 3; ++q)
+                            p.part[((long long)c * Q + r * 3 + q) * p.cap + slot[0]] = acc[r][q];
+                }
+#pragma unroll
+                for (int r = 0; r < R; ++r) acc[r][0] = acc[r][1] = acc[r][2] = 0.0;
+                ++c;
+                t_chunk_end = chunk_first_tile(bd, c + 1);
+            }
+            __syncthreads();  // everyone is done with stage it&1 before it is refilled
+        }
+    }
+}
+
+constexpr int kEvalR = 2, kEvalThreads = 256, kEvalMinB = 2;
+constexpr int kStenThreads = 128, kStenMinB = 4;
+
+cudaError_t launch_interact_eval(const InteractParams& p, int sm_count, cudaStream_t st) {
+    if (p.count <= 0) return cudaSuccess;
+    InteractParams q = p;
+    const long long spb = (long long)kEvalThreads * kEvalR;
+    const long long nblk = (q.count + spb - 1) / spb;
+    q.target_items = 8 * sm_count * kEvalMinB;
+    long long nsplit = 1;
+    if (nblk < q.target_items) {
+        nsplit = (q.target_items + nblk - 1) / nblk;
+        if (nsplit > q.bd.nchunks) nsplit = q.bd.nchunks;
+    }
+    const long long nwork = nblk * nsplit;   // one work item per CTA: the hardware balances them
+    if (nwork > 0x7fffffffLL) return cudaErrorInvalidValue;
+    interact_kernel<MODE_EVAL, kEvalR, kEvalThreads, kEvalMinB><<<(unsigned)nwork, kEvalThreads, 0, st>>>(q);
+    return cudaGetLastError();
+}
+
+cudaError_t launch_interact_stencil(const InteractParams& p, int sm_count, cudaStream_t st) {
+    InteractParams q = p;
+    q.target_items = 4 * sm_count * kStenMinB;
+    long long grid;
+    if (q.count_ptr) {
+        grid = (long long)sm_count * kStenMinB;   // persistent: the slot count lives on the device
+    } else {
+        if (q.count <= 0) return cudaSuccess;
+        const long long nblk = (q.count + kStenThreads - 1) / kStenThreads;
+        long long nsplit = 1;
+        if (nblk < q.target_items) {
+            nsplit = (q.target_items + nblk - 1) / nblk;
+            if (nsplit > q.bd.nchunks) nsplit = q.bd.nchunks;
+        }
+        grid = nblk * nsplit;
+        if (grid > 0x7fffffffLL) return cudaErrorInvalidValue;
+    }
+    interact_kernel<MODE_STENCIL, kStencil, kStenThreads, kStenMinB><<<(unsigned)grid, kStenThreads, 0, st>>>(q);
+    return cudaGetLastError();
+}
+
+// ------------------------------------------------------------------ eval epilogue ---------
+// A4: B_p = (z h^2 / 2 pi) * (sum of the chunk partial sums, in chunk order).
+__global__ void eval_finalize_kernel(int nchunks, double h2_over_2pi, long long slot0, long long count,
+                                     long long M, const double* __restrict__ z,
+                                     const double* __restrict__ lam, const double* __restrict__ part,
+                                     long long cap, double* __restrict__ B) {
+    const long long s = blockIdx.x * (long long)blockDim.x + threadIdx.x;
+    if (s >= count) return;
+    const long long id = slot0 + s;
+    const double zi = z[id];
+    bool ok = (zi > 0.0) && isfinite(zi);
+    double out[3];
+#pragma unroll
+    for (int q = 0; q < 3; ++q) {
+        double sum = part[(long long)q * cap + s];
+        for (int c = 1; c < nchunks; ++c) sum += part[((long long)c * 3 + q) * cap + s];
+        out[q] = (zi * h2_over_2pi) * sum;
+        ok = ok && isfinite(lam[q * M + id]);
+    }
+#pragma unroll
+    for (int q = 0; q < 3; ++q) B[q * M + id] = ok ? out[q] : __longlong_as_double(0x7ff8000000000000LL);
+}
+
+cudaError_t launch_eval_finalize(const BoundaryView& bd, long long slot0, long long count, long long M,
+                                 const double* z, const double* lam, const double* part, long long cap,
+                                 double* B, cudaStream_t st) {
+    if (count <= 0) return cudaSuccess;
+    const double h2_over_2pi = bd.h * bd.h / (2.0 * 3.14159265358979323846);
+    const unsigned grid = (unsigned)((count + 255) / 256);
+    eval_finalize_kernel<<<grid, 256, 0, st>>>(bd.nchunks, h2_over_2pi, slot0, count, M, z, lam, part, cap, B);
+    return cudaGetLastError();
+}
+
+// ------------------------------------------------------------------ pipe-rate probe -------
+// Register-only FMA chains: the measured denominator of the ALU roofline.
+template <typename T>
+__global__ void __launch_bounds__(256) fma_probe_kernel(int iters, T seed, T* sink) {
+    T a[8];
+#pragma unroll
+    for (int i = 0; i < 8; ++i) a[i] = seed + (T)(threadIdx.x + i);
+    const T m = (T)0.999999, c = (T)1e-7;
+    for (int k = 0; k < iters; ++k) {
+#pragma unroll
+        for (int u = 0; u < 8; ++u) {
+#pragma unroll
+            for (int i = 0; i < 8; ++i) a[i] = fma(a[i], m, c);
+        }
+    }
+    T s = 0;
+#pragma unroll
+    for (int i = 0; i < 8; ++i) s += a[i];
+    if (s == (T)-1.2345) sink[0] = s;  // never true; keeps the chains alive
+}
+
+template <typename T>
+static cudaError_t probe_one(double millis, int sm_count, double* rate) {
+    T* sink = nullptr;
+    cudaError_t e = cudaMalloc(&sink, sizeof(T));
+    if (e != cudaSuccess) return e;
+    cudaEvent_t ev0, ev1;
+    cudaEventCreate(&ev0);
+    cudaEventCreate(&ev1);
+    const int grid = sm_count * 8, threads = 256;
+    int iters = 2000;
+    float ms = 0.f;
+    for (int attempt = 0; attempt < 8; ++attempt) {
+        fma_probe_kernel<T><<<grid, threads>>>(iters / 4 + 1, (T)1, sink);  // warm-up
+        cudaEventRecord(ev0);
+        fma_probe_kernel<T><<<grid, threads>>>(iters, (T)1, sink);
+        cudaEventRecord(ev1);
+        e = cudaEventSynchronize(ev1);
+        if (e != cudaSuccess) break;
+        cudaEventElapsedTime(&ms, ev0, ev1);
+        if (ms >= millis * 0.5 || iters > (1 << 28)) break;
+        const double scale = (ms > 0.01f) ? (millis / ms) * 1.1 : 16.0;
+        iters = (int)(iters * (scale > 16.0 ? 16.0 : scale)) + 1;
+    }
+    if (e == cudaSuccess) e = cudaGetLastError();
+    if (e == cudaSuccess) *rate = (double)grid * threads * 64.0 * (double)iters / (ms * 1e-3);
+    cudaEventDestroy(ev0);
+    cudaEventDestroy(ev1);
+    cudaFree(sink);
+    return e;
+}
+
+cudaError_t launch_probe(double millis, int sm_count, double* dfma_per_s, double* ffma_per_s) {
+    cudaError_t e = cudaSuccess;
+    if (dfma_per_s) e = probe_one<double>(millis, sm_count, dfma_per_s);
+    if (e == cudaSuccess && ffma_per_s) e = probe_one<float>(millis, sm_count, ffma_per_s);
+    return e;
+}
+
+}  // namespace dbie

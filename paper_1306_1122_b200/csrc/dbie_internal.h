@@ -1,0 +1,119 @@
+// dbie_internal.h — structures shared by the translation units of libdbie_b200.so.
+// Not part of the public ABI (that is include/dbie.h).
+#pragma once
+#include <cuda_runtime.h>
+#include <stdint.h>
+
+#include "../../include/dbie.h"
+#include "dbie_nm.cuh"
+
+namespace dbie {
+
+constexpr int kTilePx = 512;     // pixels staged in shared memory at a time (16 KB fp64 records)
+constexpr int kMaxChunks = 16;   // canonical partial sums per evaluation point
+constexpr int kStencil = 4;      // r_i, r_i + delta x, + delta y, + delta z (Eq. 13, reading A-5)
+
+// Device view of the boundary as staged by dbie_create.
+// rec[k] = {x_k, Bx0[k], By0[k], Bz0[k]} (32 B, one LDS.128 pair per pixel), k = iy*nx + ix;
+// yk[iy] = y0 + (iy + 1/2) h.  x_k, y_k are formed as x0 + (ix + 0.5)*h with separately rounded
+// multiply and add, the order the paper's definition of a pixel centre (reading A-1) is
+// written in DESIGN.md.
+struct BoundaryView {
+    int nx, ny;
+    long long N;
+    double h, x0, y0;
+    const double4* rec;
+    const double* yk;
+    const float4* rec32;   // fp32 copy {x_k, Bx0, By0, Bz0} or nullptr
+    const float* yk32;
+    // tiling: a tile is `tile_rows` full rows (nx <= kTilePx) or one row segment of
+    // `seg_w` columns (nx > kTilePx); a chunk is a run of consecutive tiles.
+    int tile_rows, segs_per_row, seg_w;
+    int ntiles, nchunks;
+};
+
+struct TileDesc {
+    int row0, nrows, col0, ncols;
+    long long px0;   // index of the first record (tiles are contiguous in rec[])
+    int npx;
+};
+
+__host__ __device__ inline TileDesc tile_desc(const BoundaryView& b, int t) {
+    TileDesc d;
+    if (b.segs_per_row == 1) {
+        d.row0 = t * b.tile_rows;
+        d.nrows = (b.ny - d.row0 < b.tile_rows) ? (b.ny - d.row0) : b.tile_rows;
+        d.col0 = 0;
+        d.ncols = b.nx;
+    } else {
+        d.row0 = t / b.segs_per_row;
+        d.nrows = 1;
+        d.col0 = (t % b.segs_per_row) * b.seg_w;
+        d.ncols = (b.nx - d.col0 < b.seg_w) ? (b.nx - d.col0) : b.seg_w;
+    }
+    d.px0 = (long long)d.row0 * b.nx + d.col0;
+    d.npx = d.nrows * d.ncols;
+    return d;
+}
+
+__host__ __device__ inline int chunk_first_tile(const BoundaryView& b, int c) {
+    return (int)(((long long)c * b.ntiles) / b.nchunks);
+}
+
+// One launch of the interaction kernel.
+//  MODE_EVAL:    slot i = evaluation point i with its own lambda triple; Q = 3 sums.
+//  MODE_STENCIL: slot j = one objective evaluation of field point pid = act ? act[j] : j at the
+//                4 stencil positions with ONE lambda triple (Eq. 13); Q = 12 sums [s*3 + p].
+// Partial sums go to part[(c*Q + q)*cap + slot], one per chunk c, and are added in chunk order
+// by the consumer, so a result does not depend on how the launch was split.
+struct InteractParams {
+    BoundaryView bd;
+    const double *x, *y, *z;     // by point id
+    const double* lam;           // lam[p*ldlam + id]
+    long long ldlam;
+    const int* act;              // MODE_STENCIL: slot -> point id, or nullptr (identity)
+    const unsigned* count_ptr;   // device-resident slot count, or nullptr
+    long long count;             // host-known slot count (used when count_ptr == nullptr)
+    long long slot0;             // MODE_EVAL: id of slot 0 (batching)
+    double delta_abs;            // MODE_STENCIL: finite-difference step (length units)
+    double* part;
+    long long cap;
+    int target_items;            // split the pixel range until there are this many work items
+    unsigned* zero_ptr;          // set to 0 by the launch (the next pass's list counter), or nullptr
+};
+
+struct SolveArrays {            // per-point optimiser state, structure-of-arrays by point id
+    double* V;                  // [12][M]  simplex vertices V[(j*3+p)*M + i]
+    double* F;                  // [4][M]   Phi at the vertices
+    double* aux;                // [20][M]  (Bx,By,Bz,f,g) at the vertices, aux[(j*5+a)*M + i]
+    double* pend;               // [9][M]   reflection point kept while its follow-up is evaluated
+    double* cand;               // [3][M]   lambda triple of the outstanding evaluation
+    int* phase;                 // [M]
+    int* iters;                 // [M]
+    int* act[2];                // active lists (ping-pong)
+    unsigned* nact;             // [2] device counters
+};
+
+// launchers (defined in the .cu files; all asynchronous on `st`)
+cudaError_t launch_stage_boundary(int nx, int ny, double h, double x0, double y0, const double* bx,
+                                  const double* by, const double* bz, double4* rec, double* yk,
+                                  float4* rec32, float* yk32, cudaStream_t st);
+cudaError_t launch_interact_eval(const InteractParams& p, int sm_count, cudaStream_t st);
+cudaError_t launch_interact_stencil(const InteractParams& p, int sm_count, cudaStream_t st);
+cudaError_t launch_eval_finalize(const BoundaryView& bd, long long slot0, long long count,
+                                 long long M, const double* z, const double* lam, const double* part,
+                                 long long cap, double* B, cudaStream_t st);
+cudaError_t launch_probe(double millis, int sm_count, double* dfma_per_s, double* ffma_per_s);
+
+cudaError_t launch_solve_init(const SolveArrays& s, const NMConsts& k, long long M, long long ldo,
+                              const double* x, const double* y, const double* z, double* B, double* lam,
+                              double* resid, int* iters, int* status, cudaStream_t st);
+cudaError_t launch_solve_step(const SolveArrays& s, const NMConsts& k, const BoundaryView& bd, int pass,
+                              long long M, long long ldo, const double* z, const double* part,
+                              long long cap, double* B, double* lam, double* resid, int* iters,
+                              int* status, unsigned long long* nevals, cudaStream_t st);
+cudaError_t launch_residual_finalize(const BoundaryView& bd, const NMConsts& k, long long M,
+                                     long long ldo, const double* z, const double* part, long long cap,
+                                     double* out, double* phi, cudaStream_t st);
+
+}  // namespace dbie

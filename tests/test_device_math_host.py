@@ -1,0 +1,194 @@
+"""Host-side checks of the CUDA path's own arithmetic (no GPU, no oracle).
+
+`paper_1306_1122_b200/csrc/dbie_math.cuh` and `dbie_nm.cuh` are __host__ __device__; the host
+shim compiles them with g++ so that the polynomial sincos, the reciprocal-sqrt refinement, the
+per-interaction term, the residual formulas and the resumable Nelder-Mead state machine can be
+checked here against mpmath / NumPy / SciPy.  Nothing under oracle/ is imported.
+"""
+import ctypes as C
+import math
+
+import mpmath as mp
+import numpy as np
+import pytest
+from scipy import optimize
+
+from paper_1306_1122_b200 import build as dbuild
+
+_dp = C.POINTER(C.c_double)
+
+
+@pytest.fixture(scope="module")
+def shim():
+    lib = C.CDLL(dbuild.build_hostshim())
+    lib.shim_nm_generic.restype = C.c_int
+    return lib
+
+
+def _p(a):
+    return a.ctypes.data_as(_dp)
+
+
+def _ulp(x):
+    return np.spacing(np.abs(x))
+
+
+def test_trig_coefficients_header_is_current():
+    import subprocess, sys, os
+    script = os.path.join(os.path.dirname(dbuild.__file__), "csrc", "gen_trig_coeffs.py")
+    subprocess.check_call([sys.executable, script, "--check"])
+
+
+def test_sincos_accuracy_against_mpmath(shim):
+    """|theta| up to 1000 rad (config 4 reaches ~155): error <= 1.5 ulp of the result or, near the
+    zeros of sin/cos, <= 2^-53 absolute * |theta| scale of the reduction."""
+    rng = np.random.default_rng(1)
+    th = np.concatenate([rng.uniform(0, 2, 2000), rng.uniform(0, 200, 4000), rng.uniform(0, 1000, 2000),
+                         np.arange(0, 400) * (math.pi / 4), np.arange(1, 400) * (math.pi / 2) * (1 + 1e-12),
+                         [0.0, 1e-300, 1e-8, 0.7853981633974483, 0.7853981633974484]])
+    s = np.empty_like(th); c = np.empty_like(th)
+    shim.shim_sincos(C.c_long(th.size), _p(th), _p(s), _p(c))
+    mp.mp.dps = 50
+    worst = 0.0
+    for t, si, ci in zip(th, s, c):
+        es, ec = mp.sin(mp.mpf(float(t))), mp.cos(mp.mpf(float(t)))
+        # error budget: 1.5 ulp of the value + the reduced argument's own rounding (2^-53 relative of
+        # t <= pi/4 -> 1.2e-16 absolute)
+        for got, ex in ((si, es), (ci, ec)):
+            err = abs(mp.mpf(float(got)) - ex)
+            tol = 1.5 * float(_ulp(float(ex))) + 1.2e-16
+            worst = max(worst, float(err / tol))
+    assert worst <= 1.0, worst
+
+
+def test_kernel_n_matches_definition(shim):
+    """n(theta) = theta sin(theta) + cos(theta): relative to |theta|+1 within 3e-16."""
+    rng = np.random.default_rng(2)
+    th = np.concatenate([rng.uniform(0, 160, 5000), [0.0, 1e-9, 0.5, 100.0]])
+    out = np.empty_like(th)
+    shim.shim_kernel_n(C.c_long(th.size), _p(th), _p(out))
+    mp.mp.dps = 50
+    for t, got in zip(th, out):
+        ex = mp.mpf(float(t)) * mp.sin(mp.mpf(float(t))) + mp.cos(mp.mpf(float(t)))
+        assert abs(mp.mpf(float(got)) - ex) <= 3e-16 * (float(t) + 1.0)
+    # evenness is taken care of by the caller (|lambda|); n(0) = 1 exactly
+    assert out[-4] == 1.0
+
+
+def test_rsqrt_refinement(shim):
+    rng = np.random.default_rng(3)
+    a = np.concatenate([10.0 ** rng.uniform(-6, 8, 5000), [1.0, 4.0, 2.0, 1e-30, 1e30]])
+    out = np.empty_like(a)
+    shim.shim_rsqrt(C.c_long(a.size), _p(a), _p(out))
+    mp.mp.dps = 50
+    rel = [abs(mp.mpf(float(o)) * mp.sqrt(mp.mpf(float(x))) - 1) for x, o in zip(a, out)]
+    assert max(rel) <= 2.3e-16, float(max(rel))     # ~1 ulp
+
+
+def test_single_interaction_term(shim):
+    """One (point, pixel) term as the kernel's inner loop forms it vs the definition in mpmath."""
+    rng = np.random.default_rng(4)
+    mp.mp.dps = 40
+    for _ in range(300):
+        dx, dy = rng.uniform(-400, 400, 2)
+        z = rng.uniform(0.5, 200)
+        lam = rng.uniform(-0.2, 0.2, 3)
+        b0 = rng.uniform(-1500, 1500, 3)
+        out = np.empty(3)
+        shim.shim_interaction(C.c_double(dx), C.c_double(dy), C.c_double(z), _p(lam), _p(b0), _p(out))
+        r = mp.sqrt(mp.mpf(dx) ** 2 + mp.mpf(dy) ** 2 + mp.mpf(z) ** 2)
+        for p in range(3):
+            th = abs(mp.mpf(lam[p])) * r
+            ex = (th * mp.sin(th) + mp.cos(th)) / r ** 3 * mp.mpf(b0[p])
+            scale = (float(th) + 1.0) / float(r) ** 3 * abs(b0[p])
+            # theta = fl(lambda * r) carries 2^-53 * theta of angle error (same in the oracle)
+            assert abs(mp.mpf(out[p]) - ex) <= 4e-16 * scale * max(1.0, float(th)), (dx, dy, z, p)
+
+
+def test_residual_formulas(shim):
+    """Eq. 8, 9, 13, 14 re-derived with NumPy."""
+    rng = np.random.default_rng(5)
+    for _ in range(50):
+        Bs = rng.normal(0, 1, (4, 3))
+        Bs[1:] = Bs[0] + 1e-3 * rng.normal(0, 1, (3, 3))
+        delta, d, wg = 1e-3, 1.0, 0.7
+        out = np.empty(7)
+        shim.shim_residual(_p(Bs.ravel().copy()), C.c_double(delta), C.c_double(d), C.c_double(wg), _p(out))
+        G = (Bs[1:] - Bs[0]).T / delta            # G[p, j] = dB_p/dx_j
+        J = np.array([G[2, 1] - G[1, 2], G[0, 2] - G[2, 0], G[1, 0] - G[0, 1]])
+        div = np.trace(G)
+        B = Bs[0]
+        f = np.linalg.norm(np.cross(J, B)) / (np.linalg.norm(J) * np.linalg.norm(B))
+        g = abs(div) * (d / 6) / np.linalg.norm(B)
+        assert np.allclose(out[2:5], J, rtol=1e-13, atol=0)
+        assert np.isclose(out[5], div, rtol=1e-12, atol=1e-12)
+        assert np.isclose(out[0], f, rtol=1e-12) and np.isclose(out[1], g, rtol=1e-12)
+        assert np.isclose(out[6], f + wg * g, rtol=1e-12)
+    # |B| = 0 is an invalid point
+    out = np.empty(7)
+    shim.shim_residual(_p(np.zeros(12)), C.c_double(1e-3), C.c_double(1.0), C.c_double(1.0), _p(out))
+    assert np.isnan(out[6])
+
+
+_OBJ = C.CFUNCTYPE(C.c_double, _dp)
+
+
+def _run_nm(shim, fn, simplex, xtol, ftol, maxiter):
+    cb = _OBJ(lambda p: float(fn(np.array([p[0], p[1], p[2]]))))
+    simplex = np.ascontiguousarray(simplex, dtype=np.float64)
+    trace = np.full((maxiter + 1, 3), np.nan)
+    fs = np.empty((4, 3)); ff = np.empty(4)
+    it, nf = C.c_int(), C.c_int()
+    st = shim.shim_nm_generic(cb, _p(simplex), C.c_double(xtol), C.c_double(ftol), C.c_int(maxiter),
+                              _p(trace), _p(fs), _p(ff), C.byref(it), C.byref(nf))
+    return {"status": st, "iters": it.value, "nfev": nf.value, "simplex": fs, "f": ff,
+            "trace": trace[: it.value + 1]}
+
+
+@pytest.mark.parametrize("name", ["quadratic", "rosenbrock3", "abs_kink"])
+def test_nm_state_machine_matches_scipy(shim, name):
+    """The resumable state machine reproduces SciPy's non-adaptive Nelder-Mead vertex for vertex."""
+    fns = {
+        "quadratic": lambda v: (v[0] - 0.3) ** 2 + 2 * (v[1] + 0.1) ** 2 + 0.5 * (v[2] - 0.7) ** 2
+                               + 0.3 * v[0] * v[1],
+        "rosenbrock3": lambda v: 100 * (v[1] - v[0] ** 2) ** 2 + (1 - v[0]) ** 2
+                                 + 100 * (v[2] - v[1] ** 2) ** 2 + (1 - v[1]) ** 2,
+        "abs_kink": lambda v: abs(v[0] - 0.2) + abs(v[1] + 0.4) ** 1.5 + (v[2] - 0.1) ** 2 + 0.05 * math.sin(9 * v[0]),
+    }
+    fn = fns[name]
+    x0 = np.array([0.05, 0.05, 0.05])
+    simplex = np.vstack([x0, x0 + [0.05, 0, 0], x0 + [0, 0.05, 0], x0 + [0, 0, 0.05]])
+    xtol, ftol, maxiter = 1e-6, 1e-9, 400
+    mine = _run_nm(shim, fn, simplex, xtol, ftol, maxiter)
+    best = []
+    res = optimize.minimize(fn, x0, method="Nelder-Mead",
+                            options={"initial_simplex": simplex, "adaptive": False, "xatol": xtol,
+                                     "fatol": ftol, "maxiter": maxiter + 1, "maxfev": 10 ** 6,
+                                     "return_all": True})
+    best = np.array(res.allvecs)
+    # SciPy starts its counter at 1 (nit = 1 + simplex updates) and records allvecs[0] before
+    # its initial sort
+    assert mine["iters"] == res.nit - 1
+    assert mine["nfev"] == res.nfev
+    assert mine["status"] == (1 if res.status == 0 else 2)
+    assert np.array_equal(mine["trace"][1:], best[1: mine["iters"] + 1])
+    assert np.array_equal(mine["simplex"], res.final_simplex[0])
+    assert np.array_equal(mine["f"], res.final_simplex[1])
+
+
+def test_nm_maxiter_and_shrink_paths(shim):
+    """A function with a narrow curved valley exercises contraction and shrink; maxiter stops it."""
+    calls = []
+
+    def fn(v):
+        calls.append(tuple(v))
+        return (v[0] ** 2 + v[1] ** 2 + v[2] ** 2 - 1) ** 2 + 5 * abs(v[0] - v[1]) + abs(v[2])
+    x0 = np.array([1.0, -1.0, 0.5])
+    simplex = np.vstack([x0, x0 + [0.3, 0, 0], x0 + [0, 0.3, 0], x0 + [0, 0, 0.3]])
+    mine = _run_nm(shim, fn, simplex, 1e-10, 1e-14, 60)
+    res = optimize.minimize(fn, x0, method="Nelder-Mead",
+                            options={"initial_simplex": simplex, "adaptive": False, "xatol": 1e-10,
+                                     "fatol": 1e-14, "maxiter": 61, "maxfev": 10 ** 6})
+    assert mine["iters"] == res.nit - 1 == 60 and mine["status"] == 2
+    assert mine["nfev"] == res.nfev
+    assert np.array_equal(mine["simplex"][0], res.x)
