@@ -1,0 +1,353 @@
+#!/usr/bin/env python
+"""bench.py — throughput of the DBIE hot path on B200 (one process per GPU).
+
+    python bench.py [--gpus N] [--steps K] [--warmup W] [--impl ours|reference] [--workload cfg2|cfg3|cfg4]
+
+A "step" is one pass of the whole hot path over one batch of synthetic input:
+stage the boundary (dbie_create) and run the full per-point lambda solve (dbie_solve) on the
+volume of BASELINE.json configs[1] (Low & Lou n=1, m=1, l=0.3, Phi=pi/4; 64x64 boundary,
+64x64x32 = 131,072 points).  The metric is BASELINE.json's: point-pixel DBIE interactions/s in
+fp64 (one interaction = one (evaluation point, pixel) pair, all three components; each stencil
+offset and each objective evaluation counts).  `value` is measured with the inputs resident in
+HBM; `e2e` goes through the host-pointer C-ABI calls (dbie_create_host + dbie_solve_host) with
+the copies inside the timed region.  `roofline` is for the dominant kernel (the interaction
+kernel), timed live with CUDA-event pairs around each of its launches.  `cpu_baseline` times the
+oracle, as it stands, on the host cores over a bounded sample.  One JSON line on stdout (rank 0).
+"""
+from __future__ import annotations
+
+import argparse
+import json
+import os
+import subprocess
+import sys
+import tempfile
+import time
+
+import numpy as np
+
+ROOT = os.path.dirname(os.path.abspath(__file__))
+sys.path.insert(0, ROOT)
+
+METRIC = "point-pixel DBIE interactions/sec (fp64)"
+UNIT = "interactions/s"
+FP64_INSTR_PER_INTERACTION = 76      # DESIGN.md section 6 (SASS inner loop: 302 per 4 stencil points)
+FP64_INSTR_SURVEY = 82               # SURVEY.md 8(d) canonical count
+SM_COUNT, FP64_LANES_PER_SM = 148, 64   # B200: 148 SMs, 64 FP64 lanes per SM per clock
+
+
+def make_workload(name: str, rank: int = 0, world: int = 1):
+    """The rank's batch.  Weak scaling: every rank solves a volume of the same size; rank r's
+    layers are shifted by r*h/world in z so the ranks' point sets are disjoint."""
+    import workloads
+    wl = {"cfg2": workloads.config2, "cfg3": workloads.config3, "cfg4": workloads.config4}[name]()
+    if world > 1:
+        wl.z = wl.z + rank * wl.h / world
+    return wl
+
+
+def shard_info(M: int, rank: int, world: int) -> dict:
+    """Points are independent: no data-path collective, results stay on the rank."""
+    return {"rank": rank, "world": world, "points_per_rank": M, "points_total": M * world}
+
+
+def reduce_over_ranks(dist, device, ms: float, interactions: float):
+    """max over ranks of the time, sum over ranks of the work (the contract's aggregate)."""
+    import torch
+    if dist is None or not dist.is_initialized() or dist.get_world_size() == 1:
+        return ms, interactions
+    t = torch.tensor([ms], dtype=torch.float64, device=device)
+    w = torch.tensor([interactions], dtype=torch.float64, device=device)
+    dist.all_reduce(t, op=dist.ReduceOp.MAX)
+    dist.all_reduce(w, op=dist.ReduceOp.SUM)
+    return float(t.item()), float(w.item())
+
+
+class ClockSampler:
+    """nvidia-smi clocks line of B200_PROFILING.md, sampled during the timed region."""
+    Q = ("index,clocks.sm,clocks.max.sm,power.draw,clocks_event_reasons.active,"
+         "clocks_event_reasons.hw_slowdown,clocks_event_reasons.hw_thermal_slowdown,"
+         "clocks_event_reasons.sw_thermal_slowdown,clocks_event_reasons.sw_power_cap")
+
+    def __init__(self, gpu_index: int):
+        self.f = tempfile.NamedTemporaryFile("w+", suffix=".csv", delete=False)
+        self.p = None
+        try:
+            self.p = subprocess.Popen(["nvidia-smi", f"--id={gpu_index}", f"--query-gpu={self.Q}",
+                                       "--format=csv,noheader,nounits", "-lms", "200"],
+                                      stdout=self.f, stderr=subprocess.DEVNULL)
+        except Exception:
+            self.p = None
+
+    def stop(self) -> dict:
+        if self.p is None:
+            return {"sm_mhz": None, "sm_max_mhz": None, "reasons": ["nvidia-smi unavailable"]}
+        time.sleep(0.25)
+        self.p.terminate()
+        try:
+            self.p.wait(timeout=5)
+        except Exception:
+            self.p.kill()
+        self.f.flush()
+        rows = [r.strip().split(", ") for r in open(self.f.name) if r.strip()]
+        os.unlink(self.f.name)
+        sm, mx, pw, reasons = [], [], [], set()
+        names = ["hw_slowdown", "hw_thermal_slowdown", "sw_thermal_slowdown", "sw_power_cap"]
+        for r in rows:
+            try:
+                sm.append(float(r[1])); mx.append(float(r[2])); pw.append(float(r[3]))
+                for n, v in zip(names, r[5:9]):
+                    if v.strip().lower() == "active":
+                        reasons.add(n)
+            except Exception:
+                pass
+        if not sm:
+            return {"sm_mhz": None, "sm_max_mhz": None, "reasons": ["no samples"]}
+        hi = [s for s, p in zip(sm, pw) if p >= 0.6 * max(pw)] or sm     # samples under load
+        return {"sm_mhz": float(np.median(hi)), "sm_max_mhz": float(max(mx)), "power_w_max": float(max(pw)),
+                "samples": len(sm), "reasons": sorted(reasons)}
+
+
+# --------------------------------------------------------------------------- oracle legs ---
+def oracle_timed(wl, npoints: int, seed_offset: int, nthreads: int = 0) -> dict:
+    """Time the oracle's solve (or eval) on a seeded sample of the workload's points."""
+    import oracle
+    sub, _ = wl.seeded_subset(npoints, seed_offset=seed_offset)
+    t0 = time.perf_counter()
+    if wl.lam is None:
+        out = oracle.solve_nm(sub, nthreads=nthreads)
+        inter = float(out["nfev"].sum()) * 4.0 * wl.N
+    else:
+        oracle.eval(sub, nthreads=nthreads)
+        inter = float(sub.M) * wl.N
+    dt = time.perf_counter() - t0
+    return {"seconds": dt, "interactions": inter, "points": sub.M}
+
+
+def cpu_baseline(wl, target_s: float = 15.0) -> dict:
+    """Oracle as it stands on the host cores: a probe sample sizes a ~target_s sample."""
+    import oracle
+    cores = oracle.max_threads()
+    probe = oracle_timed(wl, min(wl.M, 8 * cores), seed_offset=50)
+    per_point = probe["seconds"] / max(probe["points"], 1)
+    n = int(min(wl.M, max(8 * cores, target_s / max(per_point, 1e-9))))
+    n = min(n, 65536)
+    r = oracle_timed(wl, n, seed_offset=51)
+    kind = "solve_nm" if wl.lam is None else "eval"
+    return {"value": r["interactions"] / r["seconds"], "unit": UNIT, "cores": cores, "kind": "oracle",
+            "sample": f"oracle.{kind} on {r['points']} seeded points of {wl.name} "
+                      f"({r['interactions']:.3e} interactions in {r['seconds']:.1f} s)"}
+
+
+def run_reference(args) -> None:
+    """--impl reference: the oracle timed on the host cores, same metric / config / unit."""
+    rank = int(os.environ.get("RANK", "0"))
+    if rank != 0:
+        return
+    import oracle
+    wl = make_workload(args.workload)
+    cores = oracle.max_threads()
+    probe = oracle_timed(wl, min(wl.M, 4 * cores), seed_offset=60)
+    per_point = probe["seconds"] / probe["points"]
+    budget = 150.0 / max(args.steps + args.warmup, 1)            # whole run within a few minutes
+    n = int(min(wl.M, max(cores, min(budget, 20.0) / per_point)))
+    for w in range(args.warmup):
+        oracle_timed(wl, n, seed_offset=100 + w)
+    tot_s = tot_i = 0.0
+    for k in range(args.steps):
+        r = oracle_timed(wl, n, seed_offset=200 + k)
+        tot_s += r["seconds"]; tot_i += r["interactions"]
+    value = tot_i / tot_s
+    line = {
+        "impl": "reference", "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": args.gpus,
+        "steps": args.steps, "warmup": args.warmup, "ms_per_step": 1e3 * tot_s / args.steps,
+        "higher_is_better": True, "scaling": "weak", "vs_baseline": None, "dtype": "f64",
+        "data": "synthetic", "gpu_launches": 0,
+        "config": workload_config(wl, args.workload, n_points_per_step=n),
+        "cpu_baseline": {"value": value, "unit": UNIT, "cores": cores, "kind": "oracle",
+                         "sample": f"each step: oracle on {n} seeded points of {wl.name}"},
+        "e2e": {"value": value, "unit": UNIT, "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0},
+    }
+    print(json.dumps(line), flush=True)
+
+
+def workload_config(wl, name, n_points_per_step=None) -> dict:
+    desc = {"cfg2": "BASELINE configs[1]: Low&Lou n=1 m=1 l=0.3 Phi=pi/4, boundary 64x64 on [-1,1]^2, "
+                    "full per-point NM lambda solve on the 64x64x32 volume",
+            "cfg3": "BASELINE configs[2]: synthetic bipolar AR 256x256 at 0.5 Mm/px, NM solve on 128x128x64",
+            "cfg4": "BASELINE configs[3]: eval at fixed lambda, boundary 512x512, M=1,048,576 random points"}[name]
+    return {"workload": desc, "boundary": [wl.nx, wl.ny], "points": wl.M if n_points_per_step is None
+            else n_points_per_step, "step": "dbie_create + dbie_solve" if wl.lam is None else "dbie_create + dbie_eval",
+            "l2": "flushed between timed steps (256 MiB write)"}
+
+
+# --------------------------------------------------------------------------- our arm -------
+def run_ours(args) -> None:
+    import torch
+    import paper_1306_1122_b200 as dbie
+    rank = int(os.environ.get("RANK", "0"))
+    world = int(os.environ.get("WORLD_SIZE", "1"))
+    local = int(os.environ.get("LOCAL_RANK", "0"))
+    dist = None
+    if world > 1:
+        import torch.distributed as dist
+        os.environ.setdefault("MASTER_ADDR", "127.0.0.1")
+        dist.init_process_group("nccl", device_id=torch.device("cuda", local))
+    if not torch.cuda.is_available():
+        raise SystemExit("bench.py: no CUDA device (the CUDA path has no CPU fallback)")
+    torch.cuda.set_device(local)
+    dev = torch.device("cuda", local)
+    dbie.load()
+
+    wl = make_workload(args.workload, rank, world)
+    is_solve = wl.lam is None
+    t = lambda a: torch.from_numpy(np.ascontiguousarray(a, dtype=np.float64)).to(dev)
+    d_bx, d_by, d_bz = t(wl.bx), t(wl.by), t(wl.bz)
+    d_x, d_y, d_z = t(wl.x), t(wl.y), t(wl.z)
+    d_lam = None if is_solve else t(wl.lam)
+    flush_buf = torch.empty(256 << 20, dtype=torch.uint8, device=dev)
+
+    def barrier():
+        if dist is not None:
+            dist.barrier()
+        torch.cuda.synchronize()
+
+    def step_device(profile=False):
+        ctx = dbie.DBIE(wl.nx, wl.ny, wl.h, wl.x0, wl.y0, d_bx, d_by, d_bz)
+        if profile:
+            ctx.profile(True)
+        out = ctx.solve(d_x, d_y, d_z) if is_solve else ctx.eval(d_x, d_y, d_z, d_lam)
+        return ctx, out
+
+    def step_host():
+        ctx = dbie.DBIE(wl.nx, wl.ny, wl.h, wl.x0, wl.y0, wl.bx, wl.by, wl.bz)
+        out = ctx.solve_host(wl.x, wl.y, wl.z) if is_solve else ctx.eval_host(wl.x, wl.y, wl.z, wl.lam)
+        return ctx, out
+
+    # ---- warm-up
+    for _ in range(max(args.warmup, 0)):
+        ctx, _ = step_device()
+        torch.cuda.synchronize()
+        ctx.close()
+
+    # ---- timed: K steps, device-resident inputs, CUDA events on the launching stream
+    sampler = ClockSampler(local) if rank == 0 else None
+    barrier()
+    ms_total = 0.0
+    inter_total = 0.0
+    launches = 0
+    kern_ms = 0.0
+    kern_launches = 0
+    evals = 0
+    for k in range(args.steps):
+        flush_buf.zero_()                       # L2 flush, outside the event pair
+        e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+        e0.record()
+        ctx, out = step_device(profile=True)
+        e1.record()
+        e1.synchronize()
+        ms_total += e0.elapsed_time(e1)
+        c = ctx.counters()
+        kt = ctx.kernel_time()
+        inter_total += c["interactions"]
+        launches += c["launches"] + 1           # + the boundary staging kernel
+        evals += c["objective_evals"]
+        kern_ms += kt["interact_ms"]
+        kern_launches += kt["interact_launches"]
+        ctx.close()
+    barrier()
+    clocks = sampler.stop() if sampler else None
+    ms_max, inter_sum = reduce_over_ranks(dist, dev, ms_total, inter_total)
+    value = inter_sum / (ms_max * 1e-3)
+
+    # ---- e2e: host buffers through the _host C-ABI calls, copies inside the timed region
+    for _ in range(1):
+        ctx, _ = step_host(); ctx.close()
+    barrier()
+    t0 = time.perf_counter()
+    e2e_inter = 0.0
+    for k in range(args.steps):
+        ctx, out = step_host()
+        e2e_inter += ctx.counters()["interactions"]
+        ctx.close()
+    torch.cuda.synchronize()
+    e2e_ms = (time.perf_counter() - t0) * 1e3
+    barrier()
+    e2e_ms, e2e_inter = reduce_over_ranks(dist, dev, e2e_ms, e2e_inter)
+    h2d = 3 * wl.N * 8 + 3 * wl.M * 8 + (0 if is_solve else 3 * wl.M * 8)
+    d2h = (3 + 3 + 2) * wl.M * 8 + 2 * wl.M * 4 if is_solve else 3 * wl.M * 8
+
+    if rank != 0:
+        if dist is not None:
+            dist.destroy_process_group()
+        return
+
+    # ---- roofline of the dominant kernel (interaction kernel), FP64-pipe bound
+    try:
+        dfma_meas, ffma_meas = dbie.probe_dfma_rate(300.0)
+    except Exception:
+        dfma_meas = ffma_meas = None
+    sm_max = (clocks or {}).get("sm_max_mhz") or 1965.0
+    peak_slots = SM_COUNT * FP64_LANES_PER_SM * sm_max * 1e6          # FP64 lane-instructions / s
+    kern_ips = inter_total / (kern_ms * 1e-3) if kern_ms > 0 else 0.0
+    achieved_slots = kern_ips * FP64_INSTR_PER_INTERACTION
+    roofline = {
+        "bound": "alu", "kernel": "dbie::interact_kernel (fp64 point-pixel sums)",
+        "achieved": 2e-12 * achieved_slots, "peak": 2e-12 * peak_slots, "unit": "TFLOP/s",
+        "frac": achieved_slots / peak_slots, "traffic": None,
+        "note": "FP64-pipe bound (no HBM/tensor step): achieved = interactions/s of the kernel x 76 FP64 "
+                "lane-instructions per interaction (DESIGN.md s6) x 2 flop per FMA slot; peak = 148 SM x 64 "
+                "FP64 lanes x clocks.max.sm (derived, DESIGN.md s7)",
+        "kernel_interactions_per_s": kern_ips, "kernel_ms_per_launch": kern_ms / max(kern_launches, 1),
+        "kernel_launches": kern_launches, "kernel_share_of_step": kern_ms / ms_total if ms_total else None,
+        "fp64_instr_per_interaction": FP64_INSTR_PER_INTERACTION,
+        "frac_survey82": kern_ips * FP64_INSTR_SURVEY / peak_slots,
+        "peak_measured_dfma_per_s": dfma_meas, "peak_measured_ffma_per_s": ffma_meas,
+        "frac_of_measured_dfma": (achieved_slots / dfma_meas) if dfma_meas else None,
+    }
+    base = cpu_baseline(make_workload(args.workload), target_s=args.cpu_seconds) if args.cpu_seconds > 0 else None
+
+    line = {
+        "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": args.steps,
+        "warmup": args.warmup, "ms_per_step": ms_max / args.steps, "higher_is_better": True,
+        "scaling": "weak", "vs_baseline": None, "dtype": "f64", "data": "synthetic",
+        "config": dict(workload_config(wl, args.workload), **shard_info(wl.M, rank, world),
+                       objective_evals_per_step=evals / args.steps),
+        "clocks": clocks,
+        "e2e": {"value": e2e_inter / (e2e_ms * 1e-3), "unit": UNIT, "h2d_bytes_per_step": h2d,
+                "d2h_bytes_per_step": d2h, "ms_per_step": e2e_ms / args.steps,
+                "api": "dbie_create_host + dbie_solve_host" if is_solve else "dbie_create_host + dbie_eval_host"},
+        "gpu_launches": launches,
+        "roofline": roofline,
+        "cpu_baseline": base,
+    }
+    if base:
+        line["gpu_over_cpu_baseline"] = value / base["value"]
+    print(json.dumps(line), flush=True)
+    if dist is not None:
+        dist.destroy_process_group()
+
+
+def main():
+    ap = argparse.ArgumentParser()
+    ap.add_argument("--gpus", type=int, default=1)
+    ap.add_argument("--steps", type=int, default=3)
+    ap.add_argument("--warmup", type=int, default=3)
+    ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
+    ap.add_argument("--workload", default="cfg2", choices=["cfg2", "cfg3", "cfg4"])
+    ap.add_argument("--cpu-seconds", type=float, default=15.0,
+                    help="target CPU time of the cpu_baseline leg (0 disables it)")
+    args = ap.parse_args()
+    if args.impl == "reference":
+        run_reference(args)
+    else:
+        if args.gpus > 1 and int(os.environ.get("WORLD_SIZE", "1")) == 1:
+            # convenience: re-launch under torchrun, one rank per GPU
+            cmd = [sys.executable, "-m", "torch.distributed.run", "--nnodes=1", f"--nproc-per-node={args.gpus}",
+                   "--master-addr", "127.0.0.1", "--master-port", "29541", os.path.abspath(__file__)] + sys.argv[1:]
+            raise SystemExit(subprocess.call(cmd))
+        run_ours(args)
+
+
+if __name__ == "__main__":
+    main()

@@ -134,6 +134,13 @@ dbie_status dbie_residual(dbie_ctx* ctx, long long M, const double* x, const dou
 dbie_status dbie_last_counters(dbie_ctx* ctx, double* interactions, long long* launches,
                                long long* objective_evals);
 
+/* Profile mode: when enabled, every later eval/residual/solve call on this context records a
+ * CUDA-event pair around each launch of the interaction kernel (on the caller's stream).
+ * dbie_last_kernel_time waits for the last call's events and returns the summed device time of
+ * its interaction-kernel launches and their number. */
+dbie_status dbie_profile(dbie_ctx* ctx, int enable);
+dbie_status dbie_last_kernel_time(dbie_ctx* ctx, double* interact_ms, long long* interact_launches);
+
 /* Measured peak of the FP64 pipe: runs a register-only DFMA loop on every SM for about
  * `millis` ms and returns DFMA instructions (per lane) per second.  Synchronises. */
 dbie_status dbie_probe_dfma_rate(double millis, double* dfma_per_s, double* ffma_per_s);

@@ -71,6 +71,8 @@ def load() -> C.CDLL:
                                   _vp]
     lib.dbie_last_counters.argtypes = [_vp, C.POINTER(C.c_double), C.POINTER(C.c_longlong),
                                        C.POINTER(C.c_longlong)]
+    lib.dbie_profile.argtypes = [_vp, C.c_int]
+    lib.dbie_last_kernel_time.argtypes = [_vp, C.POINTER(C.c_double), C.POINTER(C.c_longlong)]
     lib.dbie_probe_dfma_rate.argtypes = [C.c_double, C.POINTER(C.c_double), C.POINTER(C.c_double)]
     lib.dbie_strerror.argtypes = [C.c_int]
     lib.dbie_strerror.restype = C.c_char_p
@@ -245,6 +247,16 @@ class DBIE:
                                               _vp(lam.ctypes.data), _vp(resid.ctypes.data),
                                               _vp(iters.ctypes.data), _vp(status.ctypes.data)))
         return {"B": B, "lam": lam, "f": resid[0], "g": resid[1], "iters": iters, "status": status}
+
+    def profile(self, enable: bool = True):
+        """dbie_profile: CUDA-event pairs around every interaction-kernel launch of later calls."""
+        self._check(self._lib.dbie_profile(self._h, int(bool(enable))))
+
+    def kernel_time(self) -> dict:
+        """dbie_last_kernel_time: device ms and launch count of the last call's interaction kernels."""
+        a, b = C.c_double(), C.c_longlong()
+        self._check(self._lib.dbie_last_kernel_time(self._h, C.byref(a), C.byref(b)))
+        return {"interact_ms": a.value, "interact_launches": b.value}
 
     def counters(self) -> dict:
         """dbie_last_counters: interactions, launches, objective evaluations of the last call."""

@@ -25,6 +25,8 @@ struct dbie_ctx {
     double last_interactions;
     long long last_launches, last_evals;
     int evals_on_device;                      // last call was a solve: read nevals back on demand
+    int profile;                              // record CUDA events around every interaction launch
+    cudaEvent_t* ev;    int ev_cap, ev_n;     // event pairs of the last call (profile mode)
     char err[256];
 };
 
@@ -52,6 +54,42 @@ static dbie_status ensure(dbie_ctx* ctx, void** ptr, size_t* have, size_t need) 
     }
     CU(cudaMalloc(ptr, need));
     *have = need;
+    return DBIE_OK;
+}
+
+// profile mode: an event pair around each interaction-kernel launch of the current call
+static void prof_reset(dbie_ctx* ctx) { ctx->ev_n = 0; }
+static void prof_mark(dbie_ctx* ctx, cudaStream_t st) {
+    if (!ctx->profile) return;
+    if (ctx->ev_n == ctx->ev_cap) {
+        const int ncap = ctx->ev_cap ? 2 * ctx->ev_cap : 256;
+        cudaEvent_t* n = (cudaEvent_t*)realloc(ctx->ev, sizeof(cudaEvent_t) * ncap);
+        if (!n) return;
+        for (int i = ctx->ev_cap; i < ncap; ++i) cudaEventCreate(&n[i]);
+        ctx->ev = n;
+        ctx->ev_cap = ncap;
+    }
+    cudaEventRecord(ctx->ev[ctx->ev_n++], st);
+}
+
+extern "C" dbie_status dbie_profile(dbie_ctx* ctx, int enable) {
+    if (!ctx) return DBIE_EINVAL;
+    ctx->profile = enable != 0;
+    return DBIE_OK;
+}
+
+extern "C" dbie_status dbie_last_kernel_time(dbie_ctx* ctx, double* interact_ms, long long* interact_launches) {
+    if (!ctx) return DBIE_EINVAL;
+    double total = 0.0;
+    const int pairs = ctx->ev_n / 2;
+    if (pairs > 0) CU(cudaEventSynchronize(ctx->ev[2 * pairs - 1]));
+    for (int i = 0; i < pairs; ++i) {
+        float ms = 0.f;
+        CU(cudaEventElapsedTime(&ms, ctx->ev[2 * i], ctx->ev[2 * i + 1]));
+        total += ms;
+    }
+    if (interact_ms) *interact_ms = total;
+    if (interact_launches) *interact_launches = pairs;
     return DBIE_OK;
 }
 
@@ -116,6 +154,8 @@ extern "C" void dbie_destroy(dbie_ctx* ctx) {
     cudaFree(ctx->io);
     cudaFree(ctx->counters);
     if (ctx->own_stream) cudaStreamDestroy(ctx->own_stream);
+    for (int i = 0; i < ctx->ev_cap; ++i) cudaEventDestroy(ctx->ev[i]);
+    free(ctx->ev);
     (void)cudaGetLastError();
     free(ctx);
 }
@@ -198,6 +238,7 @@ extern "C" dbie_status dbie_eval(dbie_ctx* ctx, long long M, const double* x, co
                                  (size_t)ctx->bd.nchunks * 3 * cap * sizeof(double));
     if (s != DBIE_OK) return s;
     long long launches = 0;
+    prof_reset(ctx);
     for (long long off = 0; off < M; off += cap) {
         const long long cnt = (M - off < cap) ? (M - off) : cap;
         InteractParams p;
@@ -206,7 +247,9 @@ extern "C" dbie_status dbie_eval(dbie_ctx* ctx, long long M, const double* x, co
         p.x = x; p.y = y; p.z = z; p.lam = lam; p.ldlam = M;
         p.count = cnt; p.slot0 = off;
         p.part = ctx->part; p.cap = cap;
+        prof_mark(ctx, st);
         CU(launch_interact_eval(p, ctx->sm_count, st));
+        prof_mark(ctx, st);
         CU(launch_eval_finalize(ctx->bd, off, cnt, M, z, lam, ctx->part, cap, B, st));
         launches += 2;
     }
@@ -225,6 +268,7 @@ extern "C" dbie_status dbie_eval_host(dbie_ctx* ctx, long long M, const double* 
     if (M == 0) return DBIE_OK;
     if (!x || !y || !z || !lam || !B) return DBIE_EINVAL;
     const size_t m = (size_t)M * sizeof(double);
+    CU(cudaDeviceSynchronize());   // earlier work on this context may be in flight on another stream
     dbie_status s = io_reserve(ctx, 9 * m);
     if (s != DBIE_OK) return s;
     double* d = (double*)ctx->io;   // x, y, z, lam[3], B[3]
@@ -286,6 +330,7 @@ extern "C" dbie_status dbie_residual(dbie_ctx* ctx, long long M, const double* x
     s = ensure(ctx, (void**)&ctx->part, &ctx->part_bytes, (size_t)ctx->bd.nchunks * 12 * cap * sizeof(double));
     if (s != DBIE_OK) return s;
     long long launches = 0;
+    prof_reset(ctx);
     for (long long off = 0; off < M; off += cap) {
         const long long cnt = (M - off < cap) ? (M - off) : cap;
         InteractParams p;
@@ -296,7 +341,9 @@ extern "C" dbie_status dbie_residual(dbie_ctx* ctx, long long M, const double* x
         p.count = cnt;
         p.delta_abs = k.delta_abs;
         p.part = ctx->part; p.cap = cap;
+        prof_mark(ctx, st);
         CU(launch_interact_stencil(p, ctx->sm_count, st));
+        prof_mark(ctx, st);
         CU(launch_residual_finalize(ctx->bd, k, cnt, M, z + off, ctx->part, cap, out + off, phi ? phi + off : nullptr, st));
         launches += 2;
     }
@@ -349,6 +396,7 @@ extern "C" dbie_status dbie_solve(dbie_ctx* ctx, long long M, const double* x, c
     CU(cudaMemsetAsync(ctx->counters, 0, 64, st));
     const int maxpass = 4 + 5 * k.maxiter + 1;
     long long launches = 0;
+    prof_reset(ctx);
     for (long long off = 0; off < M; off += cap) {
         const long long cnt = (M - off < cap) ? (M - off) : cap;
         CU(cudaMemsetAsync(ctx->counters, 0, 8, st));
@@ -366,7 +414,9 @@ extern "C" dbie_status dbie_solve(dbie_ctx* ctx, long long M, const double* x, c
             p.zero_ptr = &a.nact[(pass + 1) & 1];
             p.delta_abs = k.delta_abs;
             p.part = ctx->part; p.cap = cap;
+            prof_mark(ctx, st);
             CU(launch_interact_stencil(p, ctx->sm_count, st));
+            prof_mark(ctx, st);
             CU(launch_solve_step(a, k, ctx->bd, pass, cnt, M, z + off, ctx->part, cap, B + off, lam + off,
                                  resid + off, iters + off, status + off, nevals, st));
             launches += 2;
@@ -384,6 +434,7 @@ extern "C" dbie_status dbie_solve_host(dbie_ctx* ctx, long long M, const double*
     if (M == 0) return DBIE_OK;
     if (!x || !y || !z || !B || !lam || !resid || !iters || !status) return DBIE_EINVAL;
     const size_t m = (size_t)M * sizeof(double);
+    CU(cudaDeviceSynchronize());   // earlier work on this context may be in flight on another stream
     dbie_status s = io_reserve(ctx, 11 * m + 2 * align256((size_t)M * sizeof(int)) + 512);
     if (s != DBIE_OK) return s;
     double* d = (double*)ctx->io;   // x, y, z, B[3], lam[3], resid[2], iters, status

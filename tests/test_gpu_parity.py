@@ -1,0 +1,259 @@
+"""GPU parity: the CUDA path (through the C ABI, libdbie_b200.so) against the CPU oracle on the
+same seeded inputs.  Tolerances (BASELINE.json north_star; derivation in DESIGN.md section 8):
+  B      : max_i ||dB_i|| / ||B_i||  <= 1e-9 over points with ||B_i|| >= 1e-6 max ||B||
+  lambda : | |lam|_gpu - |lam|_orc | * h <= 1e-6 on decision-stable points (protocol P-4)
+  f, g   : 1e-6 absolute;  status, iteration count: identical (integers)
+"""
+import numpy as np
+import pytest
+
+import oracle
+import workloads
+
+pytestmark = pytest.mark.gpu
+
+TOL_B = 1e-9
+TOL_LAM = 1e-6
+TOL_FG = 1e-6
+MARGIN_STABLE = 1e-7
+
+
+@pytest.fixture(scope="module")
+def dbie():
+    import torch
+    assert torch.cuda.is_available()
+    import paper_1306_1122_b200 as d
+    d.load()     # raises if the CUDA library is missing: no fallback
+    return d
+
+
+def vec_relerr(B, R, floor=1e-6):
+    n = np.linalg.norm(R, axis=0)
+    keep = n >= floor * n.max()
+    e = np.linalg.norm(B - R, axis=0)
+    return float((e[keep] / n[keep]).max()), int((~keep).sum())
+
+
+def gpu_eval(d, wl):
+    with d.DBIE.from_workload(wl) as ctx:
+        dw = d.to_device(wl)
+        return ctx.eval(dw.x, dw.y, dw.z, dw.lam).cpu().numpy()
+
+
+# ---------------------------------------------------------------------------- eval ---------
+def test_config1_dipole_eval_matches_oracle_and_closed_form(dbie):
+    """BASELINE configs[0]: lambda = 0, 16x16 window, 8x8x8 points; GPU == oracle to 1e-9 and the
+    truncation-error profile vs the closed-form dipole is the one pinned in tests/golden."""
+    w = workloads.config1()
+    B = gpu_eval(dbie, w)
+    R = oracle.eval(w)
+    err, dropped = vec_relerr(B, R)
+    assert err <= TOL_B and dropped == 0
+    ex = np.array(workloads.dipole_field(w.x, w.y, w.z))
+    rel = np.linalg.norm(B - ex, axis=0) / np.linalg.norm(ex, axis=0)
+    prof = [rel[np.isclose(w.z, zz)].max() for zz in range(1, 9)]
+    gold = np.loadtxt("tests/golden/k6_dipole_profile.txt")[:, 1]
+    assert np.all(np.abs(np.array(prof) - gold) <= 0.1 * gold)
+
+
+@pytest.mark.parametrize("nx,ny", [(1, 1), (1, 7), (7, 1), (17, 33), (513, 3), (3, 513), (1030, 2),
+                                   (64, 64), (600, 5), (512, 4), (1024, 3), (2049, 1)])
+def test_eval_ragged_boundaries(dbie, nx, ny):
+    """Tile edges: one pixel, single rows/columns, widths just above the 512-pixel tile, odd tails;
+    37 points (not a multiple of anything), h != 1, shifted origin, lambda of both signs."""
+    w = workloads.random_boundary(nx, ny, seed=nx * 7 + ny, npts=37, h=0.5, x0=-1.0, y0=2.0)
+    w.lam[:, 0] = 0.0
+    w.lam[1, 1] = -w.lam[1, 1]
+    err, _ = vec_relerr(gpu_eval(dbie, w), oracle.eval(w))
+    assert err <= TOL_B
+
+
+def test_eval_config4_first_points_fp64(dbie):
+    """BASELINE configs[3] at full boundary size (512x512), first 1536 points: spans 3 work blocks
+    with a ragged tail of the register-blocked mapping."""
+    w = workloads.config4()
+    sub = w.subset(np.arange(1536))
+    err, dropped = vec_relerr(gpu_eval(dbie, sub), oracle.eval(sub))
+    assert err <= TOL_B, err
+    assert dropped == 0
+
+
+def test_eval_config4_full_size_sampled(dbie):
+    """Full M = 1,048,576 in the launch configuration bench.py times; 192 sampled outputs are
+    recomputed one by one by the oracle; plus properties that hold at any size."""
+    import torch
+    w = workloads.config4()
+    with dbie.DBIE.from_workload(w) as ctx:
+        dw = dbie.to_device(w)
+        B = ctx.eval(dw.x, dw.y, dw.z, dw.lam)
+        B2 = ctx.eval(dw.x, dw.y, dw.z, dw.lam)
+        assert torch.equal(B, B2)                      # run-to-run bitwise reproducible
+        Bneg = ctx.eval(dw.x, dw.y, dw.z, -dw.lam)
+        assert torch.equal(B, Bneg)                    # even in lambda (reading A-3), bit for bit
+        assert bool(torch.isfinite(B).all())
+        c = ctx.counters()
+        assert c["interactions"] == float(w.M) * w.N
+        # a result does not depend on the batch it was computed in (canonical chunk sums)
+        idx = torch.arange(5000, 5000 + 777, device="cuda")
+        Bs = ctx.eval(dw.x[idx].contiguous(), dw.y[idx].contiguous(), dw.z[idx].contiguous(),
+                      dw.lam[:, idx].contiguous())
+        assert torch.equal(Bs, B[:, idx])
+        B = B.cpu().numpy()
+    sub, idx = w.seeded_subset(192)
+    err, _ = vec_relerr(B[:, idx], oracle.eval(sub))
+    assert err <= TOL_B, err
+
+
+def test_eval_edge_cases(dbie):
+    import torch
+    w = workloads.random_boundary(20, 12, seed=3, npts=9)
+    with dbie.DBIE.from_workload(w) as ctx:
+        dw = dbie.to_device(w)
+        # M = 0 is a no-op
+        e = torch.empty(0, dtype=torch.float64, device="cuda")
+        out = ctx.eval(e, e, e, torch.empty((3, 0), dtype=torch.float64, device="cuda"))
+        assert out.shape == (3, 0)
+        # invalid points give NaN without failing the call; the others are untouched
+        z = dw.z.clone(); z[2] = 0.0; z[5] = -1.0
+        lam = dw.lam.clone(); lam[1, 7] = float("nan")
+        B = ctx.eval(dw.x, dw.y, z, lam).cpu().numpy()
+        good = ctx.eval(dw.x, dw.y, dw.z, dw.lam).cpu().numpy()
+        bad = [2, 5, 7]
+        assert np.isnan(B[:, bad]).all()
+        ok = [i for i in range(9) if i not in bad]
+        assert np.array_equal(B[:, ok], good[:, ok])
+        # the host-pointer entry point gives the same bits as the device-pointer one
+        Bh = ctx.eval_host(w.x, w.y, w.z, w.lam)
+        assert np.array_equal(Bh, good)
+        # wrong dtype / device are rejected by the binding
+        with pytest.raises(TypeError):
+            ctx.eval(dw.x.float(), dw.y, dw.z, dw.lam)
+    # the oracle treats the same points as invalid
+    wb = w.subset(np.arange(9)); wb.z[2] = 0.0
+    assert np.isnan(oracle.eval(wb)[:, 2]).all()
+
+
+def test_eval_linearity_and_shift_invariance(dbie):
+    """K-8 symmetries on the GPU path: linear in B0; shifting x0, y0 and the points together."""
+    w = workloads.random_boundary(40, 24, seed=11, npts=21)
+    B1 = gpu_eval(dbie, w)
+    w2 = workloads.random_boundary(40, 24, seed=11, npts=21)
+    w2.bx, w2.by, w2.bz = 3.0 * w.bx, -2.0 * w.by, 0.5 * w.bz
+    B2 = gpu_eval(dbie, w2)
+    assert np.allclose(B2, np.array([3.0, -2.0, 0.5])[:, None] * B1, rtol=1e-13, atol=0)
+    w3 = workloads.random_boundary(40, 24, seed=11, npts=21, x0=128.0, y0=-64.0)
+    w3.bx, w3.by, w3.bz = w.bx, w.by, w.bz
+    w3.x, w3.y, w3.z, w3.lam = w.x + 128.0, w.y - 64.0, w.z, w.lam
+    assert np.allclose(gpu_eval(dbie, w3), B1, rtol=1e-11, atol=0)
+
+
+# ---------------------------------------------------------------------------- residual -----
+@pytest.mark.parametrize("case", ["random", "config3"])
+def test_residual_matches_oracle(dbie, case):
+    """A5: Eq. 8, 9, 13, 14 at given lambda triples (one objective evaluation per point)."""
+    if case == "random":
+        w = workloads.random_boundary(48, 40, seed=5, npts=133, h=0.25)
+        lam = w.lam
+    else:
+        w, _ = workloads.config3().seeded_subset(96)
+        lam = np.random.default_rng(9).uniform(0.0, 0.3, (3, w.M)) / w.h
+    ro = oracle.residual(w, lam)
+    with dbie.DBIE.from_workload(w) as ctx:
+        import torch
+        dw = dbie.to_device(w)
+        r = ctx.residual(dw.x, dw.y, dw.z, torch.from_numpy(lam).cuda())
+        r = {k: v.cpu().numpy() for k, v in r.items()}
+    err, _ = vec_relerr(r["B"], ro["B"])
+    assert err <= TOL_B
+    nB = np.linalg.norm(ro["B"], axis=0)
+    # J and div are differences of sums over delta = 1e-3 h: rounding noise 1e-13 |B| / delta
+    assert np.all(np.abs(r["J"] - ro["J"]) <= 1e-8 * nB / w.h + 1e-300)
+    assert np.all(np.abs(r["div"] - ro["div"]) <= 1e-8 * nB / w.h + 1e-300)
+    assert np.abs(r["f"] - ro["f"]).max() <= TOL_FG
+    assert np.abs(r["g"] - ro["g"]).max() <= TOL_FG
+    assert np.abs(r["phi"] - ro["phi"]).max() <= 2 * TOL_FG
+
+
+# ---------------------------------------------------------------------------- solve --------
+def _check_solve_parity(dbie, wl, opts_kw=None):
+    """Protocol P-4."""
+    opts_kw = opts_kw or {}
+    oo = oracle.Opts(**opts_kw)
+    so = oracle.solve_nm(wl, oo)
+    with dbie.DBIE.from_workload(wl) as ctx:
+        dw = dbie.to_device(wl)
+        s = ctx.solve(dw.x, dw.y, dw.z, dbie.default_opts(**opts_kw))
+        s = {k: v.cpu().numpy() for k, v in s.items()}
+        cnt = ctx.counters()
+    valid = so["status"] != 3
+    assert np.array_equal(s["status"] == 3, ~valid)
+    stable = valid & (so["margin"] >= MARGIN_STABLE)
+    # (2) decision-stable points: same path
+    assert np.array_equal(s["status"][stable], so["status"][stable])
+    assert np.array_equal(s["iters"][stable], so["iters"][stable])
+    assert (np.abs(s["lam"] - so["lam"])[:, stable] * wl.h).max() <= TOL_LAM
+    err, _ = vec_relerr(s["B"][:, stable], so["B"][:, stable])
+    assert err <= TOL_B
+    assert np.abs(s["f"] - so["f"])[stable].max() <= TOL_FG
+    assert np.abs(s["g"] - so["g"])[stable].max() <= TOL_FG
+    # (3) the rest (a comparison within finite-difference noise of a tie: paths may fork):
+    # the oracle's own objective at the GPU's lambda must be as good, and B must match there
+    rest = valid & ~stable
+    forked = rest & ((s["iters"] != so["iters"]) | (s["status"] != so["status"]))
+    if rest.any():
+        sub = wl.subset(np.where(rest)[0])
+        ro = oracle.residual(sub, s["lam"][:, rest], oo)
+        assert np.all(ro["phi"] <= so["phi"][rest] + 1e-6)
+        err, _ = vec_relerr(s["B"][:, rest], ro["B"])
+        assert err <= TOL_B
+    assert forked.sum() <= max(1, int(0.02 * valid.sum())), f"{forked.sum()} forked of {valid.sum()}"
+    # invariants S-2 on the GPU result
+    assert np.all(s["lam"][:, valid] >= 0.0)
+    st0 = s["status"] == 0
+    assert np.all(s["f"][st0] <= oo.eps_f) and np.all(s["g"][st0] <= oo.eps_g)
+    assert cnt["objective_evals"] == so["nfev"][valid].sum() or forked.any()
+    return s, so, dict(stable=int(stable.sum()), rest=int(rest.sum()), forked=int(forked.sum()))
+
+
+def test_solve_config2_lowlou_subset(dbie):
+    """BASELINE configs[1] (Low & Lou n=1, m=1, l=0.3, Phi=pi/4, 64x64 boundary): full NM solve
+    on a seeded 160-point subset of the 64x64x32 volume."""
+    w, _ = workloads.config2().seeded_subset(160)
+    s, so, info = _check_solve_parity(dbie, w)
+    # S-3: DBIE's force-free residual is far below the potential field's (lambda = 0)
+    pot = oracle.residual(w, np.zeros((3, w.M)))
+    assert np.nanmean(s["f"]) < 0.5 * np.nanmean(pot["f"])
+
+
+def test_solve_config3_bipolar_subset(dbie):
+    """BASELINE configs[2] (256x256 at 0.5 Mm/px; h != 1 exercises the units): 40 points."""
+    w, _ = workloads.config3().seeded_subset(40)
+    _check_solve_parity(dbie, w)
+
+
+def test_solve_random_boundary_options_and_invalid_points(dbie):
+    """Small ragged boundary, non-default options (no Eq. 12 exit, other simplex, low maxiter),
+    two invalid points in the batch."""
+    w = workloads.random_boundary(33, 21, seed=21, npts=70, h=2.0, zmin=1.5, zmax=6.0)
+    w.z[4] = -1.0
+    w.x[9] = float("nan")
+    s, so, info = _check_solve_parity(dbie, w, dict(use_eq12=0, lam0=0.08, step=0.03, maxiter=37,
+                                                    xtol=1e-5, ftol=1e-8, w_g=2.0, cell=0.5))
+    assert s["status"][4] == 3 and s["status"][9] == 3
+    assert np.isnan(s["lam"][:, 4]).all() and np.isnan(s["B"][:, 9]).all()
+    assert (s["status"] == 2).any()      # the iteration cap is reached by some points
+
+
+def test_solve_is_reproducible_and_host_entry_matches(dbie):
+    w, _ = workloads.config2().seeded_subset(64, seed_offset=3)
+    with dbie.DBIE.from_workload(w) as ctx:
+        dw = dbie.to_device(w)
+        a = ctx.solve(dw.x, dw.y, dw.z)
+        b = ctx.solve(dw.x, dw.y, dw.z)
+        h = ctx.solve_host(w.x, w.y, w.z)
+        for k in ("B", "lam", "f", "g", "iters", "status"):
+            assert np.array_equal(a[k].cpu().numpy(), b[k].cpu().numpy(), equal_nan=True), k
+            assert np.array_equal(a[k].cpu().numpy(), h[k], equal_nan=True), k
+        # maxiter = 0: the best initial vertex is returned with status 2
+        z = ctx.solve(dw.x, dw.y, dw.z, dbie.default_opts(maxiter=0))
+        assert (z["status"].cpu().numpy() == 2).all() and (z["iters"].cpu().numpy() == 0).all()
