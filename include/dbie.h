@@ -81,10 +81,17 @@ dbie_status dbie_eval(dbie_ctx* ctx, long long M, const double* x, const double*
 dbie_status dbie_eval_host(dbie_ctx* ctx, long long M, const double* x, const double* y,
                            const double* z, const double* lam, double* B);
 
-/* fp32-arithmetic variant of dbie_eval (BASELINE.json config 4; needs DBIE_WITH_FP32).
- * Geometry, sincos and products in fp32; partial sums are carried in fp64. */
+/* fp32-arithmetic variant of dbie_eval (BASELINE.json config 4 "fp64 and fp32"; needs a context
+ * created with DBIE_WITH_FP32, else DBIE_ESTATE).  x, y, z: M floats each; lam: 3*M floats;
+ * B: out, 3*M floats; all DEVICE pointers.  Geometry, theta, sincos and products are fp32; the
+ * sum of a row segment (<= 512 pixels) is fp32 and row sums are carried in fp64.  Target accuracy
+ * (north_star): relative vector error <= 2e-4 against the fp64 definition. */
 dbie_status dbie_eval_f32(dbie_ctx* ctx, long long M, const float* x, const float* y,
                           const float* z, const float* lam, float* B, void* cuda_stream);
+/* Tuning knob of dbie_eval_f32: bit p of mask set = component p takes sin/cos of the reduced
+ * argument from the SFU (MUFU.SIN/COS) instead of the FMA-pipe polynomials, to balance the two
+ * pipes.  Allowed masks: 0 (default), 1, 3, 7.  Results differ at the 1e-6 level between masks. */
+dbie_status dbie_set_f32_sfu_mask(dbie_ctx* ctx, int mask);
 
 /* Options of dbie_solve.  Fill with dbie_solve_default_opts, then change fields. */
 typedef struct {

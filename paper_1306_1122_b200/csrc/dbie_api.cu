@@ -25,12 +25,14 @@ struct dbie_ctx {
     double last_interactions;
     long long last_launches, last_evals;
     int evals_on_device;                      // last call was a solve: read nevals back on demand
+    int f32_sfu_mask;                         // dbie_eval_f32: components whose sincos use the SFU
     int profile;                              // record CUDA events around every interaction launch
     cudaEvent_t* ev;    int ev_cap, ev_n;     // event pairs of the last call (profile mode)
     char err[256];
 };
 
 static char g_err[256] = "no error";
+static const int kDefaultF32SfuMask = 0;   // all three components on the FMA-pipe polynomials
 
 static dbie_status fail_cuda(dbie_ctx* c, cudaError_t e, const char* where) {
     char* dst = c ? c->err : g_err;
@@ -170,6 +172,7 @@ extern "C" dbie_status dbie_create(dbie_ctx** out, int nx, int ny, double h, dou
     dbie_ctx* ctx = (dbie_ctx*)calloc(1, sizeof(dbie_ctx));
     if (!ctx) return DBIE_ENOMEM;
     strcpy(ctx->err, "no error");
+    ctx->f32_sfu_mask = kDefaultF32SfuMask;
     dbie_status st = DBIE_OK;
     do {
         cudaError_t e;
@@ -286,11 +289,45 @@ extern "C" dbie_status dbie_eval_host(dbie_ctx* ctx, long long M, const double* 
 
 extern "C" dbie_status dbie_eval_f32(dbie_ctx* ctx, long long M, const float* x, const float* y, const float* z,
                                      const float* lam, float* B, void* cuda_stream) {
-    (void)x; (void)y; (void)z; (void)lam; (void)B; (void)cuda_stream;
     if (!ctx || M < 0) return DBIE_EINVAL;
-    if (!ctx->rec32) return DBIE_ESTATE;
-    snprintf(ctx->err, 256, "dbie_eval_f32: fp32 kernel not built in this version");
-    return DBIE_ESTATE;
+    if (!ctx->rec32) {
+        snprintf(ctx->err, 256, "dbie_eval_f32: the context was created without DBIE_WITH_FP32");
+        return DBIE_ESTATE;
+    }
+    if (M == 0) return DBIE_OK;
+    if (!x || !y || !z || !lam || !B) return DBIE_EINVAL;
+    cudaStream_t st = (cudaStream_t)cuda_stream;
+    const long long cap = M < kEvalBatch ? M : kEvalBatch;
+    const dbie_status s = ensure(ctx, (void**)&ctx->part, &ctx->part_bytes,
+                                 (size_t)ctx->bd.nchunks * 3 * cap * sizeof(double));
+    if (s != DBIE_OK) return s;
+    long long launches = 0;
+    prof_reset(ctx);
+    for (long long off = 0; off < M; off += cap) {
+        const long long cnt = (M - off < cap) ? (M - off) : cap;
+        InteractParamsF32 p;
+        memset(&p, 0, sizeof p);
+        p.bd = ctx->bd;
+        p.x = x; p.y = y; p.z = z; p.lam = lam; p.ldlam = M;
+        p.count = cnt; p.slot0 = off;
+        p.part = ctx->part; p.cap = cap;
+        prof_mark(ctx, st);
+        CU(launch_interact_f32(p, ctx->sm_count, ctx->f32_sfu_mask, st));
+        prof_mark(ctx, st);
+        CU(launch_eval_finalize_f32(ctx->bd, off, cnt, M, z, lam, ctx->part, cap, B, st));
+        launches += 2;
+    }
+    ctx->last_interactions = (double)M * (double)ctx->bd.N;
+    ctx->last_launches = launches;
+    ctx->last_evals = 0;
+    ctx->evals_on_device = 0;
+    return DBIE_OK;
+}
+
+extern "C" dbie_status dbie_set_f32_sfu_mask(dbie_ctx* ctx, int mask) {
+    if (!ctx || (mask != 0 && mask != 1 && mask != 3 && mask != 7)) return DBIE_EINVAL;
+    ctx->f32_sfu_mask = mask;
+    return DBIE_OK;
 }
 
 // ------------------------------------------------------------------------------ solve -----

@@ -14,6 +14,7 @@
 
 #include "dbie_internal.h"
 #include "dbie_math.cuh"
+#include "dbie_math_f32.cuh"
 
 namespace dbie {
 
@@ -272,6 +273,187 @@ cudaError_t launch_interact_stencil(const InteractParams& p, int sm_count, cudaS
         if (grid > 0x7fffffffLL) return cudaErrorInvalidValue;
     }
     interact_kernel<MODE_STENCIL, kStencil, kStenThreads, kStenMinB><<<(unsigned)grid, kStenThreads, 0, st>>>(q);
+    return cudaGetLastError();
+}
+
+// ------------------------------------------------------------------ fp32 eval kernel ------
+// dbie_eval_f32 (BASELINE.json config 4, fp32 leg): geometry, theta, sincos and products in fp32;
+// a row segment (<= 512 pixels) is summed in fp32, row sums are carried in fp64.
+// SFU_MASK bit p set: component p takes sin/cos of the reduced argument from MUFU.SIN/COS instead
+// of the FMA-pipe polynomials, to balance the FP32 and SFU pipes (SURVEY 8(d) "fp32 variant").
+template <int R, int THREADS, int MINB, int SFU_MASK>
+__global__ void __launch_bounds__(THREADS, MINB) interact_f32_kernel(const __grid_constant__ InteractParamsF32 p) {
+    constexpr int SPB = THREADS * R;
+    __shared__ alignas(128) float4 tile[2][kTilePx];
+    __shared__ alignas(8) uint64_t full[2];
+
+    const int tid = threadIdx.x;
+    if (tid == 0) {
+        mbar_init(&full[0], 1);
+        mbar_init(&full[1], 1);
+        mbar_fence_init();
+    }
+    __syncthreads();
+
+    const long long count = p.count;
+    const long long nblk = (count + SPB - 1) / SPB;
+    const BoundaryView& bd = p.bd;
+    const int NCH = bd.nchunks;
+    int nsplit = 1;
+    if (nblk < p.target_items) {
+        nsplit = (int)((p.target_items + nblk - 1) / nblk);
+        if (nsplit > NCH) nsplit = NCH;
+    }
+    const long long nwork = nblk * nsplit;
+
+    unsigned it = 0;
+    for (long long w = blockIdx.x; w < nwork; w += gridDim.x) {
+        const long long blk = w / nsplit;
+        const int sp = (int)(w % nsplit);
+        const int c0 = (int)(((long long)sp * NCH) / nsplit);
+        const int c1 = (int)(((long long)(sp + 1) * NCH) / nsplit);
+
+        float xi[R], yi[R], z2[R], lam[R][3];
+        long long slot[R];
+#pragma unroll
+        for (int r = 0; r < R; ++r) {
+            slot[r] = blk * SPB + tid + (long long)r * THREADS;
+            const long long id = p.slot0 + (slot[r] < count ? slot[r] : count - 1);
+            xi[r] = p.x[id];
+            yi[r] = p.y[id];
+            const float z = p.z[id];
+            z2[r] = z * z;
+#pragma unroll
+            for (int c = 0; c < 3; ++c) lam[r][c] = fabsf(p.lam[c * p.ldlam + id]);
+        }
+        double acc[R][3];
+#pragma unroll
+        for (int r = 0; r < R; ++r) acc[r][0] = acc[r][1] = acc[r][2] = 0.0;
+
+        const int t0 = chunk_first_tile(bd, c0), t1 = chunk_first_tile(bd, c1);
+        int c = c0;
+        int t_chunk_end = chunk_first_tile(bd, c + 1);
+        if (tid == 0) {
+            const TileDesc d = tile_desc(bd, t0);
+            mbar_expect_tx(&full[it & 1], (unsigned)d.npx * 16u);
+            bulk_g2s(&tile[it & 1][0], bd.rec32 + d.px0, (unsigned)d.npx * 16u, &full[it & 1]);
+        }
+        for (int t = t0; t < t1; ++t, ++it) {
+            if (tid == 0 && t + 1 < t1) {
+                const TileDesc dn = tile_desc(bd, t + 1);
+                const unsigned sn = (it + 1) & 1;
+                mbar_expect_tx(&full[sn], (unsigned)dn.npx * 16u);
+                bulk_g2s(&tile[sn][0], bd.rec32 + dn.px0, (unsigned)dn.npx * 16u, &full[sn]);
+            }
+            const TileDesc d = tile_desc(bd, t);
+            mbar_wait(&full[it & 1], (it >> 1) & 1);
+            const float4* __restrict__ rp = &tile[it & 1][0];
+            for (int row = 0; row < d.nrows; ++row) {
+                const float yk = __ldg(bd.yk32 + d.row0 + row);
+                float cc[R], a32[R][3];
+#pragma unroll
+                for (int r = 0; r < R; ++r) {
+                    const float dy = yk - yi[r];
+                    cc[r] = fmaf(dy, dy, z2[r]);
+                    a32[r][0] = a32[r][1] = a32[r][2] = 0.0f;
+                }
+#pragma unroll 2
+                for (int j = 0; j < d.ncols; ++j) {
+                    const float4 px = rp[j];  // {x_k, Bx0, By0, Bz0}: one broadcast LDS.128
+#pragma unroll
+                    for (int r = 0; r < R; ++r) {
+                        const float dx = px.x - xi[r];
+                        const float r2 = fmaf(dx, dx, cc[r]);
+                        const float y = rsqrt_f32(r2);
+                        const float rr = r2 * y;
+                        const float wgt = (y * y) * y;
+                        a32[r][0] = fmaf(kernel_n_f32<(SFU_MASK & 1) != 0>(lam[r][0] * rr), wgt * px.y, a32[r][0]);
+                        a32[r][1] = fmaf(kernel_n_f32<(SFU_MASK & 2) != 0>(lam[r][1] * rr), wgt * px.z, a32[r][1]);
+                        a32[r][2] = fmaf(kernel_n_f32<(SFU_MASK & 4) != 0>(lam[r][2] * rr), wgt * px.w, a32[r][2]);
+                    }
+                }
+#pragma unroll
+                for (int r = 0; r < R; ++r)
+#pragma unroll
+                    for (int q = 0; q < 3; ++q) acc[r][q] += (double)a32[r][q];
+                rp += d.ncols;
+            }
+            if (t + 1 == t_chunk_end) {
+#pragma unroll
+                for (int r = 0; r < R; ++r)
+                    if (slot[r] < count) {
+#pragma unroll
+                        for (int q = 0; q < 3; ++q) p.part[((long long)c * 3 + q) * p.cap + slot[r]] = acc[r][q];
+                    }
+#pragma unroll
+                for (int r = 0; r < R; ++r) acc[r][0] = acc[r][1] = acc[r][2] = 0.0;
+                ++c;
+                t_chunk_end = chunk_first_tile(bd, c + 1);
+            }
+            __syncthreads();
+        }
+    }
+}
+
+constexpr int kF32R = 4, kF32Threads = 128, kF32MinB = 4;
+
+template <int MASK>
+static cudaError_t launch_f32_variant(const InteractParamsF32& q, unsigned grid, cudaStream_t st) {
+    interact_f32_kernel<kF32R, kF32Threads, kF32MinB, MASK><<<grid, kF32Threads, 0, st>>>(q);
+    return cudaGetLastError();
+}
+
+cudaError_t launch_interact_f32(const InteractParamsF32& p, int sm_count, int sfu_mask, cudaStream_t st) {
+    if (p.count <= 0) return cudaSuccess;
+    InteractParamsF32 q = p;
+    const long long spb = (long long)kF32Threads * kF32R;
+    const long long nblk = (q.count + spb - 1) / spb;
+    q.target_items = 8 * sm_count * kF32MinB;
+    long long nsplit = 1;
+    if (nblk < q.target_items) {
+        nsplit = (q.target_items + nblk - 1) / nblk;
+        if (nsplit > q.bd.nchunks) nsplit = q.bd.nchunks;
+    }
+    const long long nwork = nblk * nsplit;
+    if (nwork > 0x7fffffffLL) return cudaErrorInvalidValue;
+    switch (sfu_mask & 7) {
+        case 0: return launch_f32_variant<0>(q, (unsigned)nwork, st);
+        case 1: return launch_f32_variant<1>(q, (unsigned)nwork, st);
+        case 3: return launch_f32_variant<3>(q, (unsigned)nwork, st);
+        case 7: return launch_f32_variant<7>(q, (unsigned)nwork, st);
+        default: return cudaErrorInvalidValue;
+    }
+}
+
+// B_p = (z h^2 / 2 pi) * (chunk sums in chunk order), fp64 arithmetic, rounded to float once.
+__global__ void eval_finalize_f32_kernel(int nchunks, double h2_over_2pi, long long slot0, long long count,
+                                         long long M, const float* __restrict__ z,
+                                         const float* __restrict__ lam, const double* __restrict__ part,
+                                         long long cap, float* __restrict__ B) {
+    const long long s = blockIdx.x * (long long)blockDim.x + threadIdx.x;
+    if (s >= count) return;
+    const long long id = slot0 + s;
+    const float zi = z[id];
+    bool ok = (zi > 0.0f) && isfinite(zi);
+    float out[3];
+#pragma unroll
+    for (int q = 0; q < 3; ++q) {
+        double sum = part[(long long)q * cap + s];
+        for (int c = 1; c < nchunks; ++c) sum += part[((long long)c * 3 + q) * cap + s];
+        out[q] = (float)(((double)zi * h2_over_2pi) * sum);
+        ok = ok && isfinite(lam[q * M + id]);
+    }
+#pragma unroll
+    for (int q = 0; q < 3; ++q) B[q * M + id] = ok ? out[q] : __int_as_float(0x7fc00000);
+}
+
+cudaError_t launch_eval_finalize_f32(const BoundaryView& bd, long long slot0, long long count, long long M,
+                                     const float* z, const float* lam, const double* part, long long cap,
+                                     float* B, cudaStream_t st) {
+    if (count <= 0) return cudaSuccess;
+    const double h2_over_2pi = bd.h * bd.h / (2.0 * 3.14159265358979323846);
+    const unsigned grid = (unsigned)((count + 255) / 256);
+    eval_finalize_f32_kernel<<<grid, 256, 0, st>>>(bd.nchunks, h2_over_2pi, slot0, count, M, z, lam, part, cap, B);
     return cudaGetLastError();
 }
 

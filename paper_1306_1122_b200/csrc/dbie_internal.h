@@ -82,6 +82,18 @@ struct InteractParams {
     unsigned* zero_ptr;          // set to 0 by the launch (the next pass's list counter), or nullptr
 };
 
+// One launch of the fp32 eval kernel (dbie_eval_f32): slot i = evaluation point slot0 + i.
+struct InteractParamsF32 {
+    BoundaryView bd;
+    const float *x, *y, *z;
+    const float* lam;            // lam[p*ldlam + id]
+    long long ldlam;
+    long long count, slot0;
+    double* part;                // fp64 chunk sums, part[(c*3 + q)*cap + slot]
+    long long cap;
+    int target_items;
+};
+
 struct SolveArrays {            // per-point optimiser state, structure-of-arrays by point id
     double* V;                  // [12][M]  simplex vertices V[(j*3+p)*M + i]
     double* F;                  // [4][M]   Phi at the vertices
@@ -103,6 +115,10 @@ cudaError_t launch_interact_stencil(const InteractParams& p, int sm_count, cudaS
 cudaError_t launch_eval_finalize(const BoundaryView& bd, long long slot0, long long count,
                                  long long M, const double* z, const double* lam, const double* part,
                                  long long cap, double* B, cudaStream_t st);
+cudaError_t launch_interact_f32(const InteractParamsF32& p, int sm_count, int sfu_mask, cudaStream_t st);
+cudaError_t launch_eval_finalize_f32(const BoundaryView& bd, long long slot0, long long count, long long M,
+                                     const float* z, const float* lam, const double* part, long long cap,
+                                     float* B, cudaStream_t st);
 cudaError_t launch_probe(double millis, int sm_count, double* dfma_per_s, double* ffma_per_s);
 
 cudaError_t launch_solve_init(const SolveArrays& s, const NMConsts& k, long long M, long long ldo,
