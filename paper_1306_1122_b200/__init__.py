@@ -61,6 +61,7 @@ def load() -> C.CDLL:
     lib.dbie_eval.argtypes = [_vp, C.c_longlong, _vp, _vp, _vp, _vp, _vp, _vp]
     lib.dbie_eval_host.argtypes = [_vp, C.c_longlong, _vp, _vp, _vp, _vp, _vp]
     lib.dbie_eval_f32.argtypes = [_vp, C.c_longlong, _vp, _vp, _vp, _vp, _vp, _vp]
+    lib.dbie_set_f32_sfu_mask.argtypes = [_vp, C.c_int]
     lib.dbie_solve_default_opts.argtypes = [C.POINTER(SolveOpts)]
     lib.dbie_solve_default_opts.restype = None
     lib.dbie_solve.argtypes = [_vp, C.c_longlong, _vp, _vp, _vp, C.POINTER(SolveOpts), _vp, _vp, _vp,
@@ -115,6 +116,15 @@ def _dev_f64(t, n, name):
     torch = _torch()
     if not isinstance(t, torch.Tensor) or not t.is_cuda or t.dtype != torch.float64:
         raise TypeError(f"{name}: expected a CUDA float64 tensor")
+    if not t.is_contiguous() or t.numel() != n:
+        raise ValueError(f"{name}: expected {n} contiguous elements, got {tuple(t.shape)}")
+    return _vp(t.data_ptr())
+
+
+def _dev_f32(t, n, name):
+    torch = _torch()
+    if not isinstance(t, torch.Tensor) or not t.is_cuda or t.dtype != torch.float32:
+        raise TypeError(f"{name}: expected a CUDA float32 tensor")
     if not t.is_contiguous() or t.numel() != n:
         raise ValueError(f"{name}: expected {n} contiguous elements, got {tuple(t.shape)}")
     return _vp(t.data_ptr())
@@ -205,6 +215,22 @@ class DBIE:
         self._check(self._lib.dbie_eval_host(self._h, M, _vp(x.ctypes.data), _vp(y.ctypes.data),
                                              _vp(z.ctypes.data), _vp(lam.ctypes.data), _vp(B.ctypes.data)))
         return B
+
+    # -- dbie_eval_f32
+    def eval_f32(self, x, y, z, lam, out=None, stream=None):
+        """fp32-arithmetic variant: float32 device tensors in, B (3, M) float32 out."""
+        torch = _torch()
+        M = x.numel()
+        if out is None:
+            out = torch.empty((3, M), dtype=torch.float32, device=x.device)
+        self._check(self._lib.dbie_eval_f32(self._h, M, _dev_f32(x, M, "x"), _dev_f32(y, M, "y"),
+                                            _dev_f32(z, M, "z"), _dev_f32(lam, 3 * M, "lam"),
+                                            _dev_f32(out, 3 * M, "out"), _stream_ptr(stream)))
+        return out
+
+    def set_f32_sfu_mask(self, mask: int):
+        """dbie_set_f32_sfu_mask: which components take sin/cos from the SFU (0, 1, 3 or 7)."""
+        self._check(self._lib.dbie_set_f32_sfu_mask(self._h, int(mask)))
 
     # -- dbie_residual
     def residual(self, x, y, z, lam, opts: SolveOpts | None = None, stream=None):

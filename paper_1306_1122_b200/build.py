@@ -28,7 +28,8 @@ UNITS = [
     ("dbie_solver.cu", ["-fmad=false"]),
     ("dbie_api.cu", []),
 ]
-HEADERS = ["dbie_internal.h", "dbie_math.cuh", "dbie_nm.cuh", "trig_coeffs.h"]
+HEADERS = ["dbie_internal.h", "dbie_tma.cuh", "dbie_math.cuh", "dbie_math_f32.cuh", "dbie_nm.cuh", "trig_coeffs.h",
+           "trig_coeffs_f32.h"]
 
 
 def _newer(target: str, deps: list[str]) -> bool:
@@ -61,7 +62,8 @@ def build_lib(force: bool = False, verbose: bool = False) -> str:
 def build_hostshim(force: bool = False) -> str:
     """CPU build of the __host__ __device__ arithmetic headers, for the not-gpu tests."""
     src = os.path.join(CSRC, "host_shim.cpp")
-    deps = [src] + [os.path.join(CSRC, h) for h in ("dbie_math.cuh", "dbie_nm.cuh", "trig_coeffs.h")]
+    deps = [src] + [os.path.join(CSRC, h) for h in ("dbie_math.cuh", "dbie_math_f32.cuh", "dbie_nm.cuh", "trig_coeffs.h",
+                                                     "trig_coeffs_f32.h")]
     if force or _newer(SHIM, deps):
         tmp = SHIM + f".tmp{os.getpid()}"
         subprocess.check_call(["g++", "-O2", "-std=c++17", "-ffp-contract=off", "-fno-fast-math",

@@ -5,6 +5,7 @@
 // reciprocal-sqrt seed (MUFU.RSQ64H on the device, a float-rounded 1/sqrt here).
 // Built with g++ -O2 -ffp-contract=off; explicit fma() calls map to libm fma (correctly rounded).
 #include "dbie_math.cuh"
+#include "dbie_math_f32.cuh"
 #include "dbie_nm.cuh"
 
 extern "C" {
@@ -27,6 +28,11 @@ void shim_interaction(double dx, double dy, double z, const double lam[3], const
     const double rr = r2 * y;
     const double w = (y * y) * y;
     for (int p = 0; p < 3; ++p) out[p] = dbie::kernel_n(fabs(lam[p]) * rr) * (w * b0[p]);
+}
+
+// fp32 kernel value n(theta) on the FMA-pipe polynomials (the SFU variant is device only)
+void shim_kernel_n_f32(long n, const float* th, float* out) {
+    for (long i = 0; i < n; ++i) out[i] = dbie::kernel_n_f32<false>(th[i]);
 }
 
 typedef double (*shim_objective)(const double*);

@@ -192,3 +192,23 @@ def test_nm_maxiter_and_shrink_paths(shim):
     assert mine["iters"] == res.nit - 1 == 60 and mine["status"] == 2
     assert mine["nfev"] == res.nfev
     assert np.array_equal(mine["simplex"][0], res.x)
+
+
+def test_kernel_n_f32_polynomial_path(shim):
+    """fp32 n(theta) = theta sin theta + cos theta of dbie_math_f32.cuh (FMA-pipe path) against
+    mpmath at the float inputs: |error| <= 4 ulp_f32(theta) + 2e-7 for theta up to 400 rad
+    (config 4 reaches ~155).  The dominant term is theta * (error of sin) ~ theta * 6e-8."""
+    rng = np.random.default_rng(5)
+    th = np.concatenate([rng.uniform(0, 2, 1000), rng.uniform(0, 160, 4000), rng.uniform(0, 400, 1000),
+                         np.arange(0, 200) * (math.pi / 4), [0.0, 1e-20, 0.78539816]]).astype(np.float32)
+    out = np.empty_like(th)
+    fp = C.POINTER(C.c_float)
+    shim.shim_kernel_n_f32(C.c_long(th.size), th.ctypes.data_as(fp), out.ctypes.data_as(fp))
+    mp.mp.dps = 30
+    worst = 0.0
+    for t, got in zip(th, out):
+        tt = mp.mpf(float(t))
+        ex = tt * mp.sin(tt) + mp.cos(tt)
+        tol = 4.0 * float(np.spacing(np.float32(max(float(t), 1.0)))) + 2e-7
+        worst = max(worst, float(abs(mp.mpf(float(got)) - ex)) / tol)
+    assert worst <= 1.0, worst

@@ -147,6 +147,67 @@ def test_eval_linearity_and_shift_invariance(dbie):
     assert np.allclose(gpu_eval(dbie, w3), B1, rtol=1e-11, atol=0)
 
 
+# ---------------------------------------------------------------------------- eval, fp32 ---
+TOL_B_F32 = 2e-4
+
+
+def _f32_inputs(w):
+    """Round the points and lambda to float32 once; the oracle gets exactly those values."""
+    w32 = w.subset(np.arange(w.M))
+    for k in ("x", "y", "z"):
+        setattr(w32, k, getattr(w, k).astype(np.float32).astype(np.float64))
+    w32.lam = w.lam.astype(np.float32).astype(np.float64)
+    return w32
+
+
+def gpu_eval_f32(d, w32, mask=0):
+    import torch
+    with d.DBIE.from_workload(w32, fp32=True) as ctx:
+        ctx.set_f32_sfu_mask(mask)
+        t = lambda a: torch.from_numpy(np.ascontiguousarray(a, dtype=np.float32)).cuda()
+        return ctx.eval_f32(t(w32.x), t(w32.y), t(w32.z), t(w32.lam)).cpu().numpy().astype(np.float64)
+
+
+@pytest.mark.parametrize("mask", [0, 1, 3, 7])
+def test_eval_f32_config4_first_points(dbie, mask):
+    """BASELINE configs[3], fp32 leg: 512x512 boundary, first 2048 points (4 work blocks of the
+    128x4 mapping), every sincos variant; <= 2e-4 relative vector error vs the fp64 oracle."""
+    w = _f32_inputs(workloads.config4().subset(np.arange(2048)))
+    B = gpu_eval_f32(dbie, w, mask)
+    err, dropped = vec_relerr(B, oracle.eval(w))
+    assert err <= TOL_B_F32, err
+    assert dropped == 0
+
+
+@pytest.mark.parametrize("nx,ny", [(1, 1), (7, 5), (513, 3), (64, 64), (1030, 2)])
+def test_eval_f32_ragged_boundaries(dbie, nx, ny):
+    w = _f32_inputs(workloads.random_boundary(nx, ny, seed=nx * 3 + ny, npts=37, h=0.5, x0=-1.0, y0=2.0))
+    # the boundary values and pixel centres are rounded to float by dbie_create; use values that
+    # are exact in float so that the oracle sees the same boundary
+    for k in ("bx", "by", "bz"):
+        setattr(w, k, getattr(w, k).astype(np.float32).astype(np.float64))
+    err, _ = vec_relerr(gpu_eval_f32(dbie, w), oracle.eval(w), floor=1e-3)
+    assert err <= TOL_B_F32, err
+
+
+def test_eval_f32_needs_the_fp32_copy_and_handles_invalid_points(dbie):
+    import torch
+    w = _f32_inputs(workloads.random_boundary(20, 12, seed=3, npts=9))
+    t = lambda a: torch.from_numpy(np.ascontiguousarray(a, dtype=np.float32)).cuda()
+    with dbie.DBIE.from_workload(w) as ctx:          # no DBIE_WITH_FP32
+        with pytest.raises(dbie.DBIEError) as ei:
+            ctx.eval_f32(t(w.x), t(w.y), t(w.z), t(w.lam))
+        assert ei.value.status == dbie.DBIE_ESTATE
+    with dbie.DBIE.from_workload(w, fp32=True) as ctx:
+        z = w.z.copy(); z[2] = 0.0
+        B = ctx.eval_f32(t(w.x), t(w.y), t(z), t(w.lam)).cpu().numpy()
+        assert np.isnan(B[:, 2]).all() and np.isfinite(np.delete(B, 2, axis=1)).all()
+        B2 = ctx.eval_f32(t(w.x), t(w.y), t(z), t(w.lam)).cpu().numpy()
+        assert np.array_equal(B, B2, equal_nan=True)
+        with pytest.raises(TypeError):
+            ctx.eval_f32(t(w.x).double(), t(w.y), t(w.z), t(w.lam))
+
+
 # ---------------------------------------------------------------------------- residual -----
 @pytest.mark.parametrize("case", ["random", "config3"])
 def test_residual_matches_oracle(dbie, case):
