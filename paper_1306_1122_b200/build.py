@@ -26,10 +26,11 @@ COMMON = ["-O3", "-std=c++17", "-lineinfo", "-Xcompiler", "-fPIC", "-I", INCLUDE
 UNITS = [
     ("dbie_interact.cu", []),
     ("dbie_solver.cu", ["-fmad=false"]),
+    ("dbie_grid.cu", ["-fmad=false"]),
     ("dbie_api.cu", []),
 ]
-HEADERS = ["dbie_internal.h", "dbie_tma.cuh", "dbie_math.cuh", "dbie_math_f32.cuh", "dbie_nm.cuh", "trig_coeffs.h",
-           "trig_coeffs_f32.h"]
+HEADERS = ["dbie_internal.h", "dbie_interact_fp64.cuh", "dbie_tma.cuh", "dbie_math.cuh", "dbie_math_f32.cuh", "dbie_nm.cuh", "dbie_solver_common.cuh",
+           "trig_coeffs.h", "trig_coeffs_f32.h"]
 
 
 def _newer(target: str, deps: list[str]) -> bool:

@@ -393,6 +393,77 @@ extern "C" dbie_status dbie_residual(dbie_ctx* ctx, long long M, const double* x
 
 static size_t align256(size_t v) { return (v + 255) & ~(size_t)255; }
 
+// GRID mode (O-4; BASELINE.json config 5 reading, not in the paper): per level one
+// MODE_GRID interaction launch (4 x 3 x T sums per active point) and one grid_step launch.
+static dbie_status solve_grid(dbie_ctx* ctx, long long M, const double* x, const double* y, const double* z,
+                              const dbie_solve_opts* opts, const NMConsts& k, double* B, double* lam, double* resid,
+                              int* iters, int* status, void* cuda_stream) {
+    const int T = opts->n_trial, L = opts->n_level;
+    if (T < 2 || T > kGridMaxTrials || L < 1 || !(opts->lam_max > 0.0) || !isfinite(opts->lam_max)) return DBIE_EINVAL;
+    cudaStream_t st = (cudaStream_t)cuda_stream;
+    const BoundaryView& bd = ctx->bd;
+    // batch so that the chunk sums (nchunks x 12 T doubles per point) stay below 2 GiB
+    const size_t per_point = (size_t)bd.nchunks * 12 * T * sizeof(double);
+    long long batch = (long long)(((size_t)2 << 30) / per_point);
+    if (batch < 1024) batch = 1024;
+    const long long cap = M < batch ? M : batch;
+    dbie_status s = ensure(ctx, (void**)&ctx->part, &ctx->part_bytes, per_point * cap);
+    if (s != DBIE_OK) return s;
+    const size_t isz = align256((size_t)cap * sizeof(int));
+    const size_t dstride = (size_t)cap * sizeof(double);
+    s = ensure(ctx, (void**)&ctx->state, &ctx->state_bytes, 3 * align256(12 * dstride) + 2 * isz);
+    if (s != DBIE_OK) return s;
+    GridArrays a;
+    char* base = ctx->state;
+    a.lo = (double*)base;                base += align256(3 * dstride);
+    a.inc = (double*)base;               base += align256(12 * dstride);
+    a.il = (double*)base;                base += align256(3 * dstride);
+    a.act[0] = (int*)base;               base += isz;
+    a.act[1] = (int*)base;               base += isz;
+    a.cap = cap;
+    a.nact = ctx->counters;
+    unsigned long long* nevals = (unsigned long long*)((char*)ctx->counters + 16);
+    CU(cudaMemsetAsync(ctx->counters, 0, 64, st));
+    GridConsts gc;
+    gc.T = T;
+    gc.n_level = L;
+    gc.Lmax = opts->lam_max / bd.h;
+    long long launches = 0;
+    prof_reset(ctx);
+    for (long long off = 0; off < M; off += cap) {
+        const long long cnt = (M - off < cap) ? (M - off) : cap;
+        CU(cudaMemsetAsync(ctx->counters, 0, 8, st));
+        CU(launch_grid_init(a, cnt, M, x + off, y + off, z + off, B + off, lam + off, resid + off, iters + off,
+                            status + off, st));
+        ++launches;
+        double W = gc.Lmax;
+        for (int lev = 0; lev < L; ++lev) {
+            gc.W = W;
+            gc.Wn = 2.0 * W / (double)(T - 1);
+            InteractParams p;
+            memset(&p, 0, sizeof p);
+            p.bd = bd;
+            p.x = x + off; p.y = y + off; p.z = z + off;
+            p.act = a.act[lev & 1];
+            p.count_ptr = &a.nact[lev & 1];
+            p.zero_ptr = &a.nact[(lev + 1) & 1];
+            p.delta_abs = k.delta_abs;
+            p.part = ctx->part; p.cap = cap;
+            p.lo = a.lo; p.ldlo = cap; p.W = W; p.T = T;
+            prof_mark(ctx, st);
+            CU(launch_interact_grid(p, ctx->sm_count, st));
+            prof_mark(ctx, st);
+            CU(launch_grid_step(a, k, gc, bd, lev, cnt, M, z + off, ctx->part, cap, B + off, lam + off, resid + off,
+                                iters + off, status + off, nevals, st));
+            launches += 2;
+            W = gc.Wn;
+        }
+    }
+    ctx->last_launches = launches;
+    ctx->evals_on_device = 1;
+    return DBIE_OK;
+}
+
 extern "C" dbie_status dbie_solve(dbie_ctx* ctx, long long M, const double* x, const double* y, const double* z,
                                   const dbie_solve_opts* opts, double* B, double* lam, double* resid, int* iters,
                                   int* status, void* cuda_stream) {
@@ -403,10 +474,8 @@ extern "C" dbie_status dbie_solve(dbie_ctx* ctx, long long M, const double* x, c
     NMConsts k;
     dbie_status s = make_consts(ctx, opts, &k);
     if (s != DBIE_OK) return s;
-    if (opts && opts->method != 0) {
-        snprintf(ctx->err, 256, "dbie_solve: method %d (GRID) not built in this version", opts->method);
-        return DBIE_EINVAL;
-    }
+    if (opts && opts->method == 1) return solve_grid(ctx, M, x, y, z, opts, k, B, lam, resid, iters, status, cuda_stream);
+    if (opts && opts->method != 0) return DBIE_EINVAL;
     cudaStream_t st = (cudaStream_t)cuda_stream;
     const long long cap = M < kStencilBatch ? M : kStencilBatch;
     s = ensure(ctx, (void**)&ctx->part, &ctx->part_bytes, (size_t)ctx->bd.nchunks * 12 * cap * sizeof(double));

@@ -3,16 +3,14 @@
 //   B_p(i) = (z_i h^2/2pi) sum_k [theta sin theta + cos theta]/r^3 * B_p0[k],  theta = |lambda_p| r
 //   (Eq. 6, Eq. 16).
 //
-// Mapping (the inverse of the paper's, which strides the PIXELS of one point
-// over 80x128 threads): evaluation points are the parallel dimension, register-blocked R per
-// thread; the boundary is streamed through shared memory in 16 KB tiles by the TMA bulk-copy
-// engine (cp.async.bulk + mbarrier, double buffered) and every thread of the CTA reads the same
-// pixel record as a broadcast LDS.128 pair.  The bound is the FP64 pipe (76 FP64 instructions per
-// interaction); there are no tensor-core or HBM-bound steps.
+// This file holds the boundary staging kernel, the launchers of the fp64 interaction kernel
+// (dbie_interact_fp64.cuh), the fp32 eval kernel, the eval epilogues and the pipe-rate probe.
+// The bound is the FP64 pipe; there are no tensor-core or HBM-bound steps.
 #include <cuda_runtime.h>
 #include <stdint.h>
 
 #include "dbie_internal.h"
+#include "dbie_interact_fp64.cuh"
 #include "dbie_math.cuh"
 #include "dbie_math_f32.cuh"
 #include "dbie_tma.cuh"
@@ -51,191 +49,49 @@ cudaError_t launch_stage_boundary(int nx, int ny, double h, double x0, double y0
     return cudaGetLastError();
 }
 
-// ------------------------------------------------------------------ interaction kernel ----
-enum { MODE_EVAL = 0, MODE_STENCIL = 1 };
+// ------------------------------------------------------------------ fp64 launchers --------
+// The kernel is dbie_interact_fp64.cuh.  Shapes measured on B200 (profiles/r01_variants.md):
+// 256 threads x 2 CTAs/SM (<= 128 registers), two pixels in flight per thread; GRID mode carries
+// 4 (else 2, else 1) trial lambda triples per thread on one geometry.
+constexpr int kThreads64 = 256, kMinB64 = 2;
 
-template <int MODE, int R, int THREADS, int MINB>
-__global__ void __launch_bounds__(THREADS, MINB) interact_kernel(const __grid_constant__ InteractParams p) {
-    constexpr int Q = (MODE == MODE_EVAL) ? 3 : 3 * R;        // sums per slot
-    constexpr int SPB = (MODE == MODE_EVAL) ? THREADS * R : THREADS;  // slots per work block
-    constexpr int NL = (MODE == MODE_EVAL) ? R : 1;            // lambda triples per thread
-    static_assert(MODE == MODE_EVAL || R == kStencil, "stencil mode evaluates 4 positions");
-
-    __shared__ alignas(128) double4 tile[2][kTilePx];
-    __shared__ alignas(8) uint64_t full[2];
-
-    const int tid = threadIdx.x;
-    if (tid == 0) {
-        mbar_init(&full[0], 1);
-        mbar_init(&full[1], 1);
-        mbar_fence_init();
-    }
-    __syncthreads();
-
-    if (p.zero_ptr && blockIdx.x == 0 && tid == 0) *p.zero_ptr = 0u;  // next pass's list counter
-    const long long count = p.count_ptr ? (long long)(*p.count_ptr) : p.count;
-    const long long nblk = (count + SPB - 1) / SPB;
-    if (nblk == 0) return;
-    const BoundaryView& bd = p.bd;
-    const int NCH = bd.nchunks;
-    int nsplit = 1;
-    if (nblk < p.target_items) {
-        nsplit = (int)((p.target_items + nblk - 1) / nblk);
-        if (nsplit > NCH) nsplit = NCH;
-    }
-    const long long nwork = nblk * nsplit;
-
-    unsigned it = 0;  // tiles consumed by this CTA so far: stage = it & 1, parity = (it >> 1) & 1
-    for (long long w = blockIdx.x; w < nwork; w += gridDim.x) {
-        const long long blk = w / nsplit;
-        const int sp = (int)(w % nsplit);
-        const int c0 = (int)(((long long)sp * NCH) / nsplit);
-        const int c1 = (int)(((long long)(sp + 1) * NCH) / nsplit);
-
-        // ---- per-thread evaluation points
-        double xi[R], yi[R], z2[R], lam[NL][3];
-        long long slot[NL];
-        if (MODE == MODE_EVAL) {
-#pragma unroll
-            for (int r = 0; r < R; ++r) {
-                slot[r] = blk * SPB + tid + (long long)r * THREADS;
-                const long long id = p.slot0 + (slot[r] < count ? slot[r] : count - 1);
-                xi[r] = p.x[id];
-                yi[r] = p.y[id];
-                const double z = p.z[id];
-                z2[r] = z * z;
-#pragma unroll
-                for (int c = 0; c < 3; ++c) lam[r][c] = fabs(p.lam[c * p.ldlam + id]);
-            }
-        } else {
-            slot[0] = blk * SPB + tid;
-            const long long j = slot[0] < count ? slot[0] : count - 1;
-            const long long id = p.act ? (long long)p.act[j] : j;
-            const double x = p.x[id], y = p.y[id], z = p.z[id];
-            const double zd = __dadd_rn(z, p.delta_abs);
-#pragma unroll
-            for (int r = 0; r < R; ++r) {
-                xi[r] = (r == 1) ? __dadd_rn(x, p.delta_abs) : x;
-                yi[r] = (r == 2) ? __dadd_rn(y, p.delta_abs) : y;
-                z2[r] = (r == 3) ? zd * zd : z * z;
-            }
-#pragma unroll
-            for (int c = 0; c < 3; ++c) lam[0][c] = fabs(p.lam[c * p.ldlam + id]);
-        }
-
-        double acc[R][3];
-#pragma unroll
-        for (int r = 0; r < R; ++r) acc[r][0] = acc[r][1] = acc[r][2] = 0.0;
-
-        const int t0 = chunk_first_tile(bd, c0), t1 = chunk_first_tile(bd, c1);
-        int c = c0;
-        int t_chunk_end = chunk_first_tile(bd, c + 1);
-        if (tid == 0) {
-            const TileDesc d = tile_desc(bd, t0);
-            mbar_expect_tx(&full[it & 1], (unsigned)d.npx * 32u);
-            bulk_g2s(&tile[it & 1][0], bd.rec + d.px0, (unsigned)d.npx * 32u, &full[it & 1]);
-        }
-        for (int t = t0; t < t1; ++t, ++it) {
-            if (tid == 0 && t + 1 < t1) {  // prefetch the next tile into the other stage
-                const TileDesc dn = tile_desc(bd, t + 1);
-                const unsigned sn = (it + 1) & 1;
-                mbar_expect_tx(&full[sn], (unsigned)dn.npx * 32u);
-                bulk_g2s(&tile[sn][0], bd.rec + dn.px0, (unsigned)dn.npx * 32u, &full[sn]);
-            }
-            const TileDesc d = tile_desc(bd, t);
-            mbar_wait(&full[it & 1], (it >> 1) & 1);
-            const double4* __restrict__ rp = &tile[it & 1][0];
-            for (int row = 0; row < d.nrows; ++row) {
-                const double yk = __ldg(bd.yk + d.row0 + row);
-                double cc[R];
-#pragma unroll
-                for (int r = 0; r < R; ++r) {
-                    const double dy = yk - yi[r];
-                    cc[r] = fma(dy, dy, z2[r]);
-                }
-#pragma unroll 1
-                for (int j = 0; j < d.ncols; ++j) {
-                    const double4 px = rp[j];  // {x_k, Bx0, By0, Bz0}: two broadcast LDS.128
-#pragma unroll
-                    for (int r = 0; r < R; ++r) {
-                        const double dx = px.x - xi[r];
-                        const double r2 = fma(dx, dx, cc[r]);
-                        const double y = rsqrt_full(r2);   // 1/r
-                        const double rr = r2 * y;          // r
-                        const double w = (y * y) * y;      // 1/r^3
-                        const int l = (NL == 1) ? 0 : r;
-                        acc[r][0] = fma(kernel_n(lam[l][0] * rr), w * px.y, acc[r][0]);
-                        acc[r][1] = fma(kernel_n(lam[l][1] * rr), w * px.z, acc[r][1]);
-                        acc[r][2] = fma(kernel_n(lam[l][2] * rr), w * px.w, acc[r][2]);
-                    }
-                }
-                rp += d.ncols;
-            }
-            if (t + 1 == t_chunk_end) {  // A4: one partial sum per chunk, added in chunk order later
-                if (MODE == MODE_EVAL) {
-#pragma unroll
-                    for (int r = 0; r < R; ++r)
-                        if (slot[r] < count) {
-#pragma unroll
-                            for (int q = 0; q < 3; ++q)
-                                p.part[((long long)c * Q + q) * p.cap + slot[r]] = acc[r][q];
-                        }
-                } else if (slot[0] < count) {
-#pragma unroll
-                    for (int r = 0; r < R; ++r)
-#pragma unroll
-                        for (int q = 0; q < 3; ++q)
-                            p.part[((long long)c * Q + r * 3 + q) * p.cap + slot[0]] = acc[r][q];
-                }
-#pragma unroll
-                for (int r = 0; r < R; ++r) acc[r][0] = acc[r][1] = acc[r][2] = 0.0;
-                ++c;
-                t_chunk_end = chunk_first_tile(bd, c + 1);
-            }
-            __syncthreads();  // everyone is done with stage it&1 before it is refilled
-        }
-    }
-}
-
-constexpr int kEvalR = 2, kEvalThreads = 256, kEvalMinB = 2;
-constexpr int kStenThreads = 128, kStenMinB = 4;
-
-cudaError_t launch_interact_eval(const InteractParams& p, int sm_count, cudaStream_t st) {
-    if (p.count <= 0) return cudaSuccess;
+template <int MODE, int NT, int UNR>
+static cudaError_t launch64(const InteractParams& p, int sm_count, int waves, cudaStream_t st) {
     InteractParams q = p;
-    const long long spb = (long long)kEvalThreads * kEvalR;
-    const long long nblk = (q.count + spb - 1) / spb;
-    q.target_items = 8 * sm_count * kEvalMinB;
-    long long nsplit = 1;
-    if (nblk < q.target_items) {
-        nsplit = (q.target_items + nblk - 1) / nblk;
-        if (nsplit > q.bd.nchunks) nsplit = q.bd.nchunks;
-    }
-    const long long nwork = nblk * nsplit;   // one work item per CTA: the hardware balances them
-    if (nwork > 0x7fffffffLL) return cudaErrorInvalidValue;
-    interact_kernel<MODE_EVAL, kEvalR, kEvalThreads, kEvalMinB><<<(unsigned)nwork, kEvalThreads, 0, st>>>(q);
-    return cudaGetLastError();
-}
-
-cudaError_t launch_interact_stencil(const InteractParams& p, int sm_count, cudaStream_t st) {
-    InteractParams q = p;
-    q.target_items = 4 * sm_count * kStenMinB;
+    q.target_items = waves * sm_count * kMinB64;
     long long grid;
     if (q.count_ptr) {
-        grid = (long long)sm_count * kStenMinB;   // persistent: the slot count lives on the device
+        grid = (long long)sm_count * kMinB64;   // persistent: the slot count lives on the device
     } else {
         if (q.count <= 0) return cudaSuccess;
-        const long long nblk = (q.count + kStenThreads - 1) / kStenThreads;
+        const int G = (MODE == MODE_GRID) ? q.T / NT : 1;
+        const long long nitems = q.count * items_per_slot(MODE, G);
+        const long long nblk = (nitems + kThreads64 - 1) / kThreads64;
         long long nsplit = 1;
         if (nblk < q.target_items) {
             nsplit = (q.target_items + nblk - 1) / nblk;
             if (nsplit > q.bd.nchunks) nsplit = q.bd.nchunks;
         }
-        grid = nblk * nsplit;
+        grid = nblk * nsplit;   // one work item per CTA: the hardware balances them
         if (grid > 0x7fffffffLL) return cudaErrorInvalidValue;
     }
-    interact_kernel<MODE_STENCIL, kStencil, kStenThreads, kStenMinB><<<(unsigned)grid, kStenThreads, 0, st>>>(q);
+    interact64_kernel<MODE, NT, kThreads64, kMinB64, UNR><<<(unsigned)grid, kThreads64, 0, st>>>(q);
     return cudaGetLastError();
+}
+
+cudaError_t launch_interact_eval(const InteractParams& p, int sm_count, cudaStream_t st) {
+    return launch64<MODE_EVAL, 1, 2>(p, sm_count, 8, st);
+}
+
+cudaError_t launch_interact_stencil(const InteractParams& p, int sm_count, cudaStream_t st) {
+    return launch64<MODE_STENCIL, 1, 2>(p, sm_count, 16, st);
+}
+
+cudaError_t launch_interact_grid(const InteractParams& p, int sm_count, cudaStream_t st) {
+    if (p.T < 2) return cudaErrorInvalidValue;
+    if (p.T % 4 == 0) return launch64<MODE_GRID, 4, 1>(p, sm_count, 16, st);
+    if (p.T % 2 == 0) return launch64<MODE_GRID, 2, 2>(p, sm_count, 16, st);
+    return launch64<MODE_GRID, 1, 2>(p, sm_count, 16, st);
 }
 
 // ------------------------------------------------------------------ fp32 eval kernel ------

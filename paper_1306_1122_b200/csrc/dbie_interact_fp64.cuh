@@ -1,0 +1,184 @@
+// dbie_interact_fp64.cuh — the fp64 M x N point-pixel interaction kernel.
+//
+//   S_p(i) = sum_k [theta sin theta + cos theta]/r^3 * B_p0[k],  theta = |lambda_p| r
+//   (Eq. 6, Eq. 16; the prefactor z h^2/2pi is applied by the
+//   consumer of the chunk sums).
+//
+// Mapping (the inverse of the paper's, which strides the PIXELS of one point
+// over 80x128 threads): a thread owns ONE evaluation position (a field point, or one of the 4
+// stencil positions of Eq. 13) and NT lambda triples that share its geometry (NT = 1 except in
+// GRID mode).  The boundary is streamed through shared memory in 16 KB tiles by the TMA
+// bulk-copy engine (cp.async.bulk + mbarrier, double buffered) and every thread of the CTA reads
+// the same pixel record as a broadcast LDS.128 pair.  One position per thread keeps the kernel
+// at <= 64 registers, i.e. 8 resident warps per scheduler: the round-1 profile of the 4-positions-
+// per-thread version (profiles/r01_ncu_full_interact_stencil_cfg2.md) showed the FP64 pipe at 67 %
+// with warps stalled on fixed-latency dependencies at 3.3 warps per scheduler.
+#pragma once
+#include <cuda_runtime.h>
+#include <stdint.h>
+
+#include "dbie_internal.h"
+#include "dbie_math.cuh"
+#include "dbie_tma.cuh"
+
+namespace dbie {
+
+enum { MODE_EVAL = 0, MODE_STENCIL = 1, MODE_GRID = 2 };
+
+// items (threads' units of work) per slot
+__host__ __device__ inline long long items_per_slot(int mode, int G) {
+    return mode == MODE_EVAL ? 1 : (mode == MODE_STENCIL ? kStencil : (long long)kStencil * G);
+}
+
+template <int MODE, int NT, int THREADS, int MINB, int UNR>
+__global__ void __launch_bounds__(THREADS, MINB) interact64_kernel(const __grid_constant__ InteractParams p) {
+    static_assert(MODE == MODE_GRID || NT == 1, "only GRID mode carries several lambda triples per thread");
+    __shared__ alignas(128) double4 tile[2][kTilePx];
+    __shared__ alignas(8) uint64_t full[2];
+
+    const int tid = threadIdx.x;
+    if (tid == 0) {
+        mbar_init(&full[0], 1);
+        mbar_init(&full[1], 1);
+        mbar_fence_init();
+    }
+    __syncthreads();
+
+    if (p.zero_ptr && blockIdx.x == 0 && tid == 0) *p.zero_ptr = 0u;  // next pass's list counter
+    const long long count = p.count_ptr ? (long long)(*p.count_ptr) : p.count;   // slots
+    const int G = (MODE == MODE_GRID) ? p.T / NT : 1;
+    const long long nitems = count * items_per_slot(MODE, G);
+    const long long nblk = (nitems + THREADS - 1) / THREADS;
+    if (nblk == 0) return;
+    const BoundaryView& bd = p.bd;
+    const int NCH = bd.nchunks;
+    int nsplit = 1;
+    if (nblk < p.target_items) {
+        nsplit = (int)((p.target_items + nblk - 1) / nblk);
+        if (nsplit > NCH) nsplit = NCH;
+    }
+    const long long nwork = nblk * nsplit;
+
+    unsigned it = 0;  // tiles consumed by this CTA so far: stage = it & 1, parity = (it >> 1) & 1
+    for (long long w = blockIdx.x; w < nwork; w += gridDim.x) {
+        const long long blk = w / nsplit;
+        const int sp = (int)(w % nsplit);
+        const int c0 = (int)(((long long)sp * NCH) / nsplit);
+        const int c1 = (int)(((long long)(sp + 1) * NCH) / nsplit);
+
+        // ---- this thread's evaluation position and lambda triples
+        const long long item = blk * THREADS + tid;
+        const bool live = item < nitems;
+        const long long jt = live ? item : nitems - 1;
+        long long slot;
+        int s = 0, g = 0;
+        if (MODE == MODE_EVAL) {
+            slot = jt;
+        } else if (MODE == MODE_STENCIL) {
+            slot = jt >> 2;
+            s = (int)(jt & 3);
+        } else {
+            g = (int)(jt % G);
+            const long long js = jt / G;
+            s = (int)(js & 3);
+            slot = js >> 2;
+        }
+        const long long id = (MODE == MODE_EVAL) ? p.slot0 + slot : (p.act ? (long long)p.act[slot] : slot);
+        double xi = p.x[id], yi = p.y[id], zi = p.z[id];
+        if (MODE != MODE_EVAL) {   // Eq. 13: r_i, r_i + delta x, + delta y, + delta z
+            if (s == 1) xi = __dadd_rn(xi, p.delta_abs);
+            if (s == 2) yi = __dadd_rn(yi, p.delta_abs);
+            if (s == 3) zi = __dadd_rn(zi, p.delta_abs);
+        }
+        const double z2 = zi * zi;
+        double lam[NT][3];
+        if (MODE == MODE_GRID) {
+            // trial t of component c: lo_c + W t/(T-1), each operation rounded separately (O-4)
+#pragma unroll
+            for (int c = 0; c < 3; ++c) {
+                const double lo = p.lo[c * p.ldlo + id];
+#pragma unroll
+                for (int tt = 0; tt < NT; ++tt) {
+                    const int t = g * NT + tt;
+                    lam[tt][c] = fabs(__dadd_rn(lo, __ddiv_rn(__dmul_rn(p.W, (double)t), (double)(p.T - 1))));
+                }
+            }
+        } else {
+#pragma unroll
+            for (int c = 0; c < 3; ++c) lam[0][c] = fabs(p.lam[c * p.ldlam + id]);
+        }
+
+        double acc[NT][3];
+#pragma unroll
+        for (int tt = 0; tt < NT; ++tt) acc[tt][0] = acc[tt][1] = acc[tt][2] = 0.0;
+
+        const int t0 = chunk_first_tile(bd, c0), t1 = chunk_first_tile(bd, c1);
+        int c = c0;
+        int t_chunk_end = chunk_first_tile(bd, c + 1);
+        if (tid == 0) {
+            const TileDesc d = tile_desc(bd, t0);
+            mbar_expect_tx(&full[it & 1], (unsigned)d.npx * 32u);
+            bulk_g2s(&tile[it & 1][0], bd.rec + d.px0, (unsigned)d.npx * 32u, &full[it & 1]);
+        }
+        for (int t = t0; t < t1; ++t, ++it) {
+            if (tid == 0 && t + 1 < t1) {  // prefetch the next tile into the other stage
+                const TileDesc dn = tile_desc(bd, t + 1);
+                const unsigned sn = (it + 1) & 1;
+                mbar_expect_tx(&full[sn], (unsigned)dn.npx * 32u);
+                bulk_g2s(&tile[sn][0], bd.rec + dn.px0, (unsigned)dn.npx * 32u, &full[sn]);
+            }
+            const TileDesc d = tile_desc(bd, t);
+            mbar_wait(&full[it & 1], (it >> 1) & 1);
+            const double4* __restrict__ rp = &tile[it & 1][0];
+            for (int row = 0; row < d.nrows; ++row) {
+                const double yk = __ldg(bd.yk + d.row0 + row);
+                const double dy = yk - yi;
+                const double cc = fma(dy, dy, z2);
+#pragma unroll UNR
+                for (int j = 0; j < d.ncols; ++j) {
+                    const double4 px = rp[j];  // {x_k, Bx0, By0, Bz0}: two broadcast LDS.128
+                    const double dx = px.x - xi;
+                    const double r2 = fma(dx, dx, cc);
+                    const double y = rsqrt_full(r2);   // 1/r
+                    const double rr = r2 * y;          // r
+                    const double wgt = (y * y) * y;    // 1/r^3
+                    const double wx = wgt * px.y, wy = wgt * px.z, wz = wgt * px.w;
+#pragma unroll
+                    for (int tt = 0; tt < NT; ++tt) {
+                        acc[tt][0] = fma(kernel_n(lam[tt][0] * rr), wx, acc[tt][0]);
+                        acc[tt][1] = fma(kernel_n(lam[tt][1] * rr), wy, acc[tt][1]);
+                        acc[tt][2] = fma(kernel_n(lam[tt][2] * rr), wz, acc[tt][2]);
+                    }
+                }
+                rp += d.ncols;
+            }
+            if (t + 1 == t_chunk_end) {  // A4: one partial sum per chunk, added in chunk order later
+                if (live) {
+                    if (MODE == MODE_EVAL) {
+#pragma unroll
+                        for (int q = 0; q < 3; ++q) p.part[((long long)c * 3 + q) * p.cap + slot] = acc[0][q];
+                    } else if (MODE == MODE_STENCIL) {
+#pragma unroll
+                        for (int q = 0; q < 3; ++q)
+                            p.part[((long long)c * 12 + s * 3 + q) * p.cap + slot] = acc[0][q];
+                    } else {
+                        const long long Q = 12LL * p.T;
+#pragma unroll
+                        for (int tt = 0; tt < NT; ++tt)
+#pragma unroll
+                            for (int q = 0; q < 3; ++q)
+                                p.part[(c * Q + (long long)(s * 3 + q) * p.T + g * NT + tt) * p.cap + slot] =
+                                    acc[tt][q];
+                    }
+                }
+#pragma unroll
+                for (int tt = 0; tt < NT; ++tt) acc[tt][0] = acc[tt][1] = acc[tt][2] = 0.0;
+                ++c;
+                t_chunk_end = chunk_first_tile(bd, c + 1);
+            }
+            __syncthreads();  // everyone is done with stage it&1 before it is refilled
+        }
+    }
+}
+
+}  // namespace dbie

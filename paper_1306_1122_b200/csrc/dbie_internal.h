@@ -80,6 +80,11 @@ struct InteractParams {
     long long cap;
     int target_items;            // split the pixel range until there are this many work items
     unsigned* zero_ptr;          // set to 0 by the launch (the next pass's list counter), or nullptr
+    // MODE_GRID (O-4): trial t of component c at point id is lo[c*ldlo + id] + W t/(T-1)
+    const double* lo;
+    long long ldlo;
+    double W;
+    int T;
 };
 
 // One launch of the fp32 eval kernel (dbie_eval_f32): slot i = evaluation point slot0 + i.
@@ -106,12 +111,30 @@ struct SolveArrays {            // per-point optimiser state, structure-of-array
     unsigned* nact;             // [2] device counters
 };
 
+struct GridArrays {             // per-point GRID state (O-4), structure-of-arrays by point id
+    double* lo;                 // [3][cap]  lower end of the current window per component
+    double* inc;                // [12][cap] B at the 4 stencil positions for the incumbent, [s*3+p]
+    double* il;                 // [3][cap]  incumbent lambda
+    long long cap;
+    int* act[2];                // active lists (ping-pong)
+    unsigned* nact;             // [2] device counters
+};
+
+struct GridConsts {
+    int T, n_level;
+    double W, Wn;               // this level's window width and the next one, 2 W/(T-1)
+    double Lmax;                // lam_max / h
+};
+
+constexpr int kGridMaxTrials = 32;
+
 // launchers (defined in the .cu files; all asynchronous on `st`)
 cudaError_t launch_stage_boundary(int nx, int ny, double h, double x0, double y0, const double* bx,
                                   const double* by, const double* bz, double4* rec, double* yk,
                                   float4* rec32, float* yk32, cudaStream_t st);
 cudaError_t launch_interact_eval(const InteractParams& p, int sm_count, cudaStream_t st);
 cudaError_t launch_interact_stencil(const InteractParams& p, int sm_count, cudaStream_t st);
+cudaError_t launch_interact_grid(const InteractParams& p, int sm_count, cudaStream_t st);
 cudaError_t launch_eval_finalize(const BoundaryView& bd, long long slot0, long long count,
                                  long long M, const double* z, const double* lam, const double* part,
                                  long long cap, double* B, cudaStream_t st);
@@ -131,5 +154,13 @@ cudaError_t launch_solve_step(const SolveArrays& s, const NMConsts& k, const Bou
 cudaError_t launch_residual_finalize(const BoundaryView& bd, const NMConsts& k, long long M,
                                      long long ldo, const double* z, const double* part, long long cap,
                                      double* out, double* phi, cudaStream_t st);
+
+cudaError_t launch_grid_init(const GridArrays& s, long long M, long long ldo, const double* x, const double* y,
+                             const double* z, double* B, double* lam, double* resid, int* iters, int* status,
+                             cudaStream_t st);
+cudaError_t launch_grid_step(const GridArrays& s, const NMConsts& k, const GridConsts& gc, const BoundaryView& bd,
+                             int lev, long long M, long long ldo, const double* z, const double* part,
+                             long long cap, double* B, double* lam, double* resid, int* iters, int* status,
+                             unsigned long long* nevals, cudaStream_t st);
 
 }  // namespace dbie

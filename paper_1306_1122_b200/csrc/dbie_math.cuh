@@ -20,6 +20,21 @@
 
 namespace dbie {
 
+// On the device the polynomial / reduction constants are read as constant-bank operands of the
+// FP64 instructions (DFMA R, R, R, c[3][..]): as 64-bit literals the compiler re-materialises
+// them with ~47 UMOV / IMAD.MOV per inner-loop trip (profiles/r01_ncu_full_interact_stencil_cfg2.md).
+#if defined(__CUDACC__)
+static __constant__ double kTrigC[16] = {
+    DBIE_SIN_S0, DBIE_SIN_S1, DBIE_SIN_S2, DBIE_SIN_S3, DBIE_SIN_S4, DBIE_SIN_S5,
+    DBIE_COS_C0, DBIE_COS_C1, DBIE_COS_C2, DBIE_COS_C3, DBIE_COS_C4, DBIE_COS_C5,
+    DBIE_TWO_OVER_PI, DBIE_PIO2_HI, DBIE_PIO2_LO, DBIE_ROUND_MAGIC};
+#endif
+#if defined(__CUDA_ARCH__) && !defined(DBIE_COEF_IMMEDIATE)
+#define DBIE_K(i, name) ::dbie::kTrigC[i]
+#else
+#define DBIE_K(i, name) (name)
+#endif
+
 DBIE_HD int lo32(double v) {
 #if defined(__CUDA_ARCH__)
     return __double2loint(v);
@@ -68,48 +83,50 @@ DBIE_HD double rsqrt_full(double a) {
 // sin and cos of the REDUCED argument t, |t| <= pi/4 (1.0005 slack): 14 FP64 instructions.
 DBIE_HD void sincos_reduced(double t, double& sn, double& cs) {
     const double u = t * t;
-    double s = DBIE_SIN_S5;
-    s = fma(s, u, DBIE_SIN_S4);
-    s = fma(s, u, DBIE_SIN_S3);
-    s = fma(s, u, DBIE_SIN_S2);
-    s = fma(s, u, DBIE_SIN_S1);
-    s = fma(s, u, DBIE_SIN_S0);
-    double c = DBIE_COS_C5;
-    c = fma(c, u, DBIE_COS_C4);
-    c = fma(c, u, DBIE_COS_C3);
-    c = fma(c, u, DBIE_COS_C2);
-    c = fma(c, u, DBIE_COS_C1);
-    c = fma(c, u, DBIE_COS_C0);
+    double s = DBIE_K(5, DBIE_SIN_S5);
+    s = fma(s, u, DBIE_K(4, DBIE_SIN_S4));
+    s = fma(s, u, DBIE_K(3, DBIE_SIN_S3));
+    s = fma(s, u, DBIE_K(2, DBIE_SIN_S2));
+    s = fma(s, u, DBIE_K(1, DBIE_SIN_S1));
+    s = fma(s, u, DBIE_K(0, DBIE_SIN_S0));
+    double c = DBIE_K(11, DBIE_COS_C5);
+    c = fma(c, u, DBIE_K(10, DBIE_COS_C4));
+    c = fma(c, u, DBIE_K(9, DBIE_COS_C3));
+    c = fma(c, u, DBIE_K(8, DBIE_COS_C2));
+    c = fma(c, u, DBIE_K(7, DBIE_COS_C1));
+    c = fma(c, u, DBIE_K(6, DBIE_COS_C0));
     const double tu = t * u;
     sn = fma(tu, s, t);
     cs = fma(u, c, 1.0);
 }
 
-// Reduction theta = k pi/2 + t for 0 <= theta < 2^20 (two-term Cody-Waite; with an FMA the
-// first step is exact while k < 2^20).  4 FP64 instructions; the
-// quadrant is read from the low word of the magic-number sum, so no FP64<->int conversion.
+// Reduction theta = k pi/2 + t for 0 <= theta < 2^20.  One Cody-Waite step with the double
+// nearest to pi/2: the FMA forms theta - k*PIO2_HI exactly and rounds once.  The neglected tail
+// k*(pi/2 - PIO2_HI) = theta * 3.9e-17 is the same as evaluating sin/cos at theta (1 + 3.9e-17):
+// a perturbation that is smooth in theta (no jump at quadrant boundaries) and below the
+// half-ulp rounding (1.1e-16 theta) that theta = |lambda| r already carries.  3 FP64 instructions;
+// the quadrant is read from the low word of the magic-number sum, so no FP64<->int conversion.
 DBIE_HD double reduce_pio2(double th, int& q) {
-    const double kf = fma(th, DBIE_TWO_OVER_PI, DBIE_ROUND_MAGIC);
+    const double kf = fma(th, DBIE_K(12, DBIE_TWO_OVER_PI), DBIE_ROUND_MAGIC);
     q = lo32(kf);
     const double kd = kf - DBIE_ROUND_MAGIC;
-    double t = fma(-kd, DBIE_PIO2_HI, th);
-    t = fma(-kd, DBIE_PIO2_LO, t);
-    return t;
+    return fma(-kd, DBIE_K(13, DBIE_PIO2_HI), th);
 }
 
 // n(theta) = theta sin(theta) + cos(theta), theta >= 0 (Eq. 6 numerator).
-// 19 FP64 instructions.
+// 19 FP64 instructions.  Quadrant q&3: (sin, cos)(theta) = (sn,cs), (cs,-sn), (-sn,-cs), (-cs,sn),
+// so n = +-(theta sn + cs) for even q and +-(theta cs - sn) for odd q.  Both forms are evaluated
+// and one is selected: measured on B200, the extra DFMA is cheaper than swapping the two 64-bit
+// operands first (2 FSEL + 1 LOP3 fewer per component; the non-FP64 instructions compete with the
+// FP64 pipe for issue slots, profiles/r01_variants.md).
 DBIE_HD double kernel_n(double th) {
     int q;
     const double t = reduce_pio2(th, q);
     double sn, cs;
     sincos_reduced(t, sn, cs);
-    // quadrant q&3: sin(theta), cos(theta) = (sn,cs), (cs,-sn), (-sn,-cs), (-cs,sn).
-    // Selects and sign flips are integer-pipe work (FSEL/LOP3), not FP64-pipe instructions.
-    const bool odd = (q & 1) != 0;
-    const double a = odd ? cs : sn;
-    const double b = flip_sign_if(odd ? sn : cs, q << 31);
-    const double n = fma(th, a, b);
+    const double ne = fma(th, sn, cs);
+    const double no = fma(th, cs, -sn);
+    const double n = (q & 1) ? no : ne;
     return flip_sign_if(n, (q << 30) & (int)0x80000000);
 }
 

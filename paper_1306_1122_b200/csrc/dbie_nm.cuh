@@ -55,18 +55,16 @@ DBIE_NM_HD double norm3_(double a, double b, double c) {
     return sqrt_(add_(add_(mul_(a, a), mul_(b, b)), mul_(c, c)));
 }
 
-// B at the four stencil positions -> f, g, J, div, Phi.  Bs[s][p], s: 0 = r_i, 1 = +delta x,
-// 2 = +delta y, 3 = +delta z, all with the same lambda triple (Eq. 13).
-DBIE_NM_HD Residual residual_from_stencil(const double Bs[4][3], const NMConsts& k) {
+// Gradient G[p][j] = dB_p/dx_j (Eq. 13 forward differences) and B at r_i -> J (Eq. 14), div B,
+// f (Eq. 8), g (Eq. 9), Phi.  Split from the differencing so that GRID mode can form each
+// component's three differences once per trial value (they depend on lambda_p only).
+DBIE_NM_HD Residual residual_from_gradient(const double G[3][3], const double B0[3], const NMConsts& k) {
     Residual r;
-    double G[3][3];  // G[p][j] = dB_p/dx_j
-    for (int p = 0; p < 3; ++p)
-        for (int j = 0; j < 3; ++j) G[p][j] = div_(sub_(Bs[j + 1][p], Bs[0][p]), k.delta_abs);
     r.J[0] = sub_(G[2][1], G[1][2]);
     r.J[1] = sub_(G[0][2], G[2][0]);
     r.J[2] = sub_(G[1][0], G[0][1]);
     r.div = add_(add_(G[0][0], G[1][1]), G[2][2]);
-    for (int p = 0; p < 3; ++p) r.B[p] = Bs[0][p];
+    for (int p = 0; p < 3; ++p) r.B[p] = B0[p];
     const double nB = norm3_(r.B[0], r.B[1], r.B[2]);
     const double nJ = norm3_(r.J[0], r.J[1], r.J[2]);
     const double cx = sub_(mul_(r.J[1], r.B[2]), mul_(r.J[2], r.B[1]));
@@ -81,6 +79,15 @@ DBIE_NM_HD Residual residual_from_stencil(const double Bs[4][3], const NMConsts&
     r.g = div_(mul_(fabs(r.div), div_(k.d_abs, 6.0)), nB);               // Eq. 9, dV/dsigma = d/6
     r.phi = add_(r.f, mul_(k.w_g, r.g));
     return r;
+}
+
+// B at the four stencil positions -> f, g, J, div, Phi.  Bs[s][p], s: 0 = r_i, 1 = +delta x,
+// 2 = +delta y, 3 = +delta z, all with the same lambda triple (Eq. 13).
+DBIE_NM_HD Residual residual_from_stencil(const double Bs[4][3], const NMConsts& k) {
+    double G[3][3];  // G[p][j] = dB_p/dx_j
+    for (int p = 0; p < 3; ++p)
+        for (int j = 0; j < 3; ++j) G[p][j] = div_(sub_(Bs[j + 1][p], Bs[0][p]), k.delta_abs);
+    return residual_from_gradient(G, Bs[0], k);
 }
 
 // raw sums S[s*3+p] (Eq. 16 without the prefactor) -> B at the stencil -> residual
