@@ -1,7 +1,8 @@
 #!/usr/bin/env python
 """bench.py — throughput of the DBIE hot path on B200 (one process per GPU).
 
-    python bench.py [--gpus N] [--steps K] [--warmup W] [--impl ours|reference] [--workload cfg2|cfg3|cfg4]
+    python bench.py [--gpus N] [--steps K] [--warmup W] [--impl ours|reference]
+                    [--workload cfg2|cfg3|cfg4|cfg5] [--method nm|grid] [--points P]
 
 A "step" is one pass of the whole hot path over one batch of synthetic input:
 stage the boundary (dbie_create) and run the full per-point lambda solve (dbie_solve) on the
@@ -31,16 +32,24 @@ sys.path.insert(0, ROOT)
 
 METRIC = "point-pixel DBIE interactions/sec (fp64)"
 UNIT = "interactions/s"
-FP64_INSTR_PER_INTERACTION = 76      # DESIGN.md section 6 (SASS inner loop: 302 per 4 stencil points)
+FP64_INSTR_PER_INTERACTION = 76      # DESIGN.md section 6 (SASS inner loop: 152 per 2 pixels of one position)
+FP64_INSTR_GRID = {4: 265 / 4, 2: 139 / 2, 1: 76}   # GRID: 13 + 63 NT per NT trial triples sharing a geometry
 FP64_INSTR_SURVEY = 82               # SURVEY.md 8(d) canonical count
 SM_COUNT, FP64_LANES_PER_SM = 148, 64   # B200: 148 SMs, 64 FP64 lanes per SM per clock
 
 
-def make_workload(name: str, rank: int = 0, world: int = 1):
+def make_workload(name: str, rank: int = 0, world: int = 1, points: int = 0):
     """The rank's batch.  Weak scaling: every rank solves a volume of the same size; rank r's
-    layers are shifted by r*h/world in z so the ranks' point sets are disjoint."""
+    layers are shifted by r*h/world in z so the ranks' point sets are disjoint.  `points` > 0
+    takes a seeded subset of the volume (cfg5 defaults to 16,384 points: the full 8.4e6-point
+    GRID solve is 8.8e12 x 4 x 8 x 10 interactions, hours at the FP64 roofline)."""
     import workloads
-    wl = {"cfg2": workloads.config2, "cfg3": workloads.config3, "cfg4": workloads.config4}[name]()
+    wl = {"cfg2": workloads.config2, "cfg3": workloads.config3, "cfg4": workloads.config4,
+          "cfg5": workloads.config5}[name]()
+    if points <= 0 and name == "cfg5":
+        points = 16384
+    if 0 < points < wl.M:
+        wl, _ = wl.seeded_subset(points, seed_offset=900)
     if world > 1:
         wl.z = wl.z + rank * wl.h / world
     return wl
@@ -53,14 +62,8 @@ def shard_info(M: int, rank: int, world: int) -> dict:
 
 def reduce_over_ranks(dist, device, ms: float, interactions: float):
     """max over ranks of the time, sum over ranks of the work (the contract's aggregate)."""
-    import torch
-    if dist is None or not dist.is_initialized() or dist.get_world_size() == 1:
-        return ms, interactions
-    t = torch.tensor([ms], dtype=torch.float64, device=device)
-    w = torch.tensor([interactions], dtype=torch.float64, device=device)
-    dist.all_reduce(t, op=dist.ReduceOp.MAX)
-    dist.all_reduce(w, op=dist.ReduceOp.SUM)
-    return float(t.item()), float(w.item())
+    from paper_1306_1122_b200 import sharding
+    return sharding.reduce_over_ranks(dist, device, ms, interactions)
 
 
 class ClockSampler:
@@ -108,13 +111,20 @@ class ClockSampler:
                 "samples": len(sm), "reasons": sorted(reasons)}
 
 
+METHOD = {"grid": False}     # set by main(): GRID (O-4) instead of Nelder-Mead
+
+
 # --------------------------------------------------------------------------- oracle legs ---
 def oracle_timed(wl, npoints: int, seed_offset: int, nthreads: int = 0) -> dict:
     """Time the oracle's solve (or eval) on a seeded sample of the workload's points."""
     import oracle
     sub, _ = wl.seeded_subset(npoints, seed_offset=seed_offset)
     t0 = time.perf_counter()
-    if wl.lam is None:
+    if wl.lam is None and METHOD["grid"]:
+        o = oracle.Opts(method=1)
+        out = oracle.solve_grid(sub, o, nthreads=nthreads)
+        inter = float(out["iters"].sum()) * o.n_trial * 4.0 * wl.N
+    elif wl.lam is None:
         out = oracle.solve_nm(sub, nthreads=nthreads)
         inter = float(out["nfev"].sum()) * 4.0 * wl.N
     else:
@@ -133,7 +143,7 @@ def cpu_baseline(wl, target_s: float = 15.0) -> dict:
     n = int(min(wl.M, max(8 * cores, target_s / max(per_point, 1e-9))))
     n = min(n, 65536)
     r = oracle_timed(wl, n, seed_offset=51)
-    kind = "solve_nm" if wl.lam is None else "eval"
+    kind = ("solve_grid" if METHOD["grid"] else "solve_nm") if wl.lam is None else "eval"
     return {"value": r["interactions"] / r["seconds"], "unit": UNIT, "cores": cores, "kind": "oracle",
             "sample": f"oracle.{kind} on {r['points']} seeded points of {wl.name} "
                       f"({r['interactions']:.3e} interactions in {r['seconds']:.1f} s)"}
@@ -145,7 +155,7 @@ def run_reference(args) -> None:
     if rank != 0:
         return
     import oracle
-    wl = make_workload(args.workload)
+    wl = make_workload(args.workload, points=args.points)
     cores = oracle.max_threads()
     probe = oracle_timed(wl, min(wl.M, 4 * cores), seed_offset=60)
     per_point = probe["seconds"] / probe["points"]
@@ -175,7 +185,11 @@ def workload_config(wl, name, n_points_per_step=None) -> dict:
     desc = {"cfg2": "BASELINE configs[1]: Low&Lou n=1 m=1 l=0.3 Phi=pi/4, boundary 64x64 on [-1,1]^2, "
                     "full per-point NM lambda solve on the 64x64x32 volume",
             "cfg3": "BASELINE configs[2]: synthetic bipolar AR 256x256 at 0.5 Mm/px, NM solve on 128x128x64",
-            "cfg4": "BASELINE configs[3]: eval at fixed lambda, boundary 512x512, M=1,048,576 random points"}[name]
+            "cfg4": "BASELINE configs[3]: eval at fixed lambda, boundary 512x512, M=1,048,576 random points",
+            "cfg5": "BASELINE configs[4]: quadrupolar delta-spot 1024x1024, lambda solve on a seeded subset of "
+                    "the 256x256x128 volume"}[name]
+    if wl.lam is None:
+        desc += " [method: " + ("GRID T=8, 10 levels" if METHOD["grid"] else "Nelder-Mead") + "]"
     return {"workload": desc, "boundary": [wl.nx, wl.ny], "points": wl.M if n_points_per_step is None
             else n_points_per_step, "step": "dbie_create + dbie_solve" if wl.lam is None else "dbie_create + dbie_eval",
             "l2": "flushed between timed steps (256 MiB write)"}
@@ -199,8 +213,9 @@ def run_ours(args) -> None:
     dev = torch.device("cuda", local)
     dbie.load()
 
-    wl = make_workload(args.workload, rank, world)
+    wl = make_workload(args.workload, rank, world, points=args.points)
     is_solve = wl.lam is None
+    sopts = dbie.default_opts(method=1) if METHOD["grid"] else None
     t = lambda a: torch.from_numpy(np.ascontiguousarray(a, dtype=np.float64)).to(dev)
     d_bx, d_by, d_bz = t(wl.bx), t(wl.by), t(wl.bz)
     d_x, d_y, d_z = t(wl.x), t(wl.y), t(wl.z)
@@ -216,12 +231,12 @@ def run_ours(args) -> None:
         ctx = dbie.DBIE(wl.nx, wl.ny, wl.h, wl.x0, wl.y0, d_bx, d_by, d_bz)
         if profile:
             ctx.profile(True)
-        out = ctx.solve(d_x, d_y, d_z) if is_solve else ctx.eval(d_x, d_y, d_z, d_lam)
+        out = ctx.solve(d_x, d_y, d_z, sopts) if is_solve else ctx.eval(d_x, d_y, d_z, d_lam)
         return ctx, out
 
     def step_host():
         ctx = dbie.DBIE(wl.nx, wl.ny, wl.h, wl.x0, wl.y0, wl.bx, wl.by, wl.bz)
-        out = ctx.solve_host(wl.x, wl.y, wl.z) if is_solve else ctx.eval_host(wl.x, wl.y, wl.z, wl.lam)
+        out = ctx.solve_host(wl.x, wl.y, wl.z, sopts) if is_solve else ctx.eval_host(wl.x, wl.y, wl.z, wl.lam)
         return ctx, out
 
     # ---- warm-up
@@ -290,22 +305,24 @@ def run_ours(args) -> None:
     sm_max = (clocks or {}).get("sm_max_mhz") or 1965.0
     peak_slots = SM_COUNT * FP64_LANES_PER_SM * sm_max * 1e6          # FP64 lane-instructions / s
     kern_ips = inter_total / (kern_ms * 1e-3) if kern_ms > 0 else 0.0
-    achieved_slots = kern_ips * FP64_INSTR_PER_INTERACTION
+    per_inter = FP64_INSTR_GRID[4] if (is_solve and METHOD["grid"]) else FP64_INSTR_PER_INTERACTION
+    achieved_slots = kern_ips * per_inter
     roofline = {
-        "bound": "alu", "kernel": "dbie::interact_kernel (fp64 point-pixel sums)",
+        "bound": "alu", "kernel": "dbie::interact64_kernel (fp64 point-pixel sums)",
         "achieved": 2e-12 * achieved_slots, "peak": 2e-12 * peak_slots, "unit": "TFLOP/s",
         "frac": achieved_slots / peak_slots, "traffic": None,
-        "note": "FP64-pipe bound (no HBM/tensor step): achieved = interactions/s of the kernel x 76 FP64 "
-                "lane-instructions per interaction (DESIGN.md s6) x 2 flop per FMA slot; peak = 148 SM x 64 "
-                "FP64 lanes x clocks.max.sm (derived, DESIGN.md s7)",
+        "note": "FP64-pipe bound (no HBM/tensor step): achieved = interactions/s of the kernel x FP64 "
+                "lane-instructions per interaction (76; GRID with 4 trial triples per geometry 66.25; DESIGN.md s6) "
+                "x 2 flop per FMA slot; peak = 148 SM x 64 FP64 lanes x clocks.max.sm (derived, DESIGN.md s7)",
         "kernel_interactions_per_s": kern_ips, "kernel_ms_per_launch": kern_ms / max(kern_launches, 1),
         "kernel_launches": kern_launches, "kernel_share_of_step": kern_ms / ms_total if ms_total else None,
-        "fp64_instr_per_interaction": FP64_INSTR_PER_INTERACTION,
+        "fp64_instr_per_interaction": per_inter,
         "frac_survey82": kern_ips * FP64_INSTR_SURVEY / peak_slots,
         "peak_measured_dfma_per_s": dfma_meas, "peak_measured_ffma_per_s": ffma_meas,
         "frac_of_measured_dfma": (achieved_slots / dfma_meas) if dfma_meas else None,
     }
-    base = cpu_baseline(make_workload(args.workload), target_s=args.cpu_seconds) if args.cpu_seconds > 0 else None
+    base = (cpu_baseline(make_workload(args.workload, points=args.points), target_s=args.cpu_seconds)
+            if args.cpu_seconds > 0 else None)
 
     line = {
         "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": args.steps,
@@ -334,10 +351,15 @@ def main():
     ap.add_argument("--steps", type=int, default=3)
     ap.add_argument("--warmup", type=int, default=3)
     ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
-    ap.add_argument("--workload", default="cfg2", choices=["cfg2", "cfg3", "cfg4"])
+    ap.add_argument("--workload", default="cfg2", choices=["cfg2", "cfg3", "cfg4", "cfg5"])
+    ap.add_argument("--method", default=None, choices=["nm", "grid"],
+                    help="lambda search of the solve workloads (default: nm; cfg5: grid)")
+    ap.add_argument("--points", type=int, default=0,
+                    help="solve/eval a seeded subset of this many points (0: the whole volume; cfg5: 16384)")
     ap.add_argument("--cpu-seconds", type=float, default=15.0,
                     help="target CPU time of the cpu_baseline leg (0 disables it)")
     args = ap.parse_args()
+    METHOD["grid"] = (args.method == "grid") or (args.method is None and args.workload == "cfg5")
     if args.impl == "reference":
         run_reference(args)
     else:
