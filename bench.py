@@ -135,14 +135,16 @@ def oracle_timed(wl, npoints: int, seed_offset: int, nthreads: int = 0) -> dict:
 
 
 def cpu_baseline(wl, target_s: float = 15.0) -> dict:
-    """Oracle as it stands on the host cores: a probe sample sizes a ~target_s sample."""
+    """Oracle as it stands on the host cores: a one-point-per-core probe sizes a ~target_s sample
+    (the probe itself is the sample when it already took that long, e.g. the config-5 GRID solve
+    at ~15 s per point and core)."""
     import oracle
     cores = oracle.max_threads()
-    probe = oracle_timed(wl, min(wl.M, 8 * cores), seed_offset=50)
-    per_point = probe["seconds"] / max(probe["points"], 1)
-    n = int(min(wl.M, max(8 * cores, target_s / max(per_point, 1e-9))))
-    n = min(n, 65536)
-    r = oracle_timed(wl, n, seed_offset=51)
+    r = oracle_timed(wl, min(wl.M, cores), seed_offset=50)
+    if r["seconds"] < 0.5 * target_s:
+        per_point = r["seconds"] / max(r["points"], 1)
+        n = int(min(wl.M, 65536, max(cores, target_s / max(per_point, 1e-9))))
+        r = oracle_timed(wl, n, seed_offset=51)
     kind = ("solve_grid" if METHOD["grid"] else "solve_nm") if wl.lam is None else "eval"
     return {"value": r["interactions"] / r["seconds"], "unit": UNIT, "cores": cores, "kind": "oracle",
             "sample": f"oracle.{kind} on {r['points']} seeded points of {wl.name} "
@@ -157,7 +159,7 @@ def run_reference(args) -> None:
     import oracle
     wl = make_workload(args.workload, points=args.points)
     cores = oracle.max_threads()
-    probe = oracle_timed(wl, min(wl.M, 4 * cores), seed_offset=60)
+    probe = oracle_timed(wl, min(wl.M, cores), seed_offset=60)
     per_point = probe["seconds"] / probe["points"]
     budget = 150.0 / max(args.steps + args.warmup, 1)            # whole run within a few minutes
     n = int(min(wl.M, max(cores, min(budget, 20.0) / per_point)))
@@ -345,6 +347,94 @@ def run_ours(args) -> None:
         dist.destroy_process_group()
 
 
+# --------------------------------------------------------------------------- fp32 leg ------
+FP32_INSTR_PER_INTERACTION = 56      # FFMA/FMUL/FADD per interaction (SASS: 448 per 8 interactions)
+FP32_LANES_PER_SM = 128
+
+
+def run_ours_f32(args) -> None:
+    """BASELINE configs[3] "fp64 and fp32": dbie_eval_f32 on the config-4 workload (N = 1 only).
+    Same JSON contract; the roofline is the FP32 FMA pipe (polynomial sincos, mask 0)."""
+    import torch
+    import paper_1306_1122_b200 as dbie
+    if not torch.cuda.is_available():
+        raise SystemExit("bench.py: no CUDA device (the CUDA path has no CPU fallback)")
+    dev = torch.device("cuda", 0)
+    torch.cuda.set_device(dev)
+    dbie.load()
+    wl = make_workload("cfg4", points=args.points)
+    t64 = lambda a: torch.from_numpy(np.ascontiguousarray(a, dtype=np.float64)).to(dev)
+    h32 = lambda a: torch.from_numpy(np.ascontiguousarray(a, dtype=np.float32)).pin_memory()
+    d_bx, d_by, d_bz = t64(wl.bx), t64(wl.by), t64(wl.bz)
+    hx, hy, hz, hl = h32(wl.x), h32(wl.y), h32(wl.z), h32(wl.lam)
+    dx, dy, dz, dl = hx.to(dev), hy.to(dev), hz.to(dev), hl.to(dev)
+    flush_buf = torch.empty(256 << 20, dtype=torch.uint8, device=dev)
+    inter = float(wl.M) * wl.N
+
+    def step(profile=False):
+        ctx = dbie.DBIE(wl.nx, wl.ny, wl.h, wl.x0, wl.y0, d_bx, d_by, d_bz, fp32=True)
+        if profile:
+            ctx.profile(True)
+        return ctx, ctx.eval_f32(dx, dy, dz, dl)
+
+    for _ in range(max(args.warmup, 0)):
+        ctx, _ = step(); torch.cuda.synchronize(); ctx.close()
+    sampler = ClockSampler(0)
+    torch.cuda.synchronize()
+    ms_total = kern_ms = 0.0
+    kern_launches = 0
+    for k in range(args.steps):
+        flush_buf.zero_()
+        e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+        e0.record()
+        ctx, out = step(profile=True)
+        e1.record(); e1.synchronize()
+        ms_total += e0.elapsed_time(e1)
+        kt = ctx.kernel_time()
+        kern_ms += kt["interact_ms"]; kern_launches += kt["interact_launches"]
+        ctx.close()
+    clocks = sampler.stop()
+    # e2e: pinned host float32 points in, float32 B back out, every step
+    hb = wl.bx, wl.by, wl.bz
+    t0 = time.perf_counter()
+    for k in range(args.steps):
+        ctx = dbie.DBIE(wl.nx, wl.ny, wl.h, wl.x0, wl.y0, *hb, fp32=True)
+        o = ctx.eval_f32(hx.to(dev, non_blocking=True), hy.to(dev, non_blocking=True),
+                         hz.to(dev, non_blocking=True), hl.to(dev, non_blocking=True)).cpu()
+        ctx.close()
+    e2e_ms = (time.perf_counter() - t0) * 1e3
+    try:
+        dfma_meas, ffma_meas = dbie.probe_dfma_rate(300.0)
+    except Exception:
+        dfma_meas = ffma_meas = None
+    sm_max = (clocks or {}).get("sm_max_mhz") or 1965.0
+    peak = SM_COUNT * FP32_LANES_PER_SM * sm_max * 1e6
+    kern_ips = inter * args.steps / (kern_ms * 1e-3) if kern_ms > 0 else 0.0
+    ach = kern_ips * FP32_INSTR_PER_INTERACTION
+    line = {
+        "metric": "point-pixel DBIE interactions/sec (fp32)", "value": inter * args.steps / (ms_total * 1e-3),
+        "unit": UNIT, "n_gpus": 1, "steps": args.steps, "warmup": args.warmup, "ms_per_step": ms_total / args.steps,
+        "higher_is_better": True, "scaling": "weak", "vs_baseline": None, "dtype": "f32", "data": "synthetic",
+        "config": dict(workload_config(wl, "cfg4"), step="dbie_create(DBIE_WITH_FP32) + dbie_eval_f32"),
+        "clocks": clocks,
+        "e2e": {"value": inter * args.steps / (e2e_ms * 1e-3), "unit": UNIT,
+                "h2d_bytes_per_step": 3 * wl.N * 8 + 6 * wl.M * 4, "d2h_bytes_per_step": 3 * wl.M * 4,
+                "ms_per_step": e2e_ms / args.steps, "api": "DBIE(host boundary, fp32=True) + eval_f32 on pinned host points"},
+        "gpu_launches": 3 * args.steps,
+        "roofline": {"bound": "alu", "kernel": "dbie::interact_f32_kernel (fp32 point-pixel sums, polynomial sincos)",
+                     "achieved": 2e-12 * ach, "peak": 2e-12 * peak, "unit": "TFLOP/s", "frac": ach / peak,
+                     "traffic": None, "fp32_instr_per_interaction": FP32_INSTR_PER_INTERACTION,
+                     "note": "FP32 FMA pipe: 148 SM x 128 lanes x clocks.max.sm; the kernel issues 82 instructions per "
+                             "interaction in total, so the issue port (148 x 4 x 32 lanes/clk) bounds it at 0.68 of this peak",
+                     "kernel_interactions_per_s": kern_ips, "kernel_ms_per_launch": kern_ms / max(kern_launches, 1),
+                     "kernel_launches": kern_launches, "kernel_share_of_step": kern_ms / ms_total if ms_total else None,
+                     "peak_measured_ffma_per_s": ffma_meas,
+                     "frac_of_measured_ffma": (ach / ffma_meas) if ffma_meas else None},
+        "cpu_baseline": None,
+    }
+    print(json.dumps(line), flush=True)
+
+
 def main():
     ap = argparse.ArgumentParser()
     ap.add_argument("--gpus", type=int, default=1)
@@ -354,6 +444,8 @@ def main():
     ap.add_argument("--workload", default="cfg2", choices=["cfg2", "cfg3", "cfg4", "cfg5"])
     ap.add_argument("--method", default=None, choices=["nm", "grid"],
                     help="lambda search of the solve workloads (default: nm; cfg5: grid)")
+    ap.add_argument("--dtype", default="f64", choices=["f64", "f32"],
+                    help="f32: the dbie_eval_f32 leg of BASELINE configs[3] (implies --workload cfg4, one GPU)")
     ap.add_argument("--points", type=int, default=0,
                     help="solve/eval a seeded subset of this many points (0: the whole volume; cfg5: 16384)")
     ap.add_argument("--cpu-seconds", type=float, default=15.0,
@@ -362,6 +454,9 @@ def main():
     METHOD["grid"] = (args.method == "grid") or (args.method is None and args.workload == "cfg5")
     if args.impl == "reference":
         run_reference(args)
+    elif args.dtype == "f32":
+        if int(os.environ.get("RANK", "0")) == 0:
+            run_ours_f32(args)
     else:
         if args.gpus > 1 and int(os.environ.get("WORLD_SIZE", "1")) == 1:
             # convenience: re-launch under torchrun, one rank per GPU

@@ -1,6 +1,6 @@
 """Build libdbie_b200.so (CUDA, sm_100a) and the host test shim, in-tree.
 
-    python -m paper_1306_1122_b200.build [--force]
+    python -m paper_1306_1122_b200.build [--force] [--tune]
 
 nvcc cross-compiles without a GPU.  The shared objects are git-ignored but travel to the GPU
 box with the gpurun snapshot.
@@ -73,6 +73,14 @@ def build_hostshim(force: bool = False) -> str:
     return SHIM
 
 
+def build_tune() -> str:
+    """Developer tool: shape sweep of the fp64 interaction kernel + FP64 issue-slot probe (dbie_tune)."""
+    exe = os.path.join(HERE, "dbie_tune")
+    subprocess.check_call([NVCC, *ARCH, "-O3", "-std=c++17", "-lineinfo", "-I", INCLUDE,
+                           os.path.join(CSRC, "tune_interact.cu"), "-o", exe])
+    return exe
+
+
 def build_all(force: bool = False, verbose: bool = False) -> None:
     build_lib(force, verbose)
     build_hostshim(force)
@@ -80,5 +88,7 @@ def build_all(force: bool = False, verbose: bool = False) -> None:
 
 if __name__ == "__main__":
     build_all(force="--force" in sys.argv, verbose="-v" in sys.argv)
+    if "--tune" in sys.argv:
+        print(build_tune())
     print(LIB)
     print(SHIM)

@@ -20,7 +20,7 @@ struct dbie_ctx {
     double* part;       size_t part_bytes;    // chunk partial sums
     char* state;        size_t state_bytes;   // optimiser state
     char* io;           size_t io_bytes;      // device staging of the _host entry points
-    unsigned* counters;                       // device: nact[2], pad[2], then nevals (u64) at +16 B
+    unsigned* counters;                       // device: nact[2], pad[2], nevals (u64) at +16 B, work[2] at +32 B
     cudaStream_t own_stream;
     double last_interactions;
     long long last_launches, last_evals;
@@ -432,7 +432,8 @@ static dbie_status solve_grid(dbie_ctx* ctx, long long M, const double* x, const
     prof_reset(ctx);
     for (long long off = 0; off < M; off += cap) {
         const long long cnt = (M - off < cap) ? (M - off) : cap;
-        CU(cudaMemsetAsync(ctx->counters, 0, 8, st));
+        CU(cudaMemsetAsync(ctx->counters, 0, 8, st));        // list counters
+        CU(cudaMemsetAsync(ctx->counters + 8, 0, 8, st));    // work-item counters
         CU(launch_grid_init(a, cnt, M, x + off, y + off, z + off, B + off, lam + off, resid + off, iters + off,
                             status + off, st));
         ++launches;
@@ -447,6 +448,8 @@ static dbie_status solve_grid(dbie_ctx* ctx, long long M, const double* x, const
             p.act = a.act[lev & 1];
             p.count_ptr = &a.nact[lev & 1];
             p.zero_ptr = &a.nact[(lev + 1) & 1];
+            p.work_ctr = ctx->counters + 8 + (lev & 1);
+            p.zero_work = ctx->counters + 8 + ((lev + 1) & 1);
             p.delta_abs = k.delta_abs;
             p.part = ctx->part; p.cap = cap;
             p.lo = a.lo; p.ldlo = cap; p.W = W; p.T = T;
@@ -505,7 +508,8 @@ extern "C" dbie_status dbie_solve(dbie_ctx* ctx, long long M, const double* x, c
     prof_reset(ctx);
     for (long long off = 0; off < M; off += cap) {
         const long long cnt = (M - off < cap) ? (M - off) : cap;
-        CU(cudaMemsetAsync(ctx->counters, 0, 8, st));
+        CU(cudaMemsetAsync(ctx->counters, 0, 8, st));        // list counters
+        CU(cudaMemsetAsync(ctx->counters + 8, 0, 8, st));    // work-item counters
         CU(launch_solve_init(a, k, cnt, M, x + off, y + off, z + off, B + off, lam + off, resid + off,
                              iters + off, status + off, st));
         ++launches;
@@ -518,6 +522,8 @@ extern "C" dbie_status dbie_solve(dbie_ctx* ctx, long long M, const double* x, c
             p.act = a.act[pass & 1];
             p.count_ptr = &a.nact[pass & 1];
             p.zero_ptr = &a.nact[(pass + 1) & 1];
+            p.work_ctr = ctx->counters + 8 + (pass & 1);
+            p.zero_work = ctx->counters + 8 + ((pass + 1) & 1);
             p.delta_abs = k.delta_abs;
             p.part = ctx->part; p.cap = cap;
             prof_mark(ctx, st);

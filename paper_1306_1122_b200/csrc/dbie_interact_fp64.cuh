@@ -9,10 +9,11 @@
 // stencil positions of Eq. 13) and NT lambda triples that share its geometry (NT = 1 except in
 // GRID mode).  The boundary is streamed through shared memory in 16 KB tiles by the TMA
 // bulk-copy engine (cp.async.bulk + mbarrier, double buffered) and every thread of the CTA reads
-// the same pixel record as a broadcast LDS.128 pair.  One position per thread keeps the kernel
-// at <= 64 registers, i.e. 8 resident warps per scheduler: the round-1 profile of the 4-positions-
-// per-thread version (profiles/r01_ncu_full_interact_stencil_cfg2.md) showed the FP64 pipe at 67 %
-// with warps stalled on fixed-latency dependencies at 3.3 warps per scheduler.
+// the same pixel record as a broadcast LDS.128 pair.  UNR pixels are in flight per thread.  The
+// round-1 profile of the first version (4 stencil positions per thread, 64-bit literals
+// re-materialised in the loop; profiles/r01_ncu_full_interact_stencil_cfg2.md) had the FP64 pipe at
+// 67 %; this one reaches 79 % (profiles/r01_ncu_full_interact64_stencil_cfg2.md), and the shape sweep
+// (csrc/tune_interact.cu, profiles/r01_variants.md) picks THREADS x MINB x UNR = 256 x 2 x 2.
 #pragma once
 #include <cuda_runtime.h>
 #include <stdint.h>
@@ -35,6 +36,7 @@ __global__ void __launch_bounds__(THREADS, MINB) interact64_kernel(const __grid_
     static_assert(MODE == MODE_GRID || NT == 1, "only GRID mode carries several lambda triples per thread");
     __shared__ alignas(128) double4 tile[2][kTilePx];
     __shared__ alignas(8) uint64_t full[2];
+    __shared__ long long next_item;
 
     const int tid = threadIdx.x;
     if (tid == 0) {
@@ -44,7 +46,10 @@ __global__ void __launch_bounds__(THREADS, MINB) interact64_kernel(const __grid_
     }
     __syncthreads();
 
-    if (p.zero_ptr && blockIdx.x == 0 && tid == 0) *p.zero_ptr = 0u;  // next pass's list counter
+    if (blockIdx.x == 0 && tid == 0) {
+        if (p.zero_ptr) *p.zero_ptr = 0u;    // next pass's list counter
+        if (p.zero_work) *p.zero_work = 0u;  // next pass's work counter
+    }
     const long long count = p.count_ptr ? (long long)(*p.count_ptr) : p.count;   // slots
     const int G = (MODE == MODE_GRID) ? p.T / NT : 1;
     const long long nitems = count * items_per_slot(MODE, G);
@@ -60,7 +65,16 @@ __global__ void __launch_bounds__(THREADS, MINB) interact64_kernel(const __grid_
     const long long nwork = nblk * nsplit;
 
     unsigned it = 0;  // tiles consumed by this CTA so far: stage = it & 1, parity = (it >> 1) & 1
-    for (long long w = blockIdx.x; w < nwork; w += gridDim.x) {
+    // Work items: one per CTA when the host knows the count (the hardware scheduler balances them);
+    // a persistent grid (count on the device) takes them from an atomic counter in index order,
+    // which balances the same way (static striding measured 1-15 % slower, profiles/r01_variants.md).
+    for (long long w = blockIdx.x;; w += gridDim.x) {
+        if (p.work_ctr) {
+            if (tid == 0) next_item = (long long)atomicAdd(p.work_ctr, 1u);
+            __syncthreads();
+            w = next_item;   // every item ends with a __syncthreads, so the slot is free to rewrite
+        }
+        if (w >= nwork) break;
         const long long blk = w / nsplit;
         const int sp = (int)(w % nsplit);
         const int c0 = (int)(((long long)sp * NCH) / nsplit);

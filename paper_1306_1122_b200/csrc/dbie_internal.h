@@ -80,6 +80,8 @@ struct InteractParams {
     long long cap;
     int target_items;            // split the pixel range until there are this many work items
     unsigned* zero_ptr;          // set to 0 by the launch (the next pass's list counter), or nullptr
+    unsigned* work_ctr;          // persistent grid: atomic work-item counter (zero on entry), or nullptr
+    unsigned* zero_work;         // set to 0 by the launch (the next pass's work counter), or nullptr
     // MODE_GRID (O-4): trial t of component c at point id is lo[c*ldlo + id] + W t/(T-1)
     const double* lo;
     long long ldlo;
