@@ -35,7 +35,8 @@ class _Opts(C.Structure):
                 ("w_g", C.c_double), ("eps_f", C.c_double), ("eps_g", C.c_double),
                 ("lam0", C.c_double), ("step", C.c_double), ("xtol", C.c_double),
                 ("ftol", C.c_double), ("maxiter", C.c_int), ("n_trial", C.c_int),
-                ("n_level", C.c_int), ("lam_max", C.c_double), ("use_eq12", C.c_int)]
+                ("n_level", C.c_int), ("lam_max", C.c_double), ("use_eq12", C.c_int),
+                ("analytic", C.c_int)]
 
 
 @dataclasses.dataclass
@@ -56,6 +57,7 @@ class Opts:
     n_level: int = 10
     lam_max: float = 0.4
     use_eq12: int = 1
+    analytic: int = 0     # O-5: analytic gradient instead of Eq. 13's finite differences (NM only)
 
     def _c(self) -> _Opts:
         return _Opts(*[getattr(self, f.name) for f in dataclasses.fields(self)])
@@ -129,6 +131,21 @@ def residual(wl, lam, opts: Opts | None = None, x=None, y=None, z=None, nthreads
     lib.orc_residual(C.byref(b), C.byref(o), C.c_long(M), px, py, pz, pl,
                      out.ctypes.data_as(_dp), phi.ctypes.data_as(_dp), C.c_int(nthreads))
     return {"B": out[0:3], "f": out[3], "g": out[4], "J": out[5:8], "div": out[8], "phi": phi}
+
+
+def gradient(wl, lam=None, x=None, y=None, z=None, nthreads: int = 0):
+    """O-5: B (3, M) and the nine dB_p/dx_j (3, 3, M) from the analytic derivative of Eq. 6."""
+    lib = _load()
+    b, keep = _boundary(wl)
+    x, px = _d(wl.x if x is None else x)
+    y, py = _d(wl.y if y is None else y)
+    z, pz = _d(wl.z if z is None else z)
+    M = x.size
+    lam = np.ascontiguousarray(wl.lam if lam is None else lam, dtype=np.float64).reshape(3, M)
+    B = np.empty((3, M)); G = np.empty((3, 3, M))
+    lib.orc_gradient(C.byref(b), C.c_long(M), px, py, pz, lam.ctypes.data_as(_dp),
+                     B.ctypes.data_as(_dp), G.ctypes.data_as(_dp), C.c_int(nthreads))
+    return B, G
 
 
 def _solve(fn_name, wl, opts, x, y, z, nthreads):

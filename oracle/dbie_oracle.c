@@ -18,6 +18,13 @@
  *   orc_solve_grid      BASELINE.json config 5 reading (">= 8 trial lambda per
  *                       component per iteration"); NOT in the paper
  *                       (reading O-4).
+ *   orc_gradient        O-5 (NOT the paper's default): the nine
+ *                       dB_p/dx_j as a second sum over the same pixels, from
+ *                       d/dr[n(lambda r)/r^3] = lambda^2 cos(lambda r)/r^2
+ *                       - 3 n(lambda r)/r^4 ("possible if the function f_i can be
+ *                       calculated analytically").  With
+ *                       opts.analytic = 1 orc_residual / orc_solve_nm take J and
+ *                       div B from it instead of Eq. 13's differences.
  *   orc_nm_generic      the same Nelder-Mead driver on a caller-supplied
  *                       objective, so tests can pin it against SciPy (pin S-1).
  *
@@ -57,6 +64,8 @@ typedef struct {
     int n_trial, n_level;       /* GRID: T, number of levels                        */
     double lam_max;             /* GRID: window [0, lam_max/h]                      */
     int use_eq12;               /* 1: Eq. 12 early exit enabled                     */
+    int analytic;               /* 1: analytic gradient of Eq. 6 instead of the
+                                   finite differences of Eq. 13 (O-5, NM only)      */
 } orc_opts;
 
 /* ---------------------------------------------------------------- O-1 ---- */
@@ -147,11 +156,108 @@ static double residual_from_stencil(const double B0[3], const double Bx[3],
     return f + w_g * g;
 }
 
+/* ---------------------------------------------------------------- O-5 ---- */
+/* Analytic gradient (PAPER.md:92 allows it, Eq. 13 is the default).
+ * With K(r) = n(lambda r)/r^3, n = theta sin theta + cos theta, theta = lambda r:
+ *   dK/dr = lambda^2 cos(theta)/r^2 - 3 n/r^4,   D(r) := (dK/dr)/r,
+ *   r^2 = (x_k-x_i)^2 + (y_k-y_i)^2 + z_i^2  =>  dr/dx_i = -(x_k-x_i)/r, dr/dz_i = z_i/r,
+ *   B_p    = (z h^2/2pi) sum_k K B_p0
+ *   dB_p/dx = -(z h^2/2pi) sum_k D (x_k-x_i) B_p0      (same for y)
+ *   dB_p/dz =  (h^2/2pi) [ sum_k K B_p0 + z^2 sum_k D B_p0 ].
+ * G[p][j] = dB_p/dx_j.                                                        */
+static void eval_point_grad(const orc_boundary *b, double xi, double yi, double zi,
+                            const double lam[3], double B[3], double G[3][3])
+{
+    long double s0[3] = { 0, 0, 0 }, sx[3] = { 0, 0, 0 }, sy[3] = { 0, 0, 0 }, sd[3] = { 0, 0, 0 };
+    const double l[3] = { fabs(lam[0]), fabs(lam[1]), fabs(lam[2]) };
+    if (!(zi > 0.0) || !isfinite(xi) || !isfinite(yi) || !isfinite(zi) ||
+        !isfinite(l[0]) || !isfinite(l[1]) || !isfinite(l[2])) {
+        for (int p = 0; p < 3; ++p) { B[p] = NAN; G[p][0] = G[p][1] = G[p][2] = NAN; }
+        return;
+    }
+    for (int iy = 0; iy < b->ny; ++iy) {
+        const double yk = b->y0 + (iy + 0.5) * b->h;
+        const double dy = yk - yi;
+        for (int ix = 0; ix < b->nx; ++ix) {
+            const double xk = b->x0 + (ix + 0.5) * b->h;
+            const double dx = xk - xi;
+            const double r2 = dx * dx + dy * dy + zi * zi;
+            const double r = sqrt(r2);
+            const double r3 = r2 * r, r5 = r3 * r2;
+            const long k = (long)iy * b->nx + ix;
+            const double b0[3] = { b->bx[k], b->by[k], b->bz[k] };
+            for (int p = 0; p < 3; ++p) {
+                const double th = l[p] * r, sn = sin(th), cs = cos(th);
+                const double n = th * sn + cs;
+                const double K = n / r3;
+                const double D = l[p] * l[p] * cs / r3 - 3.0 * n / r5;
+                s0[p] += (long double)(K * b0[p]);
+                sx[p] += (long double)(D * dx * b0[p]);
+                sy[p] += (long double)(D * dy * b0[p]);
+                sd[p] += (long double)(D * b0[p]);
+            }
+        }
+    }
+    const long double c1 = (long double)b->h * (long double)b->h / (2.0L * (long double)ORC_PI);
+    const long double c = (long double)zi * c1;
+    for (int p = 0; p < 3; ++p) {
+        B[p] = (double)(c * s0[p]);
+        G[p][0] = (double)(-c * sx[p]);
+        G[p][1] = (double)(-c * sy[p]);
+        G[p][2] = (double)(c1 * (s0[p] + (long double)zi * (long double)zi * sd[p]));
+    }
+}
+
+/* Eq. 14, 8, 9 from a given gradient: the tail of residual_from_stencil, same formulas. */
+static double residual_from_gradient(const double B0[3], const double G[3][3], double d_abs,
+                                     double w_g, double out[9])
+{
+    const double Jx = G[2][1] - G[1][2];
+    const double Jy = G[0][2] - G[2][0];
+    const double Jz = G[1][0] - G[0][1];
+    const double div = G[0][0] + G[1][1] + G[2][2];
+    const double nB = sqrt(B0[0] * B0[0] + B0[1] * B0[1] + B0[2] * B0[2]);
+    const double nJ = sqrt(Jx * Jx + Jy * Jy + Jz * Jz);
+    const double cx = Jy * B0[2] - Jz * B0[1];
+    const double cy = Jz * B0[0] - Jx * B0[2];
+    const double cz = Jx * B0[1] - Jy * B0[0];
+    const double nC = sqrt(cx * cx + cy * cy + cz * cz);
+    out[0] = B0[0]; out[1] = B0[1]; out[2] = B0[2];
+    out[5] = Jx; out[6] = Jy; out[7] = Jz; out[8] = div;
+    if (!(nB > 0.0) || !isfinite(nB)) {
+        out[3] = out[4] = NAN;
+        return NAN;
+    }
+    const double f = (nJ <= 1e-300) ? 0.0 : nC / (nJ * nB);
+    const double g = fabs(div) * (d_abs / 6.0) / nB;
+    out[3] = f; out[4] = g;
+    return f + w_g * g;
+}
+
+void orc_gradient(const orc_boundary *b, long M, const double *x, const double *y,
+                  const double *z, const double *lam /* 3*M */, double *B /* 3*M */,
+                  double *G /* 9*M: G[(p*3+j)*M + i] = dB_p/dx_j */, int nthreads)
+{
+#ifdef _OPENMP
+    if (nthreads > 0) omp_set_num_threads(nthreads);
+#endif
+#pragma omp parallel for schedule(dynamic, 4)
+    for (long i = 0; i < M; ++i) {
+        double l[3] = { lam[i], lam[M + i], lam[2 * M + i] }, Bi[3], Gi[3][3];
+        eval_point_grad(b, x[i], y[i], z[i], l, Bi, Gi);
+        for (int p = 0; p < 3; ++p) {
+            B[p * M + i] = Bi[p];
+            for (int j = 0; j < 3; ++j) G[(p * 3 + j) * M + i] = Gi[p][j];
+        }
+    }
+}
+
 typedef struct {
     const orc_boundary *b;
     double xi, yi, zi;
     double delta_abs, d_abs, w_g;
     long nfev;
+    int analytic;
 } point_ctx;
 
 /* objective of the per-point search: lambda triple -> Phi; aux = (B, f, g, J, div) */
@@ -160,6 +266,11 @@ static double point_objective(const double lam[3], void *user, double aux[9])
     point_ctx *c = (point_ctx *)user;
     double B0[3], Bx[3], By[3], Bz[3];
     c->nfev++;
+    if (c->analytic) { /* O-5: one evaluation position, exact derivatives */
+        double G[3][3];
+        eval_point_grad(c->b, c->xi, c->yi, c->zi, lam, B0, G);
+        return residual_from_gradient(B0, G, c->d_abs, c->w_g, aux);
+    }
     /* Eq. 13: the same lambda triple at r_i and at its delta-neighbours */
     eval_point(c->b, c->xi, c->yi, c->zi, lam, B0);
     eval_point(c->b, c->xi + c->delta_abs, c->yi, c->zi, lam, Bx);
@@ -178,7 +289,7 @@ void orc_residual(const orc_boundary *b, const orc_opts *o, long M, const double
 #endif
 #pragma omp parallel for schedule(dynamic, 1)
     for (long i = 0; i < M; ++i) {
-        point_ctx c = { b, x[i], y[i], z[i], o->delta * b->h, o->cell * b->h, o->w_g, 0 };
+        point_ctx c = { b, x[i], y[i], z[i], o->delta * b->h, o->cell * b->h, o->w_g, 0, o->analytic };
         double l[3] = { lam[i], lam[M + i], lam[2 * M + i] }, aux[9];
         phi[i] = point_objective(l, &c, aux);
         for (int q = 0; q < 9; ++q) out[q * M + i] = aux[q];
@@ -341,7 +452,7 @@ void orc_solve_nm(const orc_boundary *b, const orc_opts *o, long M, const double
 #endif
 #pragma omp parallel for schedule(dynamic, 1)
     for (long i = 0; i < M; ++i) {
-        point_ctx c = { b, x[i], y[i], z[i], o->delta * b->h, o->cell * b->h, o->w_g, 0 };
+        point_ctx c = { b, x[i], y[i], z[i], o->delta * b->h, o->cell * b->h, o->w_g, 0, o->analytic };
         nm_state s;
         double V0[4][3];
         const double l0 = o->lam0 / b->h, st = o->step / b->h;

@@ -439,3 +439,80 @@ def test_grid_mode_brute_force_and_monotone():
                     r = oracle.residual(w.subset([i]), np.array([[a], [b], [c]]))
                     best = min(best, r["phi"][0])
         assert abs(phis[0, i] - best) < 1e-9
+
+
+# -- O-5: analytic gradient ------------------------------------
+def _mp_field(w, comp, lam):
+    """B_comp(x, y, z) of Eq. 6/16 as an mpmath function of the point (definition, 30 digits)."""
+    b0 = (w.bx, w.by, w.bz)[comp]
+    l = mp.mpf(abs(float(lam)))
+
+    def f(x, y, z):
+        tot = mp.mpf(0)
+        for iy in range(w.ny):
+            for ix in range(w.nx):
+                xk = mp.mpf(w.x0) + (ix + mp.mpf(1) / 2) * mp.mpf(w.h)
+                yk = mp.mpf(w.y0) + (iy + mp.mpf(1) / 2) * mp.mpf(w.h)
+                r = mp.sqrt((xk - x) ** 2 + (yk - y) ** 2 + z ** 2)
+                tot += (l * r * mp.sin(l * r) + mp.cos(l * r)) / r ** 3 * mp.mpf(float(b0[iy * w.nx + ix]))
+        return z * mp.mpf(w.h) ** 2 / (2 * mp.pi) * tot
+    return f
+
+
+def test_g1_analytic_gradient_vs_mpmath_numerical_derivative():
+    """The oracle's dB_p/dx_j against mpmath's numerical differentiation of the DEFINITION of B_p
+    (no derivative formula is retyped here): a wrong sign, a dropped z-term of d/dz, or a
+    transposed index fails it.  h != 1, shifted origin, lambda of both signs and lambda = 0."""
+    mp.mp.dps = 30
+    w = random_boundary(6, 5, seed=8, npts=3, h=0.5, x0=-1.0, y0=2.0, zmin=0.8, zmax=2.0)
+    w.lam[:, 0] = 0.0
+    w.lam[1, 1] = -w.lam[1, 1]
+    B, G = oracle.gradient(w)
+    assert np.allclose(B, oracle.eval(w), rtol=1e-14, atol=0)
+    for i in range(w.M):
+        pt = (mp.mpf(float(w.x[i])), mp.mpf(float(w.y[i])), mp.mpf(float(w.z[i])))
+        for p in range(3):
+            f = _mp_field(w, p, w.lam[p, i])
+            for j in range(3):
+                order = tuple(1 if q == j else 0 for q in range(3))
+                ex = mp.diff(f, pt, order)
+                scale = max(abs(G[p, :, i]).max(), 1e-300)
+                assert abs(mp.mpf(float(G[p, j, i])) - ex) <= 1e-11 * scale, (i, p, j)
+
+
+def test_g2_finite_differences_converge_to_the_analytic_gradient():
+    """Eq. 13's forward differences of the oracle's own B approach the analytic gradient linearly
+    in delta (pin K-9's statement, now between two oracle functions)."""
+    w = random_boundary(14, 11, seed=3, npts=5, zmin=1.5, zmax=5.0)
+    _, G = oracle.gradient(w)
+    errs = []
+    for d in (1e-2, 1e-3, 1e-4):
+        B0 = oracle.eval(w)
+        Gfd = np.empty_like(G)
+        Gfd[:, 0] = (oracle.eval(w, x=w.x + d) - B0) / d
+        Gfd[:, 1] = (oracle.eval(w, y=w.y + d) - B0) / d
+        Gfd[:, 2] = (oracle.eval(w, z=w.z + d) - B0) / d
+        errs.append(float((np.abs(Gfd - G).max(axis=(0, 1)) / np.abs(G).max(axis=(0, 1))).max()))
+    assert errs[0] < 5e-2 and errs[1] < 0.2 * errs[0] and errs[2] < 0.2 * errs[1]
+
+
+def test_g3_analytic_residual_and_solve_are_consistent_with_eq13():
+    """residual(analytic=1) equals Eq. 8, 9, 14 applied to the analytic gradient, stays within
+    O(delta) of the finite-difference residual, and the NM solve on it reaches an objective that is
+    as good as the finite-difference solve's (cross-evaluated with the analytic objective)."""
+    w = random_boundary(14, 11, seed=5, npts=6, zmin=1.5, zmax=5.0)
+    ra = oracle.residual(w, w.lam, oracle.Opts(analytic=1))
+    rf = oracle.residual(w, w.lam, oracle.Opts())
+    B, G = oracle.gradient(w)
+    J = np.array([G[2, 1] - G[1, 2], G[0, 2] - G[2, 0], G[1, 0] - G[0, 1]])
+    assert np.array_equal(ra["J"], J) and np.array_equal(ra["div"], G[0, 0] + G[1, 1] + G[2, 2])
+    nB = np.linalg.norm(B, axis=0)
+    f = np.linalg.norm(np.cross(J.T, B.T), axis=1) / (np.linalg.norm(J, axis=0) * nB)
+    assert np.allclose(ra["f"], f, rtol=1e-12) and np.allclose(ra["g"], np.abs(ra["div"]) * (w.h / 6.0) / nB, rtol=1e-12)
+    assert np.abs(ra["f"] - rf["f"]).max() < 2e-2 and np.abs(ra["g"] - rf["g"]).max() < 2e-2 * max(1e-3, rf["g"].max())
+    sa = oracle.solve_nm(w, oracle.Opts(analytic=1))
+    sf = oracle.solve_nm(w, oracle.Opts())
+    assert (sa["status"] != 3).all()
+    cross = oracle.residual(w, sf["lam"], oracle.Opts(analytic=1))["phi"]
+    assert np.all(sa["phi"] <= cross + 5e-3)          # both searches end in equally good minima
+    assert np.all(sa["phi"] <= oracle.residual(w, np.full((3, w.M), 0.05 / w.h), oracle.Opts(analytic=1))["phi"] + 1e-15)
