@@ -110,6 +110,13 @@ typedef struct {
     int n_level;      /* GRID: number of refinement levels; 10                                */
     double lam_max;   /* GRID: search window [0, lam_max/h]; 0.4                              */
     int use_eq12;     /* 1: stop a point as soon as f <= eps_f and g <= eps_g (Eq. 12)        */
+    int analytic;     /* 0 (default): J and div B from the finite differences of Eq. 13 (the
+                         paper's method).  1: from the analytic gradient of Eq. 6, a second sum
+                         over the same pixels with d/dr[n(lambda r)/r^3] = lambda^2 cos(lambda r)/r^2
+                         - 3 n(lambda r)/r^4 ("possible if the function f_i can be
+                         calculated analytically"; O-5): one evaluation position instead
+                         of four per objective evaluation; delta is ignored.  Method 0 (NM) and
+                         dbie_residual only; with method 1 dbie_solve returns DBIE_EINVAL.       */
 } dbie_solve_opts;
 
 void dbie_solve_default_opts(dbie_solve_opts* opts);

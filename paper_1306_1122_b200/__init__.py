@@ -38,7 +38,8 @@ class SolveOpts(C.Structure):
                 ("w_g", C.c_double), ("eps_f", C.c_double), ("eps_g", C.c_double),
                 ("lam0", C.c_double), ("step", C.c_double), ("xtol", C.c_double),
                 ("ftol", C.c_double), ("maxiter", C.c_int), ("n_trial", C.c_int),
-                ("n_level", C.c_int), ("lam_max", C.c_double), ("use_eq12", C.c_int)]
+                ("n_level", C.c_int), ("lam_max", C.c_double), ("use_eq12", C.c_int),
+                ("analytic", C.c_int)]
 
 
 _vp = C.c_void_p

@@ -25,6 +25,7 @@ struct dbie_ctx {
     double last_interactions;
     long long last_launches, last_evals;
     int evals_on_device;                      // last call was a solve: read nevals back on demand
+    int positions_per_eval;                   // evaluation positions per objective evaluation of that solve (4, or 1 analytic)
     int f32_sfu_mask;                         // dbie_eval_f32: components whose sincos use the SFU
     int profile;                              // record CUDA events around every interaction launch
     cudaEvent_t* ev;    int ev_cap, ev_n;     // event pairs of the last call (profile mode)
@@ -126,6 +127,7 @@ extern "C" void dbie_solve_default_opts(dbie_solve_opts* o) {
     o->n_level = 10;
     o->lam_max = 0.4;
     o->use_eq12 = 1;
+    o->analytic = 0;
 }
 
 static void setup_tiling(BoundaryView& b) {
@@ -350,6 +352,7 @@ static dbie_status make_consts(const dbie_ctx* ctx, const dbie_solve_opts* o, NM
     k->h2_over_2pi = h * h / (2.0 * 3.14159265358979323846);
     k->maxiter = o->maxiter;
     k->use_eq12 = o->use_eq12;
+    k->analytic = o->analytic != 0;
     return DBIE_OK;
 }
 
@@ -379,12 +382,12 @@ extern "C" dbie_status dbie_residual(dbie_ctx* ctx, long long M, const double* x
         p.delta_abs = k.delta_abs;
         p.part = ctx->part; p.cap = cap;
         prof_mark(ctx, st);
-        CU(launch_interact_stencil(p, ctx->sm_count, st));
+        CU(k.analytic ? launch_interact_analytic(p, ctx->sm_count, st) : launch_interact_stencil(p, ctx->sm_count, st));
         prof_mark(ctx, st);
         CU(launch_residual_finalize(ctx->bd, k, cnt, M, z + off, ctx->part, cap, out + off, phi ? phi + off : nullptr, st));
         launches += 2;
     }
-    ctx->last_interactions = (double)M * kStencil * (double)ctx->bd.N;
+    ctx->last_interactions = (double)M * (k.analytic ? 1 : kStencil) * (double)ctx->bd.N;
     ctx->last_launches = launches;
     ctx->last_evals = M;
     ctx->evals_on_device = 0;
@@ -464,6 +467,7 @@ static dbie_status solve_grid(dbie_ctx* ctx, long long M, const double* x, const
     }
     ctx->last_launches = launches;
     ctx->evals_on_device = 1;
+    ctx->positions_per_eval = kStencil;
     return DBIE_OK;
 }
 
@@ -477,6 +481,7 @@ extern "C" dbie_status dbie_solve(dbie_ctx* ctx, long long M, const double* x, c
     NMConsts k;
     dbie_status s = make_consts(ctx, opts, &k);
     if (s != DBIE_OK) return s;
+    if (opts && opts->method == 1 && opts->analytic) return DBIE_EINVAL;
     if (opts && opts->method == 1) return solve_grid(ctx, M, x, y, z, opts, k, B, lam, resid, iters, status, cuda_stream);
     if (opts && opts->method != 0) return DBIE_EINVAL;
     cudaStream_t st = (cudaStream_t)cuda_stream;
@@ -527,7 +532,7 @@ extern "C" dbie_status dbie_solve(dbie_ctx* ctx, long long M, const double* x, c
             p.delta_abs = k.delta_abs;
             p.part = ctx->part; p.cap = cap;
             prof_mark(ctx, st);
-            CU(launch_interact_stencil(p, ctx->sm_count, st));
+            CU(k.analytic ? launch_interact_analytic(p, ctx->sm_count, st) : launch_interact_stencil(p, ctx->sm_count, st));
             prof_mark(ctx, st);
             CU(launch_solve_step(a, k, ctx->bd, pass, cnt, M, z + off, ctx->part, cap, B + off, lam + off,
                                  resid + off, iters + off, status + off, nevals, st));
@@ -536,6 +541,7 @@ extern "C" dbie_status dbie_solve(dbie_ctx* ctx, long long M, const double* x, c
     }
     ctx->last_launches = launches;
     ctx->evals_on_device = 1;
+    ctx->positions_per_eval = k.analytic ? 1 : kStencil;
     return DBIE_OK;
 }
 
@@ -574,7 +580,7 @@ extern "C" dbie_status dbie_last_counters(dbie_ctx* ctx, double* interactions, l
         unsigned long long n = 0;
         CU(cudaMemcpy(&n, (char*)ctx->counters + 16, sizeof n, cudaMemcpyDeviceToHost));
         ctx->last_evals = (long long)n;
-        ctx->last_interactions = (double)n * kStencil * (double)ctx->bd.N;
+        ctx->last_interactions = (double)n * ctx->positions_per_eval * (double)ctx->bd.N;
     }
     if (interactions) *interactions = ctx->last_interactions;
     if (launches) *launches = ctx->last_launches;

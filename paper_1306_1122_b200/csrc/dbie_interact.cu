@@ -87,6 +87,10 @@ cudaError_t launch_interact_stencil(const InteractParams& p, int sm_count, cudaS
     return launch64<MODE_STENCIL, 1, 2>(p, sm_count, 16, st);
 }
 
+cudaError_t launch_interact_analytic(const InteractParams& p, int sm_count, cudaStream_t st) {
+    return launch64<MODE_ANALYTIC, 1, 1>(p, sm_count, 16, st);
+}
+
 cudaError_t launch_interact_grid(const InteractParams& p, int sm_count, cudaStream_t st) {
     if (p.T < 2) return cudaErrorInvalidValue;
     if (p.T % 4 == 0) return launch64<MODE_GRID, 4, 1>(p, sm_count, 16, st);

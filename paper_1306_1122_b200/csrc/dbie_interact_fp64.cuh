@@ -24,11 +24,15 @@
 
 namespace dbie {
 
-enum { MODE_EVAL = 0, MODE_STENCIL = 1, MODE_GRID = 2 };
+// MODE_ANALYTIC (O-5): one position per field point; besides the Eq. 6 sum
+// it accumulates the three sums of the analytic gradient (kinds 1..3 below), 12 sums per slot like
+// the stencil, from the same sincos: d/dr[n(lambda r)/r^3] = lambda^2 cos(lambda r)/r^2 - 3 n/r^4.
+enum { MODE_EVAL = 0, MODE_STENCIL = 1, MODE_GRID = 2, MODE_ANALYTIC = 3 };
 
 // items (threads' units of work) per slot
 __host__ __device__ inline long long items_per_slot(int mode, int G) {
-    return mode == MODE_EVAL ? 1 : (mode == MODE_STENCIL ? kStencil : (long long)kStencil * G);
+    return (mode == MODE_EVAL || mode == MODE_ANALYTIC) ? 1
+                                                         : (mode == MODE_STENCIL ? kStencil : (long long)kStencil * G);
 }
 
 template <int MODE, int NT, int THREADS, int MINB, int UNR>
@@ -86,7 +90,7 @@ __global__ void __launch_bounds__(THREADS, MINB) interact64_kernel(const __grid_
         const long long jt = live ? item : nitems - 1;
         long long slot;
         int s = 0, g = 0;
-        if (MODE == MODE_EVAL) {
+        if (MODE == MODE_EVAL || MODE == MODE_ANALYTIC) {
             slot = jt;
         } else if (MODE == MODE_STENCIL) {
             slot = jt >> 2;
@@ -99,7 +103,7 @@ __global__ void __launch_bounds__(THREADS, MINB) interact64_kernel(const __grid_
         }
         const long long id = (MODE == MODE_EVAL) ? p.slot0 + slot : (p.act ? (long long)p.act[slot] : slot);
         double xi = p.x[id], yi = p.y[id], zi = p.z[id];
-        if (MODE != MODE_EVAL) {   // Eq. 13: r_i, r_i + delta x, + delta y, + delta z
+        if (MODE == MODE_STENCIL || MODE == MODE_GRID) {   // Eq. 13: r_i, r_i + delta x, + delta y, + delta z
             if (s == 1) xi = __dadd_rn(xi, p.delta_abs);
             if (s == 2) yi = __dadd_rn(yi, p.delta_abs);
             if (s == 3) zi = __dadd_rn(zi, p.delta_abs);
@@ -122,9 +126,14 @@ __global__ void __launch_bounds__(THREADS, MINB) interact64_kernel(const __grid_
             for (int c = 0; c < 3; ++c) lam[0][c] = fabs(p.lam[c * p.ldlam + id]);
         }
 
-        double acc[NT][3];
+        // accumulators: one row per lambda triple; MODE_ANALYTIC: rows = sum K b, sum D dx b, sum D dy b, sum D b
+        constexpr int NA = (MODE == MODE_ANALYTIC) ? 4 : NT;
+        double acc[NA][3];
 #pragma unroll
-        for (int tt = 0; tt < NT; ++tt) acc[tt][0] = acc[tt][1] = acc[tt][2] = 0.0;
+        for (int tt = 0; tt < NA; ++tt) acc[tt][0] = acc[tt][1] = acc[tt][2] = 0.0;
+        double lam2[3];   // MODE_ANALYTIC: lambda^2
+#pragma unroll
+        for (int c = 0; c < 3; ++c) lam2[c] = lam[0][c] * lam[0][c];
 
         const int t0 = chunk_first_tile(bd, c0), t1 = chunk_first_tile(bd, c1);
         int c = c0;
@@ -157,6 +166,25 @@ __global__ void __launch_bounds__(THREADS, MINB) interact64_kernel(const __grid_
                     const double rr = r2 * y;          // r
                     const double wgt = (y * y) * y;    // 1/r^3
                     const double wx = wgt * px.y, wy = wgt * px.z, wz = wgt * px.w;
+                    if (MODE == MODE_ANALYTIC) {
+                        // K b = n w b;  D b = (lambda^2 cos(theta) - 3 n / r^2) w b  (w = 1/r^3)
+                        const double m3y2 = (y * y) * -3.0;
+                        const double wb[3] = {wx, wy, wz};
+#pragma unroll
+                        for (int c = 0; c < 3; ++c) {
+                            double n, cs;
+                            int sg;
+                            kernel_n_cos(lam[0][c] * rr, n, cs, sg);
+                            const double wbs = flip_sign_if(wb[c], sg);
+                            const double e = fma(lam2[c], cs, n * m3y2);
+                            const double gb = e * wbs;
+                            acc[0][c] = fma(n, wbs, acc[0][c]);
+                            acc[1][c] = fma(gb, dx, acc[1][c]);
+                            acc[2][c] = fma(gb, dy, acc[2][c]);
+                            acc[3][c] += gb;
+                        }
+                        continue;
+                    }
 #pragma unroll
                     for (int tt = 0; tt < NT; ++tt) {
                         acc[tt][0] = fma(kernel_n(lam[tt][0] * rr), wx, acc[tt][0]);
@@ -175,6 +203,12 @@ __global__ void __launch_bounds__(THREADS, MINB) interact64_kernel(const __grid_
 #pragma unroll
                         for (int q = 0; q < 3; ++q)
                             p.part[((long long)c * 12 + s * 3 + q) * p.cap + slot] = acc[0][q];
+                    } else if (MODE == MODE_ANALYTIC) {
+#pragma unroll
+                        for (int kd = 0; kd < 4; ++kd)
+#pragma unroll
+                            for (int q = 0; q < 3; ++q)
+                                p.part[((long long)c * 12 + kd * 3 + q) * p.cap + slot] = acc[kd][q];
                     } else {
                         const long long Q = 12LL * p.T;
 #pragma unroll
@@ -186,7 +220,7 @@ __global__ void __launch_bounds__(THREADS, MINB) interact64_kernel(const __grid_
                     }
                 }
 #pragma unroll
-                for (int tt = 0; tt < NT; ++tt) acc[tt][0] = acc[tt][1] = acc[tt][2] = 0.0;
+                for (int tt = 0; tt < NA; ++tt) acc[tt][0] = acc[tt][1] = acc[tt][2] = 0.0;
                 ++c;
                 t_chunk_end = chunk_first_tile(bd, c + 1);
             }

@@ -130,6 +130,22 @@ DBIE_HD double kernel_n(double th) {
     return flip_sign_if(n, (q << 30) & (int)0x80000000);
 }
 
+// n(theta) and cos(theta) up to their common sign (-1)^(q>>1), which the caller folds into the
+// weight: n' in {theta sn + cs, theta cs - sn}, c' in {cs, -sn}; sg = the sign as a bit-31 mask.
+// Used by the analytic-gradient mode (O-5).  19 FP64 instructions.
+DBIE_HD void kernel_n_cos(double th, double& n, double& c, int& sg) {
+    int q;
+    const double t = reduce_pio2(th, q);
+    double sn, cs;
+    sincos_reduced(t, sn, cs);
+    const double ne = fma(th, sn, cs);
+    const double no = fma(th, cs, -sn);
+    const bool odd = (q & 1) != 0;
+    n = odd ? no : ne;
+    c = odd ? flip_sign_if(sn, (int)0x80000000) : cs;
+    sg = (q << 30) & (int)0x80000000;
+}
+
 // full sincos (used by host accuracy tests and by nothing on the hot path)
 DBIE_HD void sincos_pos(double th, double& s, double& c) {
     int q;

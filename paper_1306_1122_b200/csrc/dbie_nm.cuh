@@ -45,6 +45,7 @@ struct NMConsts {
     double lam0_abs, step_abs;
     double h2_over_2pi;  // h^2 / (2 pi): Eq. 6 prefactor without z_i
     int maxiter, use_eq12;
+    int analytic;        // 1: sums are those of the analytic gradient (O-5), not of the Eq. 13 stencil
 };
 
 struct Residual {
@@ -98,6 +99,26 @@ DBIE_NM_HD Residual residual_from_sums(const double S[12], double z, const NMCon
     for (int s = 0; s < 4; ++s)
         for (int p = 0; p < 3; ++p) Bs[s][p] = mul_(s == 3 ? c3 : c0, S[s * 3 + p]);
     return residual_from_stencil(Bs, k);
+}
+
+// raw sums of the analytic-gradient mode (O-5): S[p] = sum K b_p, S[3+p] = sum D dx b_p,
+// S[6+p] = sum D dy b_p, S[9+p] = sum D b_p  ->  B_p = c S[p], dB_p/dx = -c S[3+p], dB_p/dy = -c S[6+p],
+// dB_p/dz = (h^2/2pi) (S[p] + z^2 S[9+p]), c = z h^2/2pi.
+DBIE_NM_HD Residual residual_from_analytic_sums(const double S[12], double z, const NMConsts& k) {
+    const double c = mul_(z, k.h2_over_2pi);
+    const double zz = mul_(z, z);
+    double G[3][3], B0[3];
+    for (int p = 0; p < 3; ++p) {
+        B0[p] = mul_(c, S[p]);
+        G[p][0] = -mul_(c, S[3 + p]);
+        G[p][1] = -mul_(c, S[6 + p]);
+        G[p][2] = mul_(k.h2_over_2pi, add_(S[p], mul_(zz, S[9 + p])));
+    }
+    return residual_from_gradient(G, B0, k);
+}
+
+DBIE_NM_HD Residual residual_any(const double S[12], double z, const NMConsts& k) {
+    return k.analytic ? residual_from_analytic_sums(S, z, k) : residual_from_sums(S, z, k);
 }
 
 enum NMPhase : int {

@@ -84,7 +84,7 @@ __global__ void solve_step_kernel(SolveArrays s, NMConsts k, int nchunks, int pa
             for (int ch = 1; ch < nchunks; ++ch) sum = __dadd_rn(sum, part[((long long)ch * 12 + q) * cap + j]);
             S[q] = sum;
         }
-        const Residual r = residual_from_sums(S, z[id], c);
+        const Residual r = residual_any(S, z[id], c);
         const double a[5] = {r.B[0], r.B[1], r.B[2], r.f, r.g};
         NMPoint p;
         load_point(s, M, id, p);
@@ -123,7 +123,7 @@ __global__ void residual_finalize_kernel(NMConsts k, int nchunks, long long M, l
         S[q] = sum;
     }
     const double zi = z[i];
-    Residual r = residual_from_sums(S, zi, c);
+    Residual r = residual_any(S, zi, c);
     const bool invalid = !(zi > 0.0) || !isfinite(zi);
     const double v[9] = {r.B[0], r.B[1], r.B[2], r.f, r.g, r.J[0], r.J[1], r.J[2], r.div};
     for (int q = 0; q < 9; ++q) out[q * ldo + i] = invalid ? qnan() : v[q];

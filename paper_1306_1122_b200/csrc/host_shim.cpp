@@ -45,7 +45,7 @@ int shim_nm_generic(shim_objective fn, const double* simplex, double xtol, doubl
     dbie::NMConsts k;
     k.delta_abs = 1.0; k.d_abs = 1.0; k.w_g = 1.0; k.eps_f = 0.0; k.eps_g = 0.0;
     k.xtol_abs = xtol; k.ftol = ftol; k.lam0_abs = 0.0; k.step_abs = 1.0; k.h2_over_2pi = 1.0;
-    k.maxiter = maxiter; k.use_eq12 = 0;
+    k.maxiter = maxiter; k.use_eq12 = 0; k.analytic = 0;
     dbie::NMPoint p;
     dbie::nm_start(p, k);
     for (int j = 0; j < 4; ++j)

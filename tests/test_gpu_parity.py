@@ -236,17 +236,23 @@ def test_residual_matches_oracle(dbie, case):
 
 
 # ---------------------------------------------------------------------------- solve --------
-def _check_solve_parity(dbie, wl, opts_kw=None):
-    """Protocol P-4; opts_kw["method"] = 1 selects GRID on both sides."""
+def _check_solve_parity(dbie, wl, opts_kw=None, gpu=None):
+    """Protocol P-4; opts_kw["method"] = 1 selects GRID on both sides.
+    `gpu`: results already computed on the GPU for exactly the points of `wl` (a sample of a
+    larger launch); otherwise the points of `wl` are solved here."""
     opts_kw = opts_kw or {}
     oo = oracle.Opts(**opts_kw)
     grid = oo.method == 1
     so = oracle.solve_grid(wl, oo) if grid else oracle.solve_nm(wl, oo)
-    with dbie.DBIE.from_workload(wl) as ctx:
-        dw = dbie.to_device(wl)
-        s = ctx.solve(dw.x, dw.y, dw.z, dbie.default_opts(**opts_kw))
-        s = {k: v.cpu().numpy() for k, v in s.items()}
-        cnt = ctx.counters()
+    cnt = None
+    if gpu is not None:
+        s = gpu
+    else:
+        with dbie.DBIE.from_workload(wl) as ctx:
+            dw = dbie.to_device(wl)
+            s = ctx.solve(dw.x, dw.y, dw.z, dbie.default_opts(**opts_kw))
+            s = {k: v.cpu().numpy() for k, v in s.items()}
+            cnt = ctx.counters()
     valid = so["status"] != 3
     assert np.array_equal(s["status"] == 3, ~valid)
     stable = valid & (so["margin"] >= MARGIN_STABLE)
@@ -274,7 +280,9 @@ def _check_solve_parity(dbie, wl, opts_kw=None):
     assert np.all(s["lam"][:, valid] >= 0.0)
     st0 = s["status"] == 0
     assert np.all(s["f"][st0] <= oo.eps_f) and np.all(s["g"][st0] <= oo.eps_g)
-    if grid:   # T candidate values per component per level a point was active in
+    if cnt is None:
+        pass
+    elif grid:   # T candidate values per component per level a point was active in
         assert cnt["objective_evals"] == oo.n_trial * so["iters"][valid].sum() or forked.any()
     else:
         assert cnt["objective_evals"] == so["nfev"][valid].sum() or forked.any()
@@ -380,3 +388,103 @@ def test_grid_is_reproducible_and_host_entry_matches(dbie):
         for bad in (dict(n_trial=1), dict(n_trial=33), dict(n_level=0), dict(lam_max=0.0)):
             with pytest.raises(dbie.DBIEError):
                 ctx.solve(dw.x, dw.y, dw.z, dbie.default_opts(method=1, **bad))
+
+
+# ------------------------------------------------------------- full-size launches, sampled -
+def _solve_full_and_sample(dbie, wl, nsample, opts_kw=None):
+    """Solve ALL points of `wl` in one call (the launch configuration bench.py times: persistent
+    grid, device-side active lists, many work blocks and a ragged tail) and hand a seeded sample of
+    the outputs to the P-4 comparison: points are independent, so a point's result must not depend
+    on the batch it was solved in."""
+    with dbie.DBIE.from_workload(wl) as ctx:
+        dw = dbie.to_device(wl)
+        s = ctx.solve(dw.x, dw.y, dw.z, dbie.default_opts(**(opts_kw or {})))
+        s = {k: v.cpu().numpy() for k, v in s.items()}
+        cnt = ctx.counters()
+    npos = 1.0 if (opts_kw or {}).get("analytic") else 4.0     # evaluation positions per objective evaluation
+    assert cnt["interactions"] == cnt["objective_evals"] * npos * wl.N
+    assert np.isin(s["status"], [0, 1, 2]).all()          # every point of the volume is valid
+    assert np.isfinite(s["B"]).all() and (s["lam"] >= 0).all()
+    sub, idx = wl.seeded_subset(nsample, seed_offset=77)
+    g = {k: (v[:, idx] if v.ndim == 2 else v[idx]) for k, v in s.items()}
+    return _check_solve_parity(dbie, sub, opts_kw, gpu=g), s
+
+
+def test_solve_config2_full_volume_sampled(dbie):
+    """BASELINE configs[1] exactly as bench.py runs it: NM solve of all 64x64x32 = 131,072 points;
+    96 sampled points are re-solved one by one by the oracle.  S-2/S-3 statistics over the volume."""
+    w = workloads.config2()
+    (_, so, info), s = _solve_full_and_sample(dbie, w, 96)
+    assert info["forked"] <= 2
+    # order of magnitude of the paper's residual statistics (PAPER.md:225: <f> 0.078, <g> 6.7e-4)
+    assert 0.005 < float(np.mean(s["f"])) < 0.3
+    assert float(np.mean(s["g"])) < 0.05
+
+
+def test_solve_config3_large_batch_sampled(dbie):
+    """BASELINE configs[2] boundary (256x256, h = 0.5): NM solve of a 16,384-point seeded subset of
+    the 128x128x64 volume in one call, 24 of them re-solved by the oracle."""
+    w, _ = workloads.config3().seeded_subset(16384, seed_offset=5)
+    _solve_full_and_sample(dbie, w, 24)
+
+
+def test_grid_config5_large_batch_sampled(dbie):
+    """BASELINE configs[4] boundary (1024x1024): GRID solve (T = 8, 3 levels) of a 4,096-point
+    seeded subset of the 256x256x128 volume in one call, 6 of them re-solved by the oracle."""
+    w, _ = workloads.config5().seeded_subset(4096, seed_offset=5)
+    _solve_full_and_sample(dbie, w, 6, dict(method=1, n_level=3))
+
+
+# ------------------------------------------- analytic gradient (SURVEY 8(f) f1, DESIGN.md O-5) -
+@pytest.mark.parametrize("case", ["random", "config3", "config5"])
+def test_analytic_residual_matches_oracle(dbie, case):
+    """dbie_residual with opts.analytic = 1 against orc_residual(analytic = 1): B to 1e-9; J and
+    div B are direct sums now (no division by delta), so they match to 1e-9 of |grad B| as well."""
+    import torch
+    if case == "random":
+        w = workloads.random_boundary(37, 23, seed=12, npts=300, h=0.5, x0=-3.0, y0=1.0, zmin=0.6, zmax=8.0)
+        lam = w.lam
+    elif case == "config3":
+        w, _ = workloads.config3().seeded_subset(96)
+        lam = np.random.default_rng(9).uniform(0.0, 0.3, (3, w.M)) / w.h
+    else:
+        w, _ = workloads.config5().seeded_subset(24)
+        lam = np.random.default_rng(10).uniform(0.0, 0.3, (3, w.M)) / w.h
+    oo = oracle.Opts(analytic=1)
+    ro = oracle.residual(w, lam, oo)
+    _, G = oracle.gradient(w, lam)
+    with dbie.DBIE.from_workload(w) as ctx:
+        dw = dbie.to_device(w)
+        r = ctx.residual(dw.x, dw.y, dw.z, torch.from_numpy(np.ascontiguousarray(lam)).cuda(),
+                         dbie.default_opts(analytic=1))
+        r = {k: v.cpu().numpy() for k, v in r.items()}
+        assert ctx.counters()["interactions"] == float(w.M) * w.N
+    err, _ = vec_relerr(r["B"], ro["B"])
+    assert err <= TOL_B
+    gscale = np.abs(G).max(axis=(0, 1))
+    assert np.all(np.abs(r["J"] - ro["J"]) <= 1e-9 * gscale)
+    assert np.all(np.abs(r["div"] - ro["div"]) <= 1e-9 * gscale)
+    assert np.abs(r["f"] - ro["f"]).max() <= TOL_FG
+    assert np.abs(r["g"] - ro["g"]).max() <= TOL_FG
+    assert np.abs(r["phi"] - ro["phi"]).max() <= 2 * TOL_FG
+
+
+def test_analytic_solve_config2_subset_and_full_volume(dbie):
+    """NM solve with the analytic gradient: P-4 parity on a 160-point subset of config 2, then the
+    whole 131,072-point volume in one call with 64 sampled points re-solved by the oracle."""
+    w, _ = workloads.config2().seeded_subset(160)
+    s, so, info = _check_solve_parity(dbie, w, dict(analytic=1))
+    assert info["forked"] <= 1          # derivative noise ~1e-13: far fewer near-ties than with Eq. 13
+    (_, _, info2), sfull = _solve_full_and_sample(dbie, workloads.config2(), 64, dict(analytic=1))
+    assert 0.005 < float(np.mean(sfull["f"])) < 0.3
+
+
+def test_analytic_solve_config3_options_and_invalid_points(dbie):
+    w, _ = workloads.config3().seeded_subset(32, seed_offset=2)
+    w.z[3] = 0.0
+    s, so, info = _check_solve_parity(dbie, w, dict(analytic=1, use_eq12=0, maxiter=60, w_g=2.0, cell=0.5))
+    assert s["status"][3] == 3
+    with dbie.DBIE.from_workload(w) as ctx:
+        dw = dbie.to_device(w)
+        with pytest.raises(dbie.DBIEError):      # GRID with the analytic gradient is not built
+            ctx.solve(dw.x, dw.y, dw.z, dbie.default_opts(method=1, analytic=1))
