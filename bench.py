@@ -33,6 +33,7 @@ sys.path.insert(0, ROOT)
 METRIC = "point-pixel DBIE interactions/sec (fp64)"
 UNIT = "interactions/s"
 FP64_INSTR_PER_INTERACTION = 76      # DESIGN.md section 6 (SASS inner loop: 152 per 2 pixels of one position)
+FP64_INSTR_ANALYTIC = 95             # analytic gradient: 11 + 3 x 28 per pixel of the one position
 FP64_INSTR_GRID = {4: 265 / 4, 2: 139 / 2, 1: 76}   # GRID: 13 + 63 NT per NT trial triples sharing a geometry
 FP64_INSTR_SURVEY = 82               # SURVEY.md 8(d) canonical count
 SM_COUNT, FP64_LANES_PER_SM = 148, 64   # B200: 148 SMs, 64 FP64 lanes per SM per clock
@@ -111,7 +112,7 @@ class ClockSampler:
                 "samples": len(sm), "reasons": sorted(reasons)}
 
 
-METHOD = {"grid": False}     # set by main(): GRID (O-4) instead of Nelder-Mead
+METHOD = {"grid": False, "analytic": False}   # set by main(): GRID (O-4) instead of NM; analytic gradient (O-5)
 
 
 # --------------------------------------------------------------------------- oracle legs ---
@@ -125,8 +126,9 @@ def oracle_timed(wl, npoints: int, seed_offset: int, nthreads: int = 0) -> dict:
         out = oracle.solve_grid(sub, o, nthreads=nthreads)
         inter = float(out["iters"].sum()) * o.n_trial * 4.0 * wl.N
     elif wl.lam is None:
-        out = oracle.solve_nm(sub, nthreads=nthreads)
-        inter = float(out["nfev"].sum()) * 4.0 * wl.N
+        an = 1 if METHOD["analytic"] else 0
+        out = oracle.solve_nm(sub, oracle.Opts(analytic=an), nthreads=nthreads)
+        inter = float(out["nfev"].sum()) * (1.0 if an else 4.0) * wl.N
     else:
         oracle.eval(sub, nthreads=nthreads)
         inter = float(sub.M) * wl.N
@@ -191,7 +193,9 @@ def workload_config(wl, name, n_points_per_step=None) -> dict:
             "cfg5": "BASELINE configs[4]: quadrupolar delta-spot 1024x1024, lambda solve on a seeded subset of "
                     "the 256x256x128 volume"}[name]
     if wl.lam is None:
-        desc += " [method: " + ("GRID T=8, 10 levels" if METHOD["grid"] else "Nelder-Mead") + "]"
+        desc += " [method: " + ("GRID T=8, 10 levels" if METHOD["grid"] else "Nelder-Mead") + (
+            "; analytic gradient (O-5): 1 evaluation position per objective evaluation instead of 4"
+            if METHOD["analytic"] else "") + "]"
     return {"workload": desc, "boundary": [wl.nx, wl.ny], "points": wl.M if n_points_per_step is None
             else n_points_per_step, "step": "dbie_create + dbie_solve" if wl.lam is None else "dbie_create + dbie_eval",
             "l2": "flushed between timed steps (256 MiB write)"}
@@ -217,7 +221,8 @@ def run_ours(args) -> None:
 
     wl = make_workload(args.workload, rank, world, points=args.points)
     is_solve = wl.lam is None
-    sopts = dbie.default_opts(method=1) if METHOD["grid"] else None
+    sopts = dbie.default_opts(method=1) if METHOD["grid"] else (
+        dbie.default_opts(analytic=1) if METHOD["analytic"] else None)
     t = lambda a: torch.from_numpy(np.ascontiguousarray(a, dtype=np.float64)).to(dev)
     d_bx, d_by, d_bz = t(wl.bx), t(wl.by), t(wl.bz)
     d_x, d_y, d_z = t(wl.x), t(wl.y), t(wl.z)
@@ -307,7 +312,8 @@ def run_ours(args) -> None:
     sm_max = (clocks or {}).get("sm_max_mhz") or 1965.0
     peak_slots = SM_COUNT * FP64_LANES_PER_SM * sm_max * 1e6          # FP64 lane-instructions / s
     kern_ips = inter_total / (kern_ms * 1e-3) if kern_ms > 0 else 0.0
-    per_inter = FP64_INSTR_GRID[4] if (is_solve and METHOD["grid"]) else FP64_INSTR_PER_INTERACTION
+    per_inter = FP64_INSTR_GRID[4] if (is_solve and METHOD["grid"]) else (
+        FP64_INSTR_ANALYTIC if (is_solve and METHOD["analytic"]) else FP64_INSTR_PER_INTERACTION)
     achieved_slots = kern_ips * per_inter
     roofline = {
         "bound": "alu", "kernel": "dbie::interact64_kernel (fp64 point-pixel sums)",
@@ -444,6 +450,8 @@ def main():
     ap.add_argument("--workload", default="cfg2", choices=["cfg2", "cfg3", "cfg4", "cfg5"])
     ap.add_argument("--method", default=None, choices=["nm", "grid"],
                     help="lambda search of the solve workloads (default: nm; cfg5: grid)")
+    ap.add_argument("--gradient", default="fd", choices=["fd", "analytic"],
+                    help="solve workloads: Eq. 13 finite differences (the paper's) or the analytic gradient (O-5)")
     ap.add_argument("--dtype", default="f64", choices=["f64", "f32"],
                     help="f32: the dbie_eval_f32 leg of BASELINE configs[3] (implies --workload cfg4, one GPU)")
     ap.add_argument("--points", type=int, default=0,
@@ -452,6 +460,7 @@ def main():
                     help="target CPU time of the cpu_baseline leg (0 disables it)")
     args = ap.parse_args()
     METHOD["grid"] = (args.method == "grid") or (args.method is None and args.workload == "cfg5")
+    METHOD["analytic"] = args.gradient == "analytic" and not METHOD["grid"]
     if args.impl == "reference":
         run_reference(args)
     elif args.dtype == "f32":

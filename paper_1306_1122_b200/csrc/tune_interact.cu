@@ -152,6 +152,11 @@ int main(int argc, char** argv) {
       run_new<1, 1, 256, 2, 2>("stencil NT1 256x2 u2 persistent static", q, sms, 16, 1, is / 4);
       run_new<1, 1, 256, 2, 2>("stencil NT1 256x2 u2 one CTA per item", q, sms, 16, 0, is / 4);
       run_new<1, 1, 256, 4, 1>("stencil NT1 256x4 u1 one CTA per item", q, sms, 16, 0, is / 4); }
+    { InteractParams q = p;   // analytic gradient: 95 FP64 instructions per interaction (frac76 x 95/76 = pipe utilisation)
+      run_new<3, 1, 256, 2, 1>("analytic NT1 256x2 u1 persistent dynamic [library]", q, sms, 16, 2, ie);
+      run_new<3, 1, 256, 2, 1>("analytic NT1 256x2 u1", q, sms, 16, 0, ie);
+      run_new<3, 1, 256, 2, 2>("analytic NT1 256x2 u2", q, sms, 16, 0, ie);
+      run_new<3, 1, 128, 4, 2>("analytic NT1 128x4 u2", q, sms, 16, 0, ie); }
     { InteractParams q = p; q.count = M / 32;
       run_new<2, 4, 256, 2, 1>("grid   NT4 256x2 u1 persistent dynamic [library]", q, sms, 16, 2, ig / 32);
       run_new<2, 4, 256, 2, 1>("grid   NT4 256x2 u1 persistent static", q, sms, 16, 1, ig / 32);

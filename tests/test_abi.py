@@ -43,7 +43,7 @@ def test_library_is_self_contained():
 
 def test_solve_opts_layout_and_defaults(lib):
     o = dbie.default_opts()
-    assert (o.method, o.maxiter, o.n_trial, o.n_level, o.use_eq12) == (0, 200, 8, 10, 1)
+    assert (o.method, o.maxiter, o.n_trial, o.n_level, o.use_eq12, o.analytic) == (0, 200, 8, 10, 1, 0)
     assert (o.delta, o.cell, o.w_g, o.eps_f, o.eps_g) == (1e-3, 1.0, 1.0, 1e-3, 1e-4)
     assert (o.lam0, o.step, o.xtol, o.ftol, o.lam_max) == (0.05, 0.05, 1e-4, 1e-6, 0.4)
     with pytest.raises(TypeError):
