@@ -65,7 +65,7 @@ typedef struct {
     double lam_max;             /* GRID: window [0, lam_max/h]                      */
     int use_eq12;               /* 1: Eq. 12 early exit enabled                     */
     int analytic;               /* 1: analytic gradient of Eq. 6 instead of the
-                                   finite differences of Eq. 13 (O-5, NM only)      */
+                                   finite differences of Eq. 13 (O-5)               */
 } orc_opts;
 
 /* ---------------------------------------------------------------- O-1 ---- */
@@ -507,6 +507,9 @@ void orc_solve_grid(const orc_boundary *b, const orc_opts *o, long M, const doub
         /* S[t][s][p]: component p at stencil position s (0, +x, +y, +z) for trial t;
          * slot T is the incumbent */
         double (*S)[4][3] = malloc(sizeof(double[4][3]) * (T + 1));
+        /* O-5 (opts.analytic): per candidate value B and the analytic gradient instead of the stencil */
+        double (*Bt)[3] = malloc(sizeof(double[3]) * (T + 1));
+        double (*Gt)[3][3] = malloc(sizeof(double[3][3]) * (T + 1));
         double *lt = malloc(sizeof(double) * 3 * (T + 1)); /* lt[p*(T+1)+t] */
         double lo[3] = { 0.0, 0.0, 0.0 }, W = Lmax;
         double best_phi = INFINITY, best_aux[9], mrg = INFINITY;
@@ -519,6 +522,7 @@ void orc_solve_grid(const orc_boundary *b, const orc_opts *o, long M, const doub
                     l[p] = lo[p] + W * (double)t / (double)(T - 1);
                     lt[p * (T + 1) + t] = l[p];
                 }
+                if (o->analytic) { eval_point_grad(b, x[i], y[i], z[i], l, Bt[t], Gt[t]); continue; }
                 eval_point(b, x[i], y[i], z[i], l, S[t][0]);
                 eval_point(b, x[i] + da, y[i], z[i], l, S[t][1]);
                 eval_point(b, x[i], y[i] + da, z[i], l, S[t][2]);
@@ -536,7 +540,16 @@ void orc_solve_grid(const orc_boundary *b, const orc_opts *o, long M, const doub
                             P0[p] = S[tt[p]][0][p]; Px[p] = S[tt[p]][1][p];
                             Py[p] = S[tt[p]][2][p]; Pz[p] = S[tt[p]][3][p];
                         }
-                        double ph = as_inf(residual_from_stencil(P0, Px, Py, Pz, da, dc,
+                        double ph;
+                        if (o->analytic) {
+                            double Gc[3][3];
+                            for (int p = 0; p < 3; ++p) {
+                                P0[p] = Bt[tt[p]][p];
+                                for (int j = 0; j < 3; ++j) Gc[p][j] = Gt[tt[p]][p][j];
+                            }
+                            ph = as_inf(residual_from_gradient(P0, Gc, dc, o->w_g, aux));
+                        } else
+                        ph = as_inf(residual_from_stencil(P0, Px, Py, Pz, da, dc,
                                                                  o->w_g, aux));
                         if (ph < lev_best) { /* strict: ties keep the lexicographically first */
                             lev_second = lev_best;
@@ -554,6 +567,11 @@ void orc_solve_grid(const orc_boundary *b, const orc_opts *o, long M, const doub
                 il[p] = lt[p * (T + 1) + bt[p]];
             }
             memcpy(S[T], inc, sizeof inc);
+            if (o->analytic)
+                for (int p = 0; p < 3; ++p) {
+                    Bt[T][p] = Bt[bt[p]][p];
+                    for (int j = 0; j < 3; ++j) Gt[T][p][j] = Gt[bt[p]][p][j];
+                }
             for (int p = 0; p < 3; ++p) lt[p * (T + 1) + T] = il[p];
             have_inc = 1;
             best_phi = lev_best; memcpy(best_aux, lev_aux, sizeof lev_aux);
@@ -586,7 +604,7 @@ void orc_solve_grid(const orc_boundary *b, const orc_opts *o, long M, const doub
             if (margin) margin[i] = mrg;
             if (phi) phi[i] = best_phi;
         }
-        free(S); free(lt);
+        free(S); free(lt); free(Bt); free(Gt);
     }
 }
 

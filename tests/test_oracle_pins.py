@@ -415,12 +415,15 @@ def test_solver_invalid_points_and_statuses():
 
 
 # -- O-4 (GRID) ---------------------------------------------------------------
-def test_grid_mode_brute_force_and_monotone():
+@pytest.mark.parametrize("analytic", [0, 1])
+def test_grid_mode_brute_force_and_monotone(analytic):
+    """O-4 with Eq. 13 differences and with the analytic gradient (O-5): the separable candidate
+    assembly must equal a direct objective evaluation at every lattice triple."""
     w = random_boundary(5, 6, seed=8, npts=3, zmin=1.0, zmax=3.0)
     T = 4
     phis = []
     for nl in (1, 2, 3, 5):
-        o = oracle.Opts(method=1, n_trial=T, n_level=nl, lam_max=0.4, use_eq12=0)
+        o = oracle.Opts(method=1, n_trial=T, n_level=nl, lam_max=0.4, use_eq12=0, analytic=analytic)
         sol = oracle.solve_grid(w, o)
         phis.append(sol["phi"].copy())
         # returned residual is the residual at the returned lambda
@@ -436,7 +439,7 @@ def test_grid_mode_brute_force_and_monotone():
         for a in ax:
             for b in ax:
                 for c in ax:
-                    r = oracle.residual(w.subset([i]), np.array([[a], [b], [c]]))
+                    r = oracle.residual(w.subset([i]), np.array([[a], [b], [c]]), oracle.Opts(analytic=analytic))
                     best = min(best, r["phi"][0])
         assert abs(phis[0, i] - best) < 1e-9
 
