@@ -112,6 +112,11 @@ class ClockSampler:
                 "samples": len(sm), "reasons": sorted(reasons)}
 
 
+# DRAM bytes of ONE launch of the interaction kernel from the committed `ncu --set full` captures
+# (dram__bytes_read.sum + dram__bytes_write.sum; profiles/r01_ncu_full_interact64_*.md).  Static evidence that
+# HBM is idle (the bound is the FP64 pipe); None where no capture of that workload/mode exists.
+NCU_TRAFFIC = {("cfg2", "nm"): 7.47e6 + 46.07e6}
+
 METHOD = {"grid": False, "analytic": False}   # set by main(): GRID (O-4) instead of NM; analytic gradient (O-5)
 
 
@@ -122,9 +127,9 @@ def oracle_timed(wl, npoints: int, seed_offset: int, nthreads: int = 0) -> dict:
     sub, _ = wl.seeded_subset(npoints, seed_offset=seed_offset)
     t0 = time.perf_counter()
     if wl.lam is None and METHOD["grid"]:
-        o = oracle.Opts(method=1)
+        o = oracle.Opts(method=1, analytic=1 if METHOD["analytic"] else 0)
         out = oracle.solve_grid(sub, o, nthreads=nthreads)
-        inter = float(out["iters"].sum()) * o.n_trial * 4.0 * wl.N
+        inter = float(out["iters"].sum()) * o.n_trial * (1.0 if o.analytic else 4.0) * wl.N
     elif wl.lam is None:
         an = 1 if METHOD["analytic"] else 0
         out = oracle.solve_nm(sub, oracle.Opts(analytic=an), nthreads=nthreads)
@@ -221,8 +226,7 @@ def run_ours(args) -> None:
 
     wl = make_workload(args.workload, rank, world, points=args.points)
     is_solve = wl.lam is None
-    sopts = dbie.default_opts(method=1) if METHOD["grid"] else (
-        dbie.default_opts(analytic=1) if METHOD["analytic"] else None)
+    sopts = dbie.default_opts(method=1 if METHOD["grid"] else 0, analytic=1 if METHOD["analytic"] else 0)
     t = lambda a: torch.from_numpy(np.ascontiguousarray(a, dtype=np.float64)).to(dev)
     d_bx, d_by, d_bz = t(wl.bx), t(wl.by), t(wl.bz)
     d_x, d_y, d_z = t(wl.x), t(wl.y), t(wl.z)
@@ -312,13 +316,17 @@ def run_ours(args) -> None:
     sm_max = (clocks or {}).get("sm_max_mhz") or 1965.0
     peak_slots = SM_COUNT * FP64_LANES_PER_SM * sm_max * 1e6          # FP64 lane-instructions / s
     kern_ips = inter_total / (kern_ms * 1e-3) if kern_ms > 0 else 0.0
-    per_inter = FP64_INSTR_GRID[4] if (is_solve and METHOD["grid"]) else (
-        FP64_INSTR_ANALYTIC if (is_solve and METHOD["analytic"]) else FP64_INSTR_PER_INTERACTION)
+    per_inter = FP64_INSTR_ANALYTIC if (is_solve and METHOD["analytic"]) else (
+        FP64_INSTR_GRID[4] if (is_solve and METHOD["grid"]) else FP64_INSTR_PER_INTERACTION)
     achieved_slots = kern_ips * per_inter
     roofline = {
         "bound": "alu", "kernel": "dbie::interact64_kernel (fp64 point-pixel sums)",
         "achieved": 2e-12 * achieved_slots, "peak": 2e-12 * peak_slots, "unit": "TFLOP/s",
-        "frac": achieved_slots / peak_slots, "traffic": None,
+        "frac": achieved_slots / peak_slots,
+        "traffic": NCU_TRAFFIC.get((args.workload, "grid" if METHOD["grid"] else ("analytic" if METHOD["analytic"] else "nm"))
+                                   if (is_solve and args.points == 0) else None),
+        "traffic_note": "bytes of the launch with all points active (ncu capture, profiles/); algorithmic: 6.8 MB of point "
+                        "data in + 100 MB of chunk partial sums out, of which the L2 keeps half",
         "note": "FP64-pipe bound (no HBM/tensor step): achieved = interactions/s of the kernel x FP64 "
                 "lane-instructions per interaction (76; GRID with 4 trial triples per geometry 66.25; DESIGN.md s6) "
                 "x 2 flop per FMA slot; peak = 148 SM x 64 FP64 lanes x clocks.max.sm (derived, DESIGN.md s7)",
@@ -460,7 +468,7 @@ def main():
                     help="target CPU time of the cpu_baseline leg (0 disables it)")
     args = ap.parse_args()
     METHOD["grid"] = (args.method == "grid") or (args.method is None and args.workload == "cfg5")
-    METHOD["analytic"] = args.gradient == "analytic" and not METHOD["grid"]
+    METHOD["analytic"] = args.gradient == "analytic"
     if args.impl == "reference":
         run_reference(args)
     elif args.dtype == "f32":

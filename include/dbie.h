@@ -115,8 +115,7 @@ typedef struct {
                          over the same pixels with d/dr[n(lambda r)/r^3] = lambda^2 cos(lambda r)/r^2
                          - 3 n(lambda r)/r^4 ("possible if the function f_i can be
                          calculated analytically"; O-5): one evaluation position instead
-                         of four per objective evaluation; delta is ignored.  Method 0 (NM) and
-                         dbie_residual only; with method 1 dbie_solve returns DBIE_EINVAL.       */
+                         of four per objective evaluation; delta is ignored.                                  */
 } dbie_solve_opts;
 
 void dbie_solve_default_opts(dbie_solve_opts* opts);

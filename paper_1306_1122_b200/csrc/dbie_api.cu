@@ -457,7 +457,7 @@ static dbie_status solve_grid(dbie_ctx* ctx, long long M, const double* x, const
             p.part = ctx->part; p.cap = cap;
             p.lo = a.lo; p.ldlo = cap; p.W = W; p.T = T;
             prof_mark(ctx, st);
-            CU(launch_interact_grid(p, ctx->sm_count, st));
+            CU(k.analytic ? launch_interact_grid_analytic(p, ctx->sm_count, st) : launch_interact_grid(p, ctx->sm_count, st));
             prof_mark(ctx, st);
             CU(launch_grid_step(a, k, gc, bd, lev, cnt, M, z + off, ctx->part, cap, B + off, lam + off, resid + off,
                                 iters + off, status + off, nevals, st));
@@ -467,7 +467,7 @@ static dbie_status solve_grid(dbie_ctx* ctx, long long M, const double* x, const
     }
     ctx->last_launches = launches;
     ctx->evals_on_device = 1;
-    ctx->positions_per_eval = kStencil;
+    ctx->positions_per_eval = k.analytic ? 1 : kStencil;
     return DBIE_OK;
 }
 
@@ -481,7 +481,6 @@ extern "C" dbie_status dbie_solve(dbie_ctx* ctx, long long M, const double* x, c
     NMConsts k;
     dbie_status s = make_consts(ctx, opts, &k);
     if (s != DBIE_OK) return s;
-    if (opts && opts->method == 1 && opts->analytic) return DBIE_EINVAL;
     if (opts && opts->method == 1) return solve_grid(ctx, M, x, y, z, opts, k, B, lam, resid, iters, status, cuda_stream);
     if (opts && opts->method != 0) return DBIE_EINVAL;
     cudaStream_t st = (cudaStream_t)cuda_stream;

@@ -70,20 +70,49 @@ grid_step_kernel(GridArrays s, NMConsts k, GridConsts gc, int nchunks, int lev, 
     const double c3 = mul_(add_(zi, k.delta_abs), k.h2_over_2pi);
     const long long Q = 12LL * T;
 
-    // A4: chunk sums in chunk order -> B at the stencil for every trial
-    for (int q = lane; q < 12 * T; q += 32) {
-        const int sp = q / T, t = q - sp * T;
-        double sum = part[(long long)q * cap + j];
-        for (int ch = 1; ch < nchunks; ++ch) sum = add_(sum, part[((long long)ch * Q + q) * cap + j]);
-        S[t * 12 + sp] = mul_(sp >= 9 ? c3 : c0, sum);
-    }
-    if (lane < 12) S[T * 12 + lane] = (lev > 0) ? s.inc[lane * s.cap + id] : 0.0;   // the incumbent
-    __syncwarp();
     const int C = (lev > 0) ? C1 : T;   // level 0 has no incumbent
-    // Eq. 13: forward differences, once per (candidate value, component)
-    for (int e = lane; e < C * 9; e += 32) {
-        const int t = e / 9, r9 = e - t * 9, p = r9 / 3, jj = r9 - p * 3;
-        G[e] = div_(sub_(S[t * 12 + (jj + 1) * 3 + p], S[t * 12 + p]), k.delta_abs);
+    if (!k.analytic) {
+        // A4: chunk sums in chunk order -> B at the stencil for every trial
+        for (int q = lane; q < 12 * T; q += 32) {
+            const int sp = q / T, t = q - sp * T;
+            double sum = part[(long long)q * cap + j];
+            for (int ch = 1; ch < nchunks; ++ch) sum = add_(sum, part[((long long)ch * Q + q) * cap + j]);
+            S[t * 12 + sp] = mul_(sp >= 9 ? c3 : c0, sum);
+        }
+        if (lane < 12) S[T * 12 + lane] = (lev > 0) ? s.inc[lane * s.cap + id] : 0.0;   // the incumbent
+        __syncwarp();
+        // Eq. 13: forward differences, once per (candidate value, component)
+        for (int e = lane; e < C * 9; e += 32) {
+            const int t = e / 9, r9 = e - t * 9, p = r9 / 3, jj = r9 - p * 3;
+            G[e] = div_(sub_(S[t * 12 + (jj + 1) * 3 + p], S[t * 12 + p]), k.delta_abs);
+        }
+    } else {
+        // O-5: raw sums S[t*12 + kind*3 + p], kind = (K b, D dx b, D dy b, D b) -> B and the gradient
+        for (int q = lane; q < 12 * T; q += 32) {
+            const int sp = q / T, t = q - sp * T;
+            double sum = part[(long long)q * cap + j];
+            for (int ch = 1; ch < nchunks; ++ch) sum = add_(sum, part[((long long)ch * Q + q) * cap + j]);
+            S[t * 12 + sp] = sum;
+        }
+        __syncwarp();
+        const double zz = mul_(zi, zi);
+        for (int e = lane; e < T * 9; e += 32) {
+            const int t = e / 9, r9 = e - t * 9, p = r9 / 3, jj = r9 - p * 3;
+            const double* St = S + t * 12;
+            G[e] = (jj == 0)   ? -mul_(c0, St[3 + p])
+                   : (jj == 1) ? -mul_(c0, St[6 + p])
+                               : mul_(k.h2_over_2pi, add_(St[p], mul_(zz, St[9 + p])));
+        }
+        __syncwarp();
+        for (int e = lane; e < T * 3; e += 32) {
+            const int t = e / 3, p = e - t * 3;
+            S[t * 12 + p] = mul_(c0, S[t * 12 + p]);   // B_p (after d/dz has used the raw sum)
+        }
+        if (lev > 0 && lane < 12) {   // the incumbent: inc[0..2] = B, inc[3 + p*3 + jj] = dB_p/dx_jj
+            const double v = s.inc[lane * s.cap + id];
+            if (lane < 3) S[T * 12 + lane] = v;
+            else G[T * 9 + lane - 3] = v;
+        }
     }
     __syncwarp();
 
@@ -142,7 +171,11 @@ grid_step_kernel(GridArrays s, NMConsts k, GridConsts gc, int nchunks, int lev, 
         return;
     }
     // the argmin becomes the incumbent; next window centred on it, clipped to [0, lam_max/h]
-    if (lane < 12) s.inc[lane * s.cap + id] = S[bt[lane % 3] * 12 + lane];
+    if (lane < 12) {
+        if (!k.analytic) s.inc[lane * s.cap + id] = S[bt[lane % 3] * 12 + lane];
+        else if (lane < 3) s.inc[lane * s.cap + id] = S[bt[lane] * 12 + lane];
+        else s.inc[lane * s.cap + id] = G[bt[(lane - 3) / 3] * 9 + lane - 3];
+    }
     if (lane == 0) {
         for (int p = 0; p < 3; ++p) {
             double l = sub_(il[p], mul_(0.5, gc.Wn));

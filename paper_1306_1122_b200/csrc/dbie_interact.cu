@@ -64,7 +64,7 @@ static cudaError_t launch64(const InteractParams& p, int sm_count, int waves, cu
         grid = (long long)sm_count * kMinB64;   // persistent: the slot count lives on the device
     } else {
         if (q.count <= 0) return cudaSuccess;
-        const int G = (MODE == MODE_GRID) ? q.T / NT : 1;
+        const int G = (MODE == MODE_GRID || MODE == MODE_GRID_ANALYTIC) ? q.T / NT : 1;
         const long long nitems = q.count * items_per_slot(MODE, G);
         const long long nblk = (nitems + kThreads64 - 1) / kThreads64;
         long long nsplit = 1;
@@ -89,6 +89,13 @@ cudaError_t launch_interact_stencil(const InteractParams& p, int sm_count, cudaS
 
 cudaError_t launch_interact_analytic(const InteractParams& p, int sm_count, cudaStream_t st) {
     return launch64<MODE_ANALYTIC, 1, 1>(p, sm_count, 16, st);
+}
+
+cudaError_t launch_interact_grid_analytic(const InteractParams& p, int sm_count, cudaStream_t st) {
+    // one trial triple per thread: two (24 accumulators + 2 x 6 lambda, lambda^2) need 168 registers,
+    // which the 256 x 2 shape does not have (spills); sharing the geometry would save 7 of 95 instructions
+    if (p.T < 2) return cudaErrorInvalidValue;
+    return launch64<MODE_GRID_ANALYTIC, 1, 2>(p, sm_count, 16, st);
 }
 
 cudaError_t launch_interact_grid(const InteractParams& p, int sm_count, cudaStream_t st) {

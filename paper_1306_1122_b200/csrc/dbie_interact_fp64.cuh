@@ -27,17 +27,21 @@ namespace dbie {
 // MODE_ANALYTIC (O-5): one position per field point; besides the Eq. 6 sum
 // it accumulates the three sums of the analytic gradient (kinds 1..3 below), 12 sums per slot like
 // the stencil, from the same sincos: d/dr[n(lambda r)/r^3] = lambda^2 cos(lambda r)/r^2 - 3 n/r^4.
-enum { MODE_EVAL = 0, MODE_STENCIL = 1, MODE_GRID = 2, MODE_ANALYTIC = 3 };
+// MODE_GRID_ANALYTIC: the same four sums for NT trial triples of GRID mode (item = slot * G + g).
+enum { MODE_EVAL = 0, MODE_STENCIL = 1, MODE_GRID = 2, MODE_ANALYTIC = 3, MODE_GRID_ANALYTIC = 4 };
 
 // items (threads' units of work) per slot
 __host__ __device__ inline long long items_per_slot(int mode, int G) {
-    return (mode == MODE_EVAL || mode == MODE_ANALYTIC) ? 1
-                                                         : (mode == MODE_STENCIL ? kStencil : (long long)kStencil * G);
+    if (mode == MODE_EVAL || mode == MODE_ANALYTIC) return 1;
+    if (mode == MODE_GRID_ANALYTIC) return G;
+    return mode == MODE_STENCIL ? kStencil : (long long)kStencil * G;
 }
 
 template <int MODE, int NT, int THREADS, int MINB, int UNR>
 __global__ void __launch_bounds__(THREADS, MINB) interact64_kernel(const __grid_constant__ InteractParams p) {
-    static_assert(MODE == MODE_GRID || NT == 1, "only GRID mode carries several lambda triples per thread");
+    constexpr bool kGridLam = (MODE == MODE_GRID || MODE == MODE_GRID_ANALYTIC);   // lambda from the GRID window
+    constexpr bool kAnalytic = (MODE == MODE_ANALYTIC || MODE == MODE_GRID_ANALYTIC);
+    static_assert(kGridLam || NT == 1, "only GRID modes carry several lambda triples per thread");
     __shared__ alignas(128) double4 tile[2][kTilePx];
     __shared__ alignas(8) uint64_t full[2];
     __shared__ long long next_item;
@@ -55,7 +59,7 @@ __global__ void __launch_bounds__(THREADS, MINB) interact64_kernel(const __grid_
         if (p.zero_work) *p.zero_work = 0u;  // next pass's work counter
     }
     const long long count = p.count_ptr ? (long long)(*p.count_ptr) : p.count;   // slots
-    const int G = (MODE == MODE_GRID) ? p.T / NT : 1;
+    const int G = kGridLam ? p.T / NT : 1;
     const long long nitems = count * items_per_slot(MODE, G);
     const long long nblk = (nitems + THREADS - 1) / THREADS;
     if (nblk == 0) return;
@@ -95,6 +99,9 @@ __global__ void __launch_bounds__(THREADS, MINB) interact64_kernel(const __grid_
         } else if (MODE == MODE_STENCIL) {
             slot = jt >> 2;
             s = (int)(jt & 3);
+        } else if (MODE == MODE_GRID_ANALYTIC) {
+            g = (int)(jt % G);
+            slot = jt / G;
         } else {
             g = (int)(jt % G);
             const long long js = jt / G;
@@ -110,7 +117,7 @@ __global__ void __launch_bounds__(THREADS, MINB) interact64_kernel(const __grid_
         }
         const double z2 = zi * zi;
         double lam[NT][3];
-        if (MODE == MODE_GRID) {
+        if (kGridLam) {
             // trial t of component c: lo_c + W t/(T-1), each operation rounded separately (O-4)
 #pragma unroll
             for (int c = 0; c < 3; ++c) {
@@ -127,13 +134,16 @@ __global__ void __launch_bounds__(THREADS, MINB) interact64_kernel(const __grid_
         }
 
         // accumulators: one row per lambda triple; MODE_ANALYTIC: rows = sum K b, sum D dx b, sum D dy b, sum D b
-        constexpr int NA = (MODE == MODE_ANALYTIC) ? 4 : NT;
+        // (row 4 tt + kind in the analytic modes)
+        constexpr int NA = kAnalytic ? 4 * NT : NT;
         double acc[NA][3];
 #pragma unroll
         for (int tt = 0; tt < NA; ++tt) acc[tt][0] = acc[tt][1] = acc[tt][2] = 0.0;
-        double lam2[3];   // MODE_ANALYTIC: lambda^2
+        double lam2[NT][3];   // analytic modes: lambda^2
 #pragma unroll
-        for (int c = 0; c < 3; ++c) lam2[c] = lam[0][c] * lam[0][c];
+        for (int tt = 0; tt < NT; ++tt)
+#pragma unroll
+            for (int c = 0; c < 3; ++c) lam2[tt][c] = lam[tt][c] * lam[tt][c];
 
         const int t0 = chunk_first_tile(bd, c0), t1 = chunk_first_tile(bd, c1);
         int c = c0;
@@ -166,23 +176,25 @@ __global__ void __launch_bounds__(THREADS, MINB) interact64_kernel(const __grid_
                     const double rr = r2 * y;          // r
                     const double wgt = (y * y) * y;    // 1/r^3
                     const double wx = wgt * px.y, wy = wgt * px.z, wz = wgt * px.w;
-                    if (MODE == MODE_ANALYTIC) {
+                    if (kAnalytic) {
                         // K b = n w b;  D b = (lambda^2 cos(theta) - 3 n / r^2) w b  (w = 1/r^3)
                         const double m3y2 = (y * y) * -3.0;
                         const double wb[3] = {wx, wy, wz};
 #pragma unroll
-                        for (int c = 0; c < 3; ++c) {
-                            double n, cs;
-                            int sg;
-                            kernel_n_cos(lam[0][c] * rr, n, cs, sg);
-                            const double wbs = flip_sign_if(wb[c], sg);
-                            const double e = fma(lam2[c], cs, n * m3y2);
-                            const double gb = e * wbs;
-                            acc[0][c] = fma(n, wbs, acc[0][c]);
-                            acc[1][c] = fma(gb, dx, acc[1][c]);
-                            acc[2][c] = fma(gb, dy, acc[2][c]);
-                            acc[3][c] += gb;
-                        }
+                        for (int tt = 0; tt < NT; ++tt)
+#pragma unroll
+                            for (int c = 0; c < 3; ++c) {
+                                double n, cs;
+                                int sg;
+                                kernel_n_cos(lam[tt][c] * rr, n, cs, sg);
+                                const double wbs = flip_sign_if(wb[c], sg);
+                                const double e = fma(lam2[tt][c], cs, n * m3y2);
+                                const double gb = e * wbs;
+                                acc[4 * tt + 0][c] = fma(n, wbs, acc[4 * tt + 0][c]);
+                                acc[4 * tt + 1][c] = fma(gb, dx, acc[4 * tt + 1][c]);
+                                acc[4 * tt + 2][c] = fma(gb, dy, acc[4 * tt + 2][c]);
+                                acc[4 * tt + 3][c] += gb;
+                            }
                         continue;
                     }
 #pragma unroll
@@ -209,6 +221,16 @@ __global__ void __launch_bounds__(THREADS, MINB) interact64_kernel(const __grid_
 #pragma unroll
                             for (int q = 0; q < 3; ++q)
                                 p.part[((long long)c * 12 + kd * 3 + q) * p.cap + slot] = acc[kd][q];
+                    } else if (MODE == MODE_GRID_ANALYTIC) {
+                        const long long Q = 12LL * p.T;
+#pragma unroll
+                        for (int tt = 0; tt < NT; ++tt)
+#pragma unroll
+                            for (int kd = 0; kd < 4; ++kd)
+#pragma unroll
+                                for (int q = 0; q < 3; ++q)
+                                    p.part[(c * Q + (long long)(kd * 3 + q) * p.T + g * NT + tt) * p.cap + slot] =
+                                        acc[4 * tt + kd][q];
                     } else {
                         const long long Q = 12LL * p.T;
 #pragma unroll

@@ -138,6 +138,7 @@ cudaError_t launch_interact_eval(const InteractParams& p, int sm_count, cudaStre
 cudaError_t launch_interact_stencil(const InteractParams& p, int sm_count, cudaStream_t st);
 cudaError_t launch_interact_grid(const InteractParams& p, int sm_count, cudaStream_t st);
 cudaError_t launch_interact_analytic(const InteractParams& p, int sm_count, cudaStream_t st);
+cudaError_t launch_interact_grid_analytic(const InteractParams& p, int sm_count, cudaStream_t st);
 cudaError_t launch_eval_finalize(const BoundaryView& bd, long long slot0, long long count,
                                  long long M, const double* z, const double* lam, const double* part,
                                  long long cap, double* B, cudaStream_t st);

@@ -484,7 +484,17 @@ def test_analytic_solve_config3_options_and_invalid_points(dbie):
     w.z[3] = 0.0
     s, so, info = _check_solve_parity(dbie, w, dict(analytic=1, use_eq12=0, maxiter=60, w_g=2.0, cell=0.5))
     assert s["status"][3] == 3
-    with dbie.DBIE.from_workload(w) as ctx:
-        dw = dbie.to_device(w)
-        with pytest.raises(dbie.DBIEError):      # GRID with the analytic gradient is not built
-            ctx.solve(dw.x, dw.y, dw.z, dbie.default_opts(method=1, analytic=1))
+
+
+@pytest.mark.parametrize("T,levels", [(8, 6), (5, 3)])
+def test_analytic_grid_config2_subset(dbie, T, levels):
+    """GRID search on the analytic gradient (O-4 + O-5): even and odd T."""
+    w, _ = workloads.config2().seeded_subset(64, seed_offset=13)
+    _check_solve_parity(dbie, w, dict(method=1, analytic=1, n_trial=T, n_level=levels))
+
+
+def test_analytic_grid_config5_large_batch_sampled(dbie):
+    """BASELINE configs[4] boundary: GRID (T = 8, 3 levels) with the analytic gradient on a
+    4,096-point subset in one call; 6 sampled points re-solved by the oracle."""
+    w, _ = workloads.config5().seeded_subset(4096, seed_offset=6)
+    _solve_full_and_sample(dbie, w, 6, dict(method=1, analytic=1, n_level=3))
