@@ -498,3 +498,26 @@ def test_analytic_grid_config5_large_batch_sampled(dbie):
     4,096-point subset in one call; 6 sampled points re-solved by the oracle."""
     w, _ = workloads.config5().seeded_subset(4096, seed_offset=6)
     _solve_full_and_sample(dbie, w, 6, dict(method=1, analytic=1, n_level=3))
+
+
+# ---------------------------------------------- the paper's own validation case (SURVEY f2) --
+def test_lowlou_case2_figures_of_merit(dbie):
+    """PAPER.md:145-163 / Table 1: Low & Lou n = 3, m = 1, l = 0.3, Phi = 4 pi/5, 192x192 boundary
+    around the 64^3 region, "bottom boundary only".  The paper prints C_vec 0.99, C_cs 0.52,
+    E'_n 0.83, E'_m -0.53, eps 1.08 for its DBIE; with the readings of DESIGN.md section 3 (its
+    quadrature, thresholds, simplex and objective are not given) this build measures
+    C_vec 0.918, C_cs 0.25, E'_n -0.48, eps 1.40, so Table 1 is NOT reproduced and stays "parity
+    unpinned".  Gated here: the pipeline runs at the paper's size, the GPU field
+    matches the oracle on sampled points, and the figures stay where this build measured them."""
+    import torch
+    w = workloads.lowlou_case2()
+    Bex = np.array(w.extra["lowlou"].field(w.x, w.y, w.z)) * w.extra["scale"]
+    (_, _, info), s = _solve_full_and_sample(dbie, w, 24, dict(analytic=1))
+    m = workloads.figures_of_merit(Bex, s["B"])
+    assert 0.88 < m["C_vec"] < 0.96 and 1.2 < m["eps"] < 1.6, m
+    with dbie.DBIE.from_workload(w) as ctx:
+        dw = dbie.to_device(w)
+        pot = ctx.eval(dw.x, dw.y, dw.z, torch.zeros((3, w.M), dtype=torch.float64, device="cuda")).cpu().numpy()
+    mp_ = workloads.figures_of_merit(Bex, pot)
+    assert 0.90 < mp_["C_vec"] < 0.97                      # lambda = 0 (potential) field, same window
+    assert float(np.mean(s["f"])) < 0.2                    # far more force-free than the potential field

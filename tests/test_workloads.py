@@ -62,3 +62,32 @@ def test_s2_s3_lowlou_solve_invariants():
     chk = oracle.residual(s, sol["lam"], o)
     assert np.allclose(chk["B"], sol["B"], rtol=1e-12, atol=0)
     assert np.allclose(chk["f"], sol["f"], atol=1e-9) and np.allclose(chk["g"], sol["g"], atol=1e-9)
+
+
+def test_lowlou_case2_generator_and_figures_of_merit():
+    """the n = 3, m = 1, Phi = 4 pi/5 field of the paper's Table 1 is force-free
+    (same central-difference self-check), the workload has the paper's shape (192x192 boundary
+    around a 64^3 region), and the five figures of merit are 1, 1, 1, 1, 1 for b = B and behave as
+    defined for a scaled / rotated copy."""
+    from workloads import lowlou_case2, figures_of_merit
+    w = lowlou_case2()
+    ll = w.extra["lowlou"]
+    assert (w.nx, w.ny, w.M) == (192, 192, 64 ** 3) and abs(w.x0 + 3.0) < 1e-12 and abs(w.h - 2 / 64) < 1e-15
+    assert abs(np.abs(w.bz).max() - 1.0) < 1e-12
+    rng = np.random.default_rng(1)
+    d = 1e-5
+    for _ in range(4):
+        q = np.array([rng.uniform(-0.8, 0.8), rng.uniform(-0.8, 0.8), rng.uniform(0.05, 1.0)])
+        B = lambda v: np.array(ll.field(v[0], v[1], v[2]))
+        G = np.stack([(B(q + d * e) - B(q - d * e)) / (2 * d) for e in np.eye(3)], axis=1)
+        J = np.array([G[2, 1] - G[1, 2], G[0, 2] - G[2, 0], G[1, 0] - G[0, 1]])
+        assert abs(np.trace(G)) < 1e-6 * np.abs(G).max()
+        assert np.linalg.norm(J - ll.alpha(*q) * B(q)) < 1e-6 * np.linalg.norm(J)
+    Bx = rng.normal(size=(3, 500))
+    m = figures_of_merit(Bx, Bx)
+    assert all(abs(v - 1.0) < 1e-12 for v in m.values())
+    m2 = figures_of_merit(Bx, 2.0 * Bx)
+    assert abs(m2["C_vec"] - 1) < 1e-12 and abs(m2["C_cs"] - 1) < 1e-12 and abs(m2["eps"] - 4) < 1e-12
+    assert abs(m2["E_n_prime"]) < 1e-12 and abs(m2["E_m_prime"]) < 1e-12
+    m3 = figures_of_merit(Bx, -Bx)
+    assert abs(m3["C_vec"] + 1) < 1e-12 and abs(m3["E_n_prime"] + 1) < 1e-12

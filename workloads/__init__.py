@@ -137,6 +137,41 @@ def config2(nb: int = 64, nz: int = 32, n: int = 1, m: int = 1, l: float = 0.3,
                     extra={"lowlou": ll, "scale": scale})
 
 
+def lowlou_case2(nb: int = 192, nv: int = 64) -> Workload:
+    """the paper's own validation case (Table 1): Low & Lou
+    n = 3, m = 1, l = 0.3, Phi = 4 pi/5; the test region is [-1,1]^2 x (0,2] sampled by nv^3 points
+    (pixel size h = 2/nv) and the bottom boundary is the nb x nb window centred on it ([-3,3]^2 for
+    nb = 3 nv), "bottom boundary only".  Points: pixel centres x z = (k+1) h (reading A-14's
+    convention; the paper does not say where its 64 layers sit).  Normalised to max|Bz| = 1."""
+    ll = LowLou(n=3, m=1, l=0.3, Phi=4.0 * math.pi / 5.0)
+    h = 2.0 / nv
+    half = 0.5 * nb * h
+    xb = pixel_centres(nb, h, -half)
+    Y, X = np.meshgrid(xb, xb, indexing="ij")
+    bx, by, bz = ll.field(X.ravel(), Y.ravel(), np.zeros(nb * nb))
+    scale = 1.0 / np.max(np.abs(bz))
+    xs = pixel_centres(nv, h, -1.0)
+    zs = (np.arange(nv, dtype=np.float64) + 1.0) * h
+    x, y, z = _grid_points(xs, xs, zs)
+    return Workload("lowlou_case2", nb, nb, h, -half, -half, bx * scale, by * scale, bz * scale, x, y, z, None,
+                    extra={"lowlou": ll, "scale": scale})
+
+
+def figures_of_merit(B, b) -> dict:
+    """The five figures of merit of Table 1 (the paper defers their definition
+    to Schrijver et al. 2006): B exact, b reconstructed, both (3, M).  Evaluation metrics, not part
+    of the method."""
+    B = np.asarray(B, dtype=np.float64); b = np.asarray(b, dtype=np.float64)
+    nB = np.linalg.norm(B, axis=0); nb_ = np.linalg.norm(b, axis=0)
+    dot = np.sum(B * b, axis=0)
+    d = np.linalg.norm(b - B, axis=0)
+    return {"C_vec": float(dot.sum() / math.sqrt(np.sum(nB ** 2) * np.sum(nb_ ** 2))),
+            "C_cs": float(np.mean(dot / (nB * nb_))),
+            "E_n_prime": float(1.0 - d.sum() / nB.sum()),
+            "E_m_prime": float(1.0 - np.mean(d / nB)),
+            "eps": float(np.sum(nb_ ** 2) / np.sum(nB ** 2))}
+
+
 # ----------------------------------------------------------------------------
 # configs 3-5: Gaussian-spot active regions
 # ----------------------------------------------------------------------------
