@@ -455,7 +455,7 @@ static dbie_status solve_grid(dbie_ctx* ctx, long long M, const double* x, const
             p.zero_work = ctx->counters + 8 + ((lev + 1) & 1);
             p.delta_abs = k.delta_abs;
             p.part = ctx->part; p.cap = cap;
-            p.lo = a.lo; p.ldlo = cap; p.W = W; p.T = T;
+            p.lo = a.lo; p.ldlo = cap; p.W = W; p.T = T; p.dlam = W / (double)(T - 1);
             prof_mark(ctx, st);
             CU(k.analytic ? launch_interact_grid_analytic(p, ctx->sm_count, st) : launch_interact_grid(p, ctx->sm_count, st));
             prof_mark(ctx, st);

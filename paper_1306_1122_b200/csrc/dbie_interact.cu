@@ -55,18 +55,18 @@ cudaError_t launch_stage_boundary(int nx, int ny, double h, double x0, double y0
 // 4 (else 2, else 1) trial lambda triples per thread on one geometry.
 constexpr int kThreads64 = 256, kMinB64 = 2;
 
-template <int MODE, int NT, int UNR>
+template <int MODE, int NT, int UNR, int THREADS = kThreads64, int MINB = kMinB64>
 static cudaError_t launch64(const InteractParams& p, int sm_count, int waves, cudaStream_t st) {
     InteractParams q = p;
-    q.target_items = waves * sm_count * kMinB64;
+    q.target_items = waves * sm_count * MINB;
     long long grid;
     if (q.count_ptr) {
-        grid = (long long)sm_count * kMinB64;   // persistent: the slot count lives on the device
+        grid = (long long)sm_count * MINB;   // persistent: the slot count lives on the device
     } else {
         if (q.count <= 0) return cudaSuccess;
         const int G = (MODE == MODE_GRID || MODE == MODE_GRID_ANALYTIC) ? q.T / NT : 1;
         const long long nitems = q.count * items_per_slot(MODE, G);
-        const long long nblk = (nitems + kThreads64 - 1) / kThreads64;
+        const long long nblk = (nitems + THREADS - 1) / THREADS;
         long long nsplit = 1;
         if (nblk < q.target_items) {
             nsplit = (q.target_items + nblk - 1) / nblk;
@@ -75,7 +75,7 @@ static cudaError_t launch64(const InteractParams& p, int sm_count, int waves, cu
         grid = nblk * nsplit;   // one work item per CTA: the hardware balances them
         if (grid > 0x7fffffffLL) return cudaErrorInvalidValue;
     }
-    interact64_kernel<MODE, NT, kThreads64, kMinB64, UNR><<<(unsigned)grid, kThreads64, 0, st>>>(q);
+    interact64_kernel<MODE, NT, THREADS, MINB, UNR><<<(unsigned)grid, THREADS, 0, st>>>(q);
     return cudaGetLastError();
 }
 
@@ -100,8 +100,11 @@ cudaError_t launch_interact_grid_analytic(const InteractParams& p, int sm_count,
 
 cudaError_t launch_interact_grid(const InteractParams& p, int sm_count, cudaStream_t st) {
     if (p.T < 2) return cudaErrorInvalidValue;
+    // NT > 1 uses the rotation recurrence, which needs window starts lo >= 0: not guaranteed for T = 2
+    // 8 trial triples per thread need 234 registers: 128 threads x 2 CTAs/SM (profiles/r01_variants.md)
+    if (p.T % 8 == 0) return launch64<MODE_GRID, 8, 1, 128, 2>(p, sm_count, 16, st);
     if (p.T % 4 == 0) return launch64<MODE_GRID, 4, 1>(p, sm_count, 16, st);
-    if (p.T % 2 == 0) return launch64<MODE_GRID, 2, 2>(p, sm_count, 16, st);
+    if (p.T % 2 == 0 && p.T > 2) return launch64<MODE_GRID, 2, 2>(p, sm_count, 16, st);
     return launch64<MODE_GRID, 1, 2>(p, sm_count, 16, st);
 }
 

@@ -197,6 +197,46 @@ __global__ void __launch_bounds__(THREADS, MINB) interact64_kernel(const __grid_
                             }
                         continue;
                     }
+                    if (MODE == MODE_GRID && NT > 1) {
+                        // The NT trial values of a component are equally spaced (lambda_t = lo + W t/(T-1)), so
+                        // theta advances by the same d_theta = W/(T-1) r for all three components: one full
+                        // sincos per component for the first trial, one for d_theta, and a plane rotation
+                        // (4 FP64 instructions) per further trial instead of a 17-instruction sincos.  The
+                        // rotated angle theta_0 + tt d_theta differs from fl(lambda_tt r) by a few ulp(theta),
+                        // the size of the rounding theta carries anyway; at most NT/2 <= 4 rotation steps from the middle trial.
+                        // Needs lo >= 0 (no |.| fold inside the group): true for T >= 3 (the launcher sends T = 2 to NT = 1).
+                        double sd, cd;
+                        sincos_pos(p.dlam * rr, sd, cd);
+                        const double wb[3] = {wx, wy, wz};
+                        constexpr int TB = NT / 2;   // the full sincos is taken at the middle trial
+#pragma unroll
+                        for (int c = 0; c < 3; ++c) {
+                            const double thb = lam[TB][c] * rr;
+                            double sb, cb;
+                            sincos_pos(thb, sb, cb);
+                            acc[TB][c] = fma(fma(thb, sb, cb), wb[c], acc[TB][c]);
+                            double sn = sb, cs = cb;
+#pragma unroll
+                            for (int tt = TB + 1; tt < NT; ++tt) {   // rotate by +d_theta
+                                const double s1 = fma(sn, cd, cs * sd);
+                                const double c1 = fma(cs, cd, -(sn * sd));
+                                sn = s1;
+                                cs = c1;
+                                acc[tt][c] = fma(fma(lam[tt][c] * rr, sn, cs), wb[c], acc[tt][c]);
+                            }
+                            sn = sb;
+                            cs = cb;
+#pragma unroll
+                            for (int tt = TB - 1; tt >= 0; --tt) {   // rotate by -d_theta
+                                const double s1 = fma(sn, cd, -(cs * sd));
+                                const double c1 = fma(cs, cd, sn * sd);
+                                sn = s1;
+                                cs = c1;
+                                acc[tt][c] = fma(fma(lam[tt][c] * rr, sn, cs), wb[c], acc[tt][c]);
+                            }
+                        }
+                        continue;
+                    }
 #pragma unroll
                     for (int tt = 0; tt < NT; ++tt) {
                         acc[tt][0] = fma(kernel_n(lam[tt][0] * rr), wx, acc[tt][0]);

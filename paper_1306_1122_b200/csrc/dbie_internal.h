@@ -86,6 +86,7 @@ struct InteractParams {
     const double* lo;
     long long ldlo;
     double W;
+    double dlam;                 // W/(T-1): spacing of the trial values
     int T;
 };
 

@@ -137,7 +137,7 @@ int main(int argc, char** argv) {
     p.bd.nx = nx; p.bd.ny = ny; p.bd.N = N; p.bd.h = 1; p.bd.x0 = 0; p.bd.y0 = 0; p.bd.rec = rec; p.bd.yk = dyk;
     setup_tiling(p.bd);
     p.x = dx; p.y = dy; p.z = dz; p.lam = dlam; p.ldlam = M; p.count = M; p.part = part; p.cap = M; p.delta_abs = 1e-3;
-    p.lo = dlo; p.ldlo = M; p.W = 0.05; p.T = T;
+    p.lo = dlo; p.ldlo = M; p.W = 0.05; p.T = T; p.dlam = p.W / (T - 1);
     printf("nx %d M %lld ntiles %d nchunks %d\n", nx, M, p.bd.ntiles, p.bd.nchunks);
     const double ie = (double)M * N, is = 4.0 * M * N, ig = 4.0 * T * M * N;
     run_new<0, 1, 256, 2, 2>("eval   NT1 256x2 u2  [library]", p, sms, 8, 0, ie);
@@ -164,7 +164,10 @@ int main(int argc, char** argv) {
       run_new<2, 2, 256, 2, 2>("grid   NT2 256x2 u2", q, sms, 16, 0, ig / 32);
       run_new<2, 1, 256, 2, 2>("grid   NT1 256x2 u2", q, sms, 16, 0, ig / 32);
       run_new<2, 4, 128, 3, 2>("grid   NT4 128x3 u2", q, sms, 16, 0, ig / 32);
-      run_new<2, 8, 128, 2, 1>("grid   NT8 128x2 u1 (spills)", q, sms, 16, 0, ig / 32); }
+      run_new<2, 8, 128, 2, 1>("grid   NT8 128x2 u1", q, sms, 16, 0, ig / 32);
+      run_new<2, 8, 128, 3, 1>("grid   NT8 128x3 u1", q, sms, 16, 0, ig / 32);
+      run_new<2, 8, 256, 1, 1>("grid   NT8 256x1 u1", q, sms, 16, 0, ig / 32);
+      run_new<2, 8, 256, 2, 1>("grid   NT8 256x2 u1", q, sms, 16, 0, ig / 32); }
     printf("FP64 pipe, 8 DFMA chains per thread, k integer-pipe instructions per DFMA:\n");
     run_probe<0>("DFMA only");
     run_probe<5>("DMUL only");
