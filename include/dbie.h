@@ -58,6 +58,11 @@ typedef enum {
 
 /* dbie_create flags */
 #define DBIE_WITH_FP32 1u /* also keep an fp32 copy of the boundary for dbie_eval_f32 */
+#define DBIE_QUAD_9NODE 2u /* Eq. 15: integrate the boundary with 9-node biquadratic
+                              elements (nodes = pixel centres, 3 x 3 Gauss points per 2h x 2h element;
+                              DESIGN.md O-6) instead of one source per pixel (Eq. 16 as read in A-1).
+                              Needs nx, ny >= 3.  The sums then run over 3 ceil((nx-1)/2) x
+                              3 ceil((ny-1)/2) weighted sources; everything else is unchanged.     */
 
 /* Boundary staging (Eq. 3, Eq. 16).
  * nx, ny: boundary grid, N = nx*ny, pixel k = iy*nx + ix (x fastest).

@@ -27,7 +27,7 @@ _ip = C.POINTER(C.c_int)
 
 class _Boundary(C.Structure):
     _fields_ = [("nx", C.c_int), ("ny", C.c_int), ("h", C.c_double), ("x0", C.c_double),
-                ("y0", C.c_double), ("bx", _dp), ("by", _dp), ("bz", _dp)]
+                ("y0", C.c_double), ("bx", _dp), ("by", _dp), ("bz", _dp), ("xs", _dp), ("ys", _dp)]
 
 
 class _Opts(C.Structure):
@@ -78,6 +78,9 @@ def _load():
     if _lib is None:
         _lib = C.CDLL(build())
         _lib.orc_max_threads.restype = C.c_int
+        _lib.orc_q9_count.restype = C.c_int
+        _lib.orc_q9_count.argtypes = [C.c_int]
+        _lib.orc_q9_stage.restype = C.c_int
     return _lib
 
 
@@ -91,6 +94,8 @@ def _d(a):
 
 
 def _boundary(wl):
+    """The boundary of a workload; `wl.quad == 9` selects the 9-node element quadrature (O-6):
+    the nodal data are staged once into the tensor grid of weighted Gauss-point sources."""
     keep = []
     ptrs = []
     for name in ("bx", "by", "bz"):
@@ -98,7 +103,29 @@ def _boundary(wl):
         assert a.size == wl.nx * wl.ny
         keep.append(a)
         ptrs.append(p)
-    return _Boundary(wl.nx, wl.ny, wl.h, wl.x0, wl.y0, *ptrs), keep
+    nodal = _Boundary(wl.nx, wl.ny, wl.h, wl.x0, wl.y0, *ptrs, None, None)
+    if getattr(wl, "quad", 0) != 9:
+        return nodal, keep
+    lib = _load()
+    nsx, nsy = lib.orc_q9_count(wl.nx), lib.orc_q9_count(wl.ny)
+    xs, ys = np.empty(nsx), np.empty(nsy)
+    sv = [np.empty(nsx * nsy) for _ in range(3)]
+    rc = lib.orc_q9_stage(C.byref(nodal), xs.ctypes.data_as(_dp), ys.ctypes.data_as(_dp),
+                          *[a.ctypes.data_as(_dp) for a in sv])
+    if rc != 0:
+        raise ValueError("9-node elements need at least 3 x 3 nodes")
+    keep += [xs, ys] + sv
+    return _Boundary(nsx, nsy, wl.h, wl.x0, wl.y0, *[a.ctypes.data_as(_dp) for a in sv],
+                     xs.ctypes.data_as(_dp), ys.ctypes.data_as(_dp)), keep
+
+
+def q9_sources(wl):
+    """O-6 staging alone: (xs, ys, sx, sy, sz) of the weighted Gauss-point source grid."""
+    import copy
+    w9 = copy.copy(wl)
+    w9.quad = 9
+    b, keep = _boundary(w9)
+    return keep[3], keep[4], keep[5], keep[6], keep[7]
 
 
 def eval(wl, x=None, y=None, z=None, lam=None, nthreads: int = 0) -> np.ndarray:

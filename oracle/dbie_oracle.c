@@ -25,6 +25,9 @@
  *                       calculated analytically").  With
  *                       opts.analytic = 1 orc_residual / orc_solve_nm take J and
  *                       div B from it instead of Eq. 13's differences.
+ *   orc_q9_stage        O-6: Eq. 15's 9-node element quadrature
+ *                        as a tensor grid of weighted sources;
+ *                       every function above then runs on it unchanged.
  *   orc_nm_generic      the same Nelder-Mead driver on a caller-supplied
  *                       objective, so tests can pin it against SciPy (pin S-1).
  *
@@ -50,6 +53,9 @@ typedef struct {
     int nx, ny;                 /* boundary grid, pixel k = iy*nx + ix              */
     double h, x0, y0;           /* pixel size; corner of pixel (0,0)                */
     const double *bx, *by, *bz; /* N = nx*ny each                                   */
+    const double *xs, *ys;      /* NULL: sources are the pixel centres (reading A-1).
+                                   Else explicit source abscissae xs[nx], ys[ny] of a
+                                   tensor grid of weighted sources (O-6, orc_q9_stage) */
 } orc_boundary;
 
 typedef struct {
@@ -68,6 +74,74 @@ typedef struct {
                                    finite differences of Eq. 13 (O-5)               */
 } orc_opts;
 
+/* ---------------------------------------------------------------- O-6 ---- */
+/* 9-node element quadrature (Eq. 15: "the boundary has
+ * been subdivided into N_e 9-nodes elements with boundary data known over each node,
+ * N_k(xi, eta) is the shape function, J the Jacobian").  Reading (the paper gives neither
+ * the node placement nor the Gauss order): nodes = pixel centres; an element spans
+ * 3 x 3 nodes (2h x 2h), biquadratic Lagrange shape functions
+ *     N_-1 = xi (xi - 1)/2,  N_0 = 1 - xi^2,  N_+1 = xi (xi + 1)/2   per direction,
+ * 3 x 3 Gauss-Legendre points xi = -sqrt(3/5), 0, +sqrt(3/5), weights 5/9, 8/9, 5/9,
+ * Jacobian h^2.  When the node count in a direction is even, the last element re-uses the
+ * last three nodes and is integrated over its outer half xi in [0, 1] only.  The integral
+ * over the boundary is from the first to the last node (the outer half pixel, where the
+ * field is assumed to vanish anyway, is dropped).
+ * Eq. 15 then reads  B_i = sum over Gauss points g of  K(r_ig) * [w_g sum_j N_j(g) B_j],
+ * i.e. the SAME sum as Eq. 16 over a tensor grid of weighted sources.  This function
+ * builds that grid: xs[nsx], ys[nsy] and the weighted values (in units of the pixel
+ * area h^2, so the prefactor z h^2/2pi of Eq. 6 is unchanged).  nsx = 3 ceil((nx-1)/2). */
+static int q9_axis(int n, double c0, double h, double *pos, double *wq, int *base, double (*shape)[3])
+{
+    /* one direction: for every Gauss abscissa its position, weight, first node and N_a */
+    const double g[3] = { -sqrt(0.6), 0.0, sqrt(0.6) }, w[3] = { 5.0 / 9.0, 8.0 / 9.0, 5.0 / 9.0 };
+    const int ne = (n - 1 + 1) / 2; /* ceil((n-1)/2) */
+    for (int e = 0; e < ne; ++e) {
+        const int half = (2 * e + 2 > n - 1);      /* even n: the last element, outer half only */
+        const int i0 = half ? n - 3 : 2 * e;
+        const double xc = c0 + (i0 + 1 + 0.5) * h; /* centre node of the element */
+        for (int q = 0; q < 3; ++q) {
+            const double xi = half ? 0.5 + 0.5 * g[q] : g[q];
+            const int k = 3 * e + q;
+            pos[k] = xc + xi * h;
+            wq[k] = half ? 0.5 * w[q] : w[q];
+            base[k] = i0;
+            shape[k][0] = xi * (xi - 1.0) / 2.0;
+            shape[k][1] = 1.0 - xi * xi;
+            shape[k][2] = xi * (xi + 1.0) / 2.0;
+        }
+    }
+    return 3 * ne;
+}
+
+int orc_q9_count(int n) { return n < 3 ? 0 : 3 * ((n - 1 + 1) / 2); }
+
+/* in: nodal boundary b (nx, ny >= 3).  out: xs[nsx], ys[nsy], sx/sy/sz[nsy*nsx].  Returns 0. */
+int orc_q9_stage(const orc_boundary *b, double *xs, double *ys, double *sx, double *sy, double *sz)
+{
+    if (b->nx < 3 || b->ny < 3) return 1;
+    const int nsx = orc_q9_count(b->nx), nsy = orc_q9_count(b->ny);
+    double *wx = malloc(sizeof(double) * nsx), *wy = malloc(sizeof(double) * nsy);
+    int *bx0 = malloc(sizeof(int) * nsx), *by0 = malloc(sizeof(int) * nsy);
+    double (*Nx)[3] = malloc(sizeof(double[3]) * nsx), (*Ny)[3] = malloc(sizeof(double[3]) * nsy);
+    q9_axis(b->nx, b->x0, b->h, xs, wx, bx0, Nx);
+    q9_axis(b->ny, b->y0, b->h, ys, wy, by0, Ny);
+    for (int gy = 0; gy < nsy; ++gy)
+        for (int gx = 0; gx < nsx; ++gx) {
+            double v[3] = { 0.0, 0.0, 0.0 };
+            for (int bb = 0; bb < 3; ++bb)
+                for (int a = 0; a < 3; ++a) {
+                    const long k = (long)(by0[gy] + bb) * b->nx + bx0[gx] + a;
+                    const double N = Ny[gy][bb] * Nx[gx][a];
+                    v[0] += N * b->bx[k]; v[1] += N * b->by[k]; v[2] += N * b->bz[k];
+                }
+            const double w = wy[gy] * wx[gx];
+            const long o = (long)gy * nsx + gx;
+            sx[o] = w * v[0]; sy[o] = w * v[1]; sz[o] = w * v[2];
+        }
+    free(wx); free(wy); free(bx0); free(by0); free(Nx); free(Ny);
+    return 0;
+}
+
 /* ---------------------------------------------------------------- O-1 ---- */
 /* B_p(i) = (z_i h^2 / 2 pi) * sum_k [theta sin theta + cos theta] / r^3 * B_p0[k],
  * theta = |lambda_p| r,  r = sqrt((x_k-x_i)^2 + (y_k-y_i)^2 + z_i^2).   Eq. 6/16. */
@@ -82,10 +156,10 @@ static void eval_point(const orc_boundary *b, double xi, double yi, double zi,
         return;
     }
     for (int iy = 0; iy < b->ny; ++iy) {
-        const double yk = b->y0 + (iy + 0.5) * b->h;
+        const double yk = b->ys ? b->ys[iy] : b->y0 + (iy + 0.5) * b->h;
         const double dy = yk - yi;
         for (int ix = 0; ix < b->nx; ++ix) {
-            const double xk = b->x0 + (ix + 0.5) * b->h;
+            const double xk = b->xs ? b->xs[ix] : b->x0 + (ix + 0.5) * b->h;
             const double dx = xk - xi;
             const double r2 = dx * dx + dy * dy + zi * zi;
             const double r = sqrt(r2);
@@ -176,10 +250,10 @@ static void eval_point_grad(const orc_boundary *b, double xi, double yi, double 
         return;
     }
     for (int iy = 0; iy < b->ny; ++iy) {
-        const double yk = b->y0 + (iy + 0.5) * b->h;
+        const double yk = b->ys ? b->ys[iy] : b->y0 + (iy + 0.5) * b->h;
         const double dy = yk - yi;
         for (int ix = 0; ix < b->nx; ++ix) {
-            const double xk = b->x0 + (ix + 0.5) * b->h;
+            const double xk = b->xs ? b->xs[ix] : b->x0 + (ix + 0.5) * b->h;
             const double dx = xk - xi;
             const double r2 = dx * dx + dy * dy + zi * zi;
             const double r = sqrt(r2);

@@ -24,6 +24,7 @@ _lib = None
 
 DBIE_OK, DBIE_EINVAL, DBIE_ENOMEM, DBIE_ECUDA, DBIE_ESTATE = range(5)
 DBIE_WITH_FP32 = 1
+DBIE_QUAD_9NODE = 2
 
 
 class DBIEError(RuntimeError):
@@ -147,13 +148,14 @@ def _stream_ptr(stream):
 class DBIE:
     """One boundary magnetogram staged on the device (dbie_create / dbie_destroy)."""
 
-    def __init__(self, nx: int, ny: int, h: float, x0: float, y0: float, bx, by, bz, fp32: bool = False):
+    def __init__(self, nx: int, ny: int, h: float, x0: float, y0: float, bx, by, bz, fp32: bool = False,
+                 quad9: bool = False):
         lib = load()
         self._lib = lib
         self._h = _vp()
         self.nx, self.ny, self.h, self.x0, self.y0 = int(nx), int(ny), float(h), float(x0), float(y0)
         self.N = self.nx * self.ny
-        flags = DBIE_WITH_FP32 if fp32 else 0
+        flags = (DBIE_WITH_FP32 if fp32 else 0) | (DBIE_QUAD_9NODE if quad9 else 0)
         if isinstance(bx, np.ndarray):
             b = [_host_f64(a, self.N, n) for a, n in ((bx, "bx"), (by, "by"), (bz, "bz"))]
             st = lib.dbie_create_host(C.byref(self._h), nx, ny, h, x0, y0, *[_vp(a.ctypes.data) for a in b],
@@ -169,7 +171,7 @@ class DBIE:
     def from_workload(cls, wl, device=None, fp32: bool = False) -> "DBIE":
         """Stage the boundary of a workloads.Workload (host arrays) on the current device."""
         return cls(wl.nx, wl.ny, wl.h, wl.x0, wl.y0, np.asarray(wl.bx), np.asarray(wl.by),
-                   np.asarray(wl.bz), fp32=fp32)
+                   np.asarray(wl.bz), fp32=fp32, quad9=getattr(wl, "quad", 0) == 9)
 
     # -- lifetime
     def close(self):

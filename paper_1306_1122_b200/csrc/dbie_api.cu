@@ -171,6 +171,7 @@ extern "C" dbie_status dbie_create(dbie_ctx** out, int nx, int ny, double h, dou
     if (nx < 1 || ny < 1 || !(h > 0.0) || !isfinite(h) || !isfinite(x0) || !isfinite(y0) || !bx || !by || !bz)
         return DBIE_EINVAL;
     if ((long long)nx * ny > (1LL << 30)) return DBIE_EINVAL;
+    if ((flags & DBIE_QUAD_9NODE) && (nx < 3 || ny < 3)) return DBIE_EINVAL;
     dbie_ctx* ctx = (dbie_ctx*)calloc(1, sizeof(dbie_ctx));
     if (!ctx) return DBIE_ENOMEM;
     strcpy(ctx->err, "no error");
@@ -183,19 +184,24 @@ extern "C" dbie_status dbie_create(dbie_ctx** out, int nx, int ny, double h, dou
             st = fail_cuda(ctx, e, "cudaDeviceGetAttribute"); break;
         }
         BoundaryView& b = ctx->bd;
-        b.nx = nx; b.ny = ny; b.N = (long long)nx * ny;
+        const bool q9 = (flags & DBIE_QUAD_9NODE) != 0;
+        // 9-node elements: the sources are 3 Gauss abscissae per element and direction (O-6)
+        const int sx = q9 ? 3 * (nx / 2) : nx, sy = q9 ? 3 * (ny / 2) : ny;
+        b.nx = sx; b.ny = sy; b.N = (long long)sx * sy;
         b.h = h; b.x0 = x0; b.y0 = y0;
         setup_tiling(b);
         if ((e = cudaMalloc(&ctx->rec, sizeof(double4) * b.N)) != cudaSuccess) { st = fail_cuda(ctx, e, "cudaMalloc(rec)"); break; }
-        if ((e = cudaMalloc(&ctx->yk, sizeof(double) * ny)) != cudaSuccess) { st = fail_cuda(ctx, e, "cudaMalloc(yk)"); break; }
+        if ((e = cudaMalloc(&ctx->yk, sizeof(double) * b.ny)) != cudaSuccess) { st = fail_cuda(ctx, e, "cudaMalloc(yk)"); break; }
         if (flags & DBIE_WITH_FP32) {
             if ((e = cudaMalloc(&ctx->rec32, sizeof(float4) * b.N)) != cudaSuccess) { st = fail_cuda(ctx, e, "cudaMalloc(rec32)"); break; }
-            if ((e = cudaMalloc(&ctx->yk32, sizeof(float) * ny)) != cudaSuccess) { st = fail_cuda(ctx, e, "cudaMalloc(yk32)"); break; }
+            if ((e = cudaMalloc(&ctx->yk32, sizeof(float) * b.ny)) != cudaSuccess) { st = fail_cuda(ctx, e, "cudaMalloc(yk32)"); break; }
         }
         if ((e = cudaMalloc(&ctx->counters, 64)) != cudaSuccess) { st = fail_cuda(ctx, e, "cudaMalloc(counters)"); break; }
         if ((e = cudaMemset(ctx->counters, 0, 64)) != cudaSuccess) { st = fail_cuda(ctx, e, "cudaMemset"); break; }
         if ((e = cudaStreamCreateWithFlags(&ctx->own_stream, cudaStreamNonBlocking)) != cudaSuccess) { st = fail_cuda(ctx, e, "cudaStreamCreate"); break; }
-        if ((e = launch_stage_boundary(nx, ny, h, x0, y0, bx, by, bz, ctx->rec, ctx->yk, ctx->rec32, ctx->yk32, 0)) != cudaSuccess) {
+        e = q9 ? launch_stage_q9(nx, ny, h, x0, y0, bx, by, bz, sx, sy, ctx->rec, ctx->yk, ctx->rec32, ctx->yk32, 0)
+               : launch_stage_boundary(nx, ny, h, x0, y0, bx, by, bz, ctx->rec, ctx->yk, ctx->rec32, ctx->yk32, 0);
+        if (e != cudaSuccess) {
             st = fail_cuda(ctx, e, "stage_boundary"); break;
         }
         if ((e = cudaDeviceSynchronize()) != cudaSuccess) { st = fail_cuda(ctx, e, "stage_boundary(sync)"); break; }

@@ -49,6 +49,71 @@ cudaError_t launch_stage_boundary(int nx, int ny, double h, double x0, double y0
     return cudaGetLastError();
 }
 
+// A1, 9-node element variant (Eq. 15; O-6): the nodes are
+// the pixel centres, an element spans 3 x 3 of them (2h x 2h), biquadratic Lagrange shape functions,
+// 3 x 3 Gauss-Legendre points.  Eq. 15 is then Eq. 16's sum over a tensor grid of Gauss-point sources
+// with values w_g sum_j N_j(g) B_j: this kernel writes that grid in the same record layout, so the
+// interaction kernels run on it unchanged (rec[].x and yk[] are explicit coordinates already).
+struct Q9Axis {
+    double pos, w, N[3];
+    int base;
+};
+// Gauss abscissa `k` of an axis with n nodes whose first node sits at c0 + h/2.  When n is even the
+// last element re-uses the last three nodes and is integrated over its outer half only.
+__device__ inline Q9Axis q9_axis(int n, double c0, double h, int k) {
+    const int e = k / 3, q = k - 3 * e;
+    const double g = (q == 0) ? -0.7745966692414834 : (q == 1 ? 0.0 : 0.7745966692414834);   // sqrt(3/5)
+    const double w = (q == 1) ? 8.0 / 9.0 : 5.0 / 9.0;
+    const bool half = 2 * e + 2 > n - 1;
+    Q9Axis a;
+    a.base = half ? n - 3 : 2 * e;
+    const double xi = half ? 0.5 + 0.5 * g : g;
+    a.pos = c0 + ((double)(a.base + 1) + 0.5) * h + xi * h;
+    a.w = half ? 0.5 * w : w;
+    a.N[0] = 0.5 * xi * (xi - 1.0);
+    a.N[1] = 1.0 - xi * xi;
+    a.N[2] = 0.5 * xi * (xi + 1.0);
+    return a;
+}
+
+__global__ void stage_q9_kernel(int nx, int ny, double h, double x0, double y0, const double* __restrict__ bx,
+                                const double* __restrict__ by, const double* __restrict__ bz, int nsx, int nsy,
+                                double4* __restrict__ rec, double* __restrict__ yk, float4* __restrict__ rec32,
+                                float* __restrict__ yk32) {
+    const long long NS = (long long)nsx * nsy;
+    for (long long k = blockIdx.x * (long long)blockDim.x + threadIdx.x; k < NS;
+         k += (long long)gridDim.x * blockDim.x) {
+        const int gy = (int)(k / nsx), gx = (int)(k - (long long)gy * nsx);
+        const Q9Axis ax = q9_axis(nx, x0, h, gx), ay = q9_axis(ny, y0, h, gy);
+        double v[3] = {0.0, 0.0, 0.0};
+        for (int b = 0; b < 3; ++b)
+            for (int a = 0; a < 3; ++a) {
+                const long long j = (long long)(ay.base + b) * nx + ax.base + a;
+                const double Nab = ay.N[b] * ax.N[a];
+                v[0] += Nab * bx[j];
+                v[1] += Nab * by[j];
+                v[2] += Nab * bz[j];
+            }
+        const double w = ay.w * ax.w;
+        rec[k] = make_double4(ax.pos, w * v[0], w * v[1], w * v[2]);
+        if (rec32) rec32[k] = make_float4((float)ax.pos, (float)(w * v[0]), (float)(w * v[1]), (float)(w * v[2]));
+        if (gx == 0) {
+            yk[gy] = ay.pos;
+            if (yk32) yk32[gy] = (float)ay.pos;
+        }
+    }
+}
+
+cudaError_t launch_stage_q9(int nx, int ny, double h, double x0, double y0, const double* bx, const double* by,
+                            const double* bz, int nsx, int nsy, double4* rec, double* yk, float4* rec32,
+                            float* yk32, cudaStream_t st) {
+    const long long NS = (long long)nsx * nsy;
+    int grid = (int)((NS + 255) / 256);
+    if (grid > 4096) grid = 4096;
+    stage_q9_kernel<<<grid, 256, 0, st>>>(nx, ny, h, x0, y0, bx, by, bz, nsx, nsy, rec, yk, rec32, yk32);
+    return cudaGetLastError();
+}
+
 // ------------------------------------------------------------------ fp64 launchers --------
 // The kernel is dbie_interact_fp64.cuh.  Shapes measured on B200 (profiles/r01_variants.md):
 // 256 threads x 2 CTAs/SM (<= 128 registers), two pixels in flight per thread; GRID mode carries

@@ -135,6 +135,9 @@ constexpr int kGridMaxTrials = 32;
 cudaError_t launch_stage_boundary(int nx, int ny, double h, double x0, double y0, const double* bx,
                                   const double* by, const double* bz, double4* rec, double* yk,
                                   float4* rec32, float* yk32, cudaStream_t st);
+cudaError_t launch_stage_q9(int nx, int ny, double h, double x0, double y0, const double* bx, const double* by,
+                            const double* bz, int nsx, int nsy, double4* rec, double* yk, float4* rec32,
+                            float* yk32, cudaStream_t st);
 cudaError_t launch_interact_eval(const InteractParams& p, int sm_count, cudaStream_t st);
 cudaError_t launch_interact_stencil(const InteractParams& p, int sm_count, cudaStream_t st);
 cudaError_t launch_interact_grid(const InteractParams& p, int sm_count, cudaStream_t st);

@@ -45,6 +45,7 @@ class Workload:
     z: np.ndarray
     lam: np.ndarray | None = None   # (3, M) float64 for eval-only configs
     extra: dict = dataclasses.field(default_factory=dict)
+    quad: int = 0           # 0: one source per pixel centre (reading A-1); 9: 9-node elements (O-6)
 
     @property
     def N(self) -> int:
