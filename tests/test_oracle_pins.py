@@ -519,3 +519,81 @@ def test_g3_analytic_residual_and_solve_are_consistent_with_eq13():
     cross = oracle.residual(w, sf["lam"], oracle.Opts(analytic=1))["phi"]
     assert np.all(sa["phi"] <= cross + 5e-3)          # both searches end in equally good minima
     assert np.all(sa["phi"] <= oracle.residual(w, np.full((3, w.M), 0.05 / w.h), oracle.Opts(analytic=1))["phi"] + 1e-15)
+
+
+# -- O-6: 9-node element quadrature (Eq. 15) ------------------
+def _nodes(n, h, c0):
+    return c0 + (np.arange(n) + 0.5) * h
+
+
+@pytest.mark.parametrize("nx,ny", [(7, 5), (6, 9), (8, 4), (3, 3)])
+def test_q1_nine_node_staging_weights_and_interpolation(nx, ny):
+    """Odd and even node counts.  (a) the weights of the Gauss-point sources sum to the integrated
+    area (first to last node) in units of h^2; (b) nodal data that are globally biquadratic are
+    reproduced exactly at every Gauss point (Lagrange interpolation on 3 x 3 nodes); (c) the rule
+    integrates x^a y^b, a, b <= 2 (data) exactly: sum of staged values = closed-form integral."""
+    h, x0, y0 = 0.5, -1.0, 2.0
+    xn, yn = _nodes(nx, h, x0), _nodes(ny, h, y0)
+    Y, X = np.meshgrid(yn, xn, indexing="ij")
+    poly = lambda x, y: 1.5 - 0.7 * x + 0.3 * y + 0.2 * x * y - 0.4 * x * x + 0.1 * y * y + 0.05 * x * x * y * y
+    one = np.ones(nx * ny)
+    w = _wl(nx, ny, h, x0, y0, one, poly(X, Y).ravel(), (X * X * Y).ravel(), [[0.0, 0.0, 1.0]])
+    xs, ys, s1, sp, sxy = oracle.q9_sources(w)
+    nsx, nsy = 3 * (nx // 2), 3 * (ny // 2)
+    assert xs.size == nsx and ys.size == nsy and s1.size == nsx * nsy
+    assert np.all(np.diff(xs) > 0) and xs[0] > xn[0] and xs[-1] < xn[-1]
+    assert abs(s1.sum() - (nx - 1) * (ny - 1)) < 1e-12 * nx * ny                       # (a)
+    YS, XS = np.meshgrid(ys, xs, indexing="ij")
+    wgt = s1.reshape(nsy, nsx)
+    assert np.allclose(sp.reshape(nsy, nsx), wgt * poly(XS, YS), rtol=1e-12, atol=1e-13)   # (b)
+    # (c) integral of x^2 y over [xn0, xn_last] x [yn0, yn_last], in units of h^2
+    ex = (xn[-1] ** 3 - xn[0] ** 3) / 3.0 * (yn[-1] ** 2 - yn[0] ** 2) / 2.0 / (h * h)
+    assert abs(sxy.sum() - ex) < 1e-12 * abs(ex)
+
+
+def test_q2_nine_node_sum_equals_element_by_element_quadrature():
+    """Eq. 15 written out independently: loop over elements, 3 x 3 Gauss points, shape functions,
+    kernel of Eq. 6 at each Gauss point (NumPy), against oracle.eval on the staged sources."""
+    import copy
+    nx, ny, h, x0, y0 = 7, 9, 1.0, 0.0, 0.0
+    w = random_boundary(nx, ny, seed=31, npts=5, h=h, x0=x0, y0=y0, zmin=1.0, zmax=4.0)
+    w9 = copy.copy(w); w9.quad = 9
+    B = oracle.eval(w9)
+    g = np.array([-math.sqrt(0.6), 0.0, math.sqrt(0.6)]); gw = np.array([5, 8, 5]) / 9.0
+    N = lambda t: np.array([t * (t - 1) / 2, 1 - t * t, t * (t + 1) / 2])
+    data = [a.reshape(ny, nx) for a in (w.bx, w.by, w.bz)]
+    for i in range(w.M):
+        tot = np.zeros(3)
+        for ey in range((ny - 1) // 2):
+            for ex in range((nx - 1) // 2):
+                for qy in range(3):
+                    for qx in range(3):
+                        xg = x0 + (2 * ex + 1.5) * h + g[qx] * h
+                        yg = y0 + (2 * ey + 1.5) * h + g[qy] * h
+                        r = math.sqrt((xg - w.x[i]) ** 2 + (yg - w.y[i]) ** 2 + w.z[i] ** 2)
+                        Nq = np.outer(N(g[qy]), N(g[qx]))
+                        for p in range(3):
+                            th = abs(w.lam[p, i]) * r
+                            val = (Nq * data[p][2 * ey:2 * ey + 3, 2 * ex:2 * ex + 3]).sum()
+                            tot[p] += gw[qy] * gw[qx] * (th * math.sin(th) + math.cos(th)) / r ** 3 * val
+        ref = w.z[i] * h * h / (2 * math.pi) * tot
+        assert np.allclose(B[:, i], ref, rtol=1e-12, atol=0)
+
+
+def test_q3_nine_node_agrees_with_the_nodal_rule_in_the_far_field():
+    """Both discretisations converge to the same integral of a field that vanishes at the window
+    edge: at z = 12 h and 24 h they agree to 5e-5 (the interpolant's flux differs from the midpoint sum by
+    O((h/sigma)^4) for this sigma = 4 h Gaussian); near the boundary the two quadratures differ."""
+    import copy
+    n = 41
+    c = (np.arange(n) + 0.5)
+    Y, X = np.meshgrid(c, c, indexing="ij")
+    bz = np.exp(-((X - 20.5) ** 2 + (Y - 20.5) ** 2) / (2 * 4.0 ** 2)).ravel()
+    pts = [[18.3, 21.1, 12.0], [22.0, 19.0, 24.0], [20.5, 20.5, 1.0]]
+    lam = np.array([[0.0, 0.1, 0.05]] * 3)
+    w = _wl(n, n, 1.0, 0.0, 0.0, bz, 0.5 * bz, -bz, pts, lam)
+    w9 = copy.copy(w); w9.quad = 9
+    a, b = oracle.eval(w), oracle.eval(w9)
+    rel = np.abs(a - b).max(axis=0) / np.abs(a).max(axis=0)
+    assert rel[0] < 5e-5 and rel[1] < 5e-5              # what remains is the Simpson-vs-midpoint flux difference
+    assert 1e-7 < rel[2] < 5e-2                         # z = h: the two quadratures differ
