@@ -521,3 +521,56 @@ def test_lowlou_case2_figures_of_merit(dbie):
     mp_ = workloads.figures_of_merit(Bex, pot)
     assert 0.90 < mp_["C_vec"] < 0.97                      # lambda = 0 (potential) field, same window
     assert float(np.mean(s["f"])) < 0.2                    # far more force-free than the potential field
+
+
+# ------------------------------------ 9-node element quadrature (O-6) -
+def _q9(w):
+    import copy
+    w9 = copy.copy(w)
+    w9.quad = 9
+    return w9
+
+
+@pytest.mark.parametrize("nx,ny", [(3, 3), (4, 3), (7, 5), (6, 9), (33, 21), (64, 64), (343, 5), (700, 4)])
+def test_q9_eval_matches_oracle(dbie, nx, ny):
+    """DBIE_QUAD_9NODE: odd / even node counts (half elements), the smallest grid, source rows longer
+    than one 512-record tile (343 nodes -> 513 sources; 700 -> 1050), h != 1, shifted origin."""
+    w = _q9(workloads.random_boundary(nx, ny, seed=nx * 5 + ny, npts=41, h=0.5, x0=-1.0, y0=2.0))
+    w.lam[:, 0] = 0.0
+    with dbie.DBIE.from_workload(w) as ctx:
+        dw = dbie.to_device(w)
+        B = ctx.eval(dw.x, dw.y, dw.z, dw.lam).cpu().numpy()
+        assert ctx.counters()["interactions"] == float(w.M) * (3 * (nx // 2)) * (3 * (ny // 2))
+    err, _ = vec_relerr(B, oracle.eval(w))
+    assert err <= TOL_B
+    # and it is a different discretisation from the one-source-per-pixel rule
+    assert not np.allclose(B, gpu_eval(dbie, workloads.random_boundary(nx, ny, seed=nx * 5 + ny, npts=41, h=0.5,
+                                                                       x0=-1.0, y0=2.0)), rtol=1e-6)
+
+
+def test_q9_solve_and_residual_config2(dbie):
+    """The whole path on the 9-node sources: Eq. 13 residual, NM solve (Eq. 13 and analytic), GRID."""
+    import torch
+    w = _q9(workloads.config2().seeded_subset(64, seed_offset=21)[0])
+    lam = np.random.default_rng(3).uniform(0.0, 0.3, (3, w.M)) / w.h
+    ro = oracle.residual(w, lam)
+    with dbie.DBIE.from_workload(w) as ctx:
+        dw = dbie.to_device(w)
+        r = {k: v.cpu().numpy() for k, v in ctx.residual(dw.x, dw.y, dw.z, torch.from_numpy(lam).cuda()).items()}
+    err, _ = vec_relerr(r["B"], ro["B"])
+    assert err <= TOL_B and np.abs(r["f"] - ro["f"]).max() <= TOL_FG and np.abs(r["g"] - ro["g"]).max() <= TOL_FG
+    _check_solve_parity(dbie, w)
+    _check_solve_parity(dbie, w, dict(analytic=1))
+    _check_solve_parity(dbie, w, dict(method=1, n_level=4))
+
+
+def test_q9_eval_f32_and_bad_sizes(dbie):
+    import torch
+    w = _q9(_f32_inputs(workloads.random_boundary(65, 40, seed=77, npts=300, zmin=1.0, zmax=30.0)))
+    with dbie.DBIE.from_workload(w, fp32=True) as ctx:
+        t = lambda a: torch.from_numpy(np.ascontiguousarray(a, dtype=np.float32)).cuda()
+        B = ctx.eval_f32(t(w.x), t(w.y), t(w.z), t(w.lam)).cpu().numpy().astype(np.float64)
+    err, _ = vec_relerr(B, oracle.eval(w))
+    assert err <= TOL_B_F32
+    with pytest.raises(dbie.DBIEError):
+        dbie.DBIE(2, 5, 1.0, 0.0, 0.0, np.ones(10), np.ones(10), np.ones(10), quad9=True)
