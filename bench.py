@@ -32,7 +32,8 @@ sys.path.insert(0, ROOT)
 
 METRIC = "point-pixel DBIE interactions/sec (fp64)"
 UNIT = "interactions/s"
-FP64_INSTR_PER_INTERACTION = 76      # DESIGN.md section 6 (SASS inner loop: 152 per 2 pixels of one position)
+FP64_INSTR_PER_INTERACTION = 76      # eval: DESIGN.md section 6 (SASS inner loop: 152 per 2 pixels of one position)
+FP64_INSTR_STENCIL = 245 / 4         # Eq. 13 stencil: 4 positions per thread, small-angle rotation (SASS: 245 per pixel)
 FP64_INSTR_ANALYTIC = 95             # analytic gradient: 11 + 3 x 28 per pixel of the one position
 FP64_INSTR_GRID = {8: 238 / 8, 4: 154 / 4, 2: 112 / 2, 1: 76}   # GRID: 31 + 3 (20 + 7 (NT-1)) per NT equally spaced trial triples
 FP64_INSTR_SURVEY = 82               # SURVEY.md 8(d) canonical count
@@ -317,7 +318,8 @@ def run_ours(args) -> None:
     peak_slots = SM_COUNT * FP64_LANES_PER_SM * sm_max * 1e6          # FP64 lane-instructions / s
     kern_ips = inter_total / (kern_ms * 1e-3) if kern_ms > 0 else 0.0
     per_inter = FP64_INSTR_ANALYTIC if (is_solve and METHOD["analytic"]) else (
-        FP64_INSTR_GRID[8] if (is_solve and METHOD["grid"]) else FP64_INSTR_PER_INTERACTION)
+        FP64_INSTR_GRID[8] if (is_solve and METHOD["grid"]) else (
+            FP64_INSTR_STENCIL if is_solve else FP64_INSTR_PER_INTERACTION))
     achieved_slots = kern_ips * per_inter
     roofline = {
         "bound": "alu", "kernel": "dbie::interact64_kernel (fp64 point-pixel sums)",
@@ -328,12 +330,14 @@ def run_ours(args) -> None:
         "traffic_note": "bytes of the launch with all points active (ncu capture, profiles/); algorithmic: 6.8 MB of point "
                         "data in + 100 MB of chunk partial sums out, of which the L2 keeps half",
         "note": "FP64-pipe bound (no HBM/tensor step): achieved = interactions/s of the kernel x FP64 "
-                "lane-instructions per interaction (76; GRID T=8: 8 equally spaced trial triples per geometry 29.75; analytic gradient 95; DESIGN.md s6) "
+                "lane-instructions per interaction (eval 76; Eq. 13 stencil 61.25; GRID T=8: 8 equally spaced trial triples per geometry 29.75; analytic gradient 95; DESIGN.md s6) "
                 "x 2 flop per FMA slot; peak = 148 SM x 64 FP64 lanes x clocks.max.sm (derived, DESIGN.md s7)",
         "kernel_interactions_per_s": kern_ips, "kernel_ms_per_launch": kern_ms / max(kern_launches, 1),
         "kernel_launches": kern_launches, "kernel_share_of_step": kern_ms / ms_total if ms_total else None,
         "fp64_instr_per_interaction": per_inter,
         "frac_survey82": kern_ips * FP64_INSTR_SURVEY / peak_slots,
+        "frac_survey82_note": "SURVEY 8(d)'s canonical 82 instructions per interaction; exceeds `frac` (and can exceed 1) "
+                              "because the kernel executes fewer: the stencil positions / GRID trials share sincos work",
         "peak_measured_dfma_per_s": dfma_meas, "peak_measured_ffma_per_s": ffma_meas,
         "frac_of_measured_dfma": (achieved_slots / dfma_meas) if dfma_meas else None,
     }

@@ -28,11 +28,16 @@ namespace dbie {
 // it accumulates the three sums of the analytic gradient (kinds 1..3 below), 12 sums per slot like
 // the stencil, from the same sincos: d/dr[n(lambda r)/r^3] = lambda^2 cos(lambda r)/r^2 - 3 n/r^4.
 // MODE_GRID_ANALYTIC: the same four sums for NT trial triples of GRID mode (item = slot * G + g).
-enum { MODE_EVAL = 0, MODE_STENCIL = 1, MODE_GRID = 2, MODE_ANALYTIC = 3, MODE_GRID_ANALYTIC = 4 };
+// MODE_STENCIL4: the Eq. 13 stencil with all 4 positions of a field point in ONE thread (item = slot).
+// The positions are delta = 1e-3 h apart, so theta_s = lambda r_s differs from theta_0 by eps <= lambda delta:
+// one full sincos per component at r_i and a small-angle rotation (rotate_small) for the other three
+// positions; geometry (dx, dy, z terms) is shared where the offsets allow.  61.25 FP64 instructions per
+// interaction instead of 76.  Threads whose lambda delta exceeds kRotateSmallMax take the plain path.
+enum { MODE_EVAL = 0, MODE_STENCIL = 1, MODE_GRID = 2, MODE_ANALYTIC = 3, MODE_GRID_ANALYTIC = 4, MODE_STENCIL4 = 5 };
 
 // items (threads' units of work) per slot
 __host__ __device__ inline long long items_per_slot(int mode, int G) {
-    if (mode == MODE_EVAL || mode == MODE_ANALYTIC) return 1;
+    if (mode == MODE_EVAL || mode == MODE_ANALYTIC || mode == MODE_STENCIL4) return 1;
     if (mode == MODE_GRID_ANALYTIC) return G;
     return mode == MODE_STENCIL ? kStencil : (long long)kStencil * G;
 }
@@ -94,7 +99,7 @@ __global__ void __launch_bounds__(THREADS, MINB) interact64_kernel(const __grid_
         const long long jt = live ? item : nitems - 1;
         long long slot;
         int s = 0, g = 0;
-        if (MODE == MODE_EVAL || MODE == MODE_ANALYTIC) {
+        if (MODE == MODE_EVAL || MODE == MODE_ANALYTIC || MODE == MODE_STENCIL4) {
             slot = jt;
         } else if (MODE == MODE_STENCIL) {
             slot = jt >> 2;
@@ -116,6 +121,9 @@ __global__ void __launch_bounds__(THREADS, MINB) interact64_kernel(const __grid_
             if (s == 3) zi = __dadd_rn(zi, p.delta_abs);
         }
         const double z2 = zi * zi;
+        // MODE_STENCIL4: the offset coordinates of positions 1 (x), 2 (y), 3 (z)
+        const double xi1 = __dadd_rn(xi, p.delta_abs), yi2 = __dadd_rn(yi, p.delta_abs);
+        const double zi3 = __dadd_rn(zi, p.delta_abs), z23 = zi3 * zi3;
         double lam[NT][3];
         if (kGridLam) {
             // trial t of component c: lo_c + W t/(T-1), each operation rounded separately (O-4)
@@ -135,10 +143,11 @@ __global__ void __launch_bounds__(THREADS, MINB) interact64_kernel(const __grid_
 
         // accumulators: one row per lambda triple; MODE_ANALYTIC: rows = sum K b, sum D dx b, sum D dy b, sum D b
         // (row 4 tt + kind in the analytic modes)
-        constexpr int NA = kAnalytic ? 4 * NT : NT;
+        constexpr int NA = (kAnalytic || MODE == MODE_STENCIL4) ? 4 * NT : NT;
         double acc[NA][3];
 #pragma unroll
         for (int tt = 0; tt < NA; ++tt) acc[tt][0] = acc[tt][1] = acc[tt][2] = 0.0;
+        const bool small_eps = fmax(fmax(lam[0][0], lam[0][1]), lam[0][2]) * p.delta_abs <= kRotateSmallMax;
         double lam2[NT][3];   // analytic modes: lambda^2
 #pragma unroll
         for (int tt = 0; tt < NT; ++tt)
@@ -167,9 +176,45 @@ __global__ void __launch_bounds__(THREADS, MINB) interact64_kernel(const __grid_
                 const double yk = __ldg(bd.yk + d.row0 + row);
                 const double dy = yk - yi;
                 const double cc = fma(dy, dy, z2);
+                const double dy2 = yk - yi2;
+                const double cc2 = fma(dy2, dy2, z2), cc3 = fma(dy, dy, z23);   // MODE_STENCIL4
 #pragma unroll UNR
                 for (int j = 0; j < d.ncols; ++j) {
                     const double4 px = rp[j];  // {x_k, Bx0, By0, Bz0}: two broadcast LDS.128
+                    if (MODE == MODE_STENCIL4) {
+                        const double dx0 = px.x - xi, dx1 = px.x - xi1;
+                        const double r2s[4] = {fma(dx0, dx0, cc), fma(dx1, dx1, cc), fma(dx0, dx0, cc2),
+                                               fma(dx0, dx0, cc3)};
+                        double rs[4], ws[4];
+#pragma unroll
+                        for (int q = 0; q < 4; ++q) {
+                            const double y = rsqrt_full(r2s[q]);
+                            rs[q] = r2s[q] * y;
+                            ws[q] = (y * y) * y;
+                        }
+                        const double b0[3] = {px.y, px.z, px.w};
+#pragma unroll
+                        for (int c = 0; c < 3; ++c) {
+                            const double th0 = lam[0][c] * rs[0];
+                            if (small_eps) {
+                                double s0, c0;
+                                sincos_pos(th0, s0, c0);
+                                acc[0][c] = fma(fma(th0, s0, c0), ws[0] * b0[c], acc[0][c]);
+#pragma unroll
+                                for (int q = 1; q < 4; ++q) {
+                                    const double thq = lam[0][c] * rs[q];
+                                    double sn, cs;
+                                    rotate_small(s0, c0, thq - th0, sn, cs);
+                                    acc[q][c] = fma(fma(thq, sn, cs), ws[q] * b0[c], acc[q][c]);
+                                }
+                            } else {
+#pragma unroll
+                                for (int q = 0; q < 4; ++q)
+                                    acc[q][c] = fma(kernel_n(lam[0][c] * rs[q]), ws[q] * b0[c], acc[q][c]);
+                            }
+                        }
+                        continue;
+                    }
                     const double dx = px.x - xi;
                     const double r2 = fma(dx, dx, cc);
                     const double y = rsqrt_full(r2);   // 1/r
@@ -255,7 +300,7 @@ __global__ void __launch_bounds__(THREADS, MINB) interact64_kernel(const __grid_
 #pragma unroll
                         for (int q = 0; q < 3; ++q)
                             p.part[((long long)c * 12 + s * 3 + q) * p.cap + slot] = acc[0][q];
-                    } else if (MODE == MODE_ANALYTIC) {
+                    } else if (MODE == MODE_ANALYTIC || MODE == MODE_STENCIL4) {   // rows = kinds / stencil positions
 #pragma unroll
                         for (int kd = 0; kd < 4; ++kd)
 #pragma unroll

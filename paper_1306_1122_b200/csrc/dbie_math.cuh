@@ -146,6 +146,19 @@ DBIE_HD void kernel_n_cos(double th, double& n, double& c, int& sg) {
     sg = (q << 30) & (int)0x80000000;
 }
 
+// (sin, cos)(theta0 + eps) from (s0, c0) = (sin, cos)(theta0) for |eps| <= 4e-3: the angle-addition
+// formulas with sin eps = eps - eps^3/6 + eps^5/120 (next term 3e-21) and cos eps = 1 - eps^2/2 + eps^4/24
+// (next term eps^6/720 <= 6e-18).  11 FP64 instructions instead of the 17 of a full sincos; the
+// DIFFERENCE to (s0, c0), which is what Eq. 13's finite differences see, is formed without cancellation.
+DBIE_HD void rotate_small(double s0, double c0, double eps, double& s, double& c) {
+    const double e2 = eps * eps;
+    const double ce = fma(e2, fma(e2, 1.0 / 24.0, -0.5), 1.0);
+    const double se = fma(eps * e2, fma(e2, 1.0 / 120.0, -1.0 / 6.0), eps);
+    s = fma(s0, ce, c0 * se);
+    c = fma(c0, ce, -(s0 * se));
+}
+constexpr double kRotateSmallMax = 4e-3;
+
 // full sincos (used by host accuracy tests and by nothing on the hot path)
 DBIE_HD void sincos_pos(double th, double& s, double& c) {
     int q;

@@ -151,7 +151,14 @@ int main(int argc, char** argv) {
       run_new<1, 1, 256, 2, 2>("stencil NT1 256x2 u2 persistent dynamic [library]", q, sms, 16, 2, is / 4);
       run_new<1, 1, 256, 2, 2>("stencil NT1 256x2 u2 persistent static", q, sms, 16, 1, is / 4);
       run_new<1, 1, 256, 2, 2>("stencil NT1 256x2 u2 one CTA per item", q, sms, 16, 0, is / 4);
-      run_new<1, 1, 256, 4, 1>("stencil NT1 256x4 u1 one CTA per item", q, sms, 16, 0, is / 4); }
+      run_new<1, 1, 256, 4, 1>("stencil NT1 256x4 u1 one CTA per item", q, sms, 16, 0, is / 4);
+      // 4 stencil positions per thread, small-angle rotation between them (61.25 FP64 instr. per interaction)
+      run_new<5, 1, 128, 2, 1>("stencil4 128x2 u1 persistent dynamic", q, sms, 16, 2, is / 4);
+      run_new<5, 1, 128, 2, 1>("stencil4 128x2 u1", q, sms, 16, 0, is / 4);
+      run_new<5, 1, 128, 3, 1>("stencil4 128x3 u1", q, sms, 16, 0, is / 4);
+      run_new<5, 1, 256, 1, 1>("stencil4 256x1 u1", q, sms, 16, 0, is / 4);
+      run_new<5, 1, 64, 4, 1>("stencil4 64x4 u1", q, sms, 16, 0, is / 4);
+      run_new<5, 1, 128, 2, 2>("stencil4 128x2 u2", q, sms, 16, 0, is / 4); }
     { InteractParams q = p;   // analytic gradient: 95 FP64 instructions per interaction (frac76 x 95/76 = pipe utilisation)
       run_new<3, 1, 256, 2, 1>("analytic NT1 256x2 u1 persistent dynamic [library]", q, sms, 16, 2, ie);
       run_new<3, 1, 256, 2, 1>("analytic NT1 256x2 u1", q, sms, 16, 0, ie);
