@@ -116,7 +116,7 @@ class ClockSampler:
 # DRAM bytes of ONE launch of the interaction kernel from the committed `ncu --set full` captures
 # (dram__bytes_read.sum + dram__bytes_write.sum; profiles/r01_ncu_full_interact64_*.md).  Static evidence that
 # HBM is idle (the bound is the FP64 pipe); None where no capture of that workload/mode exists.
-NCU_TRAFFIC = {("cfg2", "nm"): 7.47e6 + 46.07e6}
+NCU_TRAFFIC = {("cfg2", "nm"): 7.66e6 + 42.10e6, ("cfg2", "analytic"): 7.24e6 + 42.35e6}
 
 METHOD = {"grid": False, "analytic": False}   # set by main(): GRID (O-4) instead of NM; analytic gradient (O-5)
 

@@ -248,7 +248,9 @@ class DBIE:
         return {"B": out[0:3], "f": out[3], "g": out[4], "J": out[5:8], "div": out[8], "phi": phi}
 
     # -- dbie_solve
-    def solve(self, x, y, z, opts: SolveOpts | None = None, stream=None):
+    def solve(self, x, y, z, opts: SolveOpts | None = None, stream=None, with_current: bool = False):
+        """dbie_solve.  with_current=True adds J = curl B (Eq. 14) and div B at the
+        converged lambda by one more dbie_residual call with the same options."""
         torch = _torch()
         M = x.numel()
         dev = x.device
@@ -262,7 +264,11 @@ class DBIE:
                                          _dev_f64(z, M, "z"), C.byref(o), _vp(B.data_ptr()),
                                          _vp(lam.data_ptr()), _vp(resid.data_ptr()), _vp(iters.data_ptr()),
                                          _vp(status.data_ptr()), _stream_ptr(stream)))
-        return {"B": B, "lam": lam, "f": resid[0], "g": resid[1], "iters": iters, "status": status}
+        out = {"B": B, "lam": lam, "f": resid[0], "g": resid[1], "iters": iters, "status": status}
+        if with_current:
+            r = self.residual(x, y, z, lam, o, stream=stream)
+            out["J"], out["div"] = r["J"], r["div"]
+        return out
 
     def solve_host(self, x, y, z, opts: SolveOpts | None = None):
         x = np.ascontiguousarray(x, dtype=np.float64)

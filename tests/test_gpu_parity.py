@@ -328,6 +328,13 @@ def test_solve_is_reproducible_and_host_entry_matches(dbie):
         for k in ("B", "lam", "f", "g", "iters", "status"):
             assert np.array_equal(a[k].cpu().numpy(), b[k].cpu().numpy(), equal_nan=True), k
             assert np.array_equal(a[k].cpu().numpy(), h[k], equal_nan=True), k
+        # J = curl B and div B at the converged lambda (Eq. 14): consistent with the returned f, g
+        c = ctx.solve(dw.x, dw.y, dw.z, with_current=True)
+        J, B, dv = c["J"].cpu().numpy(), c["B"].cpu().numpy(), c["div"].cpu().numpy()
+        nB, nJ = np.linalg.norm(B, axis=0), np.linalg.norm(J, axis=0)
+        f = np.linalg.norm(np.cross(J.T, B.T), axis=1) / (nJ * nB)
+        assert np.allclose(f, c["f"].cpu().numpy(), atol=1e-7)
+        assert np.allclose(np.abs(dv) * (w.h / 6.0) / nB, c["g"].cpu().numpy(), atol=1e-7)
         # maxiter = 0: the best initial vertex is returned with status 2
         z = ctx.solve(dw.x, dw.y, dw.z, dbie.default_opts(maxiter=0))
         assert (z["status"].cpu().numpy() == 2).all() and (z["iters"].cpu().numpy() == 0).all()
