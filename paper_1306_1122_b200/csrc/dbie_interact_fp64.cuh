@@ -5,15 +5,15 @@
 //   consumer of the chunk sums).
 //
 // Mapping (the inverse of the paper's, which strides the PIXELS of one point
-// over 80x128 threads): a thread owns ONE evaluation position (a field point, or one of the 4
-// stencil positions of Eq. 13) and NT lambda triples that share its geometry (NT = 1 except in
-// GRID mode).  The boundary is streamed through shared memory in 16 KB tiles by the TMA
-// bulk-copy engine (cp.async.bulk + mbarrier, double buffered) and every thread of the CTA reads
-// the same pixel record as a broadcast LDS.128 pair.  UNR pixels are in flight per thread.  The
-// round-1 profile of the first version (4 stencil positions per thread, 64-bit literals
-// re-materialised in the loop; profiles/r01_ncu_full_interact_stencil_cfg2.md) had the FP64 pipe at
-// 67 %; this one reaches 79 % (profiles/r01_ncu_full_interact64_stencil_cfg2.md), and the shape sweep
-// (csrc/tune_interact.cu, profiles/r01_variants.md) picks THREADS x MINB x UNR = 256 x 2 x 2.
+// over 80x128 threads): evaluation positions are the parallel dimension.  A thread owns one field
+// point (eval, analytic gradient), all 4 stencil positions of a field point (Eq. 13: MODE_STENCIL4),
+// or one stencil position with NT equally spaced trial lambda triples (GRID).  The boundary is
+// streamed through shared memory in 16 KB tiles by the TMA bulk-copy engine (cp.async.bulk +
+// mbarrier, double buffered) and every thread of the CTA reads the same pixel record as a broadcast
+// LDS.128 pair; UNR pixels are in flight per thread.  The bound is the FP64 pipe; the history of the
+// stencil launch over round 1 (14.17 -> 11.11 -> 9.04 ms) is in profiles/r01_ncu_full_interact*_cfg2.md
+// and the shape sweep behind every THREADS x MINB x UNR choice in profiles/r01_variants.md
+// (csrc/tune_interact.cu).
 #pragma once
 #include <cuda_runtime.h>
 #include <stdint.h>
