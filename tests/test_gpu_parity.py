@@ -235,6 +235,30 @@ def test_residual_matches_oracle(dbie, case):
     assert np.abs(r["phi"] - ro["phi"]).max() <= 2 * TOL_FG
 
 
+def test_residual_large_delta_takes_the_plain_stencil_path(dbie):
+    """MODE_STENCIL4 rotates sin/cos between the stencil positions only while lambda*delta <= 4e-3;
+    with delta = 0.05 h and lambda up to 0.3/h (lambda*delta = 1.5e-2) most threads take the plain
+    four-sincos path, the lambda = 0 points of the same warps the rotated one (divergent warps)."""
+    import torch
+    w = workloads.random_boundary(48, 40, seed=15, npts=200, h=0.25)
+    lam = np.random.default_rng(4).uniform(0.0, 0.3, (3, w.M)) / w.h
+    lam[:, ::3] = 0.0
+    lam[:, 1::7] *= 0.01
+    for delta in (0.05, 1e-3):
+        oo = oracle.Opts(delta=delta)
+        ro = oracle.residual(w, lam, oo)
+        with dbie.DBIE.from_workload(w) as ctx:
+            dw = dbie.to_device(w)
+            r = ctx.residual(dw.x, dw.y, dw.z, torch.from_numpy(lam).cuda(), dbie.default_opts(delta=delta))
+            r = {k: v.cpu().numpy() for k, v in r.items()}
+        err, _ = vec_relerr(r["B"], ro["B"])
+        assert err <= TOL_B
+        nB = np.linalg.norm(ro["B"], axis=0)
+        assert np.all(np.abs(r["J"] - ro["J"]) <= 1e-11 * nB / (delta * w.h) + 1e-300)
+        assert np.all(np.abs(r["div"] - ro["div"]) <= 1e-11 * nB / (delta * w.h) + 1e-300)
+        assert np.abs(r["f"] - ro["f"]).max() <= TOL_FG and np.abs(r["g"] - ro["g"]).max() <= TOL_FG
+
+
 # ---------------------------------------------------------------------------- solve --------
 def _check_solve_parity(dbie, wl, opts_kw=None, gpu=None):
     """Protocol P-4; opts_kw["method"] = 1 selects GRID on both sides.
