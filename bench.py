@@ -366,7 +366,7 @@ def run_ours(args) -> None:
 
 
 # --------------------------------------------------------------------------- fp32 leg ------
-FP32_INSTR_PER_INTERACTION = 56      # FFMA/FMUL/FADD per interaction (SASS: 448 per 8 interactions)
+FP32_INSTR_PER_INTERACTION = 59      # FFMA/FMUL/FADD per interaction (SASS: 472 of 585 instructions per 8 interactions)
 FP32_LANES_PER_SM = 128
 
 
@@ -442,8 +442,8 @@ def run_ours_f32(args) -> None:
         "roofline": {"bound": "alu", "kernel": "dbie::interact_f32_kernel (fp32 point-pixel sums, polynomial sincos)",
                      "achieved": 2e-12 * ach, "peak": 2e-12 * peak, "unit": "TFLOP/s", "frac": ach / peak,
                      "traffic": None, "fp32_instr_per_interaction": FP32_INSTR_PER_INTERACTION,
-                     "note": "FP32 FMA pipe: 148 SM x 128 lanes x clocks.max.sm; the kernel issues 82 instructions per "
-                             "interaction in total, so the issue port (148 x 4 x 32 lanes/clk) bounds it at 0.68 of this peak",
+                     "note": "FP32 FMA pipe: 148 SM x 128 lanes x clocks.max.sm; the kernel issues 73 instructions per "
+                             "interaction in total, so the issue port (148 x 4 x 32 lanes/clk) bounds it at 0.81 of this peak",
                      "kernel_interactions_per_s": kern_ips, "kernel_ms_per_launch": kern_ms / max(kern_launches, 1),
                      "kernel_launches": kern_launches, "kernel_share_of_step": kern_ms / ms_total if ms_total else None,
                      "peak_measured_ffma_per_s": ffma_meas,

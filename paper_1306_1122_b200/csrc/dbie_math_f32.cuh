@@ -91,10 +91,11 @@ DBIE_HD32 float kernel_n_f32(float th) {
     {
         sincos_reduced_f32(t, sn, cs);
     }
-    const bool odd = (q & 1) != 0;
-    const float a = odd ? cs : sn;
-    const float b = f32_from_bits(f32_bits(odd ? sn : cs) ^ (q << 31));
-    const float n = fmaf(th, a, b);
+    // both quadrant forms, one selected (as in the fp64 kernel_n): the kernel is issue-bound, and this
+    // trades one FSEL + two LOP3/SHF per component for one FFMA
+    const float ne = fmaf(th, sn, cs);
+    const float no = fmaf(th, cs, -sn);
+    const float n = (q & 1) ? no : ne;
     return f32_from_bits(f32_bits(n) ^ ((q << 30) & (int)0x80000000));
 }
 
