@@ -34,7 +34,8 @@ METRIC = "point-pixel DBIE interactions/sec (fp64)"
 UNIT = "interactions/s"
 FP64_INSTR_PER_INTERACTION = 76      # eval: DESIGN.md section 6 (SASS inner loop: 152 per 2 pixels of one position)
 FP64_INSTR_STENCIL = 245 / 4         # Eq. 13 stencil: 4 positions per thread, small-angle rotation (SASS: 245 per pixel)
-FP64_INSTR_ANALYTIC = 95             # analytic gradient: 11 + 3 x 28 per pixel of the one position
+FP64_INSTR_ANALYTIC = 95             # analytic gradient: 11 + 3 x 28 per pixel of the one position;
+                                     # GRID on it: two trial triples per geometry, (14 + 2 x 81) / 2 = 88
 FP64_INSTR_GRID = {8: 238 / 8, 4: 154 / 4, 2: 112 / 2, 1: 76}   # GRID: 31 + 3 (20 + 7 (NT-1)) per NT equally spaced trial triples
 FP64_INSTR_SURVEY = 82               # SURVEY.md 8(d) canonical count
 SM_COUNT, FP64_LANES_PER_SM = 148, 64   # B200: 148 SMs, 64 FP64 lanes per SM per clock
@@ -317,7 +318,7 @@ def run_ours(args) -> None:
     sm_max = (clocks or {}).get("sm_max_mhz") or 1965.0
     peak_slots = SM_COUNT * FP64_LANES_PER_SM * sm_max * 1e6          # FP64 lane-instructions / s
     kern_ips = inter_total / (kern_ms * 1e-3) if kern_ms > 0 else 0.0
-    per_inter = FP64_INSTR_ANALYTIC if (is_solve and METHOD["analytic"]) else (
+    per_inter = (88.0 if METHOD["grid"] else FP64_INSTR_ANALYTIC) if (is_solve and METHOD["analytic"]) else (
         FP64_INSTR_GRID[8] if (is_solve and METHOD["grid"]) else (
             FP64_INSTR_STENCIL if is_solve else FP64_INSTR_PER_INTERACTION))
     achieved_slots = kern_ips * per_inter

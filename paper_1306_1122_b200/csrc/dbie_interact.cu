@@ -155,13 +155,14 @@ cudaError_t launch_interact_stencil(const InteractParams& p, int sm_count, cudaS
 }
 
 cudaError_t launch_interact_analytic(const InteractParams& p, int sm_count, cudaStream_t st) {
-    return launch64<MODE_ANALYTIC, 1, 1>(p, sm_count, 16, st);
+    return launch64<MODE_ANALYTIC, 1, 2>(p, sm_count, 16, st);
 }
 
 cudaError_t launch_interact_grid_analytic(const InteractParams& p, int sm_count, cudaStream_t st) {
-    // one trial triple per thread: two (24 accumulators + 2 x 6 lambda, lambda^2) need 168 registers,
-    // which the 256 x 2 shape does not have (spills); sharing the geometry would save 7 of 95 instructions
+    // two trial triples per thread share the geometry (88 instead of 95 instructions per interaction);
+    // 24 accumulators + 2 x 6 lambda, lambda^2 need 168 registers: 128 threads x 3 CTAs/SM
     if (p.T < 2) return cudaErrorInvalidValue;
+    if (p.T % 2 == 0) return launch64<MODE_GRID_ANALYTIC, 2, 1, 128, 3>(p, sm_count, 16, st);
     return launch64<MODE_GRID_ANALYTIC, 1, 2>(p, sm_count, 16, st);
 }
 
@@ -170,7 +171,7 @@ cudaError_t launch_interact_grid(const InteractParams& p, int sm_count, cudaStre
     // NT > 1 uses the rotation recurrence, which needs window starts lo >= 0: not guaranteed for T = 2
     // 8 trial triples per thread need 234 registers: 128 threads x 2 CTAs/SM (profiles/r01_variants.md)
     if (p.T % 8 == 0) return launch64<MODE_GRID, 8, 1, 128, 2>(p, sm_count, 16, st);
-    if (p.T % 4 == 0) return launch64<MODE_GRID, 4, 1>(p, sm_count, 16, st);
+    if (p.T % 4 == 0) return launch64<MODE_GRID, 4, 1, 128, 3>(p, sm_count, 16, st);
     if (p.T % 2 == 0 && p.T > 2) return launch64<MODE_GRID, 2, 2>(p, sm_count, 16, st);
     return launch64<MODE_GRID, 1, 2>(p, sm_count, 16, st);
 }
