@@ -247,9 +247,17 @@ def run_ours(args) -> None:
         out = ctx.solve(d_x, d_y, d_z, sopts) if is_solve else ctx.eval(d_x, d_y, d_z, d_lam)
         return ctx, out
 
+    # e2e inputs live in pinned host memory (numpy views of pinned tensors keep them alive)
+    pin = lambda a: torch.from_numpy(np.ascontiguousarray(a, dtype=np.float64)).pin_memory()
+    _pinned = {k: pin(getattr(wl, k)) for k in ("bx", "by", "bz", "x", "y", "z")}
+    if not is_solve:
+        _pinned["lam"] = pin(wl.lam)
+    hp = {k: v.numpy() for k, v in _pinned.items()}
+
     def step_host():
-        ctx = dbie.DBIE(wl.nx, wl.ny, wl.h, wl.x0, wl.y0, wl.bx, wl.by, wl.bz)
-        out = ctx.solve_host(wl.x, wl.y, wl.z, sopts) if is_solve else ctx.eval_host(wl.x, wl.y, wl.z, wl.lam)
+        ctx = dbie.DBIE(wl.nx, wl.ny, wl.h, wl.x0, wl.y0, hp["bx"], hp["by"], hp["bz"])
+        out = (ctx.solve_host(hp["x"], hp["y"], hp["z"], sopts) if is_solve
+               else ctx.eval_host(hp["x"], hp["y"], hp["z"], hp["lam"]))
         return ctx, out
 
     # ---- warm-up

@@ -342,6 +342,21 @@ def test_solve_random_boundary_options_and_invalid_points(dbie):
     assert (s["status"] == 2).any()      # the iteration cap is reached by some points
 
 
+def test_solve_and_residual_accept_an_empty_batch(dbie):
+    """M = 0 is a valid no-op for every entry point (no launch, empty outputs)."""
+    import torch
+    w = workloads.random_boundary(20, 12, seed=3, npts=4)
+    e = torch.empty(0, dtype=torch.float64, device="cuda")
+    with dbie.DBIE.from_workload(w) as ctx:
+        for o in (None, dbie.default_opts(method=1), dbie.default_opts(analytic=1)):
+            s = ctx.solve(e, e, e, o)
+            assert s["B"].shape == (3, 0) and s["status"].numel() == 0
+        r = ctx.residual(e, e, e, torch.empty((3, 0), dtype=torch.float64, device="cuda"))
+        assert r["J"].shape == (3, 0)
+        h = ctx.solve_host(np.empty(0), np.empty(0), np.empty(0))
+        assert h["lam"].shape == (3, 0)
+
+
 def test_solve_is_reproducible_and_host_entry_matches(dbie):
     w, _ = workloads.config2().seeded_subset(64, seed_offset=3)
     with dbie.DBIE.from_workload(w) as ctx:
