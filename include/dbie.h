@@ -111,9 +111,10 @@ typedef struct {
     double xtol;      /* NM stop: max |V_j - V_0| <= xtol/h and max |Phi_j - Phi_0| <= ftol;  */
     double ftol;      /*   1e-4, 1e-6                                                         */
     int maxiter;      /* NM iteration cap; 200                                                */
-    int n_trial;      /* GRID: T trial lambda per component per level (>= 2); 8               */
-    int n_level;      /* GRID: number of refinement levels; 10                                */
-    double lam_max;   /* GRID: search window [0, lam_max/h]; 0.4                              */
+    int n_trial;      /* GRID: T trial lambda per component per level, 2 <= T <= 32 (else
+                         DBIE_EINVAL); 8.  Multiples of 8 (then 4, then 2) run fastest.          */
+    int n_level;      /* GRID: number of refinement levels (>= 1); 10                           */
+    double lam_max;   /* GRID: search window [0, lam_max/h] (> 0); 0.4                          */
     int use_eq12;     /* 1: stop a point as soon as f <= eps_f and g <= eps_g (Eq. 12)        */
     int analytic;     /* 0 (default): J and div B from the finite differences of Eq. 13 (the
                          paper's method).  1: from the analytic gradient of Eq. 6, a second sum
@@ -130,7 +131,9 @@ void dbie_solve_default_opts(dbie_solve_opts* opts);
  * B: out 3*M, field at lambda*.  lam: out 3*M, lambda* >= 0 (reading A-3).
  * resid: out 2*M, resid[i] = f_i (Eq. 8), resid[M+i] = g_i (Eq. 9) at lambda*.
  * iters: out M (NM iterations / GRID levels done).  status: out M: 0 = Eq. 12 thresholds
- * met, 1 = simplex tolerance (GRID: all levels done), 2 = maxiter, 3 = invalid point. */
+ * met, 1 = simplex tolerance (GRID: all levels done), 2 = maxiter, 3 = invalid point.
+ * M must be < 2^31.  Large M is processed in batches (the context's scratch is bounded); a
+ * point's result does not depend on the batch or on M. */
 dbie_status dbie_solve(dbie_ctx* ctx, long long M, const double* x, const double* y,
                        const double* z, const dbie_solve_opts* opts, double* B, double* lam,
                        double* resid, int* iters, int* status, void* cuda_stream);
@@ -140,7 +143,7 @@ dbie_status dbie_solve_host(dbie_ctx* ctx, long long M, const double* x, const d
 
 /* Eq. 8, 9, 13, 14 at given lambda triples (one objective evaluation per point; the same
  * code path the solver uses).  out: 9*M, rows B_x,B_y,B_z, f, g, J_x,J_y,J_z, div B.
- * delta, cell, w_g are taken from opts (NULL = defaults).  phi: out M (may be NULL). */
+ * delta, cell, w_g, analytic are taken from opts (NULL = defaults).  phi: out M (may be NULL). */
 dbie_status dbie_residual(dbie_ctx* ctx, long long M, const double* x, const double* y,
                           const double* z, const double* lam, const dbie_solve_opts* opts,
                           double* out, double* phi, void* cuda_stream);
