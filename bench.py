@@ -33,7 +33,7 @@ sys.path.insert(0, ROOT)
 METRIC = "point-pixel DBIE interactions/sec (fp64)"
 UNIT = "interactions/s"
 FP64_INSTR_PER_INTERACTION = 76      # eval: DESIGN.md section 6 (SASS inner loop: 152 per 2 pixels of one position)
-FP64_INSTR_STENCIL = 245 / 4         # Eq. 13 stencil: 4 positions per thread, small-angle rotation (SASS: 245 per pixel)
+FP64_INSTR_STENCIL = 236 / 4         # Eq. 13 stencil: 4 positions per thread, small-angle rotation (SASS: 236 per pixel)
 FP64_INSTR_ANALYTIC = 95             # analytic gradient: 11 + 3 x 28 per pixel of the one position;
                                      # GRID on it: two trial triples per geometry, (14 + 2 x 81) / 2 = 88
 FP64_INSTR_GRID = {8: 238 / 8, 4: 154 / 4, 2: 112 / 2, 1: 76}   # GRID: 31 + 3 (20 + 7 (NT-1)) per NT equally spaced trial triples
@@ -117,7 +117,7 @@ class ClockSampler:
 # DRAM bytes of ONE launch of the interaction kernel from the committed `ncu --set full` captures
 # (dram__bytes_read.sum + dram__bytes_write.sum; profiles/r01_ncu_full_interact64_*.md).  Static evidence that
 # HBM is idle (the bound is the FP64 pipe); None where no capture of that workload/mode exists.
-NCU_TRAFFIC = {("cfg2", "nm"): 7.66e6 + 42.10e6, ("cfg2", "analytic"): 7.24e6 + 42.35e6}
+NCU_TRAFFIC = {("cfg2", "nm"): 7.22e6 + 42.92e6, ("cfg2", "analytic"): 7.24e6 + 42.35e6}
 
 METHOD = {"grid": False, "analytic": False}   # set by main(): GRID (O-4) instead of NM; analytic gradient (O-5)
 
@@ -339,7 +339,7 @@ def run_ours(args) -> None:
         "traffic_note": "bytes of the launch with all points active (ncu capture, profiles/); algorithmic: 6.8 MB of point "
                         "data in + 100 MB of chunk partial sums out, of which the L2 keeps half",
         "note": "FP64-pipe bound (no HBM/tensor step): achieved = interactions/s of the kernel x FP64 "
-                "lane-instructions per interaction (eval 76; Eq. 13 stencil 61.25; GRID T=8: 8 equally spaced trial triples per geometry 29.75; analytic gradient 95; DESIGN.md s6) "
+                "lane-instructions per interaction (eval 76; Eq. 13 stencil 59; GRID T=8: 8 equally spaced trial triples per geometry 29.75; analytic gradient 95; DESIGN.md s6) "
                 "x 2 flop per FMA slot; peak = 148 SM x 64 FP64 lanes x clocks.max.sm (derived, DESIGN.md s7)",
         "kernel_interactions_per_s": kern_ips, "kernel_ms_per_launch": kern_ms / max(kern_launches, 1),
         "kernel_launches": kern_launches, "kernel_share_of_step": kern_ms / ms_total if ms_total else None,

@@ -149,9 +149,9 @@ cudaError_t launch_interact_eval(const InteractParams& p, int sm_count, cudaStre
 }
 
 cudaError_t launch_interact_stencil(const InteractParams& p, int sm_count, cudaStream_t st) {
-    // all 4 stencil positions of a point in one thread (small-angle rotation between them): 162 registers,
-    // 128 threads x 3 CTAs/SM; +23 % over one position per thread (MODE_STENCIL, profiles/r01_variants.md)
-    return launch64<MODE_STENCIL4, 1, 1, 128, 3>(p, sm_count, 16, st);
+    // all 4 stencil positions of a point in one thread (small-angle rotation between them), two pixels in
+    // flight: 128 threads x 2 CTAs/SM; +35 % over one position per thread (MODE_STENCIL, profiles/r01_variants.md)
+    return launch64<MODE_STENCIL4, 1, 2, 128, 2>(p, sm_count, 16, st);
 }
 
 cudaError_t launch_interact_analytic(const InteractParams& p, int sm_count, cudaStream_t st) {

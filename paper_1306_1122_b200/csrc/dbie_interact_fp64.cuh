@@ -11,7 +11,7 @@
 // streamed through shared memory in 16 KB tiles by the TMA bulk-copy engine (cp.async.bulk +
 // mbarrier, double buffered) and every thread of the CTA reads the same pixel record as a broadcast
 // LDS.128 pair; UNR pixels are in flight per thread.  The bound is the FP64 pipe; the history of the
-// stencil launch over round 1 (14.17 -> 11.11 -> 9.04 ms) is in profiles/r01_ncu_full_interact*_cfg2.md
+// stencil launch over round 1 (14.17 -> 11.11 -> 9.04 -> 8.39 ms) is in profiles/r01_ncu_full_interact*_cfg2.md
 // and the shape sweep behind every THREADS x MINB x UNR choice in profiles/r01_variants.md
 // (csrc/tune_interact.cu).
 #pragma once
@@ -31,7 +31,7 @@ namespace dbie {
 // MODE_STENCIL4: the Eq. 13 stencil with all 4 positions of a field point in ONE thread (item = slot).
 // The positions are delta = 1e-3 h apart, so theta_s = lambda r_s differs from theta_0 by eps <= lambda delta:
 // one full sincos per component at r_i and a small-angle rotation (rotate_small) for the other three
-// positions; geometry (dx, dy, z terms) is shared where the offsets allow.  61.25 FP64 instructions per
+// positions; geometry (dx, dy, z terms) is shared where the offsets allow.  59 FP64 instructions per
 // interaction instead of 76.  Threads whose lambda delta exceeds kRotateSmallMax take the plain path.
 enum { MODE_EVAL = 0, MODE_STENCIL = 1, MODE_GRID = 2, MODE_ANALYTIC = 3, MODE_GRID_ANALYTIC = 4, MODE_STENCIL4 = 5 };
 
@@ -40,6 +40,42 @@ __host__ __device__ inline long long items_per_slot(int mode, int G) {
     if (mode == MODE_EVAL || mode == MODE_ANALYTIC || mode == MODE_STENCIL4) return 1;
     if (mode == MODE_GRID_ANALYTIC) return G;
     return mode == MODE_STENCIL ? kStencil : (long long)kStencil * G;
+}
+
+// One pixel of MODE_STENCIL4: the 4 stencil positions (x_i, x_i + delta | y, y + delta | z, z + delta share
+// dx / dy^2 + z^2 terms where they can).  FAST: one sincos per component at r_i, rotate_small for the rest.
+template <bool FAST>
+__device__ __forceinline__ void stencil4_pixel(const double4 px, double xi, double xi1, double cc, double cc2,
+                                               double cc3, const double (&lam)[3], double (&acc)[4][3]) {
+    const double dx0 = px.x - xi, dx1 = px.x - xi1;
+    const double r2s[4] = {fma(dx0, dx0, cc), fma(dx1, dx1, cc), fma(dx0, dx0, cc2), fma(dx0, dx0, cc3)};
+    double rs[4], ws[4];
+#pragma unroll
+    for (int q = 0; q < 4; ++q) {
+        const double y = rsqrt_full(r2s[q]);
+        rs[q] = r2s[q] * y;
+        ws[q] = (y * y) * y;
+    }
+    const double b0[3] = {px.y, px.z, px.w};
+#pragma unroll
+    for (int c = 0; c < 3; ++c) {
+        if (FAST) {
+            const double th0 = lam[c] * rs[0];
+            double s0, c0;
+            sincos_pos(th0, s0, c0);
+            acc[0][c] = fma(fma(th0, s0, c0), ws[0] * b0[c], acc[0][c]);
+#pragma unroll
+            for (int q = 1; q < 4; ++q) {
+                const double thq = lam[c] * rs[q];
+                double sn, cs;
+                rotate_small(s0, c0, thq - th0, sn, cs);
+                acc[q][c] = fma(fma(thq, sn, cs), ws[q] * b0[c], acc[q][c]);
+            }
+        } else {
+#pragma unroll
+            for (int q = 0; q < 4; ++q) acc[q][c] = fma(kernel_n(lam[c] * rs[q]), ws[q] * b0[c], acc[q][c]);
+        }
+    }
 }
 
 template <int MODE, int NT, int THREADS, int MINB, int UNR>
@@ -178,43 +214,21 @@ __global__ void __launch_bounds__(THREADS, MINB) interact64_kernel(const __grid_
                 const double cc = fma(dy, dy, z2);
                 const double dy2 = yk - yi2;
                 const double cc2 = fma(dy2, dy2, z2), cc3 = fma(dy, dy, z23);   // MODE_STENCIL4
+                if constexpr (MODE == MODE_STENCIL4) {
+                    // the small-angle / plain decision is per thread: two loops instead of a branch per pixel
+                    if (small_eps) {
+#pragma unroll UNR
+                        for (int j = 0; j < d.ncols; ++j) stencil4_pixel<true>(rp[j], xi, xi1, cc, cc2, cc3, lam[0], acc);
+                    } else {
+#pragma unroll UNR
+                        for (int j = 0; j < d.ncols; ++j) stencil4_pixel<false>(rp[j], xi, xi1, cc, cc2, cc3, lam[0], acc);
+                    }
+                    rp += d.ncols;
+                    continue;
+                }
 #pragma unroll UNR
                 for (int j = 0; j < d.ncols; ++j) {
                     const double4 px = rp[j];  // {x_k, Bx0, By0, Bz0}: two broadcast LDS.128
-                    if (MODE == MODE_STENCIL4) {
-                        const double dx0 = px.x - xi, dx1 = px.x - xi1;
-                        const double r2s[4] = {fma(dx0, dx0, cc), fma(dx1, dx1, cc), fma(dx0, dx0, cc2),
-                                               fma(dx0, dx0, cc3)};
-                        double rs[4], ws[4];
-#pragma unroll
-                        for (int q = 0; q < 4; ++q) {
-                            const double y = rsqrt_full(r2s[q]);
-                            rs[q] = r2s[q] * y;
-                            ws[q] = (y * y) * y;
-                        }
-                        const double b0[3] = {px.y, px.z, px.w};
-#pragma unroll
-                        for (int c = 0; c < 3; ++c) {
-                            const double th0 = lam[0][c] * rs[0];
-                            if (small_eps) {
-                                double s0, c0;
-                                sincos_pos(th0, s0, c0);
-                                acc[0][c] = fma(fma(th0, s0, c0), ws[0] * b0[c], acc[0][c]);
-#pragma unroll
-                                for (int q = 1; q < 4; ++q) {
-                                    const double thq = lam[0][c] * rs[q];
-                                    double sn, cs;
-                                    rotate_small(s0, c0, thq - th0, sn, cs);
-                                    acc[q][c] = fma(fma(thq, sn, cs), ws[q] * b0[c], acc[q][c]);
-                                }
-                            } else {
-#pragma unroll
-                                for (int q = 0; q < 4; ++q)
-                                    acc[q][c] = fma(kernel_n(lam[0][c] * rs[q]), ws[q] * b0[c], acc[q][c]);
-                            }
-                        }
-                        continue;
-                    }
                     const double dx = px.x - xi;
                     const double r2 = fma(dx, dx, cc);
                     const double y = rsqrt_full(r2);   // 1/r

@@ -158,7 +158,13 @@ int main(int argc, char** argv) {
       run_new<5, 1, 128, 3, 1>("stencil4 128x3 u1", q, sms, 16, 0, is / 4);
       run_new<5, 1, 256, 1, 1>("stencil4 256x1 u1", q, sms, 16, 0, is / 4);
       run_new<5, 1, 64, 4, 1>("stencil4 64x4 u1", q, sms, 16, 0, is / 4);
-      run_new<5, 1, 128, 2, 2>("stencil4 128x2 u2", q, sms, 16, 0, is / 4); }
+      run_new<5, 1, 128, 2, 2>("stencil4 128x2 u2", q, sms, 16, 0, is / 4);
+      run_new<5, 1, 128, 2, 2>("stencil4 128x2 u2 persistent dynamic [library]", q, sms, 16, 2, is / 4);
+      run_new<5, 1, 128, 2, 3>("stencil4 128x2 u3", q, sms, 16, 0, is / 4);
+      run_new<5, 1, 128, 2, 4>("stencil4 128x2 u4", q, sms, 16, 0, is / 4);
+      run_new<5, 1, 256, 1, 2>("stencil4 256x1 u2", q, sms, 16, 0, is / 4);
+      run_new<5, 1, 64, 4, 2>("stencil4 64x4 u2", q, sms, 16, 0, is / 4);
+      run_new<5, 1, 128, 3, 2>("stencil4 128x3 u2", q, sms, 16, 0, is / 4); }
     { InteractParams q = p;   // analytic gradient: 95 FP64 instructions per interaction (frac76 x 95/76 = pipe utilisation)
       run_new<3, 1, 256, 2, 1>("analytic NT1 256x2 u1 persistent dynamic [library]", q, sms, 16, 2, ie);
       run_new<3, 1, 256, 2, 1>("analytic NT1 256x2 u1", q, sms, 16, 0, ie);
