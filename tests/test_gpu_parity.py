@@ -468,16 +468,19 @@ def test_solve_config2_full_volume_sampled(dbie):
 
 
 def test_solve_config3_large_batch_sampled(dbie):
-    """BASELINE configs[2] boundary (256x256, h = 0.5): NM solve of a 16,384-point seeded subset of
-    the 128x128x64 volume in one call, 24 of them re-solved by the oracle."""
-    w, _ = workloads.config3().seeded_subset(16384, seed_offset=5)
+    """BASELINE configs[2] boundary (256x256, h = 0.5): NM solve of the 65,536-point seeded subset of
+    the 128x128x64 volume that `bench.py --workload cfg3 --points 65536` times (same seed), in one
+    call; 24 of them re-solved by the oracle."""
+    w, _ = workloads.config3().seeded_subset(65536, seed_offset=900)
     _solve_full_and_sample(dbie, w, 24)
 
 
 def test_grid_config5_large_batch_sampled(dbie):
-    """BASELINE configs[4] boundary (1024x1024): GRID solve (T = 8, 3 levels) of a 4,096-point
-    seeded subset of the 256x256x128 volume in one call, 6 of them re-solved by the oracle."""
-    w, _ = workloads.config5().seeded_subset(4096, seed_offset=5)
+    """BASELINE configs[4] boundary (1024x1024): GRID solve (T = 8; 3 of the 10 levels, the oracle
+    costs 1.3e8 interactions per point and level) of the 16,384-point seeded subset of the
+    256x256x128 volume that `bench.py --workload cfg5` times (same seed), in one call; 6 of them
+    re-solved by the oracle."""
+    w, _ = workloads.config5().seeded_subset(16384, seed_offset=900)
     _solve_full_and_sample(dbie, w, 6, dict(method=1, n_level=3))
 
 
