@@ -22,6 +22,8 @@ struct dbie_ctx {
     char* io;           size_t io_bytes;      // device staging of the _host entry points
     unsigned* counters;                       // device: nact[2], pad[2], nevals (u64) at +16 B, work[2] at +32 B
     cudaStream_t own_stream;
+    unsigned* h_probe;                        // pinned host: active-list lengths read back by the solve loop
+    cudaEvent_t probe_ev[2];
     double last_interactions;
     long long last_launches, last_evals;
     int evals_on_device;                      // last call was a solve: read nevals back on demand
@@ -158,6 +160,9 @@ extern "C" void dbie_destroy(dbie_ctx* ctx) {
     cudaFree(ctx->io);
     cudaFree(ctx->counters);
     if (ctx->own_stream) cudaStreamDestroy(ctx->own_stream);
+    if (ctx->h_probe) cudaFreeHost(ctx->h_probe);
+    for (int i = 0; i < 2; ++i)
+        if (ctx->probe_ev[i]) cudaEventDestroy(ctx->probe_ev[i]);
     for (int i = 0; i < ctx->ev_cap; ++i) cudaEventDestroy(ctx->ev[i]);
     free(ctx->ev);
     (void)cudaGetLastError();
@@ -199,6 +204,11 @@ extern "C" dbie_status dbie_create(dbie_ctx** out, int nx, int ny, double h, dou
         if ((e = cudaMalloc(&ctx->counters, 64)) != cudaSuccess) { st = fail_cuda(ctx, e, "cudaMalloc(counters)"); break; }
         if ((e = cudaMemset(ctx->counters, 0, 64)) != cudaSuccess) { st = fail_cuda(ctx, e, "cudaMemset"); break; }
         if ((e = cudaStreamCreateWithFlags(&ctx->own_stream, cudaStreamNonBlocking)) != cudaSuccess) { st = fail_cuda(ctx, e, "cudaStreamCreate"); break; }
+        if ((e = cudaHostAlloc((void**)&ctx->h_probe, 64, cudaHostAllocDefault)) != cudaSuccess) { st = fail_cuda(ctx, e, "cudaHostAlloc"); break; }
+        if ((e = cudaEventCreateWithFlags(&ctx->probe_ev[0], cudaEventDisableTiming)) != cudaSuccess ||
+            (e = cudaEventCreateWithFlags(&ctx->probe_ev[1], cudaEventDisableTiming)) != cudaSuccess) {
+            st = fail_cuda(ctx, e, "cudaEventCreate"); break;
+        }
         e = q9 ? launch_stage_q9(nx, ny, h, x0, y0, bx, by, bz, sx, sy, ctx->rec, ctx->yk, ctx->rec32, ctx->yk32, 0)
                : launch_stage_boundary(nx, ny, h, x0, y0, bx, by, bz, ctx->rec, ctx->yk, ctx->rec32, ctx->yk32, 0);
         if (e != cudaSuccess) {
@@ -523,7 +533,29 @@ extern "C" dbie_status dbie_solve(dbie_ctx* ctx, long long M, const double* x, c
         CU(launch_solve_init(a, k, cnt, M, x + off, y + off, z + off, B + off, lam + off, resid + off,
                              iters + off, status + off, st));
         ++launches;
+        // The pass schedule is fixed, but every kProbeEvery passes the length of the next active list is
+        // copied to pinned host memory behind an event; when a copy that has ALREADY completed shows an
+        // empty list the rest of the schedule is not enqueued.  The host never waits: a large batch (the
+        // host runs far ahead of the device) enqueues everything, a small launch-bound one stops early.
+        const int kProbeEvery = 32;
+        int probe_pending[2] = {0, 0};
         for (int pass = 0; pass < maxpass; ++pass) {
+            if (pass % kProbeEvery == 0 && pass > 0) {
+                bool done = false;
+                for (int q = 0; q < 2; ++q)
+                    if (probe_pending[q] && cudaEventQuery(ctx->probe_ev[q]) == cudaSuccess) {
+                        probe_pending[q] = 0;
+                        done = done || ctx->h_probe[q] == 0u;
+                    }
+                (void)cudaGetLastError();   // cudaErrorNotReady of a pending probe is not an error
+                if (done) break;
+                const int q = (pass / kProbeEvery) & 1;
+                if (!probe_pending[q]) {
+                    CU(cudaMemcpyAsync(&ctx->h_probe[q], &a.nact[pass & 1], sizeof(unsigned), cudaMemcpyDeviceToHost, st));
+                    CU(cudaEventRecord(ctx->probe_ev[q], st));
+                    probe_pending[q] = 1;
+                }
+            }
             InteractParams p;
             memset(&p, 0, sizeof p);
             p.bd = ctx->bd;
