@@ -183,6 +183,7 @@ __global__ void __launch_bounds__(THREADS, MINB) interact64_kernel(const __grid_
         double acc[NA][3];
 #pragma unroll
         for (int tt = 0; tt < NA; ++tt) acc[tt][0] = acc[tt][1] = acc[tt][2] = 0.0;
+        const bool lam_all_zero = (lam[0][0] == 0.0) && (lam[0][1] == 0.0) && (lam[0][2] == 0.0);   // MODE_EVAL
         const bool small_eps = fmax(fmax(lam[0][0], lam[0][1]), lam[0][2]) * p.delta_abs <= kRotateSmallMax;
         double lam2[NT][3];   // analytic modes: lambda^2
 #pragma unroll
@@ -225,6 +226,26 @@ __global__ void __launch_bounds__(THREADS, MINB) interact64_kernel(const __grid_
                     }
                     rp += d.ncols;
                     continue;
+                }
+                if constexpr (MODE == MODE_EVAL) {
+                    // lambda = 0 in all three components (the potential field, BASELINE config 1): n(0) = 1
+                    // exactly, so the term is w B_p0 and the sum is bit-identical to the general loop's
+                    // fma(1, w B, acc) at 16 instead of 76 FP64 instructions.  Per-thread decision.
+                    if (lam_all_zero) {
+#pragma unroll 4
+                        for (int j = 0; j < d.ncols; ++j) {
+                            const double4 px = rp[j];
+                            const double dx = px.x - xi;
+                            const double r2 = fma(dx, dx, cc);
+                            const double y = rsqrt_full(r2);
+                            const double wgt = (y * y) * y;
+                            acc[0][0] = __dadd_rn(acc[0][0], __dmul_rn(wgt, px.y));   // no contraction: same
+                            acc[0][1] = __dadd_rn(acc[0][1], __dmul_rn(wgt, px.z));   // roundings as fma(1, w B, acc)
+                            acc[0][2] = __dadd_rn(acc[0][2], __dmul_rn(wgt, px.w));
+                        }
+                        rp += d.ncols;
+                        continue;
+                    }
                 }
 #pragma unroll UNR
                 for (int j = 0; j < d.ncols; ++j) {

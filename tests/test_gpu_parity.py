@@ -133,6 +133,25 @@ def test_eval_edge_cases(dbie):
     assert np.isnan(oracle.eval(wb)[:, 2]).all()
 
 
+def test_eval_potential_field_fast_path_is_bit_identical(dbie):
+    """Points with lambda = 0 in all three components take a loop without sincos (n(0) = 1 exactly).  Their
+    result must equal, bit for bit, what the general loop gives: lambda = 1e-300 r underflows theta to a
+    value whose n(theta) is exactly 1 as well, but takes the general path.  Mixed warps included."""
+    import torch
+    w = workloads.random_boundary(150, 90, seed=41, npts=700, h=0.5, zmin=0.5, zmax=40.0)
+    lam0 = np.zeros((3, w.M))
+    lam_tiny = np.full((3, w.M), 1e-300)
+    lam_mixed = lam0.copy(); lam_mixed[:, ::2] = w.lam[:, ::2]
+    with dbie.DBIE.from_workload(w) as ctx:
+        dw = dbie.to_device(w)
+        ev = lambda l: ctx.eval(dw.x, dw.y, dw.z, torch.from_numpy(np.ascontiguousarray(l)).cuda()).cpu().numpy()
+        B0, Bt, Bm, Bg = ev(lam0), ev(lam_tiny), ev(lam_mixed), ev(w.lam)
+    assert np.array_equal(B0, Bt)
+    assert np.array_equal(Bm[:, 1::2], B0[:, 1::2]) and np.array_equal(Bm[:, ::2], Bg[:, ::2])
+    err, _ = vec_relerr(B0, oracle.eval(w, lam=lam0))
+    assert err <= TOL_B
+
+
 def test_eval_linearity_and_shift_invariance(dbie):
     """K-8 symmetries on the GPU path: linear in B0; shifting x0, y0 and the points together."""
     w = workloads.random_boundary(40, 24, seed=11, npts=21)
