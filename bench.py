@@ -375,8 +375,9 @@ def run_ours(args) -> None:
 
 
 # --------------------------------------------------------------------------- fp32 leg ------
-FP32_INSTR_PER_INTERACTION = 59      # FFMA/FMUL/FADD per interaction (SASS: 472 of 585 instructions per 8 interactions)
-FP32_LANES_PER_SM = 128
+MUFU_PER_INTERACTION = 7             # default dbie_eval_f32 (SFU sincos): 1 rsqrt + 3 x (sin, cos); SASS: 56 MUFU,
+                                     # 280 FP32 of 439 instructions per 8 interactions
+MUFU_LANES_PER_SM = 16
 
 
 def run_ours_f32(args) -> None:
@@ -435,9 +436,9 @@ def run_ours_f32(args) -> None:
     except Exception:
         dfma_meas = ffma_meas = None
     sm_max = (clocks or {}).get("sm_max_mhz") or 1965.0
-    peak = SM_COUNT * FP32_LANES_PER_SM * sm_max * 1e6
+    peak = SM_COUNT * MUFU_LANES_PER_SM * sm_max * 1e6
     kern_ips = inter * args.steps / (kern_ms * 1e-3) if kern_ms > 0 else 0.0
-    ach = kern_ips * FP32_INSTR_PER_INTERACTION
+    ach = kern_ips * MUFU_PER_INTERACTION
     line = {
         "metric": "point-pixel DBIE interactions/sec (fp32)", "value": inter * args.steps / (ms_total * 1e-3),
         "unit": UNIT, "n_gpus": 1, "steps": args.steps, "warmup": args.warmup, "ms_per_step": ms_total / args.steps,
@@ -448,15 +449,14 @@ def run_ours_f32(args) -> None:
                 "h2d_bytes_per_step": 3 * wl.N * 8 + 6 * wl.M * 4, "d2h_bytes_per_step": 3 * wl.M * 4,
                 "ms_per_step": e2e_ms / args.steps, "api": "DBIE(host boundary, fp32=True) + eval_f32 on pinned host points"},
         "gpu_launches": 3 * args.steps,
-        "roofline": {"bound": "alu", "kernel": "dbie::interact_f32_kernel (fp32 point-pixel sums, polynomial sincos)",
-                     "achieved": 2e-12 * ach, "peak": 2e-12 * peak, "unit": "TFLOP/s", "frac": ach / peak,
-                     "traffic": None, "fp32_instr_per_interaction": FP32_INSTR_PER_INTERACTION,
-                     "note": "FP32 FMA pipe: 148 SM x 128 lanes x clocks.max.sm; the kernel issues 73 instructions per "
-                             "interaction in total, so the issue port (148 x 4 x 32 lanes/clk) bounds it at 0.81 of this peak",
+        "roofline": {"bound": "alu", "kernel": "dbie::interact_f32_kernel (fp32 point-pixel sums, SFU sincos of the reduced argument)",
+                     "achieved": 1e-12 * ach, "peak": 1e-12 * peak, "unit": "T MUFU lane-op/s", "frac": ach / peak,
+                     "traffic": None, "mufu_per_interaction": MUFU_PER_INTERACTION,
+                     "note": "SFU-bound: 148 SM x 16 MUFU lanes x clocks.max.sm / 7 MUFU per interaction (the issue port, 55 "
+                             "instructions per interaction, allows 2 % more; the FP32 FMA pipe 60 % more)",
                      "kernel_interactions_per_s": kern_ips, "kernel_ms_per_launch": kern_ms / max(kern_launches, 1),
                      "kernel_launches": kern_launches, "kernel_share_of_step": kern_ms / ms_total if ms_total else None,
-                     "peak_measured_ffma_per_s": ffma_meas,
-                     "frac_of_measured_ffma": (ach / ffma_meas) if ffma_meas else None},
+                     "peak_measured_ffma_per_s": ffma_meas},
         "cpu_baseline": None,
     }
     print(json.dumps(line), flush=True)

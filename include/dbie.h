@@ -95,7 +95,8 @@ dbie_status dbie_eval_f32(dbie_ctx* ctx, long long M, const float* x, const floa
                           const float* z, const float* lam, float* B, void* cuda_stream);
 /* Tuning knob of dbie_eval_f32: bit p of mask set = component p takes sin/cos of the reduced
  * argument from the SFU (MUFU.SIN/COS) instead of the FMA-pipe polynomials, to balance the two
- * pipes.  Allowed masks: 0 (default), 1, 3, 7.  Results differ at the 1e-6 level between masks. */
+ * pipes.  Allowed masks: 0, 1, 3, 7 (default: all three from the SFU, the fastest measured).  Results
+ * differ at the 1e-6 level between masks; all meet the 2e-4 target. */
 dbie_status dbie_set_f32_sfu_mask(dbie_ctx* ctx, int mask);
 
 /* Options of dbie_solve.  Fill with dbie_solve_default_opts, then change fields. */
