@@ -173,7 +173,16 @@ int main(int argc, char** argv) {
       run_new<3, 1, 256, 2, 1>("analytic NT1 256x2 u1 persistent dynamic [library]", q, sms, 16, 2, ie);
       run_new<3, 1, 256, 2, 1>("analytic NT1 256x2 u1", q, sms, 16, 0, ie);
       run_new<3, 1, 256, 2, 2>("analytic NT1 256x2 u2", q, sms, 16, 0, ie);
-      run_new<3, 1, 128, 4, 2>("analytic NT1 128x4 u2", q, sms, 16, 0, ie); }
+      run_new<3, 1, 128, 4, 2>("analytic NT1 128x4 u2", q, sms, 16, 0, ie);
+      run_new<3, 1, 128, 2, 2>("analytic NT1 128x2 u2", q, sms, 16, 0, ie);
+      run_new<3, 1, 128, 2, 4>("analytic NT1 128x2 u4", q, sms, 16, 0, ie);
+      run_new<3, 1, 256, 1, 4>("analytic NT1 256x1 u4", q, sms, 16, 0, ie); }
+    { InteractParams q = p; q.count = M / 8;   // GRID on the analytic gradient (88 instr. per interaction at NT2)
+      const double iga = (double)T * (M / 8) * N;
+      run_new<4, 2, 128, 3, 1>("grid-analytic NT2 128x3 u1 [library]", q, sms, 16, 0, iga);
+      run_new<4, 2, 128, 2, 1>("grid-analytic NT2 128x2 u1", q, sms, 16, 0, iga);
+      run_new<4, 2, 128, 2, 2>("grid-analytic NT2 128x2 u2", q, sms, 16, 0, iga);
+      run_new<4, 1, 256, 2, 2>("grid-analytic NT1 256x2 u2", q, sms, 16, 0, iga); }
     { InteractParams q = p; q.count = M / 32;
       run_new<2, 4, 256, 2, 1>("grid   NT4 256x2 u1 persistent dynamic [library]", q, sms, 16, 2, ig / 32);
       run_new<2, 4, 256, 2, 1>("grid   NT4 256x2 u1 persistent static", q, sms, 16, 1, ig / 32);
