@@ -151,6 +151,9 @@ int main(int argc, char** argv) {
     run_new<0, 1, 128, 2, 4>("eval   NT1 128x2 u4", p, sms, 8, 0, ie);
     run_new<0, 1, 128, 3, 4>("eval   NT1 128x3 u4", p, sms, 8, 0, ie);
     run_new<0, 1, 256, 1, 4>("eval   NT1 256x1 u4", p, sms, 8, 0, ie);
+    run_new<0, 1, 128, 2, 8>("eval   NT1 128x2 u8", p, sms, 8, 0, ie);
+    run_new<0, 1, 128, 2, 6>("eval   NT1 128x2 u6", p, sms, 8, 0, ie);
+    run_new<0, 1, 64, 4, 8>("eval   NT1 64x4 u8", p, sms, 8, 0, ie);
     { InteractParams q = p; q.count = M / 4;
       run_new<1, 1, 256, 2, 2>("stencil NT1 256x2 u2 persistent dynamic [library]", q, sms, 16, 2, is / 4);
       run_new<1, 1, 256, 2, 2>("stencil NT1 256x2 u2 persistent static", q, sms, 16, 1, is / 4);
