@@ -117,7 +117,7 @@ class ClockSampler:
 # DRAM bytes of ONE launch of the interaction kernel from the committed `ncu --set full` captures
 # (dram__bytes_read.sum + dram__bytes_write.sum; profiles/r01_ncu_full_interact64_*.md).  Static evidence that
 # HBM is idle (the bound is the FP64 pipe); None where no capture of that workload/mode exists.
-NCU_TRAFFIC = {("cfg4", "eval"): 96.0e6 + 383.3e6, ("cfg2", "nm"): 7.22e6 + 42.92e6, ("cfg2", "analytic"): 7.24e6 + 42.35e6}
+NCU_TRAFFIC = {("cfg4", "eval"): 60.2e6 + 5.8e6, ("cfg2", "nm"): 7.22e6 + 42.92e6, ("cfg2", "analytic"): 7.24e6 + 42.35e6}
 
 METHOD = {"grid": False, "analytic": False}   # set by main(): GRID (O-4) instead of NM; analytic gradient (O-5)
 
@@ -338,7 +338,7 @@ def run_ours(args) -> None:
                                    if (is_solve and args.points == 0) else NCU_TRAFFIC.get((args.workload, "eval"))),
         "traffic_note": "bytes of one launch with all points active (ncu captures, profiles/).  Solve: algorithmic 6.8 MB of "
                         "point data in + 100 MB of chunk partial sums out, of which the L2 keeps half.  Eval (cfg4): "
-                        "algorithmic 84 MB; the rest are the 16 canonical chunk partial sums per output (403 MB) - 0.35 GB/s",
+                        "algorithmic 72 M + 32 N = 84 MB (the 25 MB of output sums are read back from L2)",
         "note": "FP64-pipe bound (no HBM/tensor step): achieved = interactions/s of the kernel x FP64 "
                 "lane-instructions per interaction (eval 76; Eq. 13 stencil 59; GRID T=8: 8 equally spaced trial triples per geometry 29.75; analytic gradient 95; DESIGN.md s6) "
                 "x 2 flop per FMA slot; peak = 148 SM x 64 FP64 lanes x clocks.max.sm (derived, DESIGN.md s7)",

@@ -270,9 +270,10 @@ extern "C" dbie_status dbie_eval(dbie_ctx* ctx, long long M, const double* x, co
         p.count = cnt; p.slot0 = off;
         p.part = ctx->part; p.cap = cap;
         prof_mark(ctx, st);
-        CU(launch_interact_eval(p, ctx->sm_count, st));
+        int nparts = ctx->bd.nchunks;
+        CU(launch_interact_eval(p, ctx->sm_count, &nparts, st));
         prof_mark(ctx, st);
-        CU(launch_eval_finalize(ctx->bd, off, cnt, M, z, lam, ctx->part, cap, B, st));
+        CU(launch_eval_finalize(ctx->bd, nparts, off, cnt, M, z, lam, ctx->part, cap, B, st));
         launches += 2;
     }
     ctx->last_interactions = (double)M * (double)ctx->bd.N;
@@ -331,9 +332,10 @@ extern "C" dbie_status dbie_eval_f32(dbie_ctx* ctx, long long M, const float* x,
         p.count = cnt; p.slot0 = off;
         p.part = ctx->part; p.cap = cap;
         prof_mark(ctx, st);
-        CU(launch_interact_f32(p, ctx->sm_count, ctx->f32_sfu_mask, st));
+        int nparts = ctx->bd.nchunks;
+        CU(launch_interact_f32(p, ctx->sm_count, ctx->f32_sfu_mask, &nparts, st));
         prof_mark(ctx, st);
-        CU(launch_eval_finalize_f32(ctx->bd, off, cnt, M, z, lam, ctx->part, cap, B, st));
+        CU(launch_eval_finalize_f32(ctx->bd, nparts, off, cnt, M, z, lam, ctx->part, cap, B, st));
         launches += 2;
     }
     ctx->last_interactions = (double)M * (double)ctx->bd.N;

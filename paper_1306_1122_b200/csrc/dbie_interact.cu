@@ -144,7 +144,11 @@ static cudaError_t launch64(const InteractParams& p, int sm_count, int waves, cu
     return cudaGetLastError();
 }
 
-cudaError_t launch_interact_eval(const InteractParams& p, int sm_count, cudaStream_t st) {
+// *nparts: how many chunk slots the launch fills per output (1 when every CTA covers all chunks and adds
+// them itself, else nchunks); the epilogue adds exactly that many, in chunk order.
+cudaError_t launch_interact_eval(const InteractParams& p, int sm_count, int* nparts, cudaStream_t st) {
+    const long long nblk = (p.count + kThreads64 - 1) / kThreads64;
+    *nparts = (nblk >= 8LL * sm_count * kMinB64 || p.bd.nchunks == 1) ? 1 : p.bd.nchunks;
     return launch64<MODE_EVAL, 1, 2>(p, sm_count, 8, st);
 }
 
@@ -226,7 +230,7 @@ __global__ void __launch_bounds__(THREADS, MINB) interact_f32_kernel(const __gri
 #pragma unroll
             for (int c = 0; c < 3; ++c) lam[r][c] = fabsf(p.lam[c * p.ldlam + id]);
         }
-        double acc[R][3];
+        double acc[R][3], run[R][3];   // run: running sum of the chunk sums of an unsplit launch
 #pragma unroll
         for (int r = 0; r < R; ++r) acc[r][0] = acc[r][1] = acc[r][2] = 0.0;
 
@@ -279,12 +283,27 @@ __global__ void __launch_bounds__(THREADS, MINB) interact_f32_kernel(const __gri
                 rp += d.ncols;
             }
             if (t + 1 == t_chunk_end) {
+                if (nsplit == 1) {   // unsplit launch: add the chunk sums here, in chunk order (as the epilogue would)
 #pragma unroll
-                for (int r = 0; r < R; ++r)
-                    if (slot[r] < count) {
+                    for (int r = 0; r < R; ++r)
 #pragma unroll
-                        for (int q = 0; q < 3; ++q) p.part[((long long)c * 3 + q) * p.cap + slot[r]] = acc[r][q];
+                        for (int q = 0; q < 3; ++q) run[r][q] = (c == 0) ? acc[r][q] : __dadd_rn(run[r][q], acc[r][q]);
+                    if (c == NCH - 1) {
+#pragma unroll
+                        for (int r = 0; r < R; ++r)
+                            if (slot[r] < count) {
+#pragma unroll
+                                for (int q = 0; q < 3; ++q) p.part[(long long)q * p.cap + slot[r]] = run[r][q];
+                            }
                     }
+                } else {
+#pragma unroll
+                    for (int r = 0; r < R; ++r)
+                        if (slot[r] < count) {
+#pragma unroll
+                            for (int q = 0; q < 3; ++q) p.part[((long long)c * 3 + q) * p.cap + slot[r]] = acc[r][q];
+                        }
+                }
 #pragma unroll
                 for (int r = 0; r < R; ++r) acc[r][0] = acc[r][1] = acc[r][2] = 0.0;
                 ++c;
@@ -303,7 +322,8 @@ static cudaError_t launch_f32_variant(const InteractParamsF32& q, unsigned grid,
     return cudaGetLastError();
 }
 
-cudaError_t launch_interact_f32(const InteractParamsF32& p, int sm_count, int sfu_mask, cudaStream_t st) {
+cudaError_t launch_interact_f32(const InteractParamsF32& p, int sm_count, int sfu_mask, int* nparts, cudaStream_t st) {
+    *nparts = p.bd.nchunks;
     if (p.count <= 0) return cudaSuccess;
     InteractParamsF32 q = p;
     const long long spb = (long long)kF32Threads * kF32R;
@@ -314,6 +334,7 @@ cudaError_t launch_interact_f32(const InteractParamsF32& p, int sm_count, int sf
         nsplit = (q.target_items + nblk - 1) / nblk;
         if (nsplit > q.bd.nchunks) nsplit = q.bd.nchunks;
     }
+    *nparts = (nsplit == 1) ? 1 : q.bd.nchunks;
     const long long nwork = nblk * nsplit;
     if (nwork > 0x7fffffffLL) return cudaErrorInvalidValue;
     switch (sfu_mask & 7) {
@@ -347,13 +368,13 @@ __global__ void eval_finalize_f32_kernel(int nchunks, double h2_over_2pi, long l
     for (int q = 0; q < 3; ++q) B[q * M + id] = ok ? out[q] : __int_as_float(0x7fc00000);
 }
 
-cudaError_t launch_eval_finalize_f32(const BoundaryView& bd, long long slot0, long long count, long long M,
+cudaError_t launch_eval_finalize_f32(const BoundaryView& bd, int nparts, long long slot0, long long count, long long M,
                                      const float* z, const float* lam, const double* part, long long cap,
                                      float* B, cudaStream_t st) {
     if (count <= 0) return cudaSuccess;
     const double h2_over_2pi = bd.h * bd.h / (2.0 * 3.14159265358979323846);
     const unsigned grid = (unsigned)((count + 255) / 256);
-    eval_finalize_f32_kernel<<<grid, 256, 0, st>>>(bd.nchunks, h2_over_2pi, slot0, count, M, z, lam, part, cap, B);
+    eval_finalize_f32_kernel<<<grid, 256, 0, st>>>(nparts, h2_over_2pi, slot0, count, M, z, lam, part, cap, B);
     return cudaGetLastError();
 }
 
@@ -380,13 +401,13 @@ __global__ void eval_finalize_kernel(int nchunks, double h2_over_2pi, long long 
     for (int q = 0; q < 3; ++q) B[q * M + id] = ok ? out[q] : __longlong_as_double(0x7ff8000000000000LL);
 }
 
-cudaError_t launch_eval_finalize(const BoundaryView& bd, long long slot0, long long count, long long M,
+cudaError_t launch_eval_finalize(const BoundaryView& bd, int nparts, long long slot0, long long count, long long M,
                                  const double* z, const double* lam, const double* part, long long cap,
                                  double* B, cudaStream_t st) {
     if (count <= 0) return cudaSuccess;
     const double h2_over_2pi = bd.h * bd.h / (2.0 * 3.14159265358979323846);
     const unsigned grid = (unsigned)((count + 255) / 256);
-    eval_finalize_kernel<<<grid, 256, 0, st>>>(bd.nchunks, h2_over_2pi, slot0, count, M, z, lam, part, cap, B);
+    eval_finalize_kernel<<<grid, 256, 0, st>>>(nparts, h2_over_2pi, slot0, count, M, z, lam, part, cap, B);
     return cudaGetLastError();
 }
 

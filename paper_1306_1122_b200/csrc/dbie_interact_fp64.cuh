@@ -185,6 +185,7 @@ __global__ void __launch_bounds__(THREADS, MINB) interact64_kernel(const __grid_
         for (int tt = 0; tt < NA; ++tt) acc[tt][0] = acc[tt][1] = acc[tt][2] = 0.0;
         const bool lam_all_zero = (lam[0][0] == 0.0) && (lam[0][1] == 0.0) && (lam[0][2] == 0.0);   // MODE_EVAL
         const bool small_eps = fmax(fmax(lam[0][0], lam[0][1]), lam[0][2]) * p.delta_abs <= kRotateSmallMax;
+        double run[3] = {0.0, 0.0, 0.0};   // MODE_EVAL, unsplit launch: running sum of the chunk sums
         double lam2[NT][3];   // analytic modes: lambda^2
 #pragma unroll
         for (int tt = 0; tt < NT; ++tt)
@@ -329,8 +330,19 @@ __global__ void __launch_bounds__(THREADS, MINB) interact64_kernel(const __grid_
             if (t + 1 == t_chunk_end) {  // A4: one partial sum per chunk, added in chunk order later
                 if (live) {
                     if (MODE == MODE_EVAL) {
+                        if (nsplit == 1) {
+                            // this CTA sees every chunk: add them here, in chunk order with the epilogue's own
+                            // operation (bit-identical), and write one sum instead of nchunks partial sums
 #pragma unroll
-                        for (int q = 0; q < 3; ++q) p.part[((long long)c * 3 + q) * p.cap + slot] = acc[0][q];
+                            for (int q = 0; q < 3; ++q) run[q] = (c == 0) ? acc[0][q] : __dadd_rn(run[q], acc[0][q]);
+                            if (c == NCH - 1) {
+#pragma unroll
+                                for (int q = 0; q < 3; ++q) p.part[(long long)q * p.cap + slot] = run[q];
+                            }
+                        } else {
+#pragma unroll
+                            for (int q = 0; q < 3; ++q) p.part[((long long)c * 3 + q) * p.cap + slot] = acc[0][q];
+                        }
                     } else if (MODE == MODE_STENCIL) {
 #pragma unroll
                         for (int q = 0; q < 3; ++q)

@@ -138,16 +138,16 @@ cudaError_t launch_stage_boundary(int nx, int ny, double h, double x0, double y0
 cudaError_t launch_stage_q9(int nx, int ny, double h, double x0, double y0, const double* bx, const double* by,
                             const double* bz, int nsx, int nsy, double4* rec, double* yk, float4* rec32,
                             float* yk32, cudaStream_t st);
-cudaError_t launch_interact_eval(const InteractParams& p, int sm_count, cudaStream_t st);
+cudaError_t launch_interact_eval(const InteractParams& p, int sm_count, int* nparts, cudaStream_t st);
 cudaError_t launch_interact_stencil(const InteractParams& p, int sm_count, cudaStream_t st);
 cudaError_t launch_interact_grid(const InteractParams& p, int sm_count, cudaStream_t st);
 cudaError_t launch_interact_analytic(const InteractParams& p, int sm_count, cudaStream_t st);
 cudaError_t launch_interact_grid_analytic(const InteractParams& p, int sm_count, cudaStream_t st);
-cudaError_t launch_eval_finalize(const BoundaryView& bd, long long slot0, long long count,
+cudaError_t launch_eval_finalize(const BoundaryView& bd, int nparts, long long slot0, long long count,
                                  long long M, const double* z, const double* lam, const double* part,
                                  long long cap, double* B, cudaStream_t st);
-cudaError_t launch_interact_f32(const InteractParamsF32& p, int sm_count, int sfu_mask, cudaStream_t st);
-cudaError_t launch_eval_finalize_f32(const BoundaryView& bd, long long slot0, long long count, long long M,
+cudaError_t launch_interact_f32(const InteractParamsF32& p, int sm_count, int sfu_mask, int* nparts, cudaStream_t st);
+cudaError_t launch_eval_finalize_f32(const BoundaryView& bd, int nparts, long long slot0, long long count, long long M,
                                      const float* z, const float* lam, const double* part, long long cap,
                                      float* B, cudaStream_t st);
 cudaError_t launch_probe(double millis, int sm_count, double* dfma_per_s, double* ffma_per_s);
