@@ -223,9 +223,9 @@ def nm_generic(fn, simplex, xtol: float, ftol: float, maxiter: int):
     simplex, ps = _d(np.asarray(simplex).reshape(4, 3))
     trace = np.full((maxiter + 1, 3), np.nan)
     fs = np.empty((4, 3)); ff = np.empty(4)
-    it = C.c_int(); nf = C.c_int(); st = C.c_int()
+    it = C.c_int(); nf = C.c_int(); st = C.c_int(); mg = C.c_double()
     lib.orc_nm_generic(cb, ps, C.c_double(xtol), C.c_double(ftol), C.c_int(maxiter),
                        trace.ctypes.data_as(_dp), fs.ctypes.data_as(_dp), ff.ctypes.data_as(_dp),
-                       C.byref(it), C.byref(nf), C.byref(st))
+                       C.byref(it), C.byref(nf), C.byref(st), C.byref(mg))
     return {"trace": trace[: it.value + 1], "simplex": fs, "f": ff, "iters": it.value,
-            "nfev": nf.value, "status": st.value}
+            "nfev": nf.value, "status": st.value, "margin": mg.value}

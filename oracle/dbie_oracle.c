@@ -503,7 +503,7 @@ static double generic_adapter(const double lam[3], void *user, double aux[9])
 void orc_nm_generic(orc_objective3 fn, const double *simplex /* 4*3 */, double xtol,
                     double ftol, int maxiter, double *trace /* (maxiter+1)*3 */,
                     double *final_simplex /* 12 */, double *final_f /* 4 */,
-                    int *iters, int *nfev, int *status)
+                    int *iters, int *nfev, int *status, double *margin /* 1 or NULL */)
 {
     nm_state s;
     double V0[4][3];
@@ -512,6 +512,7 @@ void orc_nm_generic(orc_objective3 fn, const double *simplex /* 4*3 */, double x
     memcpy(final_simplex, s.V, sizeof s.V);
     memcpy(final_f, s.F, sizeof s.F);
     *iters = s.iters; *nfev = s.nfev; *status = s.status;
+    if (margin) *margin = s.margin;
 }
 
 void orc_solve_nm(const orc_boundary *b, const orc_opts *o, long M, const double *x,
@@ -610,21 +611,22 @@ void orc_solve_grid(const orc_boundary *b, const orc_opts *o, long M, const doub
                     for (int tz = 0; tz < C; ++tz) {
                         const int tt[3] = { tx, ty, tz };
                         double P0[3], Px[3], Py[3], Pz[3], aux[9];
-                        for (int p = 0; p < 3; ++p) {
-                            P0[p] = S[tt[p]][0][p]; Px[p] = S[tt[p]][1][p];
-                            Py[p] = S[tt[p]][2][p]; Pz[p] = S[tt[p]][3][p];
-                        }
                         double ph;
-                        if (o->analytic) {
+                        if (o->analytic) { /* the stencil table S is not filled in this mode */
                             double Gc[3][3];
                             for (int p = 0; p < 3; ++p) {
                                 P0[p] = Bt[tt[p]][p];
                                 for (int j = 0; j < 3; ++j) Gc[p][j] = Gt[tt[p]][p][j];
                             }
                             ph = as_inf(residual_from_gradient(P0, Gc, dc, o->w_g, aux));
-                        } else
-                        ph = as_inf(residual_from_stencil(P0, Px, Py, Pz, da, dc,
-                                                                 o->w_g, aux));
+                        } else {
+                            for (int p = 0; p < 3; ++p) {
+                                P0[p] = S[tt[p]][0][p]; Px[p] = S[tt[p]][1][p];
+                                Py[p] = S[tt[p]][2][p]; Pz[p] = S[tt[p]][3][p];
+                            }
+                            ph = as_inf(residual_from_stencil(P0, Px, Py, Pz, da, dc,
+                                                              o->w_g, aux));
+                        }
                         if (ph < lev_best) { /* strict: ties keep the lexicographically first */
                             lev_second = lev_best;
                             lev_best = ph; bt[0] = tx; bt[1] = ty; bt[2] = tz;
@@ -636,12 +638,12 @@ void orc_solve_grid(const orc_boundary *b, const orc_opts *o, long M, const doub
                 mrg = lev_second - lev_best;
             /* the argmin becomes the incumbent (slot T) */
             double inc[4][3], il[3];
-            for (int p = 0; p < 3; ++p) {
-                for (int s = 0; s < 4; ++s) inc[s][p] = S[bt[p]][s][p];
-                il[p] = lt[p * (T + 1) + bt[p]];
-            }
-            memcpy(S[T], inc, sizeof inc);
-            if (o->analytic)
+            for (int p = 0; p < 3; ++p) il[p] = lt[p * (T + 1) + bt[p]];
+            if (!o->analytic) {
+                for (int p = 0; p < 3; ++p)
+                    for (int s = 0; s < 4; ++s) inc[s][p] = S[bt[p]][s][p];
+                memcpy(S[T], inc, sizeof inc);
+            } else
                 for (int p = 0; p < 3; ++p) {
                     Bt[T][p] = Bt[bt[p]][p];
                     for (int j = 0; j < 3; ++j) Gt[T][p][j] = Gt[bt[p]][p][j];

@@ -597,3 +597,160 @@ def test_q3_nine_node_agrees_with_the_nodal_rule_in_the_far_field():
     rel = np.abs(a - b).max(axis=0) / np.abs(a).max(axis=0)
     assert rel[0] < 5e-5 and rel[1] < 5e-5              # what remains is the Simpson-vs-midpoint flux difference
     assert 1e-7 < rel[2] < 5e-2                         # z = h: the two quadratures differ
+
+
+# -- margin (protocol P-4 rests on it) ---------------------------------------
+def _table_objective(values):
+    """Objective defined ONLY at the points one Nelder-Mead iteration can visit from the unit
+    simplex V0 = 0, V1 = e1, V2 = e2, V3 = e3 (Phi = 10, 20, 30, 40): reflection (2/3, 2/3, -1),
+    expansion (1, 1, -2), outside contraction (1/2, 1/2, -1/2), inside contraction (1/6, 1/6, 1/2),
+    shrink vertices e_j / 2.  The geometry is O-3's formulas worked out by hand, not code."""
+    pts = {"v0": (0, 0, 0), "v1": (1, 0, 0), "v2": (0, 1, 0), "v3": (0, 0, 1), "r": (2 / 3, 2 / 3, -1),
+           "e": (1, 1, -2), "oc": (0.5, 0.5, -0.5), "ic": (1 / 6, 1 / 6, 0.5),
+           "s1": (0.5, 0, 0), "s2": (0, 0.5, 0), "s3": (0, 0, 0.5)}
+    vals = dict(v0=10.0, v1=20.0, v2=30.0, v3=40.0)
+    vals.update(values)
+
+    def fn(x):
+        for k, p in pts.items():
+            if np.allclose(x, p, atol=1e-12):
+                return vals[k]       # KeyError = the driver visited a point this case does not define
+        raise KeyError(tuple(x))
+    return fn
+
+
+@pytest.mark.parametrize("values,ftol,expect", [
+    # reflection 9.7 < Phi_0 = 10 (gap 0.3, the closest) -> expansion 5 < 9.7 (gap 4.7); new order 5,10,20,30
+    (dict(r=9.7, e=5.0), 1e-6, 0.3),
+    # expansion not better than the reflection: 9.02 vs 9 (gap 0.02) -> reflection kept; order 9,10,20,30 (gap 1)
+    (dict(r=9.0, e=9.02), 1e-6, 0.02),
+    # 29.6: not < Phi_0 (19.6), < Phi_2 = 30 (gap 0.4) -> accepted; the new order 10,20,29.6,30 has the same gap
+    (dict(r=29.6), 1e-6, 0.4),
+    # 35: not < 30 (5), < Phi_3 = 40 (5) -> outside contraction 34.9 <= 35 (gap 0.1) accepted; order 10,20,30,34.9
+    (dict(r=35.0, oc=34.9), 1e-6, 0.1),
+    # 45 >= Phi_3 (5) -> inside contraction 39.95 < 40 (gap 0.05) accepted
+    (dict(r=45.0, ic=39.95), 1e-6, 0.05),
+    # inside contraction 41 not < 40 (gap 1) -> shrink; the new vertices 12, 12.25, 17 sort with gap 0.25
+    (dict(r=45.0, ic=41.0, s1=12.0, s2=12.25, s3=17.0), 1e-6, 0.25),
+    # the termination test max |Phi_j - Phi_0| = 30 against ftol = 29.99 is a decision too (gap 0.01)
+    (dict(r=25.0), 29.99, 0.01),
+])
+def test_margin_is_the_closest_comparison_of_the_search(values, ftol, expect):
+    """`margin` = the smallest |a - b| over every comparison a < b the search took (sorts, the ftol
+    test, reflection / expansion / contraction decisions).  One iteration on a hand-built objective
+    whose closest comparison is known.  The sort notes all six pairs; the smallest pair gap is always
+    between neighbours of the sorted order, which the insertion sort compares directly, so this is the
+    same number as the smallest gap over the comparisons actually executed."""
+    sim = np.array([[0, 0, 0], [1, 0, 0], [0, 1, 0], [0, 0, 1]], float)
+    out = oracle.nm_generic(_table_objective(values), sim, 1e-9, ftol, 1)
+    assert out["iters"] == 1
+    assert out["margin"] == pytest.approx(expect, abs=1e-12)
+
+
+def test_margin_of_the_point_solve_includes_the_eq12_tests():
+    """orc_solve_nm also notes f vs eps_f and g vs eps_g (Eq. 12) at the best vertex: with eps_f set a
+    hair below the f of the best initial vertex, the one iteration that follows has a margin of at most
+    that hair (and exactly that hair when every other comparison is wider)."""
+    w = random_boundary(9, 8, seed=12, npts=3, zmin=1.5, zmax=4.0)
+    start = oracle.solve_nm(w, oracle.Opts(use_eq12=0, maxiter=0))     # best initial vertex, no iteration
+    wide = oracle.solve_nm(w, oracle.Opts(use_eq12=0, maxiter=1))
+    hair = 3e-9
+    for i in range(w.M):
+        o = oracle.Opts(use_eq12=1, maxiter=1, eps_f=float(start["f"][i]) - hair, eps_g=1e300)
+        s = oracle.solve_nm(w.subset([i]), o)
+        assert s["iters"][0] == 1 and s["status"][0] == 2          # the threshold was not met
+        assert s["margin"][0] == pytest.approx(min(hair, wide["margin"][i]), rel=1e-6, abs=1e-15)
+    assert (wide["margin"] > hair).any()
+
+
+# -- O-4 (GRID): the refinement rule of levels >= 1 ---------------------------------------------
+def _grid_by_the_book(w, i, T, L, lam_max, analytic, events):
+    """DESIGN.md O-4 written out with the NumPy objective (no separability shortcut: every candidate
+    triple is evaluated directly): window [lo, lo + W], trials lo + W t/(T-1), candidates = trials plus
+    the incumbent (index T, levels >= 1), strict '<' in (t_x, t_y, t_z) order, next window of width
+    2W/(T-1) centred on the argmin and clipped to [0, lam_max/h]."""
+    p = np.array([w.x[i], w.y[i], w.z[i]])
+    Lmax = lam_max / w.h
+    lo, W, inc, best = np.zeros(3), Lmax, None, np.inf
+
+    def phi_of(lam):
+        if not analytic:
+            return _numpy_phi(w, p, lam)[0]
+        G, B0 = _analytic_grad(w, p, lam), _numpy_eval(w, p, lam)
+        J = np.array([G[2, 1] - G[1, 2], G[0, 2] - G[2, 0], G[1, 0] - G[0, 1]])
+        f = np.linalg.norm(np.cross(J, B0)) / (np.linalg.norm(J) * np.linalg.norm(B0))
+        return f + abs(np.trace(G)) * (w.h / 6.0) / np.linalg.norm(B0)
+
+    for lev in range(L):
+        cands = [[lo[c] + W * t / (T - 1) for t in range(T)] + ([inc[c]] if inc is not None else [])
+                 for c in range(3)]
+        best, arg, second = np.inf, None, np.inf
+        for tx, a in enumerate(cands[0]):
+            for ty, b in enumerate(cands[1]):
+                for tz, c in enumerate(cands[2]):
+                    ph = phi_of(np.array([a, b, c]))
+                    if ph < best:
+                        second, best, arg = best, ph, (tx, ty, tz)
+                    elif ph < second:
+                        second = ph
+        inc = np.array([cands[c][arg[c]] for c in range(3)])
+        events["gap"] = min(events.get("gap", np.inf), second - best)
+        events["incumbent_kept"] = events.get("incumbent_kept", 0) + sum(1 for c in range(3) if arg[c] == T)
+        Wn = 2.0 * W / (T - 1)
+        for c in range(3):
+            l = inc[c] - 0.5 * Wn
+            if l < 0.0:
+                l = 0.0
+                events["clip_lo"] = events.get("clip_lo", 0) + 1
+            if l + Wn > Lmax:
+                l = Lmax - Wn
+                events["clip_hi"] = events.get("clip_hi", 0) + 1
+            lo[c] = l
+        W = Wn
+    return inc, best
+
+
+@pytest.mark.parametrize("T,lam_max,analytic", [(3, 0.4, 1), (4, 0.4, 1), (5, 0.03, 1), (4, 0.4, 0), (3, 0.03, 0)])
+def test_grid_refinement_levels_by_brute_force(T, lam_max, analytic):
+    """Pins levels 1-2 of O-4 (window recentring, clipping at 0 and at lam_max, the incumbent slot),
+    not only level 0: orc_solve_grid after 1, 2 and 3 levels against the rule written out in NumPy.
+    lam_max = 0.03 puts the optimum above the window, so the upper clip is exercised; lambda = 0
+    winners exercise the lower one."""
+    w = random_boundary(6, 5, seed=40 + T, npts=4, zmin=1.0, zmax=3.0)
+    events = {}
+    for L in (1, 2, 3):
+        o = oracle.Opts(method=1, n_trial=T, n_level=L, lam_max=lam_max, use_eq12=0, analytic=analytic)
+        sol = oracle.solve_grid(w, o)
+        for i in range(w.M):
+            ev = {}
+            lam, phi = _grid_by_the_book(w, i, T, L, lam_max, analytic, ev)
+            if ev["gap"] < (1e-10 if analytic else 1e-7):
+                continue        # a near-tie of two candidates: the two evaluation orders may pick either
+            for k, v in ev.items():
+                events[k] = (min(events[k], v) if k == "gap" else events[k] + v) if k in events else v
+            assert np.allclose(sol["lam"][:, i], lam, rtol=0, atol=1e-13 / w.h), (L, i)
+            assert abs(sol["phi"][i] - phi) < (1e-12 if analytic else 1e-8)
+    assert events.get("clip_lo", 0) + events.get("clip_hi", 0) > 0      # a window was clipped ...
+    if lam_max < 0.1:
+        assert events.get("clip_hi", 0) > 0                              # ... at lam_max
+    assert "gap" in events                                               # some point was compared
+
+
+# -- SURVEY section 5: the oracle under ASan / UBSan ------------------------------------------------
+def test_oracle_runs_clean_under_address_and_undefined_sanitizers(tmp_path):
+    import shutil
+    import subprocess
+    if shutil.which("gcc") is None:
+        pytest.skip("no gcc")
+    exe = tmp_path / "orc_san"
+    src = os.path.join(os.path.dirname(oracle.__file__), "sanitize_main.c")
+    cc = ["gcc", "-O1", "-g", "-fsanitize=address,undefined", "-fno-sanitize-recover=all",
+          "-ffp-contract=off", "-fopenmp", "-o", str(exe), src, "-lm"]
+    r = subprocess.run(cc, capture_output=True, text=True)
+    if r.returncode != 0 and "sanitize" in r.stderr:
+        pytest.skip("sanitizer runtime not installed: " + r.stderr.splitlines()[0])
+    assert r.returncode == 0, r.stderr
+    r = subprocess.run([str(exe)], capture_output=True, text=True,
+                       env=dict(os.environ, ASAN_OPTIONS="detect_leaks=1", OMP_NUM_THREADS="2"))
+    assert r.returncode == 0, r.stdout + r.stderr
+    assert "sanitize_main ok" in r.stdout
