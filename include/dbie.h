@@ -38,6 +38,19 @@
  *    status 3 in dbie_solve).
  *  - There is no CPU fallback: without a CUDA device every compute entry point returns
  *    DBIE_ECUDA.
+ *  - Devices: a context belongs to the CUDA device that was current in dbie_create.  Every later
+ *    entry point makes that device current for the duration of the call and restores the caller's
+ *    device before returning; the arrays and the stream passed in must belong to the context's device.
+ *  - Range of lambda: theta = |lambda| r must stay below 2^20 (about 1e6 rad) for every point-pixel
+ *    pair; the one-step argument reduction of the kernel is exact up to theta * 4e-17 there (relative
+ *    to theta: the same size as the rounding of theta itself).  Beyond that the result is unspecified
+ *    (finite, wrong).  The paper's lambda are ~0.1 / pixel on windows of <= 1500 pixels: theta < 200.
+ *  - Const-ness: eval / residual / solve take a NON-const context although they do not change the
+ *    boundary: they grow and use the context's scratch memory and record counters (SURVEY 8(b)
+ *    wrote `const dbie_ctx*`; the deviation is deliberate and is why one context serves one stream
+ *    at a time).
+ *  - dbie_last_cuda_error(NULL) reads a process-global buffer (the last failure that had no
+ *    context, i.e. inside dbie_create): it is not synchronised between threads.
  */
 #ifndef DBIE_H
 #define DBIE_H
@@ -93,11 +106,6 @@ dbie_status dbie_eval_host(dbie_ctx* ctx, long long M, const double* x, const do
  * (north_star): relative vector error <= 2e-4 against the fp64 definition. */
 dbie_status dbie_eval_f32(dbie_ctx* ctx, long long M, const float* x, const float* y,
                           const float* z, const float* lam, float* B, void* cuda_stream);
-/* Tuning knob of dbie_eval_f32: bit p of mask set = component p takes sin/cos of the reduced
- * argument from the SFU (MUFU.SIN/COS) instead of the FMA-pipe polynomials, to balance the two
- * pipes.  Allowed masks: 0, 1, 3, 7 (default: all three from the SFU, the fastest measured).  Results
- * differ at the 1e-6 level between masks; all meet the 2e-4 target. */
-dbie_status dbie_set_f32_sfu_mask(dbie_ctx* ctx, int mask);
 
 /* Options of dbie_solve.  Fill with dbie_solve_default_opts, then change fields. */
 typedef struct {
@@ -112,8 +120,9 @@ typedef struct {
     double xtol;      /* NM stop: max |V_j - V_0| <= xtol/h and max |Phi_j - Phi_0| <= ftol;  */
     double ftol;      /*   1e-4, 1e-6                                                         */
     int maxiter;      /* NM iteration cap; 200                                                */
-    int n_trial;      /* GRID: T trial lambda per component per level, 2 <= T <= 32 (else
-                         DBIE_EINVAL); 8.  Multiples of 8 (then 4, then 2) run fastest.          */
+    int n_trial;      /* GRID: T trial lambda per component per level, 4 <= T <= 32 (else
+                         DBIE_EINVAL: below 4 the refined window 2W/(T-1) does not shrink); 8.
+                         Multiples of 8 (then 4, then 2) run fastest.                            */
     int n_level;      /* GRID: number of refinement levels (>= 1); 10                           */
     double lam_max;   /* GRID: search window [0, lam_max/h] (> 0); 0.4                          */
     int use_eq12;     /* 1: stop a point as soon as f <= eps_f and g <= eps_g (Eq. 12)        */
@@ -149,6 +158,10 @@ dbie_status dbie_residual(dbie_ctx* ctx, long long M, const double* x, const dou
                           const double* z, const double* lam, const dbie_solve_opts* opts,
                           double* out, double* phi, void* cuda_stream);
 
+/* ------------------------------------------------------------------------------------------------
+ * Diagnostics and measurement.  Not needed to use the library; bench.py and the tests call them.
+ * ---------------------------------------------------------------------------------------------- */
+
 /* Counters of the last eval/solve/residual call on this context (host values, valid after
  * the stream has been synchronised): point-pixel interactions evaluated (one interaction =
  * one (evaluation point, pixel) pair, all three components), kernel launches enqueued, and
@@ -167,11 +180,23 @@ dbie_status dbie_last_kernel_time(dbie_ctx* ctx, double* interact_ms, long long*
  * `millis` ms and returns DFMA instructions (per lane) per second.  Synchronises. */
 dbie_status dbie_probe_dfma_rate(double millis, double* dfma_per_s, double* ffma_per_s);
 
+/* Tuning knob of dbie_eval_f32: bit p of mask set = component p takes sin/cos of the reduced
+ * argument from the SFU (MUFU.SIN/COS) instead of the FMA-pipe polynomials, to balance the two
+ * pipes.  Allowed masks: 0, 1, 3, 7 (default: all three from the SFU, the fastest measured).  Results
+ * differ at the 1e-6 level between masks; all meet the 2e-4 target. */
+dbie_status dbie_set_f32_sfu_mask(dbie_ctx* ctx, int mask);
+
+/* Test knob: process eval / residual / solve in internal batches of at most `points` points
+ * (0 restores the defaults: 2^21 for eval, 2^22 for residual and the Nelder-Mead solve, a 2 GiB
+ * scratch bound for GRID).  Results do not depend on it, bit for bit; the tests use it to run the
+ * multi-batch paths at small sizes. */
+dbie_status dbie_debug_set_batch_limit(dbie_ctx* ctx, long long points);
+
 const char* dbie_strerror(dbie_status s);
 /* CUDA error string of the last DBIE_ECUDA on this context (or of the last failure with
  * no context when ctx is NULL).  Never NULL. */
 const char* dbie_last_cuda_error(const dbie_ctx* ctx);
-/* Library version string, e.g. "dbie-b200 0.1 (sm_100a)". */
+/* Library version string, e.g. "dbie-b200 0.2 (sm_100a)". */
 const char* dbie_version(void);
 
 #ifdef __cplusplus

@@ -64,6 +64,7 @@ def load() -> C.CDLL:
     lib.dbie_eval_host.argtypes = [_vp, C.c_longlong, _vp, _vp, _vp, _vp, _vp]
     lib.dbie_eval_f32.argtypes = [_vp, C.c_longlong, _vp, _vp, _vp, _vp, _vp, _vp]
     lib.dbie_set_f32_sfu_mask.argtypes = [_vp, C.c_int]
+    lib.dbie_debug_set_batch_limit.argtypes = [_vp, C.c_longlong]
     lib.dbie_solve_default_opts.argtypes = [C.POINTER(SolveOpts)]
     lib.dbie_solve_default_opts.restype = None
     lib.dbie_solve.argtypes = [_vp, C.c_longlong, _vp, _vp, _vp, C.POINTER(SolveOpts), _vp, _vp, _vp,
@@ -234,6 +235,10 @@ class DBIE:
     def set_f32_sfu_mask(self, mask: int):
         """dbie_set_f32_sfu_mask: which components take sin/cos from the SFU (0, 1, 3 or 7)."""
         self._check(self._lib.dbie_set_f32_sfu_mask(self._h, int(mask)))
+
+    def set_batch_limit(self, points: int):
+        """dbie_debug_set_batch_limit: internal batches of at most `points` points (0: defaults)."""
+        self._check(self._lib.dbie_debug_set_batch_limit(self._h, int(points)))
 
     # -- dbie_residual
     def residual(self, x, y, z, lam, opts: SolveOpts | None = None, stream=None):

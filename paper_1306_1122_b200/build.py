@@ -1,6 +1,6 @@
 """Build libdbie_b200.so (CUDA, sm_100a) and the host test shim, in-tree.
 
-    python -m paper_1306_1122_b200.build [--force] [--tune]
+    python -m paper_1306_1122_b200.build [--force] [-v]
 
 nvcc cross-compiles without a GPU.  The shared objects are git-ignored but travel to the GPU
 box with the gpurun snapshot.
@@ -25,6 +25,7 @@ COMMON = ["-O3", "-std=c++17", "-lineinfo", "-Xcompiler", "-fPIC", "-I", INCLUDE
 # decisions are comparisons of separately rounded IEEE operations.
 UNITS = [
     ("dbie_interact.cu", []),
+    ("dbie_solve_fused.cu", []),     # same flags as dbie_interact.cu: identical interaction arithmetic
     ("dbie_solver.cu", ["-fmad=false"]),
     ("dbie_grid.cu", ["-fmad=false"]),
     ("dbie_api.cu", []),
@@ -73,14 +74,6 @@ def build_hostshim(force: bool = False) -> str:
     return SHIM
 
 
-def build_tune() -> str:
-    """Developer tool: shape sweep of the fp64 interaction kernel + FP64 issue-slot probe (dbie_tune)."""
-    exe = os.path.join(HERE, "dbie_tune")
-    subprocess.check_call([NVCC, *ARCH, "-O3", "-std=c++17", "-lineinfo", "-I", INCLUDE,
-                           os.path.join(CSRC, "tune_interact.cu"), "-o", exe])
-    return exe
-
-
 def build_all(force: bool = False, verbose: bool = False) -> None:
     build_lib(force, verbose)
     build_hostshim(force)
@@ -88,7 +81,5 @@ def build_all(force: bool = False, verbose: bool = False) -> None:
 
 if __name__ == "__main__":
     build_all(force="--force" in sys.argv, verbose="-v" in sys.argv)
-    if "--tune" in sys.argv:
-        print(build_tune())
     print(LIB)
     print(SHIM)

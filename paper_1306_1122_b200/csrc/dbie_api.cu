@@ -6,9 +6,18 @@
 #include <stdlib.h>
 #include <string.h>
 
+#include <nvtx3/nvToolsExt.h>   // header-only; ranges show up in Nsight tools, a no-op otherwise
+
 #include "dbie_internal.h"
 
 using namespace dbie;
+
+namespace {
+struct NvtxRange {   // ranges around create / eval / residual / solve
+    explicit NvtxRange(const char* name) { nvtxRangePushA(name); }
+    ~NvtxRange() { nvtxRangePop(); }
+};
+}  // namespace
 
 struct dbie_ctx {
     int device, sm_count;
@@ -20,21 +29,21 @@ struct dbie_ctx {
     double* part;       size_t part_bytes;    // chunk partial sums
     char* state;        size_t state_bytes;   // optimiser state
     char* io;           size_t io_bytes;      // device staging of the _host entry points
-    unsigned* counters;                       // device: nact[2], pad[2], nevals (u64) at +16 B, work[2] at +32 B
+    unsigned* counters;                       // device: list lengths [0..2], nevals (u64) at +16 B, work-item counters at +32 B
     cudaStream_t own_stream;
-    unsigned* h_probe;                        // pinned host: active-list lengths read back by the solve loop
-    cudaEvent_t probe_ev[2];
     double last_interactions;
     long long last_launches, last_evals;
     int evals_on_device;                      // last call was a solve: read nevals back on demand
     int positions_per_eval;                   // evaluation positions per objective evaluation of that solve (4, or 1 analytic)
     int f32_sfu_mask;                         // dbie_eval_f32: components whose sincos use the SFU
+    long long batch_limit;                    // dbie_debug_set_batch_limit: points per internal batch (0: defaults)
     int profile;                              // record CUDA events around every interaction launch
     cudaEvent_t* ev;    int ev_cap, ev_n;     // event pairs of the last call (profile mode)
     char err[256];
 };
 
 static char g_err[256] = "no error";
+static const size_t kCounterBytes = 128;   // device counters: list lengths [0..2], objective evaluations (u64) at +16 B, work items at +32 B
 static const int kDefaultF32SfuMask = 7;   // sin/cos of the reduced argument from the SFU for all three components:
                                            // measured fastest (4.90e11 vs 4.26e11 interactions/s with polynomials), same accuracy
 
@@ -51,6 +60,19 @@ static dbie_status fail_cuda(dbie_ctx* c, cudaError_t e, const char* where) {
         if (e_ != cudaSuccess) return fail_cuda(ctx, e_, #call);   \
     } while (0)
 
+// A context belongs to the device that was current in dbie_create.  Every entry point makes that device
+// current for the duration of the call and restores the caller's device on return, so a context can be
+// used after the caller switched devices (pointers must still belong to the context's device).
+struct DeviceGuard {
+    int prev = -1;
+    bool switched = false;
+    cudaError_t err = cudaSuccess;
+    explicit DeviceGuard(const dbie_ctx* c);
+    ~DeviceGuard() {
+        if (switched) (void)cudaSetDevice(prev);
+    }
+};
+
 static dbie_status ensure(dbie_ctx* ctx, void** ptr, size_t* have, size_t need) {
     if (need <= *have) return DBIE_OK;
     if (*ptr) {
@@ -62,6 +84,17 @@ static dbie_status ensure(dbie_ctx* ctx, void** ptr, size_t* have, size_t need) 
     *have = need;
     return DBIE_OK;
 }
+
+DeviceGuard::DeviceGuard(const dbie_ctx* c) {
+    err = cudaGetDevice(&prev);
+    if (err == cudaSuccess && c && prev != c->device) {
+        err = cudaSetDevice(c->device);
+        switched = err == cudaSuccess;
+    }
+}
+#define GUARD_DEVICE()                                                          \
+    DeviceGuard guard_(ctx);                                                    \
+    if (guard_.err != cudaSuccess) return fail_cuda(ctx, guard_.err, "cudaSetDevice(context's device)")
 
 // profile mode: an event pair around each interaction-kernel launch of the current call
 static void prof_reset(dbie_ctx* ctx) { ctx->ev_n = 0; }
@@ -86,6 +119,7 @@ extern "C" dbie_status dbie_profile(dbie_ctx* ctx, int enable) {
 
 extern "C" dbie_status dbie_last_kernel_time(dbie_ctx* ctx, double* interact_ms, long long* interact_launches) {
     if (!ctx) return DBIE_EINVAL;
+    GUARD_DEVICE();
     double total = 0.0;
     const int pairs = ctx->ev_n / 2;
     if (pairs > 0) CU(cudaEventSynchronize(ctx->ev[2 * pairs - 1]));
@@ -110,7 +144,7 @@ extern "C" const char* dbie_strerror(dbie_status s) {
     return "unknown status";
 }
 extern "C" const char* dbie_last_cuda_error(const dbie_ctx* ctx) { return ctx ? ctx->err : g_err; }
-extern "C" const char* dbie_version(void) { return "dbie-b200 0.1 (sm_100a)"; }
+extern "C" const char* dbie_version(void) { return "dbie-b200 0.2 (sm_100a)"; }
 
 extern "C" void dbie_solve_default_opts(dbie_solve_opts* o) {
     if (!o) return;
@@ -152,6 +186,7 @@ static void setup_tiling(BoundaryView& b) {
 
 extern "C" void dbie_destroy(dbie_ctx* ctx) {
     if (!ctx) return;
+    DeviceGuard guard_(ctx->device >= 0 ? ctx : nullptr);
     cudaFree(ctx->rec);
     cudaFree(ctx->yk);
     cudaFree(ctx->rec32);
@@ -161,9 +196,6 @@ extern "C" void dbie_destroy(dbie_ctx* ctx) {
     cudaFree(ctx->io);
     cudaFree(ctx->counters);
     if (ctx->own_stream) cudaStreamDestroy(ctx->own_stream);
-    if (ctx->h_probe) cudaFreeHost(ctx->h_probe);
-    for (int i = 0; i < 2; ++i)
-        if (ctx->probe_ev[i]) cudaEventDestroy(ctx->probe_ev[i]);
     for (int i = 0; i < ctx->ev_cap; ++i) cudaEventDestroy(ctx->ev[i]);
     free(ctx->ev);
     (void)cudaGetLastError();
@@ -178,6 +210,7 @@ extern "C" dbie_status dbie_create(dbie_ctx** out, int nx, int ny, double h, dou
         return DBIE_EINVAL;
     if ((long long)nx * ny > (1LL << 30)) return DBIE_EINVAL;
     if ((flags & DBIE_QUAD_9NODE) && (nx < 3 || ny < 3)) return DBIE_EINVAL;
+    NvtxRange nvtx_("dbie_create");
     dbie_ctx* ctx = (dbie_ctx*)calloc(1, sizeof(dbie_ctx));
     if (!ctx) return DBIE_ENOMEM;
     strcpy(ctx->err, "no error");
@@ -202,14 +235,9 @@ extern "C" dbie_status dbie_create(dbie_ctx** out, int nx, int ny, double h, dou
             if ((e = cudaMalloc(&ctx->rec32, sizeof(float4) * b.N)) != cudaSuccess) { st = fail_cuda(ctx, e, "cudaMalloc(rec32)"); break; }
             if ((e = cudaMalloc(&ctx->yk32, sizeof(float) * b.ny)) != cudaSuccess) { st = fail_cuda(ctx, e, "cudaMalloc(yk32)"); break; }
         }
-        if ((e = cudaMalloc(&ctx->counters, 64)) != cudaSuccess) { st = fail_cuda(ctx, e, "cudaMalloc(counters)"); break; }
-        if ((e = cudaMemset(ctx->counters, 0, 64)) != cudaSuccess) { st = fail_cuda(ctx, e, "cudaMemset"); break; }
+        if ((e = cudaMalloc(&ctx->counters, kCounterBytes)) != cudaSuccess) { st = fail_cuda(ctx, e, "cudaMalloc(counters)"); break; }
+        if ((e = cudaMemset(ctx->counters, 0, kCounterBytes)) != cudaSuccess) { st = fail_cuda(ctx, e, "cudaMemset"); break; }
         if ((e = cudaStreamCreateWithFlags(&ctx->own_stream, cudaStreamNonBlocking)) != cudaSuccess) { st = fail_cuda(ctx, e, "cudaStreamCreate"); break; }
-        if ((e = cudaHostAlloc((void**)&ctx->h_probe, 64, cudaHostAllocDefault)) != cudaSuccess) { st = fail_cuda(ctx, e, "cudaHostAlloc"); break; }
-        if ((e = cudaEventCreateWithFlags(&ctx->probe_ev[0], cudaEventDisableTiming)) != cudaSuccess ||
-            (e = cudaEventCreateWithFlags(&ctx->probe_ev[1], cudaEventDisableTiming)) != cudaSuccess) {
-            st = fail_cuda(ctx, e, "cudaEventCreate"); break;
-        }
         e = q9 ? launch_stage_q9(nx, ny, h, x0, y0, bx, by, bz, sx, sy, ctx->rec, ctx->yk, ctx->rec32, ctx->yk32, 0)
                : launch_stage_boundary(nx, ny, h, x0, y0, bx, by, bz, ctx->rec, ctx->yk, ctx->rec32, ctx->yk32, 0);
         if (e != cudaSuccess) {
@@ -248,14 +276,24 @@ extern "C" dbie_status dbie_create_host(dbie_ctx** out, int nx, int ny, double h
 // ------------------------------------------------------------------------------ eval ------
 static const long long kEvalBatch = 1LL << 21;
 static const long long kStencilBatch = 1LL << 22;
+static long long eval_batch(const dbie_ctx* c) { return c->batch_limit > 0 ? c->batch_limit : kEvalBatch; }
+static long long stencil_batch(const dbie_ctx* c) { return c->batch_limit > 0 ? c->batch_limit : kStencilBatch; }
+
+extern "C" dbie_status dbie_debug_set_batch_limit(dbie_ctx* ctx, long long points) {
+    if (!ctx || points < 0) return DBIE_EINVAL;
+    ctx->batch_limit = points;
+    return DBIE_OK;
+}
 
 extern "C" dbie_status dbie_eval(dbie_ctx* ctx, long long M, const double* x, const double* y, const double* z,
                                  const double* lam, double* B, void* cuda_stream) {
     if (!ctx || M < 0) return DBIE_EINVAL;
     if (M == 0) return DBIE_OK;
     if (!x || !y || !z || !lam || !B) return DBIE_EINVAL;
+    GUARD_DEVICE();
+    NvtxRange nvtx_("dbie_eval");
     cudaStream_t st = (cudaStream_t)cuda_stream;
-    const long long cap = M < kEvalBatch ? M : kEvalBatch;
+    const long long cap = M < eval_batch(ctx) ? M : eval_batch(ctx);
     const dbie_status s = ensure(ctx, (void**)&ctx->part, &ctx->part_bytes,
                                  (size_t)ctx->bd.nchunks * 3 * cap * sizeof(double));
     if (s != DBIE_OK) return s;
@@ -290,6 +328,7 @@ extern "C" dbie_status dbie_eval_host(dbie_ctx* ctx, long long M, const double* 
     if (!ctx || M < 0) return DBIE_EINVAL;
     if (M == 0) return DBIE_OK;
     if (!x || !y || !z || !lam || !B) return DBIE_EINVAL;
+    GUARD_DEVICE();
     const size_t m = (size_t)M * sizeof(double);
     CU(cudaDeviceSynchronize());   // earlier work on this context may be in flight on another stream
     dbie_status s = io_reserve(ctx, 9 * m);
@@ -316,8 +355,10 @@ extern "C" dbie_status dbie_eval_f32(dbie_ctx* ctx, long long M, const float* x,
     }
     if (M == 0) return DBIE_OK;
     if (!x || !y || !z || !lam || !B) return DBIE_EINVAL;
+    GUARD_DEVICE();
+    NvtxRange nvtx_("dbie_eval_f32");
     cudaStream_t st = (cudaStream_t)cuda_stream;
-    const long long cap = M < kEvalBatch ? M : kEvalBatch;
+    const long long cap = M < eval_batch(ctx) ? M : eval_batch(ctx);
     const dbie_status s = ensure(ctx, (void**)&ctx->part, &ctx->part_bytes,
                                  (size_t)ctx->bd.nchunks * 3 * cap * sizeof(double));
     if (s != DBIE_OK) return s;
@@ -381,11 +422,13 @@ extern "C" dbie_status dbie_residual(dbie_ctx* ctx, long long M, const double* x
     if (!ctx || M < 0) return DBIE_EINVAL;
     if (M == 0) return DBIE_OK;
     if (!x || !y || !z || !lam || !out) return DBIE_EINVAL;
+    GUARD_DEVICE();
+    NvtxRange nvtx_("dbie_residual");
     NMConsts k;
     dbie_status s = make_consts(ctx, opts, &k);
     if (s != DBIE_OK) return s;
     cudaStream_t st = (cudaStream_t)cuda_stream;
-    const long long cap = M < kStencilBatch ? M : kStencilBatch;
+    const long long cap = M < stencil_batch(ctx) ? M : stencil_batch(ctx);
     s = ensure(ctx, (void**)&ctx->part, &ctx->part_bytes, (size_t)ctx->bd.nchunks * 12 * cap * sizeof(double));
     if (s != DBIE_OK) return s;
     long long launches = 0;
@@ -421,13 +464,15 @@ static dbie_status solve_grid(dbie_ctx* ctx, long long M, const double* x, const
                               const dbie_solve_opts* opts, const NMConsts& k, double* B, double* lam, double* resid,
                               int* iters, int* status, void* cuda_stream) {
     const int T = opts->n_trial, L = opts->n_level;
-    if (T < 2 || T > kGridMaxTrials || L < 1 || !(opts->lam_max > 0.0) || !isfinite(opts->lam_max)) return DBIE_EINVAL;
+    // T < 4: the refined window 2W/(T-1) would not shrink (T = 3) or would grow (T = 2)
+    if (T < 4 || T > kGridMaxTrials || L < 1 || !(opts->lam_max > 0.0) || !isfinite(opts->lam_max)) return DBIE_EINVAL;
     cudaStream_t st = (cudaStream_t)cuda_stream;
     const BoundaryView& bd = ctx->bd;
     // batch so that the chunk sums (nchunks x 12 T doubles per point) stay below 2 GiB
     const size_t per_point = (size_t)bd.nchunks * 12 * T * sizeof(double);
     long long batch = (long long)(((size_t)2 << 30) / per_point);
     if (batch < 1024) batch = 1024;
+    if (ctx->batch_limit > 0) batch = ctx->batch_limit;
     const long long cap = M < batch ? M : batch;
     dbie_status s = ensure(ctx, (void**)&ctx->part, &ctx->part_bytes, per_point * cap);
     if (s != DBIE_OK) return s;
@@ -445,7 +490,7 @@ static dbie_status solve_grid(dbie_ctx* ctx, long long M, const double* x, const
     a.cap = cap;
     a.nact = ctx->counters;
     unsigned long long* nevals = (unsigned long long*)((char*)ctx->counters + 16);
-    CU(cudaMemsetAsync(ctx->counters, 0, 64, st));
+    CU(cudaMemsetAsync(ctx->counters, 0, kCounterBytes, st));
     GridConsts gc;
     gc.T = T;
     gc.n_level = L;
@@ -497,22 +542,25 @@ extern "C" dbie_status dbie_solve(dbie_ctx* ctx, long long M, const double* x, c
     if (M == 0) return DBIE_OK;
     if (!x || !y || !z || !B || !lam || !resid || !iters || !status) return DBIE_EINVAL;
     if (M > 0x7fffffffLL) return DBIE_EINVAL;
+    GUARD_DEVICE();
+    NvtxRange nvtx_("dbie_solve");
     NMConsts k;
     dbie_status s = make_consts(ctx, opts, &k);
     if (s != DBIE_OK) return s;
     if (opts && opts->method == 1) return solve_grid(ctx, M, x, y, z, opts, k, B, lam, resid, iters, status, cuda_stream);
     if (opts && opts->method != 0) return DBIE_EINVAL;
     cudaStream_t st = (cudaStream_t)cuda_stream;
-    const long long cap = M < kStencilBatch ? M : kStencilBatch;
+    const long long cap = M < stencil_batch(ctx) ? M : stencil_batch(ctx);
     s = ensure(ctx, (void**)&ctx->part, &ctx->part_bytes, (size_t)ctx->bd.nchunks * 12 * cap * sizeof(double));
     if (s != DBIE_OK) return s;
-    // state layout: 48 doubles + 4 ints per point
+    // state layout: 48 doubles + 4 ints per point (structure-of-arrays, rows of `count` points of the current
+    // batch, count <= cap) + the arrival counters of the fused kernel
     const size_t isz = align256((size_t)cap * sizeof(int));
-    s = ensure(ctx, (void**)&ctx->state, &ctx->state_bytes, 48 * (size_t)cap * sizeof(double) + 5 * 256 + 4 * isz);
+    const size_t dsz = align256(((size_t)cap / 4 + 2) * sizeof(unsigned));
+    s = ensure(ctx, (void**)&ctx->state, &ctx->state_bytes, 48 * (size_t)cap * sizeof(double) + 5 * 256 + 4 * isz + dsz);
     if (s != DBIE_OK) return s;
     SolveArrays a;
     char* base = ctx->state;
-    // arrays are indexed [q*cap + i], so each block of q rows must be contiguous with stride cap
     const size_t dstride = (size_t)cap * sizeof(double);
     a.V = (double*)base;                 base += align256(12 * dstride);
     a.F = (double*)base;                 base += align256(4 * dstride);
@@ -523,61 +571,44 @@ extern "C" dbie_status dbie_solve(dbie_ctx* ctx, long long M, const double* x, c
     a.iters = (int*)base;                base += isz;
     a.act[0] = (int*)base;               base += isz;
     a.act[1] = (int*)base;               base += isz;
+    unsigned* done = (unsigned*)base;
     a.nact = ctx->counters;
     unsigned long long* nevals = (unsigned long long*)((char*)ctx->counters + 16);
-    CU(cudaMemsetAsync(ctx->counters, 0, 64, st));
-    const int maxpass = 4 + 5 * k.maxiter + 1;
+    CU(cudaMemsetAsync(ctx->counters, 0, kCounterBytes, st));
+    CU(cudaMemsetAsync(done, 0, dsz, st));
     long long launches = 0;
     prof_reset(ctx);
     for (long long off = 0; off < M; off += cap) {
         const long long cnt = (M - off < cap) ? (M - off) : cap;
-        CU(cudaMemsetAsync(ctx->counters, 0, 8, st));        // list counters
-        CU(cudaMemsetAsync(ctx->counters + 8, 0, 8, st));    // work-item counters
+        CU(cudaMemsetAsync(ctx->counters, 0, 16, st));        // list counters (three rotating slots)
+        CU(cudaMemsetAsync(ctx->counters + 8, 0, 16, st));    // work-item counters
         CU(launch_solve_init(a, k, cnt, M, x + off, y + off, z + off, B + off, lam + off, resid + off,
                              iters + off, status + off, st));
         ++launches;
-        // The pass schedule is fixed, but every kProbeEvery passes the length of the next active list is
-        // copied to pinned host memory behind an event; when a copy that has ALREADY completed shows an
-        // empty list the rest of the schedule is not enqueued.  The host never waits: a large batch (the
-        // host runs far ahead of the device) enqueues everything, a small launch-bound one stops early.
-        const int kProbeEvery = 32;
-        int probe_pending[2] = {0, 0};
-        for (int pass = 0; pass < maxpass; ++pass) {
-            if (pass % kProbeEvery == 0 && pass > 0) {
-                bool done = false;
-                for (int q = 0; q < 2; ++q)
-                    if (probe_pending[q] && cudaEventQuery(ctx->probe_ev[q]) == cudaSuccess) {
-                        probe_pending[q] = 0;
-                        done = done || ctx->h_probe[q] == 0u;
-                    }
-                (void)cudaGetLastError();   // cudaErrorNotReady of a pending probe is not an error
-                if (done) break;
-                const int q = (pass / kProbeEvery) & 1;
-                if (!probe_pending[q]) {
-                    CU(cudaMemcpyAsync(&ctx->h_probe[q], &a.nact[pass & 1], sizeof(unsigned), cudaMemcpyDeviceToHost, st));
-                    CU(cudaEventRecord(ctx->probe_ev[q], st));
-                    probe_pending[q] = 1;
-                }
-            }
-            InteractParams p;
-            memset(&p, 0, sizeof p);
-            p.bd = ctx->bd;
-            p.x = x + off; p.y = y + off; p.z = z + off;
-            p.lam = a.cand; p.ldlam = cnt;
-            p.act = a.act[pass & 1];
-            p.count_ptr = &a.nact[pass & 1];
-            p.zero_ptr = &a.nact[(pass + 1) & 1];
-            p.work_ctr = ctx->counters + 8 + (pass & 1);
-            p.zero_work = ctx->counters + 8 + ((pass + 1) & 1);
-            p.delta_abs = k.delta_abs;
-            p.part = ctx->part; p.cap = cap;
-            prof_mark(ctx, st);
-            CU(k.analytic ? launch_interact_analytic(p, ctx->sm_count, st) : launch_interact_stencil(p, ctx->sm_count, st));
-            prof_mark(ctx, st);
-            CU(launch_solve_step(a, k, ctx->bd, pass, cnt, M, z + off, ctx->part, cap, B + off, lam + off,
-                                 resid + off, iters + off, status + off, nevals, st));
-            launches += 2;
-        }
+        // One cooperative launch runs every pass of the search (dbie_solve_fused.cu): no per-pass host work,
+        // no read-back, no partial-sum round trip for large batches.
+        FusedParams f;
+        memset(&f, 0, sizeof f);
+        f.ip.bd = ctx->bd;
+        f.ip.x = x + off; f.ip.y = y + off; f.ip.z = z + off;
+        f.ip.lam = a.cand; f.ip.ldlam = cnt;
+        f.ip.delta_abs = k.delta_abs;
+        f.ip.part = ctx->part; f.ip.cap = cap;
+        f.s = a;
+        f.k = k;
+        f.count = cnt; f.ldo = M;
+        f.B = B + off; f.lam = lam + off; f.resid = resid + off;
+        f.iters = iters + off; f.status = status + off;
+        f.nevals = nevals;
+        f.nact3 = ctx->counters;
+        f.work3 = ctx->counters + 8;
+        f.done = done;
+        f.maxpass = 4 + 5 * k.maxiter + 1;
+        prof_mark(ctx, st);
+        int nl = 0;
+        CU(launch_solve_nm_fused(f, ctx->sm_count, &nl, st));
+        prof_mark(ctx, st);
+        launches += nl;
     }
     ctx->last_launches = launches;
     ctx->evals_on_device = 1;
@@ -591,6 +622,7 @@ extern "C" dbie_status dbie_solve_host(dbie_ctx* ctx, long long M, const double*
     if (!ctx || M < 0) return DBIE_EINVAL;
     if (M == 0) return DBIE_OK;
     if (!x || !y || !z || !B || !lam || !resid || !iters || !status) return DBIE_EINVAL;
+    GUARD_DEVICE();
     const size_t m = (size_t)M * sizeof(double);
     CU(cudaDeviceSynchronize());   // earlier work on this context may be in flight on another stream
     dbie_status s = io_reserve(ctx, 11 * m + 2 * align256((size_t)M * sizeof(int)) + 512);
@@ -616,6 +648,7 @@ extern "C" dbie_status dbie_solve_host(dbie_ctx* ctx, long long M, const double*
 extern "C" dbie_status dbie_last_counters(dbie_ctx* ctx, double* interactions, long long* launches,
                                           long long* objective_evals) {
     if (!ctx) return DBIE_EINVAL;
+    GUARD_DEVICE();
     if (ctx->evals_on_device) {
         unsigned long long n = 0;
         CU(cudaMemcpy(&n, (char*)ctx->counters + 16, sizeof n, cudaMemcpyDeviceToHost));

@@ -11,9 +11,13 @@
 // streamed through shared memory in 16 KB tiles by the TMA bulk-copy engine (cp.async.bulk +
 // mbarrier, double buffered) and every thread of the CTA reads the same pixel record as a broadcast
 // LDS.128 pair; UNR pixels are in flight per thread.  The bound is the FP64 pipe; the history of the
-// stencil launch over round 1 (14.17 -> 11.11 -> 9.04 -> 8.39 ms) is in profiles/r01_ncu_full_interact*_cfg2.md
-// and the shape sweep behind every THREADS x MINB x UNR choice in profiles/r01_variants.md
-// (csrc/tune_interact.cu).
+// stencil launch over round 1 (14.17 -> 11.11 -> 9.04 -> 8.39 ms) is in profiles/r01_ncu_full_interact64_*_cfg2.md
+// and the shape sweep behind every THREADS x MINB x UNR choice in profiles/r01_variants.md.
+//
+// The body of one work item (a block of evaluation positions x a range of canonical chunks) is the
+// device function interact_item; what happens to a finished chunk sum is the caller's `sink`:
+// interact64_kernel writes it to the partial-sum scratch (PartSink), the fused Nelder-Mead kernel
+// (dbie_solve_fused.cu) keeps it in registers or hands it to the CTA that finishes the point block last.
 #pragma once
 #include <cuda_runtime.h>
 #include <stdint.h>
@@ -33,20 +37,23 @@ namespace dbie {
 // one full sincos per component at r_i and a small-angle rotation (rotate_small) for the other three
 // positions; geometry (dx, dy, z terms) is shared where the offsets allow.  59 FP64 instructions per
 // interaction instead of 76.  Threads whose lambda delta exceeds kRotateSmallMax take the plain path.
-enum { MODE_EVAL = 0, MODE_STENCIL = 1, MODE_GRID = 2, MODE_ANALYTIC = 3, MODE_GRID_ANALYTIC = 4, MODE_STENCIL4 = 5 };
+enum { MODE_EVAL = 0, MODE_GRID = 2, MODE_ANALYTIC = 3, MODE_GRID_ANALYTIC = 4, MODE_STENCIL4 = 5 };
 
 // items (threads' units of work) per slot
 __host__ __device__ inline long long items_per_slot(int mode, int G) {
     if (mode == MODE_EVAL || mode == MODE_ANALYTIC || mode == MODE_STENCIL4) return 1;
     if (mode == MODE_GRID_ANALYTIC) return G;
-    return mode == MODE_STENCIL ? kStencil : (long long)kStencil * G;
+    return (long long)kStencil * G;   // MODE_GRID: one item per stencil position and group of NT trials
 }
 
 // One pixel of MODE_STENCIL4: the 4 stencil positions (x_i, x_i + delta | y, y + delta | z, z + delta share
 // dx / dy^2 + z^2 terms where they can).  FAST: one sincos per component at r_i, rotate_small for the rest.
+// The pixel's 12 terms are returned as factor pairs: the accumulation is acc[q][c] = fma(nv[q][c], wb[q][c], acc[q][c]),
+// in pixel order, whoever performs it (the owning thread, or a chain lane of the warp-per-point path).
 template <bool FAST>
-__device__ __forceinline__ void stencil4_pixel(const double4 px, double xi, double xi1, double cc, double cc2,
-                                               double cc3, const double (&lam)[3], double (&acc)[4][3]) {
+__device__ __forceinline__ void stencil4_terms(const double4 px, double xi, double xi1, double cc, double cc2,
+                                               double cc3, const double (&lam)[3], double (&nv)[4][3],
+                                               double (&wb)[4][3]) {
     const double dx0 = px.x - xi, dx1 = px.x - xi1;
     const double r2s[4] = {fma(dx0, dx0, cc), fma(dx1, dx1, cc), fma(dx0, dx0, cc2), fma(dx0, dx0, cc3)};
     double rs[4], ws[4];
@@ -63,26 +70,358 @@ __device__ __forceinline__ void stencil4_pixel(const double4 px, double xi, doub
             const double th0 = lam[c] * rs[0];
             double s0, c0;
             sincos_pos(th0, s0, c0);
-            acc[0][c] = fma(fma(th0, s0, c0), ws[0] * b0[c], acc[0][c]);
+            nv[0][c] = fma(th0, s0, c0);
+            wb[0][c] = ws[0] * b0[c];
 #pragma unroll
             for (int q = 1; q < 4; ++q) {
                 const double thq = lam[c] * rs[q];
                 double sn, cs;
                 rotate_small(s0, c0, thq - th0, sn, cs);
-                acc[q][c] = fma(fma(thq, sn, cs), ws[q] * b0[c], acc[q][c]);
+                nv[q][c] = fma(thq, sn, cs);
+                wb[q][c] = ws[q] * b0[c];
             }
         } else {
 #pragma unroll
-            for (int q = 0; q < 4; ++q) acc[q][c] = fma(kernel_n(lam[c] * rs[q]), ws[q] * b0[c], acc[q][c]);
+            for (int q = 0; q < 4; ++q) {
+                nv[q][c] = kernel_n(lam[c] * rs[q]);
+                wb[q][c] = ws[q] * b0[c];
+            }
         }
     }
 }
 
-template <int MODE, int NT, int THREADS, int MINB, int UNR>
-__global__ void __launch_bounds__(THREADS, MINB) interact64_kernel(const __grid_constant__ InteractParams p) {
+template <bool FAST>
+__device__ __forceinline__ void stencil4_pixel(const double4 px, double xi, double xi1, double cc, double cc2,
+                                               double cc3, const double (&lam)[3], double (&acc)[4][3]) {
+    double nv[4][3], wb[4][3];
+    stencil4_terms<FAST>(px, xi, xi1, cc, cc2, cc3, lam, nv, wb);
+#pragma unroll
+    for (int c = 0; c < 3; ++c)
+#pragma unroll
+        for (int q = 0; q < 4; ++q) acc[q][c] = fma(nv[q][c], wb[q][c], acc[q][c]);
+}
+
+// One pixel of MODE_ANALYTIC (one lambda triple) as factor pairs, kind = 0: sum K b, 1: sum D dx b, 2: sum D dy b,
+// 3: sum D b; the accumulation is acc[kind][c] = fma(fa[kind][c], fb[kind][c], acc[kind][c]) (kind 3 has fb = 1, which
+// rounds exactly like acc + fa).  The same expressions as the thread-per-point loop of interact_item below.
+__device__ __forceinline__ void analytic_terms(const double4 px, double xi, double dy, double cc, const double (&lam)[3],
+                                               const double (&lam2)[3], double (&fa)[4][3], double (&fb)[4][3]) {
+    const double dx = px.x - xi;
+    const double r2 = fma(dx, dx, cc);
+    const double y = rsqrt_full(r2);
+    const double rr = r2 * y;
+    const double wgt = (y * y) * y;
+    const double wb[3] = {wgt * px.y, wgt * px.z, wgt * px.w};
+    const double m3y2 = (y * y) * -3.0;
+#pragma unroll
+    for (int c = 0; c < 3; ++c) {
+        double n, cs;
+        int sg;
+        kernel_n_cos(lam[c] * rr, n, cs, sg);
+        const double wbs = flip_sign_if(wb[c], sg);
+        const double e = fma(lam2[c], cs, n * m3y2);
+        const double gb = e * wbs;
+        fa[0][c] = n;  fb[0][c] = wbs;
+        fa[1][c] = gb; fb[1][c] = dx;
+        fa[2][c] = gb; fb[2][c] = dy;
+        fa[3][c] = gb; fb[3][c] = 1.0;
+    }
+}
+
+struct ItemCtx {      // what a sink needs to know about the calling thread's work item
+    bool live;        // the thread owns a real item (not padding of the last block)
+    long long slot;   // its slot
+    int s, g;         // MODE_GRID: stencil position and trial group; MODE_GRID_ANALYTIC: trial group
+};
+
+// The sink of interact64_kernel: chunk sums go to the scratch, part[(c*Q + q)*cap + slot] (A4).
+template <int MODE, int NT>
+struct PartSink {
+    const InteractParams& p;
+    int nsplit, nch;
+    double run[3];   // MODE_EVAL, unsplit launch: running sum of the chunk sums
+    template <int NA>
+    __device__ __forceinline__ void operator()(const ItemCtx& ic, int c, const double (&acc)[NA][3]) {
+        if (!ic.live) return;
+        const long long slot = ic.slot;
+        if (MODE == MODE_EVAL) {
+            if (nsplit == 1) {
+                // this CTA sees every chunk: add them here, in chunk order with the epilogue's own
+                // operation (bit-identical), and write one sum instead of nchunks partial sums
+#pragma unroll
+                for (int q = 0; q < 3; ++q) run[q] = (c == 0) ? acc[0][q] : __dadd_rn(run[q], acc[0][q]);
+                if (c == nch - 1) {
+#pragma unroll
+                    for (int q = 0; q < 3; ++q) p.part[(long long)q * p.cap + slot] = run[q];
+                }
+            } else {
+#pragma unroll
+                for (int q = 0; q < 3; ++q) p.part[((long long)c * 3 + q) * p.cap + slot] = acc[0][q];
+            }
+        } else if (MODE == MODE_ANALYTIC || MODE == MODE_STENCIL4) {   // rows = kinds / stencil positions
+#pragma unroll
+            for (int kd = 0; kd < 4; ++kd)
+#pragma unroll
+                for (int q = 0; q < 3; ++q) p.part[((long long)c * 12 + kd * 3 + q) * p.cap + slot] = acc[kd][q];
+        } else if (MODE == MODE_GRID_ANALYTIC) {
+            const long long Q = 12LL * p.T;
+#pragma unroll
+            for (int tt = 0; tt < NT; ++tt)
+#pragma unroll
+                for (int kd = 0; kd < 4; ++kd)
+#pragma unroll
+                    for (int q = 0; q < 3; ++q)
+                        p.part[(c * Q + (long long)(kd * 3 + q) * p.T + ic.g * NT + tt) * p.cap + slot] =
+                            acc[4 * tt + kd][q];
+        } else {
+            const long long Q = 12LL * p.T;
+#pragma unroll
+            for (int tt = 0; tt < NT; ++tt)
+#pragma unroll
+                for (int q = 0; q < 3; ++q)
+                    p.part[(c * Q + (long long)(ic.s * 3 + q) * p.T + ic.g * NT + tt) * p.cap + slot] = acc[tt][q];
+        }
+    }
+};
+
+// One work item: the evaluation positions of block `blk` (THREADS items) against the canonical chunks
+// [c0, c1).  `it` counts the tiles this CTA has consumed (stage = it & 1, mbarrier parity = (it >> 1) & 1).
+// At the end of every chunk the chunk sums go to sink(ctx, c, acc) and the accumulators restart from zero.
+// Every tile ends with a __syncthreads, so the caller may reuse its shared scalars after the call.
+template <int MODE, int NT, int THREADS, int UNR, class Sink>
+__device__ __forceinline__ void interact_item(const InteractParams& p, double4 (*tile)[kTilePx], uint64_t* full,
+                                              unsigned& it, long long nitems, int G, long long blk, int c0, int c1,
+                                              Sink& sink) {
     constexpr bool kGridLam = (MODE == MODE_GRID || MODE == MODE_GRID_ANALYTIC);   // lambda from the GRID window
     constexpr bool kAnalytic = (MODE == MODE_ANALYTIC || MODE == MODE_GRID_ANALYTIC);
     static_assert(kGridLam || NT == 1, "only GRID modes carry several lambda triples per thread");
+    const int tid = threadIdx.x;
+    const BoundaryView& bd = p.bd;
+
+    // ---- this thread's evaluation position and lambda triples
+    const long long item = blk * THREADS + tid;
+    ItemCtx ic;
+    ic.live = item < nitems;
+    const long long jt = ic.live ? item : nitems - 1;
+    int s = 0, g = 0;
+    long long slot;
+    if (MODE == MODE_EVAL || MODE == MODE_ANALYTIC || MODE == MODE_STENCIL4) {
+        slot = jt;
+    } else if (MODE == MODE_GRID_ANALYTIC) {
+        g = (int)(jt % G);
+        slot = jt / G;
+    } else {
+        g = (int)(jt % G);
+        const long long js = jt / G;
+        s = (int)(js & 3);
+        slot = js >> 2;
+    }
+    ic.slot = slot;
+    ic.s = s;
+    ic.g = g;
+    // the active list and the trial lambda may have been written earlier in the SAME launch by another SM
+    // (fused solver): read them through L2
+    const long long id = (MODE == MODE_EVAL) ? p.slot0 + slot : (p.act ? (long long)__ldcg(p.act + slot) : slot);
+    double xi = p.x[id], yi = p.y[id], zi = p.z[id];
+    if (MODE == MODE_GRID) {   // Eq. 13: r_i, r_i + delta x, + delta y, + delta z
+        if (s == 1) xi = __dadd_rn(xi, p.delta_abs);
+        if (s == 2) yi = __dadd_rn(yi, p.delta_abs);
+        if (s == 3) zi = __dadd_rn(zi, p.delta_abs);
+    }
+    const double z2 = zi * zi;
+    // MODE_STENCIL4: the offset coordinates of positions 1 (x), 2 (y), 3 (z)
+    const double xi1 = __dadd_rn(xi, p.delta_abs), yi2 = __dadd_rn(yi, p.delta_abs);
+    const double zi3 = __dadd_rn(zi, p.delta_abs), z23 = zi3 * zi3;
+    double lam[NT][3];
+    if (kGridLam) {
+        // trial t of component c: lo_c + W t/(T-1), each operation rounded separately (O-4)
+#pragma unroll
+        for (int c = 0; c < 3; ++c) {
+            const double lo = p.lo[c * p.ldlo + id];
+#pragma unroll
+            for (int tt = 0; tt < NT; ++tt) {
+                const int t = g * NT + tt;
+                lam[tt][c] = fabs(__dadd_rn(lo, __ddiv_rn(__dmul_rn(p.W, (double)t), (double)(p.T - 1))));
+            }
+        }
+    } else {
+#pragma unroll
+        for (int c = 0; c < 3; ++c) lam[0][c] = fabs(__ldcg(p.lam + c * p.ldlam + id));
+    }
+
+    // accumulators: one row per lambda triple; MODE_ANALYTIC: rows = sum K b, sum D dx b, sum D dy b, sum D b
+    // (row 4 tt + kind in the analytic modes)
+    constexpr int NA = (kAnalytic || MODE == MODE_STENCIL4) ? 4 * NT : NT;
+    double acc[NA][3];
+#pragma unroll
+    for (int tt = 0; tt < NA; ++tt) acc[tt][0] = acc[tt][1] = acc[tt][2] = 0.0;
+    const bool lam_all_zero = (lam[0][0] == 0.0) && (lam[0][1] == 0.0) && (lam[0][2] == 0.0);   // MODE_EVAL
+    const bool small_eps = fmax(fmax(lam[0][0], lam[0][1]), lam[0][2]) * p.delta_abs <= kRotateSmallMax;
+    double lam2[NT][3];   // analytic modes: lambda^2
+#pragma unroll
+    for (int tt = 0; tt < NT; ++tt)
+#pragma unroll
+        for (int c = 0; c < 3; ++c) lam2[tt][c] = lam[tt][c] * lam[tt][c];
+
+    const int t0 = chunk_first_tile(bd, c0), t1 = chunk_first_tile(bd, c1);
+    int c = c0;
+    int t_chunk_end = chunk_first_tile(bd, c + 1);
+    if (tid == 0) {
+        const TileDesc d = tile_desc(bd, t0);
+        mbar_expect_tx(&full[it & 1], (unsigned)d.npx * 32u);
+        bulk_g2s(&tile[it & 1][0], bd.rec + d.px0, (unsigned)d.npx * 32u, &full[it & 1]);
+    }
+    for (int t = t0; t < t1; ++t, ++it) {
+        if (tid == 0 && t + 1 < t1) {  // prefetch the next tile into the other stage
+            const TileDesc dn = tile_desc(bd, t + 1);
+            const unsigned sn = (it + 1) & 1;
+            mbar_expect_tx(&full[sn], (unsigned)dn.npx * 32u);
+            bulk_g2s(&tile[sn][0], bd.rec + dn.px0, (unsigned)dn.npx * 32u, &full[sn]);
+        }
+        const TileDesc d = tile_desc(bd, t);
+        mbar_wait(&full[it & 1], (it >> 1) & 1);
+        const double4* __restrict__ rp = &tile[it & 1][0];
+        for (int row = 0; row < d.nrows; ++row) {
+            const double yk = __ldg(bd.yk + d.row0 + row);
+            const double dy = yk - yi;
+            const double cc = fma(dy, dy, z2);
+            const double dy2 = yk - yi2;
+            const double cc2 = fma(dy2, dy2, z2), cc3 = fma(dy, dy, z23);   // MODE_STENCIL4
+            if constexpr (MODE == MODE_STENCIL4) {
+                // the small-angle / plain decision is per thread: two loops instead of a branch per pixel
+                if (small_eps) {
+#pragma unroll UNR
+                    for (int j = 0; j < d.ncols; ++j) stencil4_pixel<true>(rp[j], xi, xi1, cc, cc2, cc3, lam[0], acc);
+                } else {
+#pragma unroll UNR
+                    for (int j = 0; j < d.ncols; ++j) stencil4_pixel<false>(rp[j], xi, xi1, cc, cc2, cc3, lam[0], acc);
+                }
+                rp += d.ncols;
+                continue;
+            }
+            if constexpr (MODE == MODE_EVAL) {
+                // lambda = 0 in all three components (the potential field, BASELINE config 1): n(0) = 1
+                // exactly, so the term is w B_p0 and the sum is bit-identical to the general loop's
+                // fma(1, w B, acc) at 16 instead of 76 FP64 instructions.  Per-thread decision.
+                if (lam_all_zero) {
+#pragma unroll 4
+                    for (int j = 0; j < d.ncols; ++j) {
+                        const double4 px = rp[j];
+                        const double dx = px.x - xi;
+                        const double r2 = fma(dx, dx, cc);
+                        const double y = rsqrt_full(r2);
+                        const double wgt = (y * y) * y;
+                        acc[0][0] = __dadd_rn(acc[0][0], __dmul_rn(wgt, px.y));   // no contraction: same
+                        acc[0][1] = __dadd_rn(acc[0][1], __dmul_rn(wgt, px.z));   // roundings as fma(1, w B, acc)
+                        acc[0][2] = __dadd_rn(acc[0][2], __dmul_rn(wgt, px.w));
+                    }
+                    rp += d.ncols;
+                    continue;
+                }
+            }
+#pragma unroll UNR
+            for (int j = 0; j < d.ncols; ++j) {
+                const double4 px = rp[j];  // {x_k, Bx0, By0, Bz0}: two broadcast LDS.128
+                const double dx = px.x - xi;
+                const double r2 = fma(dx, dx, cc);
+                const double y = rsqrt_full(r2);   // 1/r
+                const double rr = r2 * y;          // r
+                const double wgt = (y * y) * y;    // 1/r^3
+                const double wx = wgt * px.y, wy = wgt * px.z, wz = wgt * px.w;
+                if (kAnalytic) {
+                    // K b = n w b;  D b = (lambda^2 cos(theta) - 3 n / r^2) w b  (w = 1/r^3)
+                    const double m3y2 = (y * y) * -3.0;
+                    const double wb[3] = {wx, wy, wz};
+#pragma unroll
+                    for (int tt = 0; tt < NT; ++tt)
+#pragma unroll
+                        for (int c = 0; c < 3; ++c) {
+                            double n, cs;
+                            int sg;
+                            kernel_n_cos(lam[tt][c] * rr, n, cs, sg);
+                            const double wbs = flip_sign_if(wb[c], sg);
+                            const double e = fma(lam2[tt][c], cs, n * m3y2);
+                            const double gb = e * wbs;
+                            acc[4 * tt + 0][c] = fma(n, wbs, acc[4 * tt + 0][c]);
+                            acc[4 * tt + 1][c] = fma(gb, dx, acc[4 * tt + 1][c]);
+                            acc[4 * tt + 2][c] = fma(gb, dy, acc[4 * tt + 2][c]);
+                            acc[4 * tt + 3][c] += gb;
+                        }
+                    continue;
+                }
+                if (MODE == MODE_GRID && NT > 1) {
+                    // The NT trial values of a component are equally spaced (lambda_t = lo + W t/(T-1)), so
+                    // theta advances by the same d_theta = W/(T-1) r for all three components: one full
+                    // sincos per component for the first trial, one for d_theta, and a plane rotation
+                    // (4 FP64 instructions) per further trial instead of a 17-instruction sincos.  The
+                    // rotated angle theta_0 + tt d_theta differs from fl(lambda_tt r) by a few ulp(theta),
+                    // the size of the rounding theta carries anyway; at most NT/2 <= 4 rotation steps from the middle trial.
+                    // Needs lo >= 0 (no |.| fold inside the group): true for T >= 3 (dbie_solve rejects T < 4).
+                    double sd, cd;
+                    sincos_pos(p.dlam * rr, sd, cd);
+                    const double wb[3] = {wx, wy, wz};
+                    constexpr int TB = NT / 2;   // the full sincos is taken at the middle trial
+#pragma unroll
+                    for (int c = 0; c < 3; ++c) {
+                        const double thb = lam[TB][c] * rr;
+                        double sb, cb;
+                        sincos_pos(thb, sb, cb);
+                        acc[TB][c] = fma(fma(thb, sb, cb), wb[c], acc[TB][c]);
+                        double sn = sb, cs = cb;
+#pragma unroll
+                        for (int tt = TB + 1; tt < NT; ++tt) {   // rotate by +d_theta
+                            const double s1 = fma(sn, cd, cs * sd);
+                            const double c1 = fma(cs, cd, -(sn * sd));
+                            sn = s1;
+                            cs = c1;
+                            acc[tt][c] = fma(fma(lam[tt][c] * rr, sn, cs), wb[c], acc[tt][c]);
+                        }
+                        sn = sb;
+                        cs = cb;
+#pragma unroll
+                        for (int tt = TB - 1; tt >= 0; --tt) {   // rotate by -d_theta
+                            const double s1 = fma(sn, cd, -(cs * sd));
+                            const double c1 = fma(cs, cd, sn * sd);
+                            sn = s1;
+                            cs = c1;
+                            acc[tt][c] = fma(fma(lam[tt][c] * rr, sn, cs), wb[c], acc[tt][c]);
+                        }
+                    }
+                    continue;
+                }
+#pragma unroll
+                for (int tt = 0; tt < NT; ++tt) {
+                    acc[tt][0] = fma(kernel_n(lam[tt][0] * rr), wx, acc[tt][0]);
+                    acc[tt][1] = fma(kernel_n(lam[tt][1] * rr), wy, acc[tt][1]);
+                    acc[tt][2] = fma(kernel_n(lam[tt][2] * rr), wz, acc[tt][2]);
+                }
+            }
+            rp += d.ncols;
+        }
+        if (t + 1 == t_chunk_end) {  // A4: one partial sum per chunk, added in chunk order later
+            sink(ic, c, acc);
+#pragma unroll
+            for (int tt = 0; tt < NA; ++tt) acc[tt][0] = acc[tt][1] = acc[tt][2] = 0.0;
+            ++c;
+            t_chunk_end = chunk_first_tile(bd, c + 1);
+        }
+        __syncthreads();  // everyone is done with stage it&1 before it is refilled
+    }
+}
+
+// split of the chunk range of a launch with `nblk` position blocks (shared by the kernels and their launchers)
+__host__ __device__ inline int chunk_split(long long nblk, int target_items, int nchunks) {
+    int nsplit = 1;
+    if (nblk < target_items) {
+        nsplit = (int)((target_items + nblk - 1) / nblk);
+        if (nsplit > nchunks) nsplit = nchunks;
+    }
+    return nsplit;
+}
+
+template <int MODE, int NT, int THREADS, int MINB, int UNR>
+__global__ void __launch_bounds__(THREADS, MINB) interact64_kernel(const __grid_constant__ InteractParams p) {
+    constexpr bool kGridLam = (MODE == MODE_GRID || MODE == MODE_GRID_ANALYTIC);
     __shared__ alignas(128) double4 tile[2][kTilePx];
     __shared__ alignas(8) uint64_t full[2];
     __shared__ long long next_item;
@@ -104,16 +443,11 @@ __global__ void __launch_bounds__(THREADS, MINB) interact64_kernel(const __grid_
     const long long nitems = count * items_per_slot(MODE, G);
     const long long nblk = (nitems + THREADS - 1) / THREADS;
     if (nblk == 0) return;
-    const BoundaryView& bd = p.bd;
-    const int NCH = bd.nchunks;
-    int nsplit = 1;
-    if (nblk < p.target_items) {
-        nsplit = (int)((p.target_items + nblk - 1) / nblk);
-        if (nsplit > NCH) nsplit = NCH;
-    }
+    const int NCH = p.bd.nchunks;
+    const int nsplit = chunk_split(nblk, p.target_items, NCH);
     const long long nwork = nblk * nsplit;
 
-    unsigned it = 0;  // tiles consumed by this CTA so far: stage = it & 1, parity = (it >> 1) & 1
+    unsigned it = 0;  // tiles consumed by this CTA so far
     // Work items: one per CTA when the host knows the count (the hardware scheduler balances them);
     // a persistent grid (count on the device) takes them from an atomic counter in index order,
     // which balances the same way (static striding measured 1-15 % slower, profiles/r01_variants.md).
@@ -128,258 +462,8 @@ __global__ void __launch_bounds__(THREADS, MINB) interact64_kernel(const __grid_
         const int sp = (int)(w % nsplit);
         const int c0 = (int)(((long long)sp * NCH) / nsplit);
         const int c1 = (int)(((long long)(sp + 1) * NCH) / nsplit);
-
-        // ---- this thread's evaluation position and lambda triples
-        const long long item = blk * THREADS + tid;
-        const bool live = item < nitems;
-        const long long jt = live ? item : nitems - 1;
-        long long slot;
-        int s = 0, g = 0;
-        if (MODE == MODE_EVAL || MODE == MODE_ANALYTIC || MODE == MODE_STENCIL4) {
-            slot = jt;
-        } else if (MODE == MODE_STENCIL) {
-            slot = jt >> 2;
-            s = (int)(jt & 3);
-        } else if (MODE == MODE_GRID_ANALYTIC) {
-            g = (int)(jt % G);
-            slot = jt / G;
-        } else {
-            g = (int)(jt % G);
-            const long long js = jt / G;
-            s = (int)(js & 3);
-            slot = js >> 2;
-        }
-        const long long id = (MODE == MODE_EVAL) ? p.slot0 + slot : (p.act ? (long long)p.act[slot] : slot);
-        double xi = p.x[id], yi = p.y[id], zi = p.z[id];
-        if (MODE == MODE_STENCIL || MODE == MODE_GRID) {   // Eq. 13: r_i, r_i + delta x, + delta y, + delta z
-            if (s == 1) xi = __dadd_rn(xi, p.delta_abs);
-            if (s == 2) yi = __dadd_rn(yi, p.delta_abs);
-            if (s == 3) zi = __dadd_rn(zi, p.delta_abs);
-        }
-        const double z2 = zi * zi;
-        // MODE_STENCIL4: the offset coordinates of positions 1 (x), 2 (y), 3 (z)
-        const double xi1 = __dadd_rn(xi, p.delta_abs), yi2 = __dadd_rn(yi, p.delta_abs);
-        const double zi3 = __dadd_rn(zi, p.delta_abs), z23 = zi3 * zi3;
-        double lam[NT][3];
-        if (kGridLam) {
-            // trial t of component c: lo_c + W t/(T-1), each operation rounded separately (O-4)
-#pragma unroll
-            for (int c = 0; c < 3; ++c) {
-                const double lo = p.lo[c * p.ldlo + id];
-#pragma unroll
-                for (int tt = 0; tt < NT; ++tt) {
-                    const int t = g * NT + tt;
-                    lam[tt][c] = fabs(__dadd_rn(lo, __ddiv_rn(__dmul_rn(p.W, (double)t), (double)(p.T - 1))));
-                }
-            }
-        } else {
-#pragma unroll
-            for (int c = 0; c < 3; ++c) lam[0][c] = fabs(p.lam[c * p.ldlam + id]);
-        }
-
-        // accumulators: one row per lambda triple; MODE_ANALYTIC: rows = sum K b, sum D dx b, sum D dy b, sum D b
-        // (row 4 tt + kind in the analytic modes)
-        constexpr int NA = (kAnalytic || MODE == MODE_STENCIL4) ? 4 * NT : NT;
-        double acc[NA][3];
-#pragma unroll
-        for (int tt = 0; tt < NA; ++tt) acc[tt][0] = acc[tt][1] = acc[tt][2] = 0.0;
-        const bool lam_all_zero = (lam[0][0] == 0.0) && (lam[0][1] == 0.0) && (lam[0][2] == 0.0);   // MODE_EVAL
-        const bool small_eps = fmax(fmax(lam[0][0], lam[0][1]), lam[0][2]) * p.delta_abs <= kRotateSmallMax;
-        double run[3] = {0.0, 0.0, 0.0};   // MODE_EVAL, unsplit launch: running sum of the chunk sums
-        double lam2[NT][3];   // analytic modes: lambda^2
-#pragma unroll
-        for (int tt = 0; tt < NT; ++tt)
-#pragma unroll
-            for (int c = 0; c < 3; ++c) lam2[tt][c] = lam[tt][c] * lam[tt][c];
-
-        const int t0 = chunk_first_tile(bd, c0), t1 = chunk_first_tile(bd, c1);
-        int c = c0;
-        int t_chunk_end = chunk_first_tile(bd, c + 1);
-        if (tid == 0) {
-            const TileDesc d = tile_desc(bd, t0);
-            mbar_expect_tx(&full[it & 1], (unsigned)d.npx * 32u);
-            bulk_g2s(&tile[it & 1][0], bd.rec + d.px0, (unsigned)d.npx * 32u, &full[it & 1]);
-        }
-        for (int t = t0; t < t1; ++t, ++it) {
-            if (tid == 0 && t + 1 < t1) {  // prefetch the next tile into the other stage
-                const TileDesc dn = tile_desc(bd, t + 1);
-                const unsigned sn = (it + 1) & 1;
-                mbar_expect_tx(&full[sn], (unsigned)dn.npx * 32u);
-                bulk_g2s(&tile[sn][0], bd.rec + dn.px0, (unsigned)dn.npx * 32u, &full[sn]);
-            }
-            const TileDesc d = tile_desc(bd, t);
-            mbar_wait(&full[it & 1], (it >> 1) & 1);
-            const double4* __restrict__ rp = &tile[it & 1][0];
-            for (int row = 0; row < d.nrows; ++row) {
-                const double yk = __ldg(bd.yk + d.row0 + row);
-                const double dy = yk - yi;
-                const double cc = fma(dy, dy, z2);
-                const double dy2 = yk - yi2;
-                const double cc2 = fma(dy2, dy2, z2), cc3 = fma(dy, dy, z23);   // MODE_STENCIL4
-                if constexpr (MODE == MODE_STENCIL4) {
-                    // the small-angle / plain decision is per thread: two loops instead of a branch per pixel
-                    if (small_eps) {
-#pragma unroll UNR
-                        for (int j = 0; j < d.ncols; ++j) stencil4_pixel<true>(rp[j], xi, xi1, cc, cc2, cc3, lam[0], acc);
-                    } else {
-#pragma unroll UNR
-                        for (int j = 0; j < d.ncols; ++j) stencil4_pixel<false>(rp[j], xi, xi1, cc, cc2, cc3, lam[0], acc);
-                    }
-                    rp += d.ncols;
-                    continue;
-                }
-                if constexpr (MODE == MODE_EVAL) {
-                    // lambda = 0 in all three components (the potential field, BASELINE config 1): n(0) = 1
-                    // exactly, so the term is w B_p0 and the sum is bit-identical to the general loop's
-                    // fma(1, w B, acc) at 16 instead of 76 FP64 instructions.  Per-thread decision.
-                    if (lam_all_zero) {
-#pragma unroll 4
-                        for (int j = 0; j < d.ncols; ++j) {
-                            const double4 px = rp[j];
-                            const double dx = px.x - xi;
-                            const double r2 = fma(dx, dx, cc);
-                            const double y = rsqrt_full(r2);
-                            const double wgt = (y * y) * y;
-                            acc[0][0] = __dadd_rn(acc[0][0], __dmul_rn(wgt, px.y));   // no contraction: same
-                            acc[0][1] = __dadd_rn(acc[0][1], __dmul_rn(wgt, px.z));   // roundings as fma(1, w B, acc)
-                            acc[0][2] = __dadd_rn(acc[0][2], __dmul_rn(wgt, px.w));
-                        }
-                        rp += d.ncols;
-                        continue;
-                    }
-                }
-#pragma unroll UNR
-                for (int j = 0; j < d.ncols; ++j) {
-                    const double4 px = rp[j];  // {x_k, Bx0, By0, Bz0}: two broadcast LDS.128
-                    const double dx = px.x - xi;
-                    const double r2 = fma(dx, dx, cc);
-                    const double y = rsqrt_full(r2);   // 1/r
-                    const double rr = r2 * y;          // r
-                    const double wgt = (y * y) * y;    // 1/r^3
-                    const double wx = wgt * px.y, wy = wgt * px.z, wz = wgt * px.w;
-                    if (kAnalytic) {
-                        // K b = n w b;  D b = (lambda^2 cos(theta) - 3 n / r^2) w b  (w = 1/r^3)
-                        const double m3y2 = (y * y) * -3.0;
-                        const double wb[3] = {wx, wy, wz};
-#pragma unroll
-                        for (int tt = 0; tt < NT; ++tt)
-#pragma unroll
-                            for (int c = 0; c < 3; ++c) {
-                                double n, cs;
-                                int sg;
-                                kernel_n_cos(lam[tt][c] * rr, n, cs, sg);
-                                const double wbs = flip_sign_if(wb[c], sg);
-                                const double e = fma(lam2[tt][c], cs, n * m3y2);
-                                const double gb = e * wbs;
-                                acc[4 * tt + 0][c] = fma(n, wbs, acc[4 * tt + 0][c]);
-                                acc[4 * tt + 1][c] = fma(gb, dx, acc[4 * tt + 1][c]);
-                                acc[4 * tt + 2][c] = fma(gb, dy, acc[4 * tt + 2][c]);
-                                acc[4 * tt + 3][c] += gb;
-                            }
-                        continue;
-                    }
-                    if (MODE == MODE_GRID && NT > 1) {
-                        // The NT trial values of a component are equally spaced (lambda_t = lo + W t/(T-1)), so
-                        // theta advances by the same d_theta = W/(T-1) r for all three components: one full
-                        // sincos per component for the first trial, one for d_theta, and a plane rotation
-                        // (4 FP64 instructions) per further trial instead of a 17-instruction sincos.  The
-                        // rotated angle theta_0 + tt d_theta differs from fl(lambda_tt r) by a few ulp(theta),
-                        // the size of the rounding theta carries anyway; at most NT/2 <= 4 rotation steps from the middle trial.
-                        // Needs lo >= 0 (no |.| fold inside the group): true for T >= 3 (the launcher sends T = 2 to NT = 1).
-                        double sd, cd;
-                        sincos_pos(p.dlam * rr, sd, cd);
-                        const double wb[3] = {wx, wy, wz};
-                        constexpr int TB = NT / 2;   // the full sincos is taken at the middle trial
-#pragma unroll
-                        for (int c = 0; c < 3; ++c) {
-                            const double thb = lam[TB][c] * rr;
-                            double sb, cb;
-                            sincos_pos(thb, sb, cb);
-                            acc[TB][c] = fma(fma(thb, sb, cb), wb[c], acc[TB][c]);
-                            double sn = sb, cs = cb;
-#pragma unroll
-                            for (int tt = TB + 1; tt < NT; ++tt) {   // rotate by +d_theta
-                                const double s1 = fma(sn, cd, cs * sd);
-                                const double c1 = fma(cs, cd, -(sn * sd));
-                                sn = s1;
-                                cs = c1;
-                                acc[tt][c] = fma(fma(lam[tt][c] * rr, sn, cs), wb[c], acc[tt][c]);
-                            }
-                            sn = sb;
-                            cs = cb;
-#pragma unroll
-                            for (int tt = TB - 1; tt >= 0; --tt) {   // rotate by -d_theta
-                                const double s1 = fma(sn, cd, -(cs * sd));
-                                const double c1 = fma(cs, cd, sn * sd);
-                                sn = s1;
-                                cs = c1;
-                                acc[tt][c] = fma(fma(lam[tt][c] * rr, sn, cs), wb[c], acc[tt][c]);
-                            }
-                        }
-                        continue;
-                    }
-#pragma unroll
-                    for (int tt = 0; tt < NT; ++tt) {
-                        acc[tt][0] = fma(kernel_n(lam[tt][0] * rr), wx, acc[tt][0]);
-                        acc[tt][1] = fma(kernel_n(lam[tt][1] * rr), wy, acc[tt][1]);
-                        acc[tt][2] = fma(kernel_n(lam[tt][2] * rr), wz, acc[tt][2]);
-                    }
-                }
-                rp += d.ncols;
-            }
-            if (t + 1 == t_chunk_end) {  // A4: one partial sum per chunk, added in chunk order later
-                if (live) {
-                    if (MODE == MODE_EVAL) {
-                        if (nsplit == 1) {
-                            // this CTA sees every chunk: add them here, in chunk order with the epilogue's own
-                            // operation (bit-identical), and write one sum instead of nchunks partial sums
-#pragma unroll
-                            for (int q = 0; q < 3; ++q) run[q] = (c == 0) ? acc[0][q] : __dadd_rn(run[q], acc[0][q]);
-                            if (c == NCH - 1) {
-#pragma unroll
-                                for (int q = 0; q < 3; ++q) p.part[(long long)q * p.cap + slot] = run[q];
-                            }
-                        } else {
-#pragma unroll
-                            for (int q = 0; q < 3; ++q) p.part[((long long)c * 3 + q) * p.cap + slot] = acc[0][q];
-                        }
-                    } else if (MODE == MODE_STENCIL) {
-#pragma unroll
-                        for (int q = 0; q < 3; ++q)
-                            p.part[((long long)c * 12 + s * 3 + q) * p.cap + slot] = acc[0][q];
-                    } else if (MODE == MODE_ANALYTIC || MODE == MODE_STENCIL4) {   // rows = kinds / stencil positions
-#pragma unroll
-                        for (int kd = 0; kd < 4; ++kd)
-#pragma unroll
-                            for (int q = 0; q < 3; ++q)
-                                p.part[((long long)c * 12 + kd * 3 + q) * p.cap + slot] = acc[kd][q];
-                    } else if (MODE == MODE_GRID_ANALYTIC) {
-                        const long long Q = 12LL * p.T;
-#pragma unroll
-                        for (int tt = 0; tt < NT; ++tt)
-#pragma unroll
-                            for (int kd = 0; kd < 4; ++kd)
-#pragma unroll
-                                for (int q = 0; q < 3; ++q)
-                                    p.part[(c * Q + (long long)(kd * 3 + q) * p.T + g * NT + tt) * p.cap + slot] =
-                                        acc[4 * tt + kd][q];
-                    } else {
-                        const long long Q = 12LL * p.T;
-#pragma unroll
-                        for (int tt = 0; tt < NT; ++tt)
-#pragma unroll
-                            for (int q = 0; q < 3; ++q)
-                                p.part[(c * Q + (long long)(s * 3 + q) * p.T + g * NT + tt) * p.cap + slot] =
-                                    acc[tt][q];
-                    }
-                }
-#pragma unroll
-                for (int tt = 0; tt < NA; ++tt) acc[tt][0] = acc[tt][1] = acc[tt][2] = 0.0;
-                ++c;
-                t_chunk_end = chunk_first_tile(bd, c + 1);
-            }
-            __syncthreads();  // everyone is done with stage it&1 before it is refilled
-        }
+        PartSink<MODE, NT> sink{p, nsplit, NCH, {0.0, 0.0, 0.0}};
+        interact_item<MODE, NT, THREADS, UNR>(p, tile, full, it, nitems, G, blk, c0, c1, sink);
     }
 }
 

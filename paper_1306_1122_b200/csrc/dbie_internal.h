@@ -62,8 +62,9 @@ __host__ __device__ inline int chunk_first_tile(const BoundaryView& b, int c) {
 
 // One launch of the interaction kernel.
 //  MODE_EVAL:    slot i = evaluation point i with its own lambda triple; Q = 3 sums.
-//  MODE_STENCIL: slot j = one objective evaluation of field point pid = act ? act[j] : j at the
-//                4 stencil positions with ONE lambda triple (Eq. 13); Q = 12 sums [s*3 + p].
+//  MODE_STENCIL4 / MODE_ANALYTIC: slot j = one objective evaluation of field point pid = act ? act[j] : j
+//                with ONE lambda triple: the 4 stencil positions of Eq. 13, Q = 12 sums [s*3 + p], or the
+//                four sums of the analytic gradient (O-5), Q = 12 sums [kind*3 + p].
 // Partial sums go to part[(c*Q + q)*cap + slot], one per chunk c, and are added in chunk order
 // by the consumer, so a result does not depend on how the launch was split.
 struct InteractParams {
@@ -71,11 +72,11 @@ struct InteractParams {
     const double *x, *y, *z;     // by point id
     const double* lam;           // lam[p*ldlam + id]
     long long ldlam;
-    const int* act;              // MODE_STENCIL: slot -> point id, or nullptr (identity)
+    const int* act;              // solver modes: slot -> point id, or nullptr (identity)
     const unsigned* count_ptr;   // device-resident slot count, or nullptr
     long long count;             // host-known slot count (used when count_ptr == nullptr)
     long long slot0;             // MODE_EVAL: id of slot 0 (batching)
-    double delta_abs;            // MODE_STENCIL: finite-difference step (length units)
+    double delta_abs;            // finite-difference step of Eq. 13 (length units)
     double* part;
     long long cap;
     int target_items;            // split the pixel range until there are this many work items
@@ -112,6 +113,24 @@ struct SolveArrays {            // per-point optimiser state, structure-of-array
     int* iters;                 // [M]
     int* act[2];                // active lists (ping-pong)
     unsigned* nact;             // [2] device counters
+};
+
+// The fused Nelder-Mead solve (dbie_solve_fused.cu): ONE cooperative launch runs every pass of the search.
+// List and work counters rotate over three slots: pass p consumes [p % 3], fills [(p+1) % 3] and clears
+// [(p+2) % 3], so no counter is cleared while another CTA may still read or bump it.
+struct FusedParams {
+    InteractParams ip;          // bd, x, y, z, lam = s.cand, ldlam = count, delta_abs, part, cap, target_items
+    SolveArrays s;              // s.act[2]: ping-pong lists; s.nact is unused here (nact3)
+    NMConsts k;
+    long long count, ldo;       // points of the batch; stride of the caller's output arrays
+    double *B, *lam, *resid;
+    int *iters, *status;
+    unsigned long long* nevals;
+    unsigned* nact3;            // [3] list lengths
+    unsigned* work3;            // [3] work-item counters
+    unsigned* done;             // [cap/4 + 2] arrivals per point block (thread mode) / point group (warp mode)
+    int maxpass;
+    int warp_items_max;         // warp-per-point path when ceil(n/4) * nchunks <= this
 };
 
 struct GridArrays {             // per-point GRID state (O-4), structure-of-arrays by point id
@@ -155,10 +174,7 @@ cudaError_t launch_probe(double millis, int sm_count, double* dfma_per_s, double
 cudaError_t launch_solve_init(const SolveArrays& s, const NMConsts& k, long long M, long long ldo,
                               const double* x, const double* y, const double* z, double* B, double* lam,
                               double* resid, int* iters, int* status, cudaStream_t st);
-cudaError_t launch_solve_step(const SolveArrays& s, const NMConsts& k, const BoundaryView& bd, int pass,
-                              long long M, long long ldo, const double* z, const double* part,
-                              long long cap, double* B, double* lam, double* resid, int* iters,
-                              int* status, unsigned long long* nevals, cudaStream_t st);
+cudaError_t launch_solve_nm_fused(const FusedParams& p, int sm_count, int* launches, cudaStream_t st);
 cudaError_t launch_residual_finalize(const BoundaryView& bd, const NMConsts& k, long long M,
                                      long long ldo, const double* z, const double* part, long long cap,
                                      double* out, double* phi, cudaStream_t st);

@@ -4,6 +4,9 @@
 #pragma once
 #include <cuda_runtime.h>
 
+#include "dbie_internal.h"
+#include "dbie_nm.cuh"
+
 namespace dbie {
 
 static __device__ __forceinline__ double qnan() { return __longlong_as_double(0x7ff8000000000000LL); }
@@ -32,6 +35,32 @@ static __device__ void write_invalid(long long ldo, long long i, double* B, doub
     resid[ldo + i] = qnan();
     iters[i] = 0;
     status[i] = 3;
+}
+
+// Per-point optimiser state <-> registers.  The loads go through L2 (__ldcg): in the fused solver the state
+// was written earlier in the same launch, possibly by another SM.
+static __device__ __forceinline__ void load_point(const SolveArrays& s, long long M, long long i, NMPoint& p) {
+    for (int j = 0; j < 4; ++j) {
+        for (int c = 0; c < 3; ++c) p.V[j][c] = __ldcg(s.V + (j * 3 + c) * M + i);
+        p.F[j] = __ldcg(s.F + j * M + i);
+        for (int a = 0; a < 5; ++a) p.A[j][a] = __ldcg(s.aux + (j * 5 + a) * M + i);
+    }
+    for (int a = 0; a < 9; ++a) p.P[a] = __ldcg(s.pend + a * M + i);
+    for (int c = 0; c < 3; ++c) p.cand[c] = __ldcg(s.cand + c * M + i);
+    p.phase = __ldcg(s.phase + i);
+    p.iters = __ldcg(s.iters + i);
+}
+
+static __device__ __forceinline__ void store_point(const SolveArrays& s, long long M, long long i, const NMPoint& p) {
+    for (int j = 0; j < 4; ++j) {
+        for (int c = 0; c < 3; ++c) s.V[(j * 3 + c) * M + i] = p.V[j][c];
+        s.F[j * M + i] = p.F[j];
+        for (int a = 0; a < 5; ++a) s.aux[(j * 5 + a) * M + i] = p.A[j][a];
+    }
+    for (int a = 0; a < 9; ++a) s.pend[a * M + i] = p.P[a];
+    for (int c = 0; c < 3; ++c) s.cand[c * M + i] = p.cand[c];
+    s.phase[i] = p.phase;
+    s.iters[i] = p.iters;
 }
 
 }  // namespace dbie

@@ -1,8 +1,9 @@
 """GPU parity: the CUDA path (through the C ABI, libdbie_b200.so) against the CPU oracle on the
 same seeded inputs.  Tolerances (BASELINE.json north_star; derivation in DESIGN.md section 8):
   B      : max_i ||dB_i|| / ||B_i||  <= 1e-9 over points with ||B_i|| >= 1e-6 max ||B||
-  lambda : | |lam|_gpu - |lam|_orc | * h <= 1e-6 on decision-stable points (protocol P-4)
-  f, g   : 1e-6 absolute;  status, iteration count: identical (integers)
+  lambda : | |lam|_gpu - |lam|_orc | * h <= 1e-6 with identical status and iteration count on >= 95 %
+           of the valid points of every solve batch; the rest must be explained forks (protocol P-4)
+  f, g   : 1e-6 absolute
 """
 import numpy as np
 import pytest
@@ -279,10 +280,19 @@ def test_residual_large_delta_takes_the_plain_stencil_path(dbie):
 
 
 # ---------------------------------------------------------------------------- solve --------
-def _check_solve_parity(dbie, wl, opts_kw=None, gpu=None):
+def _check_solve_parity(dbie, wl, opts_kw=None, gpu=None, min_same=0.95):
     """Protocol P-4; opts_kw["method"] = 1 selects GRID on both sides.
     `gpu`: results already computed on the GPU for exactly the points of `wl` (a sample of a
-    larger launch); otherwise the points of `wl` are solved here."""
+    larger launch); otherwise the points of `wl` are solved here.
+
+    Every valid point falls in one of two classes, decided from the OUTPUTS only:
+      same   : identical status and iteration count AND | |lam|_gpu - |lam|_orc | h <= 1e-6 in all three
+               components.  There B must agree to 1e-9 and f, g to 1e-6.  At least `min_same` of the
+               valid points must be in this class (north_star: "converged lambda must agree to <= 1e-6").
+      forked : everything else.  A fork is legitimate only where some comparison of the oracle's search
+               was within the noise of a tie (margin < MARGIN_STABLE); there the ORACLE's objective at the
+               GPU's lambda must be as good as its own (<= Phi* + 1e-6) and the oracle's B at the GPU's
+               lambda must match the GPU's B to 1e-9."""
     opts_kw = opts_kw or {}
     oo = oracle.Opts(**opts_kw)
     grid = oo.method == 1
@@ -298,27 +308,37 @@ def _check_solve_parity(dbie, wl, opts_kw=None, gpu=None):
             cnt = ctx.counters()
     valid = so["status"] != 3
     assert np.array_equal(s["status"] == 3, ~valid)
+    nvalid = int(valid.sum())
+    with np.errstate(invalid="ignore"):
+        dlam = np.abs(s["lam"] - so["lam"]).max(axis=0) * wl.h
+    same = valid & (s["status"] == so["status"]) & (s["iters"] == so["iters"]) & (dlam <= TOL_LAM)
+    forked = valid & ~same
     stable = valid & (so["margin"] >= MARGIN_STABLE)
-    # (2) decision-stable points: same path
-    if stable.any():
-        assert np.array_equal(s["status"][stable], so["status"][stable])
-        assert np.array_equal(s["iters"][stable], so["iters"][stable])
-        assert (np.abs(s["lam"] - so["lam"])[:, stable] * wl.h).max() <= TOL_LAM
-        err, _ = vec_relerr(s["B"][:, stable], so["B"][:, stable])
+    info = dict(valid=nvalid, same=int(same.sum()), forked=int(forked.sum()), stable=int(stable.sum()),
+                same_frac=float(same.sum()) / max(nvalid, 1),
+                max_dlam_h=float(dlam[same].max()) if same.any() else 0.0)
+    print(f"P-4 {wl.name}{' ' + str(opts_kw) if opts_kw else ''}: valid {nvalid}, same path and lambda {info['same']} "
+          f"({100 * info['same_frac']:.1f} %, max |dlam| h {info['max_dlam_h']:.1e}), forked {info['forked']}, "
+          f"oracle margin >= {MARGIN_STABLE:g}: {info['stable']}")
+    # class `same`: the whole output agrees
+    if nvalid:
+        assert same.any(), "no point of the batch follows the oracle's path"
+        err, _ = vec_relerr(s["B"][:, same], so["B"][:, same])
+        assert err <= TOL_B, err
+        assert np.abs(s["f"] - so["f"])[same].max() <= TOL_FG
+        assert np.abs(s["g"] - so["g"])[same].max() <= TOL_FG
+        # small samples: one fork of a handful of points is allowed
+        assert info["same_frac"] >= min(min_same, 1.0 - 1.5 / nvalid), info
+    # a point whose every comparison was clear of the noise must not fork
+    assert not (forked & stable).any(), (np.where(forked & stable)[0], so["margin"][forked & stable])
+    # class `forked`: the oracle's own objective at the GPU's lambda is as good, and B matches there
+    if forked.any():
+        sub = wl.subset(np.where(forked)[0])
+        ro = oracle.residual(sub, s["lam"][:, forked], oo)
+        assert np.all(ro["phi"] <= so["phi"][forked] + 1e-6)
+        err, _ = vec_relerr(s["B"][:, forked], ro["B"])
         assert err <= TOL_B
-        assert np.abs(s["f"] - so["f"])[stable].max() <= TOL_FG
-        assert np.abs(s["g"] - so["g"])[stable].max() <= TOL_FG
-    # (3) the rest (a comparison within finite-difference noise of a tie: paths may fork):
-    # the oracle's own objective at the GPU's lambda must be as good, and B must match there
-    rest = valid & ~stable
-    forked = rest & ((s["iters"] != so["iters"]) | (s["status"] != so["status"]))
-    if rest.any():
-        sub = wl.subset(np.where(rest)[0])
-        ro = oracle.residual(sub, s["lam"][:, rest], oo)
-        assert np.all(ro["phi"] <= so["phi"][rest] + 1e-6)
-        err, _ = vec_relerr(s["B"][:, rest], ro["B"])
-        assert err <= TOL_B
-    assert forked.sum() <= max(1, int(0.02 * valid.sum())), f"{forked.sum()} forked of {valid.sum()}"
+        assert np.abs(s["f"][forked] - ro["f"]).max() <= TOL_FG and np.abs(s["g"][forked] - ro["g"]).max() <= TOL_FG
     # invariants S-2 on the GPU result
     assert np.all(s["lam"][:, valid] >= 0.0)
     st0 = s["status"] == 0
@@ -329,7 +349,7 @@ def _check_solve_parity(dbie, wl, opts_kw=None, gpu=None):
         assert cnt["objective_evals"] == oo.n_trial * so["iters"][valid].sum() or forked.any()
     else:
         assert cnt["objective_evals"] == so["nfev"][valid].sum() or forked.any()
-    return s, so, dict(stable=int(stable.sum()), rest=int(rest.sum()), forked=int(forked.sum()))
+    return s, so, info
 
 
 def test_solve_config2_lowlou_subset(dbie):
@@ -421,12 +441,13 @@ def test_grid_config5_delta_spot_subset(dbie):
     _check_solve_parity(dbie, w, dict(method=1, n_level=4))
 
 
-@pytest.mark.parametrize("T,levels", [(2, 3), (5, 4), (6, 3), (12, 2)])
+@pytest.mark.parametrize("T,levels", [(4, 3), (5, 4), (6, 3), (12, 2)])
 def test_grid_trial_counts_options_and_invalid_points(dbie, T, levels):
-    """T not a multiple of 4 (2 or 1 trial triples per thread); odd T (the centre trial of every
-    refined window coincides with the incumbent, so the level argmin is an exact or near tie at
-    every point and the whole batch is checked by part (3) of the protocol); the degenerate T = 2 (the window
-    does not shrink: W_next = 2W/(T-1) = 2W), non-default options, invalid points in the batch, h != 1."""
+    """T not a multiple of 8 (4, 2 or 1 trial triples per thread); odd T (the centre trial of every
+    refined window coincides with the incumbent, so the level argmin is an exact or near tie at every
+    point: whichever of the two wins, lambda is the same to an ulp, so these points still land in the
+    `same` class), non-default options, invalid points in the batch, h != 1.  T < 4 is rejected (the
+    window 2W/(T-1) would not shrink)."""
     w = workloads.random_boundary(33, 21, seed=50 + T, npts=45, h=2.0, zmin=1.5, zmax=6.0)
     w.z[4] = -1.0
     w.x[9] = float("nan")
@@ -435,8 +456,7 @@ def test_grid_trial_counts_options_and_invalid_points(dbie, T, levels):
     assert s["status"][4] == 3 and s["status"][9] == 3
     valid = so["status"] != 3
     assert np.all(s["iters"][valid] == levels) and np.all(s["status"][valid] == 1)
-    if T >= 3:
-        assert np.all(s["lam"][:, valid] * w.h <= 0.6 + 1e-12)
+    assert np.all(s["lam"][:, valid] * w.h <= 0.6 + 1e-12)
 
 
 def test_grid_is_reproducible_and_host_entry_matches(dbie):
@@ -450,7 +470,8 @@ def test_grid_is_reproducible_and_host_entry_matches(dbie):
         for k in ("B", "lam", "f", "g", "iters", "status"):
             assert np.array_equal(a[k].cpu().numpy(), b[k].cpu().numpy(), equal_nan=True), k
             assert np.array_equal(a[k].cpu().numpy(), h[k], equal_nan=True), k
-        for bad in (dict(n_trial=1), dict(n_trial=33), dict(n_level=0), dict(lam_max=0.0)):
+        for bad in (dict(n_trial=1), dict(n_trial=2), dict(n_trial=3), dict(n_trial=33), dict(n_level=0),
+                    dict(lam_max=0.0)):
             with pytest.raises(dbie.DBIEError):
                 ctx.solve(dw.x, dw.y, dw.z, dbie.default_opts(method=1, **bad))
 
@@ -472,6 +493,13 @@ def _solve_full_and_sample(dbie, wl, nsample, opts_kw=None):
     assert np.isfinite(s["B"]).all() and (s["lam"] >= 0).all()
     sub, idx = wl.seeded_subset(nsample, seed_offset=77)
     g = {k: (v[:, idx] if v.ndim == 2 else v[idx]) for k, v in s.items()}
+    # the same points solved alone (a few dozen points: the warp-per-point shape of the fused kernel, one
+    # batch) give the same bits as inside the large launch (thread-per-point shape)
+    with dbie.DBIE.from_workload(sub) as ctx:
+        dw = dbie.to_device(sub)
+        alone = {k: v.cpu().numpy() for k, v in ctx.solve(dw.x, dw.y, dw.z, dbie.default_opts(**(opts_kw or {}))).items()}
+    for k in g:
+        assert np.array_equal(alone[k], g[k], equal_nan=True), k
     return _check_solve_parity(dbie, sub, opts_kw, gpu=g), s
 
 
@@ -492,6 +520,28 @@ def test_solve_config3_large_batch_sampled(dbie):
     call; 24 of them re-solved by the oracle."""
     w, _ = workloads.config3().seeded_subset(65536, seed_offset=900)
     _solve_full_and_sample(dbie, w, 24)
+
+
+def test_solve_config3_whole_volume_sampled(dbie):
+    """BASELINE configs[2] at full size: NM solve of all 128 x 128 x 64 = 1,048,576 points of the 256x256
+    boundary in ONE dbie_solve call (about 3 minutes of FP64 work); 64 sampled points are re-solved by the
+    oracle, and solved again alone on the GPU (bit-identical)."""
+    w = workloads.config3()
+    assert w.M == 1048576
+    (_, _, info), s = _solve_full_and_sample(dbie, w, 64)
+    assert info["same_frac"] >= 0.95
+    assert 0.005 < float(np.mean(s["f"])) < 0.5
+
+
+def test_grid_config5_ten_levels_as_benched(dbie):
+    """BASELINE configs[4] with exactly the options bench.py times (GRID, T = 8, 10 levels) on the
+    1024x1024 boundary: 16 seeded points against orc_solve_grid, Eq. 13 differences and the analytic
+    gradient.  After ten levels the window is 0.4 (2/7)^9 = 5e-6 wide, so late near-ties move lambda by
+    less than the 1e-6 tolerance; a fork at an early level would not."""
+    w, _ = workloads.config5().seeded_subset(16, seed_offset=31)
+    for kw in (dict(method=1), dict(method=1, analytic=1)):
+        s, so, info = _check_solve_parity(dbie, w, kw)
+        assert np.all(so["iters"][so["status"] == 1] == 10)
 
 
 def test_grid_config5_large_batch_sampled(dbie):
@@ -642,3 +692,68 @@ def test_q9_eval_f32_and_bad_sizes(dbie):
     assert err <= TOL_B_F32
     with pytest.raises(dbie.DBIEError):
         dbie.DBIE(2, 5, 1.0, 0.0, 0.0, np.ones(10), np.ones(10), np.ones(10), quad9=True)
+
+
+# ------------------------------------------------ internal batching (dbie_debug_set_batch_limit) -
+def test_internal_batches_do_not_change_a_bit(dbie):
+    """eval, eval_f32, residual, the Nelder-Mead solve and GRID process large M in internal batches
+    (2^21 / 2^22 points, a 2 GiB scratch bound): never reached by the other tests.  With the test knob
+    the same paths run with 3-4 uneven batches (offsets > 0, a ragged last batch) and must reproduce the
+    single-batch results bit for bit, for every output array."""
+    import torch
+    w, _ = workloads.config2().seeded_subset(700, seed_offset=4)
+    lam = np.random.default_rng(2).uniform(0.0, 0.3, (3, w.M)) / w.h
+    w.z[11] = -1.0                                   # an invalid point in the second batch
+    t64 = lambda a: torch.from_numpy(np.ascontiguousarray(a, dtype=np.float64)).cuda()
+    t32 = lambda a: torch.from_numpy(np.ascontiguousarray(a, dtype=np.float32)).cuda()
+
+    def run_all(ctx):
+        dw = dbie.to_device(w)
+        out = {"eval": ctx.eval(dw.x, dw.y, dw.z, t64(lam)),
+               "f32": ctx.eval_f32(t32(w.x), t32(w.y), t32(w.z), t32(lam))}
+        for name, o in (("res", None), ("res_an", dbie.default_opts(analytic=1))):
+            for k, v in ctx.residual(dw.x, dw.y, dw.z, t64(lam), o).items():
+                out[f"{name}.{k}"] = v
+        for name, o in (("nm", dbie.default_opts(maxiter=40)), ("nm_an", dbie.default_opts(maxiter=40, analytic=1)),
+                        ("grid", dbie.default_opts(method=1, n_level=3)),
+                        ("grid_an", dbie.default_opts(method=1, n_level=3, analytic=1, n_trial=6))):
+            for k, v in ctx.solve(dw.x, dw.y, dw.z, o).items():
+                out[f"{name}.{k}"] = v
+        return {k: v.cpu().numpy() for k, v in out.items()}
+
+    with dbie.DBIE.from_workload(w, fp32=True) as ctx:
+        one = run_all(ctx)
+        for limit in (256, 199):                     # 3 batches (256, 256, 188) and 4 (199, 199, 199, 103)
+            ctx.set_batch_limit(limit)
+            many = run_all(ctx)
+            for k in one:
+                assert np.array_equal(one[k], many[k], equal_nan=True), (limit, k)
+        ctx.set_batch_limit(0)
+    assert one["nm.status"][11] == 3 and np.isnan(one["eval"][:, 11]).all()
+
+
+# ------------------------------------------------------------- range of theta (include/dbie.h) --
+@pytest.mark.parametrize("theta", [1e3, 1e4, 1e5])
+def test_eval_large_theta_against_oracle(dbie, theta):
+    """include/dbie.h: theta = |lambda| r < 2^20.  The kernel's one-step Cody-Waite reduction leaves
+    k (pi/2 - fl(pi/2)) = 3.9e-17 theta, and theta = lambda r itself carries half an ulp (1.1e-16 theta) on
+    both sides, r possibly one more: each term n(theta) w b is then off by about |theta| * ulp(theta), i.e.
+    2^-52 theta relative to its own amplitude.  Gate: |dB| <= 8 * 2^-52 * theta_max * sum |terms|."""
+    w = workloads.random_boundary(40, 24, seed=77, npts=64, zmin=2.0, zmax=9.0)
+    lam = np.full((3, w.M), 1.0)
+    xk = w.x0 + (np.arange(w.nx) + 0.5) * w.h
+    yk = w.y0 + (np.arange(w.ny) + 0.5) * w.h
+    r = np.sqrt((xk[None, None, :] - w.x[:, None, None]) ** 2 + (yk[None, :, None] - w.y[:, None, None]) ** 2
+                + w.z[:, None, None] ** 2)
+    lam *= theta / r.max(axis=(1, 2))                         # theta_max = theta at every point
+    lam[1] *= 0.37; lam[2] *= 0.81
+    with dbie.DBIE.from_workload(w) as ctx:
+        import torch
+        dw = dbie.to_device(w)
+        B = ctx.eval(dw.x, dw.y, dw.z, torch.from_numpy(lam).cuda()).cpu().numpy()
+    R = oracle.eval(w, lam=lam)
+    c = w.z * w.h ** 2 / (2 * np.pi)
+    for p, b0 in enumerate((w.bx, w.by, w.bz)):
+        th = lam[p][:, None, None] * r
+        mag = c * np.sum((th + 1.0) / r ** 3 * np.abs(b0.reshape(w.ny, w.nx))[None], axis=(1, 2))
+        assert np.all(np.abs(B[p] - R[p]) <= 8 * 2.0 ** -52 * theta * mag), (p, np.abs(B[p] - R[p]).max(), mag.min())
