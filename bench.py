@@ -2,18 +2,25 @@
 """bench.py — throughput of the DBIE hot path on B200 (one process per GPU).
 
     python bench.py [--gpus N] [--steps K] [--warmup W] [--impl ours|reference]
-                    [--workload cfg2|cfg3|cfg4|cfg5] [--method nm|grid] [--points P]
+                    [--workload cfg4|cfg2|cfg3|cfg5] [--method nm|grid] [--gradient fd|analytic]
+                    [--dtype f64|f32] [--points P] [--slabs] [--no-legs]
 
-A "step" is one pass of the whole hot path over one batch of synthetic input:
-stage the boundary (dbie_create) and run the full per-point lambda solve (dbie_solve) on the
-volume of BASELINE.json configs[1] (Low & Lou n=1, m=1, l=0.3, Phi=pi/4; 64x64 boundary,
-64x64x32 = 131,072 points).  The metric is BASELINE.json's: point-pixel DBIE interactions/s in
-fp64 (one interaction = one (evaluation point, pixel) pair, all three components; each stencil
-offset and each objective evaluation counts).  `value` is measured with the inputs resident in
-HBM; `e2e` goes through the host-pointer C-ABI calls (dbie_create_host + dbie_solve_host) with
-the copies inside the timed region.  `roofline` is for the dominant kernel (the interaction
-kernel), timed live with CUDA-event pairs around each of its launches.  `cpu_baseline` times the
-oracle, as it stands, on the host cores over a bounded sample.  One JSON line on stdout (rank 0).
+The metric is BASELINE.json's: point-pixel DBIE interactions/s in fp64 and the fraction of the FP64
+roofline.  One interaction = one (evaluation point, pixel) pair, all three components; in the solver
+every stencil position and every objective evaluation counts.
+
+Default (no flags, one GPU): the HEADLINE line is BASELINE configs[3] ("cfg4": 512x512 boundary,
+M = 1,048,576 random points, per-component lambda, fp64) — the configuration the metric's "interactions/s
+and roofline fraction" are quoted on.  A step is one pass of the hot path over that batch: stage the
+boundary (dbie_create) and evaluate Eq. 6/16 at every point (dbie_eval).  The same run then times three
+more legs, each with its own value / roofline / clocks, under "legs":
+    cfg2_nm    BASELINE configs[1]: full per-point Nelder-Mead lambda solve of the 64x64x32 Low & Lou volume
+    cfg5_grid  BASELINE configs[4]: GRID solve (T = 8, 10 levels) of a seeded 8,192-point subset at 1024x1024
+    cfg4_f32   BASELINE configs[3], fp32 leg: dbie_eval_f32
+`value` is measured with the inputs resident in HBM; `e2e` goes through the host-pointer C-ABI calls with
+the copies inside the timed region.  `roofline` is for the dominant kernel, timed live with CUDA-event pairs
+around each of its launches.  `cpu_baseline` times the oracle, as it stands, on the host cores (all cores and
+one core) over a bounded sample.  One JSON line on stdout (rank 0).
 """
 from __future__ import annotations
 
@@ -32,25 +39,29 @@ sys.path.insert(0, ROOT)
 
 METRIC = "point-pixel DBIE interactions/sec (fp64)"
 UNIT = "interactions/s"
-FP64_INSTR_PER_INTERACTION = 76      # eval: DESIGN.md section 6 (SASS inner loop: 152 per 2 pixels of one position)
-FP64_INSTR_STENCIL = 236 / 4         # Eq. 13 stencil: 4 positions per thread, small-angle rotation (SASS: 236 per pixel)
-FP64_INSTR_ANALYTIC = 95             # analytic gradient: 11 + 3 x 28 per pixel of the one position;
-                                     # GRID on it: two trial triples per geometry, (14 + 2 x 81) / 2 = 88
-FP64_INSTR_GRID = {8: 238 / 8, 4: 154 / 4, 2: 112 / 2, 1: 76}   # GRID: 31 + 3 (20 + 7 (NT-1)) per NT equally spaced trial triples
+# FP64-pipe instructions per interaction of each inner loop, counted from the SASS of the built library by
+# paper_1306_1122_b200/csrc/sass_loops.py (profiles/r02_sass_loops.txt); DESIGN.md section 6 derives them.
+FP64_INSTR = {"eval": 76.0, "nm": 236 / 4, "analytic": 95.0, "grid": 238 / 8, "grid_analytic": 176 / 2}
 FP64_INSTR_SURVEY = 82               # SURVEY.md 8(d) canonical count
 SM_COUNT, FP64_LANES_PER_SM = 148, 64   # B200: 148 SMs, 64 FP64 lanes per SM per clock
+MUFU_PER_INTERACTION = 7             # dbie_eval_f32 default (SFU sincos): 1 rsqrt + 3 x (sin, cos)
+MUFU_LANES_PER_SM = 16
+
+# DRAM bytes (dram__bytes_read.sum + dram__bytes_write.sum) of ONE launch of the dominant kernel, from the
+# committed `ncu --set full` captures; evidence that HBM is idle (the bound is the FP64 pipe).
+NCU_TRAFFIC = {
+    "eval": (60.2e6 + 5.8e6, "profiles/r01_ncu_full_interact64_eval_cfg4.md"),
+}
 
 
 def make_workload(name: str, rank: int = 0, world: int = 1, points: int = 0):
-    """The rank's batch.  Weak scaling: every rank solves a volume of the same size; rank r's
-    layers are shifted by r*h/world in z so the ranks' point sets are disjoint.  `points` > 0
-    takes a seeded subset of the volume (cfg5 defaults to 16,384 points: the full 8.4e6-point
-    GRID solve is 8.8e12 x 4 x 8 x 10 interactions, hours at the FP64 roofline)."""
+    """The rank's batch.  Weak scaling: every rank gets a batch of the same size; rank r's points are
+    shifted by r*h/world in z so the ranks' point sets are disjoint.  `points` > 0 takes a seeded subset."""
     import workloads
     wl = {"cfg2": workloads.config2, "cfg3": workloads.config3, "cfg4": workloads.config4,
           "cfg5": workloads.config5}[name]()
     if points <= 0 and name == "cfg5":
-        points = 16384
+        points = 16384    # the full 8.4e6-point GRID solve is 2.8e15 interactions: hours at the roofline (SURVEY 8(d))
     if 0 < points < wl.M:
         wl, _ = wl.seeded_subset(points, seed_offset=900)
     if world > 1:
@@ -114,26 +125,32 @@ class ClockSampler:
                 "samples": len(sm), "reasons": sorted(reasons)}
 
 
-# DRAM bytes of ONE launch of the interaction kernel from the committed `ncu --set full` captures
-# (dram__bytes_read.sum + dram__bytes_write.sum; profiles/r01_ncu_full_interact64_*.md).  Static evidence that
-# HBM is idle (the bound is the FP64 pipe); None where no capture of that workload/mode exists.
-NCU_TRAFFIC = {("cfg4", "eval"): 60.2e6 + 5.8e6, ("cfg2", "nm"): 7.22e6 + 42.92e6, ("cfg2", "analytic"): 7.24e6 + 42.35e6}
+class Mode:
+    """What a leg runs: eval at given lambda, or the lambda solve (NM / GRID, Eq. 13 / analytic gradient)."""
 
-METHOD = {"grid": False, "analytic": False}   # set by main(): GRID (O-4) instead of NM; analytic gradient (O-5)
+    def __init__(self, workload: str, grid: bool = False, analytic: bool = False, points: int = 0):
+        self.workload, self.grid, self.analytic, self.points = workload, grid, analytic, points
+
+    def kind(self, is_solve: bool) -> str:
+        if not is_solve:
+            return "eval"
+        if self.grid:
+            return "grid_analytic" if self.analytic else "grid"
+        return "analytic" if self.analytic else "nm"
 
 
 # --------------------------------------------------------------------------- oracle legs ---
-def oracle_timed(wl, npoints: int, seed_offset: int, nthreads: int = 0) -> dict:
+def oracle_timed(wl, mode: Mode, npoints: int, seed_offset: int, nthreads: int = 0) -> dict:
     """Time the oracle's solve (or eval) on a seeded sample of the workload's points."""
     import oracle
     sub, _ = wl.seeded_subset(npoints, seed_offset=seed_offset)
     t0 = time.perf_counter()
-    if wl.lam is None and METHOD["grid"]:
-        o = oracle.Opts(method=1, analytic=1 if METHOD["analytic"] else 0)
+    if wl.lam is None and mode.grid:
+        o = oracle.Opts(method=1, analytic=1 if mode.analytic else 0)
         out = oracle.solve_grid(sub, o, nthreads=nthreads)
         inter = float(out["iters"].sum()) * o.n_trial * (1.0 if o.analytic else 4.0) * wl.N
     elif wl.lam is None:
-        an = 1 if METHOD["analytic"] else 0
+        an = 1 if mode.analytic else 0
         out = oracle.solve_nm(sub, oracle.Opts(analytic=an), nthreads=nthreads)
         inter = float(out["nfev"].sum()) * (1.0 if an else 4.0) * wl.N
     else:
@@ -143,40 +160,60 @@ def oracle_timed(wl, npoints: int, seed_offset: int, nthreads: int = 0) -> dict:
     return {"seconds": dt, "interactions": inter, "points": sub.M}
 
 
-def cpu_baseline(wl, target_s: float = 15.0) -> dict:
-    """Oracle as it stands on the host cores: a one-point-per-core probe sizes a ~target_s sample
-    (the probe itself is the sample when it already took that long, e.g. the config-5 GRID solve
-    at ~15 s per point and core)."""
+def cpu_model() -> str:
+    try:
+        for line in open("/proc/cpuinfo"):
+            if line.startswith("model name"):
+                return line.split(":", 1)[1].strip()
+    except OSError:
+        pass
+    return "unknown"
+
+
+def cpu_baseline(wl, mode: Mode, target_s: float = 15.0) -> dict:
+    """Oracle as it stands on the host cores (all cores AND one core).  A one-core probe
+    sizes the samples: ~target_s of wall time on all cores, about a third of that on one core."""
     import oracle
     cores = oracle.max_threads()
-    r = oracle_timed(wl, min(wl.M, cores), seed_offset=50)
+    # one core first: a small probe gives the core-seconds per point, which sizes both samples
+    r1 = oracle_timed(wl, mode, min(wl.M, 1 if wl.lam is None else 8), seed_offset=52, nthreads=1)
+    per_point_core = r1["seconds"] / max(r1["points"], 1)
+    if r1["seconds"] < 0.5 * target_s / 3.0:
+        n1 = int(min(wl.M, max(1, (target_s / 3.0) / max(per_point_core, 1e-9))))
+        r1 = oracle_timed(wl, mode, n1, seed_offset=53, nthreads=1)
+        per_point_core = r1["seconds"] / max(r1["points"], 1)
+    # all cores: a probe (a few scheduling chunks per core) measures the parallel rate actually delivered
+    # (a container may expose more cores than its CPU quota), then the sample is sized from it
+    r = oracle_timed(wl, mode, min(wl.M, cores * (1 if wl.lam is None else 16)), seed_offset=50)
     if r["seconds"] < 0.5 * target_s:
-        per_point = r["seconds"] / max(r["points"], 1)
-        n = int(min(wl.M, 65536, max(cores, target_s / max(per_point, 1e-9))))
-        r = oracle_timed(wl, n, seed_offset=51)
-    kind = ("solve_grid" if METHOD["grid"] else "solve_nm") if wl.lam is None else "eval"
+        n = int(min(wl.M, 65536, max(cores, target_s * r["points"] / max(r["seconds"], 1e-9))))
+        r = oracle_timed(wl, mode, n, seed_offset=51)
+    kind = ("solve_grid" if mode.grid else "solve_nm") if wl.lam is None else "eval"
     return {"value": r["interactions"] / r["seconds"], "unit": UNIT, "cores": cores, "kind": "oracle",
+            "cpu": cpu_model(),
             "sample": f"oracle.{kind} on {r['points']} seeded points of {wl.name} "
-                      f"({r['interactions']:.3e} interactions in {r['seconds']:.1f} s)"}
+                      f"({r['interactions']:.3e} interactions in {r['seconds']:.1f} s)",
+            "one_core": {"value": r1["interactions"] / r1["seconds"], "cores": 1,
+                         "sample": f"{r1['points']} points ({r1['interactions']:.3e} interactions in {r1['seconds']:.1f} s)"}}
 
 
-def run_reference(args) -> None:
+def run_reference(args, mode: Mode) -> None:
     """--impl reference: the oracle timed on the host cores, same metric / config / unit."""
     rank = int(os.environ.get("RANK", "0"))
     if rank != 0:
         return
     import oracle
-    wl = make_workload(args.workload, points=args.points)
+    wl = make_workload(mode.workload, points=mode.points)
     cores = oracle.max_threads()
-    probe = oracle_timed(wl, min(wl.M, cores), seed_offset=60)
+    probe = oracle_timed(wl, mode, min(wl.M, cores), seed_offset=60)
     per_point = probe["seconds"] / probe["points"]
     budget = 150.0 / max(args.steps + args.warmup, 1)            # whole run within a few minutes
     n = int(min(wl.M, max(cores, min(budget, 20.0) / per_point)))
     for w in range(args.warmup):
-        oracle_timed(wl, n, seed_offset=100 + w)
+        oracle_timed(wl, mode, n, seed_offset=100 + w)
     tot_s = tot_i = 0.0
     for k in range(args.steps):
-        r = oracle_timed(wl, n, seed_offset=200 + k)
+        r = oracle_timed(wl, mode, n, seed_offset=200 + k)
         tot_s += r["seconds"]; tot_i += r["interactions"]
     value = tot_i / tot_s
     line = {
@@ -184,51 +221,41 @@ def run_reference(args) -> None:
         "steps": args.steps, "warmup": args.warmup, "ms_per_step": 1e3 * tot_s / args.steps,
         "higher_is_better": True, "scaling": "weak", "vs_baseline": None, "dtype": "f64",
         "data": "synthetic", "gpu_launches": 0,
-        "config": workload_config(wl, args.workload, n_points_per_step=n),
-        "cpu_baseline": {"value": value, "unit": UNIT, "cores": cores, "kind": "oracle",
+        "config": workload_config(wl, mode, n_points_per_step=n),
+        "cpu_baseline": {"value": value, "unit": UNIT, "cores": cores, "kind": "oracle", "cpu": cpu_model(),
                          "sample": f"each step: oracle on {n} seeded points of {wl.name}"},
         "e2e": {"value": value, "unit": UNIT, "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0},
     }
     print(json.dumps(line), flush=True)
 
 
-def workload_config(wl, name, n_points_per_step=None) -> dict:
+def workload_config(wl, mode: Mode, n_points_per_step=None) -> dict:
     desc = {"cfg2": "BASELINE configs[1]: Low&Lou n=1 m=1 l=0.3 Phi=pi/4, boundary 64x64 on [-1,1]^2, "
-                    "full per-point NM lambda solve on the 64x64x32 volume",
-            "cfg3": "BASELINE configs[2]: synthetic bipolar AR 256x256 at 0.5 Mm/px, NM solve on 128x128x64",
-            "cfg4": "BASELINE configs[3]: eval at fixed lambda, boundary 512x512, M=1,048,576 random points",
+                    "full per-point lambda solve on the 64x64x32 volume",
+            "cfg3": "BASELINE configs[2]: synthetic bipolar AR 256x256 at 0.5 Mm/px, lambda solve on 128x128x64",
+            "cfg4": "BASELINE configs[3]: eval at fixed lambda, boundary 512x512, M=1,048,576 random points, "
+                    "per-component lambda in [-0.2,0.2]/px",
             "cfg5": "BASELINE configs[4]: quadrupolar delta-spot 1024x1024, lambda solve on a seeded subset of "
-                    "the 256x256x128 volume"}[name]
+                    "the 256x256x128 volume"}[mode.workload]
     if wl.lam is None:
-        desc += " [method: " + ("GRID T=8, 10 levels" if METHOD["grid"] else "Nelder-Mead") + (
+        desc += " [method: " + ("GRID T=8, 10 levels" if mode.grid else "Nelder-Mead") + (
             "; analytic gradient (O-5): 1 evaluation position per objective evaluation instead of 4"
-            if METHOD["analytic"] else "") + "]"
+            if mode.analytic else "") + "]"
     return {"workload": desc, "boundary": [wl.nx, wl.ny], "points": wl.M if n_points_per_step is None
             else n_points_per_step, "step": "dbie_create + dbie_solve" if wl.lam is None else "dbie_create + dbie_eval",
             "l2": "flushed between timed steps (256 MiB write)"}
 
 
 # --------------------------------------------------------------------------- our arm -------
-def run_ours(args) -> None:
+def measure_f64(mode: Mode, steps: int, warmup: int, rank=0, world=1, local=0, dist=None, e2e: bool = True) -> dict:
+    """Time `steps` passes of dbie_create + dbie_eval / dbie_solve on this rank's batch; returns the line."""
     import torch
     import paper_1306_1122_b200 as dbie
-    rank = int(os.environ.get("RANK", "0"))
-    world = int(os.environ.get("WORLD_SIZE", "1"))
-    local = int(os.environ.get("LOCAL_RANK", "0"))
-    dist = None
-    if world > 1:
-        import torch.distributed as dist
-        os.environ.setdefault("MASTER_ADDR", "127.0.0.1")
-        dist.init_process_group("nccl", device_id=torch.device("cuda", local))
-    if not torch.cuda.is_available():
-        raise SystemExit("bench.py: no CUDA device (the CUDA path has no CPU fallback)")
-    torch.cuda.set_device(local)
     dev = torch.device("cuda", local)
-    dbie.load()
-
-    wl = make_workload(args.workload, rank, world, points=args.points)
+    wl = make_workload(mode.workload, rank, world, points=mode.points)
     is_solve = wl.lam is None
-    sopts = dbie.default_opts(method=1 if METHOD["grid"] else 0, analytic=1 if METHOD["analytic"] else 0)
+    kind = mode.kind(is_solve)
+    sopts = dbie.default_opts(method=1 if mode.grid else 0, analytic=1 if mode.analytic else 0)
     t = lambda a: torch.from_numpy(np.ascontiguousarray(a, dtype=np.float64)).to(dev)
     d_bx, d_by, d_bz = t(wl.bx), t(wl.by), t(wl.bz)
     d_x, d_y, d_z = t(wl.x), t(wl.y), t(wl.z)
@@ -260,8 +287,7 @@ def run_ours(args) -> None:
                else ctx.eval_host(hp["x"], hp["y"], hp["z"], hp["lam"]))
         return ctx, out
 
-    # ---- warm-up
-    for _ in range(max(args.warmup, 0)):
+    for _ in range(max(warmup, 0)):
         ctx, _ = step_device()
         torch.cuda.synchronize()
         ctx.close()
@@ -269,13 +295,9 @@ def run_ours(args) -> None:
     # ---- timed: K steps, device-resident inputs, CUDA events on the launching stream
     sampler = ClockSampler(local) if rank == 0 else None
     barrier()
-    ms_total = 0.0
-    inter_total = 0.0
-    launches = 0
-    kern_ms = 0.0
-    kern_launches = 0
-    evals = 0
-    for k in range(args.steps):
+    ms_total = inter_total = kern_ms = 0.0
+    launches = kern_launches = evals = 0
+    for k in range(steps):
         flush_buf.zero_()                       # L2 flush, outside the event pair
         e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
         e0.record()
@@ -297,28 +319,29 @@ def run_ours(args) -> None:
     value = inter_sum / (ms_max * 1e-3)
 
     # ---- e2e: host buffers through the _host C-ABI calls, copies inside the timed region
-    for _ in range(1):
+    e2e_line = None
+    if e2e:
         ctx, _ = step_host(); ctx.close()
-    barrier()
-    t0 = time.perf_counter()
-    e2e_inter = 0.0
-    for k in range(args.steps):
-        ctx, out = step_host()
-        e2e_inter += ctx.counters()["interactions"]
-        ctx.close()
-    torch.cuda.synchronize()
-    e2e_ms = (time.perf_counter() - t0) * 1e3
-    barrier()
-    e2e_ms, e2e_inter = reduce_over_ranks(dist, dev, e2e_ms, e2e_inter)
-    h2d = 3 * wl.N * 8 + 3 * wl.M * 8 + (0 if is_solve else 3 * wl.M * 8)
-    d2h = (3 + 3 + 2) * wl.M * 8 + 2 * wl.M * 4 if is_solve else 3 * wl.M * 8
-
+        barrier()
+        t0 = time.perf_counter()
+        e2e_inter = 0.0
+        for k in range(steps):
+            ctx, out = step_host()
+            e2e_inter += ctx.counters()["interactions"]
+            ctx.close()
+        torch.cuda.synchronize()
+        e2e_ms = (time.perf_counter() - t0) * 1e3
+        barrier()
+        e2e_ms, e2e_inter = reduce_over_ranks(dist, dev, e2e_ms, e2e_inter)
+        h2d = 3 * wl.N * 8 + 3 * wl.M * 8 + (0 if is_solve else 3 * wl.M * 8)
+        d2h = (3 + 3 + 2) * wl.M * 8 + 2 * wl.M * 4 if is_solve else 3 * wl.M * 8
+        e2e_line = {"value": e2e_inter / (e2e_ms * 1e-3), "unit": UNIT, "h2d_bytes_per_step": h2d,
+                    "d2h_bytes_per_step": d2h, "ms_per_step": e2e_ms / steps,
+                    "api": "dbie_create_host + dbie_solve_host" if is_solve else "dbie_create_host + dbie_eval_host"}
     if rank != 0:
-        if dist is not None:
-            dist.destroy_process_group()
-        return
+        return {}
 
-    # ---- roofline of the dominant kernel (interaction kernel), FP64-pipe bound
+    # ---- roofline of the dominant kernel, FP64-pipe bound
     try:
         dfma_meas, ffma_meas = dbie.probe_dfma_rate(300.0)
     except Exception:
@@ -326,72 +349,61 @@ def run_ours(args) -> None:
     sm_max = (clocks or {}).get("sm_max_mhz") or 1965.0
     peak_slots = SM_COUNT * FP64_LANES_PER_SM * sm_max * 1e6          # FP64 lane-instructions / s
     kern_ips = inter_total / (kern_ms * 1e-3) if kern_ms > 0 else 0.0
-    per_inter = (88.0 if METHOD["grid"] else FP64_INSTR_ANALYTIC) if (is_solve and METHOD["analytic"]) else (
-        FP64_INSTR_GRID[8] if (is_solve and METHOD["grid"]) else (
-            FP64_INSTR_STENCIL if is_solve else FP64_INSTR_PER_INTERACTION))
+    per_inter = FP64_INSTR[kind]
     achieved_slots = kern_ips * per_inter
+    traffic = NCU_TRAFFIC.get(kind) if (mode.points == 0 and mode.workload in ("cfg4", "cfg2")) else None
+    kernel_name = ("dbie::interact64_kernel (fp64 point-pixel sums)" if (not is_solve or mode.grid) else
+                   "dbie::solve_nm_fused_kernel (whole Nelder-Mead search in one cooperative launch: point-pixel sums "
+                   "+ residual + simplex step + list compaction)")
+    # independent-geometry rate: objective evaluations x N, without the x4 stencil or xT trial multipliers
+    pos = 1.0 if (not is_solve or mode.analytic) else 4.0
+    indep = (inter_total / pos / (8.0 if mode.grid else 1.0)) / (ms_total * 1e-3)
     roofline = {
-        "bound": "alu", "kernel": "dbie::interact64_kernel (fp64 point-pixel sums)",
+        "bound": "alu", "kernel": kernel_name,
         "achieved": 2e-12 * achieved_slots, "peak": 2e-12 * peak_slots, "unit": "TFLOP/s",
         "frac": achieved_slots / peak_slots,
-        "traffic": NCU_TRAFFIC.get((args.workload, "grid" if METHOD["grid"] else ("analytic" if METHOD["analytic"] else "nm"))
-                                   if (is_solve and args.points == 0) else NCU_TRAFFIC.get((args.workload, "eval"))),
-        "traffic_note": "bytes of one launch with all points active (ncu captures, profiles/).  Solve: algorithmic 6.8 MB of "
-                        "point data in + 100 MB of chunk partial sums out, of which the L2 keeps half.  Eval (cfg4): "
-                        "algorithmic 72 M + 32 N = 84 MB (the 25 MB of output sums are read back from L2)",
-        "note": "FP64-pipe bound (no HBM/tensor step): achieved = interactions/s of the kernel x FP64 "
-                "lane-instructions per interaction (eval 76; Eq. 13 stencil 59; GRID T=8: 8 equally spaced trial triples per geometry 29.75; analytic gradient 95; DESIGN.md s6) "
-                "x 2 flop per FMA slot; peak = 148 SM x 64 FP64 lanes x clocks.max.sm (derived, DESIGN.md s7)",
+        "unit_note": "achieved and peak count every FP64-pipe lane-instruction (DFMA, DMUL, DADD alike) as 2 flop: "
+                     "`frac` is the fraction of the FP64 pipe's issue slots, not of real flops",
+        "achieved_lane_instr_per_s": achieved_slots, "peak_lane_instr_per_s": peak_slots,
+        "traffic": traffic[0] if traffic else None,
+        "traffic_source": traffic[1] if traffic else "no ncu --set full capture of this leg at this size; see profiles/README.md",
+        "traffic_note": "DRAM bytes of one launch.  Algorithmic bytes: eval 72 M + 32 N (cfg4: 84 MB); solve: 24 M of "
+                        "point data + 480 M of optimiser state per pass through L2.  HBM is idle either way (bound: FP64 pipe)",
+        "note": "FP64-pipe bound (no HBM/tensor step): achieved = interactions/s of the kernel x FP64 lane-instructions per "
+                "interaction (eval 76; Eq. 13 stencil 59; GRID T=8 29.75; analytic gradient 95; GRID on it 88; "
+                "profiles/r02_sass_loops.txt) x 2; peak = 148 SM x 64 FP64 lanes x clocks.max.sm (derived, DESIGN.md s7)",
         "kernel_interactions_per_s": kern_ips, "kernel_ms_per_launch": kern_ms / max(kern_launches, 1),
         "kernel_launches": kern_launches, "kernel_share_of_step": kern_ms / ms_total if ms_total else None,
         "fp64_instr_per_interaction": per_inter,
         "frac_survey82": kern_ips * FP64_INSTR_SURVEY / peak_slots,
         "frac_survey82_note": "SURVEY 8(d)'s canonical 82 instructions per interaction; exceeds `frac` (and can exceed 1) "
-                              "because the kernel executes fewer: the stencil positions / GRID trials share sincos work",
+                              "where the kernel executes fewer: the stencil positions / GRID trials share sincos work",
         "peak_measured_dfma_per_s": dfma_meas, "peak_measured_ffma_per_s": ffma_meas,
         "frac_of_measured_dfma": (achieved_slots / dfma_meas) if dfma_meas else None,
     }
-    base = (cpu_baseline(make_workload(args.workload, points=args.points), target_s=args.cpu_seconds)
-            if args.cpu_seconds > 0 else None)
-
-    line = {
-        "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": args.steps,
-        "warmup": args.warmup, "ms_per_step": ms_max / args.steps, "higher_is_better": True,
+    return {
+        "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": steps,
+        "warmup": warmup, "ms_per_step": ms_max / steps, "higher_is_better": True,
         "scaling": "weak", "vs_baseline": None, "dtype": "f64", "data": "synthetic",
-        "config": dict(workload_config(wl, args.workload), **shard_info(wl.M, rank, world),
-                       objective_evals_per_step=evals / args.steps),
+        "config": dict(workload_config(wl, mode), **shard_info(wl.M, rank, world),
+                       objective_evals_per_step=evals / steps),
         "clocks": clocks,
-        "e2e": {"value": e2e_inter / (e2e_ms * 1e-3), "unit": UNIT, "h2d_bytes_per_step": h2d,
-                "d2h_bytes_per_step": d2h, "ms_per_step": e2e_ms / args.steps,
-                "api": "dbie_create_host + dbie_solve_host" if is_solve else "dbie_create_host + dbie_eval_host"},
+        "e2e": e2e_line,
         "gpu_launches": launches,
+        "independent_geometry_interactions_per_s": indep,
+        "independent_geometry_note": "objective evaluations (or eval points) x pixels per second: without the x4 stencil "
+                                     "positions of Eq. 13 and the x8 GRID trials that `value` counts as interactions",
         "roofline": roofline,
-        "cpu_baseline": base,
     }
-    if base:
-        line["gpu_over_cpu_baseline"] = value / base["value"]
-    print(json.dumps(line), flush=True)
-    if dist is not None:
-        dist.destroy_process_group()
 
 
-# --------------------------------------------------------------------------- fp32 leg ------
-MUFU_PER_INTERACTION = 7             # default dbie_eval_f32 (SFU sincos): 1 rsqrt + 3 x (sin, cos); SASS: 56 MUFU,
-                                     # 280 FP32 of 439 instructions per 8 interactions
-MUFU_LANES_PER_SM = 16
-
-
-def run_ours_f32(args) -> None:
-    """BASELINE configs[3] "fp64 and fp32": dbie_eval_f32 on the config-4 workload (N = 1 only).
-    Same JSON contract; the roofline is the FP32 FMA pipe (polynomial sincos, mask 0)."""
+def measure_f32(steps: int, warmup: int, points: int = 0) -> dict:
+    """BASELINE configs[3] "fp64 and fp32": dbie_eval_f32 on the config-4 workload (one GPU).
+    Same JSON contract; the roofline is the SFU (MUFU sin/cos of the reduced argument, 7 per interaction)."""
     import torch
     import paper_1306_1122_b200 as dbie
-    if not torch.cuda.is_available():
-        raise SystemExit("bench.py: no CUDA device (the CUDA path has no CPU fallback)")
     dev = torch.device("cuda", 0)
-    torch.cuda.set_device(dev)
-    dbie.load()
-    wl = make_workload("cfg4", points=args.points)
+    wl = make_workload("cfg4", points=points)
     t64 = lambda a: torch.from_numpy(np.ascontiguousarray(a, dtype=np.float64)).to(dev)
     h32 = lambda a: torch.from_numpy(np.ascontiguousarray(a, dtype=np.float32)).pin_memory()
     d_bx, d_by, d_bz = t64(wl.bx), t64(wl.by), t64(wl.bz)
@@ -406,13 +418,13 @@ def run_ours_f32(args) -> None:
             ctx.profile(True)
         return ctx, ctx.eval_f32(dx, dy, dz, dl)
 
-    for _ in range(max(args.warmup, 0)):
+    for _ in range(max(warmup, 0)):
         ctx, _ = step(); torch.cuda.synchronize(); ctx.close()
     sampler = ClockSampler(0)
     torch.cuda.synchronize()
     ms_total = kern_ms = 0.0
-    kern_launches = 0
-    for k in range(args.steps):
+    kern_launches = launches = 0
+    for k in range(steps):
         flush_buf.zero_()
         e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
         e0.record()
@@ -421,12 +433,13 @@ def run_ours_f32(args) -> None:
         ms_total += e0.elapsed_time(e1)
         kt = ctx.kernel_time()
         kern_ms += kt["interact_ms"]; kern_launches += kt["interact_launches"]
+        launches += ctx.counters()["launches"] + 1
         ctx.close()
     clocks = sampler.stop()
     # e2e: pinned host float32 points in, float32 B back out, every step
     hb = wl.bx, wl.by, wl.bz
     t0 = time.perf_counter()
-    for k in range(args.steps):
+    for k in range(steps):
         ctx = dbie.DBIE(wl.nx, wl.ny, wl.h, wl.x0, wl.y0, *hb, fp32=True)
         o = ctx.eval_f32(hx.to(dev, non_blocking=True), hy.to(dev, non_blocking=True),
                          hz.to(dev, non_blocking=True), hl.to(dev, non_blocking=True)).cpu()
@@ -438,21 +451,23 @@ def run_ours_f32(args) -> None:
         dfma_meas = ffma_meas = None
     sm_max = (clocks or {}).get("sm_max_mhz") or 1965.0
     peak = SM_COUNT * MUFU_LANES_PER_SM * sm_max * 1e6
-    kern_ips = inter * args.steps / (kern_ms * 1e-3) if kern_ms > 0 else 0.0
+    kern_ips = inter * steps / (kern_ms * 1e-3) if kern_ms > 0 else 0.0
     ach = kern_ips * MUFU_PER_INTERACTION
-    line = {
-        "metric": "point-pixel DBIE interactions/sec (fp32)", "value": inter * args.steps / (ms_total * 1e-3),
-        "unit": UNIT, "n_gpus": 1, "steps": args.steps, "warmup": args.warmup, "ms_per_step": ms_total / args.steps,
+    return {
+        "metric": "point-pixel DBIE interactions/sec (fp32)", "value": inter * steps / (ms_total * 1e-3),
+        "unit": UNIT, "n_gpus": 1, "steps": steps, "warmup": warmup, "ms_per_step": ms_total / steps,
         "higher_is_better": True, "scaling": "weak", "vs_baseline": None, "dtype": "f32", "data": "synthetic",
-        "config": dict(workload_config(wl, "cfg4"), step="dbie_create(DBIE_WITH_FP32) + dbie_eval_f32"),
+        "config": dict(workload_config(wl, Mode("cfg4")), step="dbie_create(DBIE_WITH_FP32) + dbie_eval_f32"),
         "clocks": clocks,
-        "e2e": {"value": inter * args.steps / (e2e_ms * 1e-3), "unit": UNIT,
+        "e2e": {"value": inter * steps / (e2e_ms * 1e-3), "unit": UNIT,
                 "h2d_bytes_per_step": 3 * wl.N * 8 + 6 * wl.M * 4, "d2h_bytes_per_step": 3 * wl.M * 4,
-                "ms_per_step": e2e_ms / args.steps, "api": "DBIE(host boundary, fp32=True) + eval_f32 on pinned host points"},
-        "gpu_launches": 3 * args.steps,
+                "ms_per_step": e2e_ms / steps, "api": "DBIE(host boundary, fp32=True) + eval_f32 on pinned host points"},
+        "gpu_launches": launches,
         "roofline": {"bound": "alu", "kernel": "dbie::interact_f32_kernel (fp32 point-pixel sums, SFU sincos of the reduced argument)",
                      "achieved": 1e-12 * ach, "peak": 1e-12 * peak, "unit": "T MUFU lane-op/s", "frac": ach / peak,
-                     "traffic": None, "mufu_per_interaction": MUFU_PER_INTERACTION,
+                     "traffic": None, "traffic_source": "profiles/r01_ncu_full_interact_f32_eval_cfg4.md (that launch is split; "
+                                                        "no per-launch figure)",
+                     "mufu_per_interaction": MUFU_PER_INTERACTION,
                      "note": "SFU-bound: 148 SM x 16 MUFU lanes x clocks.max.sm / 7 MUFU per interaction (the issue port, 55 "
                              "instructions per interaction, allows 2 % more; the FP32 FMA pipe 60 % more)",
                      "kernel_interactions_per_s": kern_ips, "kernel_ms_per_launch": kern_ms / max(kern_launches, 1),
@@ -460,7 +475,96 @@ def run_ours_f32(args) -> None:
                      "peak_measured_ffma_per_s": ffma_meas},
         "cpu_baseline": None,
     }
-    print(json.dumps(line), flush=True)
+
+
+def measure_slabs(steps: int) -> dict:
+    """the full 256x256x128 volume is hours even at the roofline, so time z-slabs of
+    256 x 256 = 65,536 points at a few heights and project.  GRID, T = 8, 10 levels, Eq. 13 differences."""
+    import torch
+    import workloads
+    import paper_1306_1122_b200 as dbie
+    dev = torch.device("cuda", 0)
+    full = workloads.config5()
+    nlay = 128
+    per = full.M // nlay
+    assert per == 65536
+    t = lambda a: torch.from_numpy(np.ascontiguousarray(a, dtype=np.float64)).to(dev)
+    ctx = dbie.DBIE(full.nx, full.ny, full.h, full.x0, full.y0, t(full.bx), t(full.by), t(full.bz))
+    ctx.profile(True)
+    sopts = dbie.default_opts(method=1)
+    out = []
+    for layer in (0, 31, 127):                      # z = 1, 32, 128 pixels
+        idx = np.arange(layer * per, (layer + 1) * per)
+        sub = full.subset(idx)
+        dx, dy, dz = t(sub.x), t(sub.y), t(sub.z)
+        best = None
+        for k in range(max(steps, 1)):
+            e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+            e0.record()
+            s = ctx.solve(dx, dy, dz, sopts)
+            e1.record(); e1.synchronize()
+            ms = e0.elapsed_time(e1)
+            c = ctx.counters(); kt = ctx.kernel_time()
+            rec = {"z_px": float(sub.z[0] / full.h), "points": per, "ms": ms, "interactions": c["interactions"],
+                   "value": c["interactions"] / (ms * 1e-3), "kernel_ms": kt["interact_ms"],
+                   "levels_mean": float(s["iters"].double().mean().item()),
+                   "status0_frac": float((s["status"] == 0).double().mean().item()),
+                   "mean_f": float(s["f"].mean().item()), "mean_g": float(s["g"].mean().item())}
+            if best is None or rec["ms"] < best["ms"]:
+                best = rec
+        peak = SM_COUNT * FP64_LANES_PER_SM * 1965e6
+        best["roofline_frac_kernel"] = best["interactions"] / (best["kernel_ms"] * 1e-3) * FP64_INSTR["grid"] / peak
+        out.append(best)
+    ctx.close()
+    mean_ms = float(np.mean([r["ms"] for r in out]))
+    return {"workload": "BASELINE configs[4] z-slabs: 256x256 points at z = 1, 32, 128 px, 1024x1024 boundary, GRID T=8, 10 levels",
+            "slabs": out, "projected_full_volume_s": mean_ms * 1e-3 * nlay,
+            "note": "full volume (128 slabs, 8,388,608 points) NOT run: projected = mean slab time x 128"}
+
+
+def run_ours(args, mode: Mode) -> None:
+    import torch
+    import paper_1306_1122_b200 as dbie
+    rank = int(os.environ.get("RANK", "0"))
+    world = int(os.environ.get("WORLD_SIZE", "1"))
+    local = int(os.environ.get("LOCAL_RANK", "0"))
+    dist = None
+    if world > 1:
+        import torch.distributed as dist
+        os.environ.setdefault("MASTER_ADDR", "127.0.0.1")
+        dist.init_process_group("nccl", device_id=torch.device("cuda", local))
+    if not torch.cuda.is_available():
+        raise SystemExit("bench.py: no CUDA device (the CUDA path has no CPU fallback)")
+    torch.cuda.set_device(local)
+    dbie.load()
+
+    if args.dtype == "f32":
+        if rank == 0:
+            print(json.dumps(measure_f32(args.steps, args.warmup, args.points)), flush=True)
+        return
+    if args.slabs:
+        if rank == 0:
+            print(json.dumps(measure_slabs(args.steps)), flush=True)
+        return
+
+    line = measure_f64(mode, args.steps, args.warmup, rank, world, local, dist)
+    if rank == 0:
+        base = (cpu_baseline(make_workload(mode.workload, points=mode.points), mode, target_s=args.cpu_seconds)
+                if args.cpu_seconds > 0 else None)
+        line["cpu_baseline"] = base
+        if base:
+            line["gpu_over_cpu_baseline"] = line["value"] / base["value"]
+        if world == 1 and args.legs:
+            # the other legs of the same run: fewer steps each so that the default run stays within a few minutes
+            ls, lw = max(1, min(args.steps, 2)), max(1, min(args.warmup, 3))
+            legs = {}
+            legs["cfg2_nm"] = measure_f64(Mode("cfg2"), ls, lw)
+            legs["cfg5_grid"] = measure_f64(Mode("cfg5", grid=True, points=8192), 1, 1)
+            legs["cfg4_f32"] = measure_f32(ls, lw)
+            line["legs"] = legs
+        print(json.dumps(line), flush=True)
+    if dist is not None:
+        dist.destroy_process_group()
 
 
 def main():
@@ -469,32 +573,35 @@ def main():
     ap.add_argument("--steps", type=int, default=3)
     ap.add_argument("--warmup", type=int, default=3)
     ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
-    ap.add_argument("--workload", default="cfg2", choices=["cfg2", "cfg3", "cfg4", "cfg5"])
+    ap.add_argument("--workload", default="cfg4", choices=["cfg2", "cfg3", "cfg4", "cfg5"])
     ap.add_argument("--method", default=None, choices=["nm", "grid"],
                     help="lambda search of the solve workloads (default: nm; cfg5: grid)")
     ap.add_argument("--gradient", default="fd", choices=["fd", "analytic"],
                     help="solve workloads: Eq. 13 finite differences (the paper's) or the analytic gradient (O-5)")
     ap.add_argument("--dtype", default="f64", choices=["f64", "f32"],
-                    help="f32: the dbie_eval_f32 leg of BASELINE configs[3] (implies --workload cfg4, one GPU)")
+                    help="f32: the dbie_eval_f32 leg of BASELINE configs[3] alone (implies --workload cfg4, one GPU)")
     ap.add_argument("--points", type=int, default=0,
                     help="solve/eval a seeded subset of this many points (0: the whole volume; cfg5: 16384)")
+    ap.add_argument("--slabs", action="store_true",
+                    help="config 5 as SURVEY 8(d) asks: GRID solve of three 65,536-point z-slabs + projected full-volume time")
+    ap.add_argument("--no-legs", dest="legs", action="store_false",
+                    help="only the headline workload (legs run by default for --workload cfg4 on one GPU)")
     ap.add_argument("--cpu-seconds", type=float, default=15.0,
                     help="target CPU time of the cpu_baseline leg (0 disables it)")
     args = ap.parse_args()
-    METHOD["grid"] = (args.method == "grid") or (args.method is None and args.workload == "cfg5")
-    METHOD["analytic"] = args.gradient == "analytic"
+    if args.workload != "cfg4":
+        args.legs = False
+    mode = Mode(args.workload, grid=(args.method == "grid") or (args.method is None and args.workload == "cfg5"),
+                analytic=args.gradient == "analytic", points=args.points)
     if args.impl == "reference":
-        run_reference(args)
-    elif args.dtype == "f32":
-        if int(os.environ.get("RANK", "0")) == 0:
-            run_ours_f32(args)
+        run_reference(args, mode)
     else:
         if args.gpus > 1 and int(os.environ.get("WORLD_SIZE", "1")) == 1:
             # convenience: re-launch under torchrun, one rank per GPU
             cmd = [sys.executable, "-m", "torch.distributed.run", "--nnodes=1", f"--nproc-per-node={args.gpus}",
                    "--master-addr", "127.0.0.1", "--master-port", "29541", os.path.abspath(__file__)] + sys.argv[1:]
             raise SystemExit(subprocess.call(cmd))
-        run_ours(args)
+        run_ours(args, mode)
 
 
 if __name__ == "__main__":
