@@ -219,16 +219,37 @@ __global__ void __launch_bounds__(kFusedThreads, kFusedMinB) solve_nm_fused_kern
 
         if (ngrp * NCH > P.warp_items_max) {
             // ---------------- thread per point: 128 points x a range of chunks
+            // Schedule: as many whole rounds of the grid as the point blocks fill run with one item per block
+            // covering ALL chunks (sums stay in registers); only the remaining blocks of the last, partial
+            // round are split over chunk ranges, as finely as it takes to fill the grid once more.
             const long long nblk = (n + kFusedThreads - 1) / kFusedThreads;
-            const int nsplit = chunk_split(nblk, ip.target_items, NCH);
-            const long long nwork = nblk * nsplit;
+            const long long G = gridDim.x;
+            const long long nwhole = (nblk / G) * G;
+            const long long rem = nblk - nwhole;
+            int nsplit_t = 1;
+            if (rem > 0) {   // smallest split minimising rounds x longest item, in chunks
+                long long best = -1;
+                for (int sc = 1; sc <= NCH; ++sc) {
+                    const long long cost = ((rem * sc + G - 1) / G) * ((NCH + sc - 1) / sc);
+                    if (best < 0 || cost < best) {
+                        best = cost;
+                        nsplit_t = sc;
+                    }
+                }
+            }
+            const long long nwork = nwhole + rem * nsplit_t;
             for (;;) {
                 if (tid == 0) *next_item = (long long)atomicAdd(P.work3 + r0, 1u);
                 __syncthreads();
                 const long long w = *next_item;
                 if (w >= nwork) break;
-                const long long blk = w / nsplit;
-                const int sp = (int)(w % nsplit);
+                long long blk = w;
+                int nsplit = 1, sp = 0;
+                if (w >= nwhole) {
+                    nsplit = nsplit_t;
+                    blk = nwhole + (w - nwhole) / nsplit;
+                    sp = (int)((w - nwhole) % nsplit);
+                }
                 const int c0 = (int)(((long long)sp * NCH) / nsplit);
                 const int c1 = (int)(((long long)(sp + 1) * NCH) / nsplit);
                 FusedSink sink{q, nsplit == 1, {}};
@@ -323,7 +344,6 @@ static cudaError_t launch_fused(const FusedParams& p, int sm_count, cudaStream_t
     if (blocks_per_sm > kFusedMinB) blocks_per_sm = kFusedMinB;
     FusedParams q = p;
     const int grid = sm_count * blocks_per_sm;
-    q.ip.target_items = 16 * grid;
     q.warp_items_max = 11 * grid;   // warp shape while its items fit ~11 rounds of the grid (one item costs ~1/11 of a thread-shape item)
     void* args[] = {(void*)&q};
     return cudaLaunchCooperativeKernel((const void*)kern, dim3(grid), dim3(kFusedThreads), args, kFusedSmem, st);
