@@ -158,6 +158,35 @@ dbie_status dbie_residual(dbie_ctx* ctx, long long M, const double* x, const dou
                           const double* z, const double* lam, const dbie_solve_opts* opts,
                           double* out, double* phi, void* cuda_stream);
 
+/* Field-line and current-line tracing.  The paper draws lines of the reconstructed B
+ * and "current lines" of J = curl B (Eq. 14) in its Figs. 5-11
+ * without giving the integrator; reading T-1 of DESIGN.md: dr/ds = direction * v/|v| in arc length s,
+ * classical RK4 at a fixed step, v = B or J evaluated by this library AT the four stage points of
+ * every step (nothing is interpolated): B and lambda from the per-point search of dbie_solve (or Eq. 6
+ * at a fixed lambda triple), J from the stencil of Eq. 13 at that lambda. */
+typedef struct {
+    double ds;         /* arc-length step as a FRACTION of h; 0.5                                       */
+    int max_steps;     /* S: steps per line (each line stores up to S + 1 points); 100                  */
+    int direction;     /* +1: along v; -1: against v                                                    */
+    int current;       /* 0: field lines (v = B); 1: current lines (v = J, Eq. 14)                      */
+    int fixed_lambda;  /* 0: lambda from the per-point search (solve options); 1: the triple `lam`      */
+    double lam[3];     /* fixed lambda triple, units 1/length (0, 0, 0 = the potential field)           */
+    double z_min;      /* a line lives in z_min h < z <= z_max h and inside the magnetogram window;     */
+    double z_max;      /*   0, 1e300                                                                    */
+} dbie_trace_opts;
+
+void dbie_trace_default_opts(dbie_trace_opts* opts);
+
+/* x0, y0, z0: L seed points (device).  sopts: options of the lambda search and of Eq. 13 (NULL = defaults).
+ * path: out, 3*(S+1)*L doubles, point k of line i at path[(c*(S+1) + k)*L + i], c = 0, 1, 2; NaN beyond a
+ * line's last point.  npts: out L, points stored (0 if the seed is outside the region).  status: out L:
+ * 0 = max_steps reached, 1 = left the region (a stage point or the new point), 2 = v zero or not finite at
+ * a stage point.  Asynchronous on the stream; 4 S field evaluations of L points are enqueued, lines that
+ * have stopped cost nothing in the lambda search. */
+dbie_status dbie_trace(dbie_ctx* ctx, long long L, const double* x0, const double* y0, const double* z0,
+                       const dbie_solve_opts* sopts, const dbie_trace_opts* topts, double* path, int* npts,
+                       int* status, void* cuda_stream);
+
 /* ------------------------------------------------------------------------------------------------
  * Diagnostics and measurement.  Not needed to use the library; bench.py and the tests call them.
  * ---------------------------------------------------------------------------------------------- */

@@ -43,6 +43,12 @@ class SolveOpts(C.Structure):
                 ("analytic", C.c_int)]
 
 
+class TraceOpts(C.Structure):
+    """Mirror of dbie_trace_opts (include/dbie.h)."""
+    _fields_ = [("ds", C.c_double), ("max_steps", C.c_int), ("direction", C.c_int), ("current", C.c_int),
+                ("fixed_lambda", C.c_int), ("lam", C.c_double * 3), ("z_min", C.c_double), ("z_max", C.c_double)]
+
+
 _vp = C.c_void_p
 
 
@@ -73,6 +79,10 @@ def load() -> C.CDLL:
                                     _vp, _vp, _vp]
     lib.dbie_residual.argtypes = [_vp, C.c_longlong, _vp, _vp, _vp, _vp, C.POINTER(SolveOpts), _vp, _vp,
                                   _vp]
+    lib.dbie_trace_default_opts.argtypes = [C.POINTER(TraceOpts)]
+    lib.dbie_trace_default_opts.restype = None
+    lib.dbie_trace.argtypes = [_vp, C.c_longlong, _vp, _vp, _vp, C.POINTER(SolveOpts), C.POINTER(TraceOpts), _vp, _vp,
+                               _vp, _vp]
     lib.dbie_last_counters.argtypes = [_vp, C.POINTER(C.c_double), C.POINTER(C.c_longlong),
                                        C.POINTER(C.c_longlong)]
     lib.dbie_profile.argtypes = [_vp, C.c_int]
@@ -94,6 +104,21 @@ def default_opts(**kw) -> SolveOpts:
         if not hasattr(o, k):
             raise TypeError(f"unknown solve option {k!r}")
         setattr(o, k, v)
+    return o
+
+
+def default_trace_opts(**kw) -> TraceOpts:
+    """dbie_trace_default_opts, then keyword overrides; lam=(lx, ly, lz) also sets fixed_lambda = 1."""
+    o = TraceOpts()
+    load().dbie_trace_default_opts(C.byref(o))
+    for k, v in kw.items():
+        if k == "lam":
+            o.lam[0], o.lam[1], o.lam[2] = (float(t) for t in v)
+            o.fixed_lambda = 1
+        elif not hasattr(o, k):
+            raise TypeError(f"unknown trace option {k!r}")
+        else:
+            setattr(o, k, v)
     return o
 
 
@@ -274,6 +299,22 @@ class DBIE:
             r = self.residual(x, y, z, lam, o, stream=stream)
             out["J"], out["div"] = r["J"], r["div"]
         return out
+
+    # -- dbie_trace
+    def trace(self, x0, y0, z0, topts: TraceOpts | None = None, sopts: SolveOpts | None = None, stream=None):
+        """Field lines (or current lines) through the seeds: dict path (3, S+1, L), npts (L,), status (L,)."""
+        torch = _torch()
+        L = x0.numel()
+        t = topts if topts is not None else default_trace_opts()
+        o = sopts if sopts is not None else default_opts()
+        S = int(t.max_steps)
+        path = torch.empty((3, S + 1, L), dtype=torch.float64, device=x0.device)
+        npts = torch.empty((L,), dtype=torch.int32, device=x0.device)
+        status = torch.empty((L,), dtype=torch.int32, device=x0.device)
+        self._check(self._lib.dbie_trace(self._h, L, _dev_f64(x0, L, "x0"), _dev_f64(y0, L, "y0"),
+                                         _dev_f64(z0, L, "z0"), C.byref(o), C.byref(t), _vp(path.data_ptr()),
+                                         _vp(npts.data_ptr()), _vp(status.data_ptr()), _stream_ptr(stream)))
+        return {"path": path, "npts": npts, "status": status}
 
     def solve_host(self, x, y, z, opts: SolveOpts | None = None):
         x = np.ascontiguousarray(x, dtype=np.float64)

@@ -28,6 +28,7 @@ UNITS = [
     ("dbie_solve_fused.cu", []),     # same flags as dbie_interact.cu: identical interaction arithmetic
     ("dbie_solver.cu", ["-fmad=false"]),
     ("dbie_grid.cu", ["-fmad=false"]),
+    ("dbie_trace.cu", ["-fmad=false"]),
     ("dbie_api.cu", []),
 ]
 HEADERS = ["dbie_internal.h", "dbie_interact_fp64.cuh", "dbie_tma.cuh", "dbie_math.cuh", "dbie_math_f32.cuh", "dbie_nm.cuh", "dbie_solver_common.cuh",

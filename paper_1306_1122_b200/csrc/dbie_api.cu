@@ -21,6 +21,7 @@ struct NvtxRange {   // ranges around create / eval / residual
 
 struct dbie_ctx {
     int device, sm_count;
+    int win_nx, win_ny;                       // the magnetogram's pixel grid (bd.nx, bd.ny count SOURCES: 9-node staging changes them)
     BoundaryView bd;
     double4* rec;
     double* yk;
@@ -29,6 +30,7 @@ struct dbie_ctx {
     double* part;       size_t part_bytes;    // chunk partial sums
     char* state;        size_t state_bytes;   // optimiser state
     char* io;           size_t io_bytes;      // device staging of the _host entry points
+    char* trace;        size_t trace_bytes;   // dbie_trace: line state and the field at the line heads
     unsigned* counters;                       // device: list lengths [0..2], nevals (u64) at +16 B, work-item counters at +32 B
     cudaStream_t own_stream;
     double last_interactions;
@@ -194,6 +196,7 @@ extern "C" void dbie_destroy(dbie_ctx* ctx) {
     cudaFree(ctx->part);
     cudaFree(ctx->state);
     cudaFree(ctx->io);
+    cudaFree(ctx->trace);
     cudaFree(ctx->counters);
     if (ctx->own_stream) cudaStreamDestroy(ctx->own_stream);
     for (int i = 0; i < ctx->ev_cap; ++i) cudaEventDestroy(ctx->ev[i]);
@@ -226,6 +229,7 @@ extern "C" dbie_status dbie_create(dbie_ctx** out, int nx, int ny, double h, dou
         const bool q9 = (flags & DBIE_QUAD_9NODE) != 0;
         // 9-node elements: the sources are 3 Gauss abscissae per element and direction (O-6)
         const int sx = q9 ? 3 * (nx / 2) : nx, sy = q9 ? 3 * (ny / 2) : ny;
+        ctx->win_nx = nx; ctx->win_ny = ny;
         b.nx = sx; b.ny = sy; b.N = (long long)sx * sy;
         b.h = h; b.x0 = x0; b.y0 = y0;
         setup_tiling(b);
@@ -642,6 +646,100 @@ extern "C" dbie_status dbie_solve_host(dbie_ctx* ctx, long long M, const double*
     CU(cudaMemcpyAsync(iters, di, (size_t)M * sizeof(int), cudaMemcpyDeviceToHost, st));
     CU(cudaMemcpyAsync(status, ds, (size_t)M * sizeof(int), cudaMemcpyDeviceToHost, st));
     CU(cudaStreamSynchronize(st));
+    return DBIE_OK;
+}
+
+// ------------------------------------------------------------------------------ trace -----
+extern "C" void dbie_trace_default_opts(dbie_trace_opts* o) {
+    if (!o) return;
+    memset(o, 0, sizeof *o);
+    o->ds = 0.5;
+    o->max_steps = 100;
+    o->direction = 1;
+    o->current = 0;
+    o->fixed_lambda = 0;
+    o->z_min = 0.0;
+    o->z_max = 1e300;
+}
+
+extern "C" dbie_status dbie_trace(dbie_ctx* ctx, long long L, const double* x0, const double* y0, const double* z0,
+                                  const dbie_solve_opts* sopts, const dbie_trace_opts* topts, double* path, int* npts,
+                                  int* status, void* cuda_stream) {
+    if (!ctx || L < 0) return DBIE_EINVAL;
+    if (L == 0) return DBIE_OK;
+    if (!x0 || !y0 || !z0 || !path || !npts || !status || L > 0x7fffffffLL) return DBIE_EINVAL;
+    dbie_trace_opts td;
+    if (!topts) { dbie_trace_default_opts(&td); topts = &td; }
+    if (!(topts->ds > 0.0) || !isfinite(topts->ds) || topts->max_steps < 0 || (topts->direction != 1 && topts->direction != -1) ||
+        !(topts->z_max > topts->z_min))
+        return DBIE_EINVAL;
+    if (topts->fixed_lambda && !(isfinite(topts->lam[0]) && isfinite(topts->lam[1]) && isfinite(topts->lam[2]))) return DBIE_EINVAL;
+    GUARD_DEVICE();
+    NvtxRange nvtx_("dbie_trace");
+    cudaStream_t st = (cudaStream_t)cuda_stream;
+    const BoundaryView& bd = ctx->bd;
+    const double h = bd.h;
+    // layout of the scratch: r[3], k[12], px, py, pz, B[3], lam[3], resid[2], out9[9] doubles; 5 ints per line
+    const size_t dl = (size_t)L * sizeof(double), il = align256((size_t)L * sizeof(int));
+    dbie_status s = ensure(ctx, (void**)&ctx->trace, &ctx->trace_bytes, align256(35 * dl) + 5 * il);
+    if (s != DBIE_OK) return s;
+    double* d = (double*)ctx->trace;
+    TraceState t;
+    t.r = d;               d += 3 * L;
+    t.k = d;               d += 12 * L;
+    t.px = d;              d += L;
+    t.py = d;              d += L;
+    t.pz = d;              d += L;
+    double* fB = d;        d += 3 * L;
+    double* flam = d;      d += 3 * L;
+    double* fres = d;      d += 2 * L;
+    double* fout = d;      d += 9 * L;
+    char* ib = ctx->trace + align256(35 * dl);
+    t.alive = (int*)ib;    ib += il;
+    t.good = (int*)ib;     ib += il;
+    t.why = (int*)ib;      ib += il;
+    int* fit = (int*)ib;   ib += il;
+    int* fst = (int*)ib;
+    TraceBox box;
+    // the region written as the oracle writes it: x0 + nx h etc. (nx, ny of the magnetogram, not of a 9-node source grid)
+    box.x0 = bd.x0; box.x1 = bd.x0 + (double)ctx->win_nx * h;
+    box.y0 = bd.y0; box.y1 = bd.y0 + (double)ctx->win_ny * h;
+    box.z0 = topts->z_min * h; box.z1 = topts->z_max * h;
+    const double ds = topts->ds * h;
+    const int S = topts->max_steps;
+    CU(launch_trace_init(t, box, L, S, x0, y0, z0, path, npts, status, st));
+    if (topts->fixed_lambda) CU(launch_trace_fill_lambda(flam, L, topts->lam, st));
+    double interactions = 0.0;
+    long long launches = 1, evals = 0;
+    for (int step = 0; step < S; ++step)
+        for (int stage = 0; stage < 4; ++stage) {
+            const double* v = fB;
+            if (!topts->fixed_lambda) {
+                s = dbie_solve(ctx, L, t.px, t.py, t.pz, sopts, fB, flam, fres, fit, fst, st);
+                if (s != DBIE_OK) return s;
+                launches += ctx->last_launches;
+            } else if (!topts->current) {
+                s = dbie_eval(ctx, L, t.px, t.py, t.pz, flam, fB, st);
+                if (s != DBIE_OK) return s;
+                launches += ctx->last_launches;
+                interactions += ctx->last_interactions;
+            }
+            if (topts->current) {
+                s = dbie_residual(ctx, L, t.px, t.py, t.pz, flam, sopts, fout, nullptr, st);
+                if (s != DBIE_OK) return s;
+                launches += ctx->last_launches;
+                interactions += ctx->last_interactions;
+                evals += L;
+                v = fout + 5 * L;   // rows 5..7 of dbie_residual's output: J (Eq. 14)
+            }
+            CU(launch_trace_stage(t, box, L, S, step, stage, topts->direction, ds, v, L, path, npts, status, st));
+            ++launches;
+        }
+    // counters: the interactions of the lambda searches live on the device (they are not summed over the calls)
+    ctx->last_interactions = interactions;
+    ctx->last_launches = launches;
+    ctx->last_evals = evals;
+    ctx->evals_on_device = 0;
     return DBIE_OK;
 }
 

@@ -142,6 +142,17 @@ struct GridArrays {             // per-point GRID state (O-4), structu
     unsigned* nact;             // [2] device counters
 };
 
+// Line tracing (dbie_trace.cu): per-line state, structure-of-arrays over L lines
+struct TraceState {
+    double* r;                  // [3][L] current point r_n
+    double* k;                  // [3 stages][3][L] k1..k3 (k4 is consumed at once)
+    double *px, *py, *pz;       // [L] the stage point handed to the field evaluation (z = -1: skip)
+    int *alive, *good, *why;    // [L] line still traced; still integrating this step; stop reason if not
+};
+struct TraceBox {
+    double x0, x1, y0, y1, z0, z1;   // region: x0 <= x <= x1, y0 <= y <= y1, z0 < z <= z1
+};
+
 struct GridConsts {
     int T, n_level;
     double W, Wn;               // this level's window width and the next one, 2 W/(T-1)
@@ -186,5 +197,13 @@ cudaError_t launch_grid_step(const GridArrays& s, const NMConsts& k, const GridC
                              int lev, long long M, long long ldo, const double* z, const double* part,
                              long long cap, double* B, double* lam, double* resid, int* iters, int* status,
                              unsigned long long* nevals, cudaStream_t st);
+
+cudaError_t launch_trace_init(const TraceState& t, const TraceBox& box, long long L, int S, const double* sx,
+                              const double* sy, const double* sz, double* path, int* npts, int* status,
+                              cudaStream_t st);
+cudaError_t launch_trace_stage(const TraceState& t, const TraceBox& box, long long L, int S, int step, int stage,
+                               int direction, double ds, const double* v, long long ldv, double* path, int* npts,
+                               int* status, cudaStream_t st);
+cudaError_t launch_trace_fill_lambda(double* lam, long long L, const double l[3], cudaStream_t st);
 
 }  // namespace dbie

@@ -763,3 +763,82 @@ def test_eval_large_theta_against_oracle(dbie, theta):
         th = lam[p][:, None, None] * r
         mag = c * np.sum((th + 1.0) / r ** 3 * np.abs(b0.reshape(w.ny, w.nx))[None], axis=(1, 2))
         assert np.all(np.abs(B[p] - R[p]) <= 8 * 2.0 ** -52 * theta * mag), (p, np.abs(B[p] - R[p]).max(), mag.min())
+
+
+# ---------------------------------------- field-line / current-line tracing -----
+def _gpu_trace(dbie, w, seeds, topts_kw, sopts_kw=None):
+    import torch
+    t = lambda a: torch.from_numpy(np.ascontiguousarray(a, dtype=np.float64)).cuda()
+    with dbie.DBIE.from_workload(w) as ctx:
+        out = ctx.trace(t(seeds[0]), t(seeds[1]), t(seeds[2]), dbie.default_trace_opts(**topts_kw),
+                        dbie.default_opts(**(sopts_kw or {})))
+        return {k: v.cpu().numpy() for k, v in out.items()}
+
+
+def _check_trace(g, o, h, tol=1e-8):
+    path, npts, status = o
+    assert np.array_equal(g["npts"], npts), (g["npts"], npts)
+    assert np.array_equal(g["status"], status)
+    assert np.array_equal(np.isnan(g["path"]), np.isnan(path))
+    d = np.nanmax(np.abs(g["path"] - path)) if np.isfinite(path).any() else 0.0
+    assert d <= tol * h, d / h
+    return d / h
+
+
+def test_trace_potential_field_lines_of_the_dipole(dbie):
+    """lambda = 0 (fixed): lines of the DBIE field of the buried dipole's magnetogram, GPU against the tracing
+    oracle point by point, both directions, with lines that leave through z_min, through the window side and
+    seeds outside the region; the GPU lines keep the dipole invariant r / sin^2(theta) like the oracle's (T-4)."""
+    from oracle import trace as otrace
+    w = workloads.config1(n=64)
+    seeds = np.array([[9.5, 8.0, 6.0], [8.0, 6.0, 6.5], [10.0, 10.0, 6.0], [8.0 + 31.0, 8.0, 3.0], [8.0, 8.0 - 31.5, 3.0],
+                      [200.0, 8.0, 3.0], [9.0, 9.0, 2.4]]).T.copy()
+    for direction in (1, -1):
+        kw = dict(ds=0.25, max_steps=50, direction=direction, z_min=2.5)
+        g = _gpu_trace(dbie, w, seeds, dict(kw, lam=(0.0, 0.0, 0.0)))
+        o = otrace.trace_dbie(w, seeds, otrace.TraceOpts(fixed_lam=(0.0, 0.0, 0.0), **kw))
+        _check_trace(g, o, w.h)
+        assert list(g["npts"][-2:]) == [0, 0] and (g["status"][-2:] == 1).all()
+    p = g["path"][:, :g["npts"][0], 0]
+    X, Y, Z = p[0] - 8.0, p[1] - 8.0, p[2] + 4.0
+    R = np.sqrt(X * X + Y * Y + Z * Z)
+    Lsh = R ** 3 / (X * X + Y * Y)
+    assert np.abs(Lsh / Lsh[0] - 1.0).max() < 5e-3       # 64x64 window: truncation 1.4e-3 (pin K-6)
+
+
+@pytest.mark.parametrize("current", [0, 1])
+def test_trace_with_the_lambda_solve_matches_the_oracle(dbie, current):
+    """Lines of B (and current lines of J, Eq. 14) with lambda from the per-point Nelder-Mead search at every
+    stage point, on the Low & Lou boundary of BASELINE configs[1]: 12 seeds x 6 steps = 288 point solves per
+    line set, compared point by point with the oracle's sequential RK4 (1e-8 h).  The search runs in the
+    warp-per-point shape of the fused kernel (12 points)."""
+    from oracle import trace as otrace
+    w, _ = workloads.config2().seeded_subset(12, seed_offset=5)
+    seeds = np.stack([w.x, w.y, w.z + 3 * w.h])
+    kw = dict(ds=0.5, max_steps=6, direction=1, current=current)
+    g = _gpu_trace(dbie, w, seeds, kw)
+    o = otrace.trace_dbie(w, seeds, otrace.TraceOpts(**kw))
+    d = _check_trace(g, o, w.h)
+    print(f"trace current={current}: max |dr| = {d:.1e} h over {int(g['npts'].sum())} points")
+    assert g["npts"].max() >= 4
+
+
+def test_trace_analytic_gradient_and_options(dbie):
+    """The analytic-gradient search (O-5) under the tracer, against the field, with a z_max lid, on the config-3
+    boundary (h = 0.5); bad options are rejected."""
+    import torch
+    from oracle import trace as otrace
+    w, _ = workloads.config3().seeded_subset(8, seed_offset=8)
+    seeds = np.stack([w.x, w.y, np.minimum(w.z, 6.0 * w.h)])
+    kw = dict(ds=0.4, max_steps=4, direction=-1, z_min=0.5, z_max=7.0)
+    g = _gpu_trace(dbie, w, seeds, kw, dict(analytic=1))
+    o = otrace.trace_dbie(w, seeds, otrace.TraceOpts(**kw), oracle.Opts(analytic=1))
+    _check_trace(g, o, w.h)
+    e = torch.empty(0, dtype=torch.float64, device="cuda")
+    with dbie.DBIE.from_workload(w) as ctx:
+        out = ctx.trace(e, e, e)
+        assert out["path"].shape == (3, 101, 0)
+        t = lambda a: torch.from_numpy(np.ascontiguousarray(a)).cuda()
+        for bad in (dict(ds=0.0), dict(direction=0), dict(max_steps=-1), dict(z_min=2.0, z_max=1.0)):
+            with pytest.raises(dbie.DBIEError):
+                ctx.trace(t(seeds[0]), t(seeds[1]), t(seeds[2]), dbie.default_trace_opts(**bad))
