@@ -140,7 +140,11 @@ static cudaError_t launch64(const InteractParams& p, int sm_count, int waves, cu
         grid = nblk * nsplit;   // one work item per CTA: the hardware balances them
         if (grid > 0x7fffffffLL) return cudaErrorInvalidValue;
     }
-    interact64_kernel<MODE, NT, THREADS, MINB, UNR><<<(unsigned)grid, THREADS, 0, st>>>(q);
+    auto kern = interact64_kernel<MODE, NT, THREADS, MINB, UNR>;
+    // per launch: the attribute belongs to the current device's copy of the kernel
+    cudaError_t e = cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)kInteractSmem);
+    if (e != cudaSuccess) return e;
+    kern<<<(unsigned)grid, THREADS, kInteractSmem, st>>>(q);
     return cudaGetLastError();
 }
 
@@ -149,7 +153,7 @@ static cudaError_t launch64(const InteractParams& p, int sm_count, int waves, cu
 cudaError_t launch_interact_eval(const InteractParams& p, int sm_count, int* nparts, cudaStream_t st) {
     const long long nblk = (p.count + kThreads64 - 1) / kThreads64;
     *nparts = (nblk >= 8LL * sm_count * kMinB64 || p.bd.nchunks == 1) ? 1 : p.bd.nchunks;
-    return launch64<MODE_EVAL, 1, 2>(p, sm_count, 8, st);
+    return launch64<MODE_EVAL, 1, 3>(p, sm_count, 8, st);   // three pixels in flight (_work sweep: u1 .822, u2 .835, u3 .848, u4 .842)
 }
 
 cudaError_t launch_interact_stencil(const InteractParams& p, int sm_count, cudaStream_t st) {

@@ -51,8 +51,8 @@ __host__ __device__ inline long long items_per_slot(int mode, int G) {
 // The pixel's 12 terms are returned as factor pairs: the accumulation is acc[q][c] = fma(nv[q][c], wb[q][c], acc[q][c]),
 // in pixel order, whoever performs it (the owning thread, or a chain lane of the warp-per-point path).
 template <bool FAST>
-__device__ __forceinline__ void stencil4_terms(const double4 px, double xi, double xi1, double cc, double cc2,
-                                               double cc3, const double (&lam)[3], double (&nv)[4][3],
+__device__ __forceinline__ void stencil4_terms(const TrigRef& tr, const double4 px, double xi, double xi1, double cc,
+                                               double cc2, double cc3, const double (&lam)[3], double (&nv)[4][3],
                                                double (&wb)[4][3]) {
     const double dx0 = px.x - xi, dx1 = px.x - xi1;
     const double r2s[4] = {fma(dx0, dx0, cc), fma(dx1, dx1, cc), fma(dx0, dx0, cc2), fma(dx0, dx0, cc3)};
@@ -69,7 +69,7 @@ __device__ __forceinline__ void stencil4_terms(const double4 px, double xi, doub
         if (FAST) {
             const double th0 = lam[c] * rs[0];
             double s0, c0;
-            sincos_pos(th0, s0, c0);
+            sincos_pos(th0, tr, s0, c0);
             nv[0][c] = fma(th0, s0, c0);
             wb[0][c] = ws[0] * b0[c];
 #pragma unroll
@@ -83,7 +83,7 @@ __device__ __forceinline__ void stencil4_terms(const double4 px, double xi, doub
         } else {
 #pragma unroll
             for (int q = 0; q < 4; ++q) {
-                nv[q][c] = kernel_n(lam[c] * rs[q]);
+                nv[q][c] = kernel_n(lam[c] * rs[q], tr);
                 wb[q][c] = ws[q] * b0[c];
             }
         }
@@ -91,10 +91,10 @@ __device__ __forceinline__ void stencil4_terms(const double4 px, double xi, doub
 }
 
 template <bool FAST>
-__device__ __forceinline__ void stencil4_pixel(const double4 px, double xi, double xi1, double cc, double cc2,
-                                               double cc3, const double (&lam)[3], double (&acc)[4][3]) {
+__device__ __forceinline__ void stencil4_pixel(const TrigRef& tr, const double4 px, double xi, double xi1, double cc,
+                                               double cc2, double cc3, const double (&lam)[3], double (&acc)[4][3]) {
     double nv[4][3], wb[4][3];
-    stencil4_terms<FAST>(px, xi, xi1, cc, cc2, cc3, lam, nv, wb);
+    stencil4_terms<FAST>(tr, px, xi, xi1, cc, cc2, cc3, lam, nv, wb);
 #pragma unroll
     for (int c = 0; c < 3; ++c)
 #pragma unroll
@@ -104,8 +104,9 @@ __device__ __forceinline__ void stencil4_pixel(const double4 px, double xi, doub
 // One pixel of MODE_ANALYTIC (one lambda triple) as factor pairs, kind = 0: sum K b, 1: sum D dx b, 2: sum D dy b,
 // 3: sum D b; the accumulation is acc[kind][c] = fma(fa[kind][c], fb[kind][c], acc[kind][c]) (kind 3 has fb = 1, which
 // rounds exactly like acc + fa).  The same expressions as the thread-per-point loop of interact_item below.
-__device__ __forceinline__ void analytic_terms(const double4 px, double xi, double dy, double cc, const double (&lam)[3],
-                                               const double (&lam2)[3], double (&fa)[4][3], double (&fb)[4][3]) {
+__device__ __forceinline__ void analytic_terms(const TrigRef& tr, const double4 px, double xi, double dy, double cc,
+                                               const double (&lam)[3], const double (&lam2)[3], double (&fa)[4][3],
+                                               double (&fb)[4][3]) {
     const double dx = px.x - xi;
     const double r2 = fma(dx, dx, cc);
     const double y = rsqrt_full(r2);
@@ -116,12 +117,10 @@ __device__ __forceinline__ void analytic_terms(const double4 px, double xi, doub
 #pragma unroll
     for (int c = 0; c < 3; ++c) {
         double n, cs;
-        int sg;
-        kernel_n_cos(lam[c] * rr, n, cs, sg);
-        const double wbs = flip_sign_if(wb[c], sg);
+        kernel_n_cos(lam[c] * rr, tr, n, cs);
         const double e = fma(lam2[c], cs, n * m3y2);
-        const double gb = e * wbs;
-        fa[0][c] = n;  fb[0][c] = wbs;
+        const double gb = e * wb[c];
+        fa[0][c] = n;  fb[0][c] = wb[c];
         fa[1][c] = gb; fb[1][c] = dx;
         fa[2][c] = gb; fb[2][c] = dy;
         fa[3][c] = gb; fb[3][c] = 1.0;
@@ -189,9 +188,9 @@ struct PartSink {
 // At the end of every chunk the chunk sums go to sink(ctx, c, acc) and the accumulators restart from zero.
 // Every tile ends with a __syncthreads, so the caller may reuse its shared scalars after the call.
 template <int MODE, int NT, int THREADS, int UNR, class Sink>
-__device__ __forceinline__ void interact_item(const InteractParams& p, double4 (*tile)[kTilePx], uint64_t* full,
-                                              unsigned& it, long long nitems, int G, long long blk, int c0, int c1,
-                                              Sink& sink) {
+__device__ __forceinline__ void interact_item(const InteractParams& p, const TrigRef& tr, double4 (*tile)[kTilePx],
+                                              uint64_t* full, unsigned& it, long long nitems, int G, long long blk,
+                                              int c0, int c1, Sink& sink) {
     constexpr bool kGridLam = (MODE == MODE_GRID || MODE == MODE_GRID_ANALYTIC);   // lambda from the GRID window
     constexpr bool kAnalytic = (MODE == MODE_ANALYTIC || MODE == MODE_GRID_ANALYTIC);
     static_assert(kGridLam || NT == 1, "only GRID modes carry several lambda triples per thread");
@@ -291,10 +290,10 @@ __device__ __forceinline__ void interact_item(const InteractParams& p, double4 (
                 // the small-angle / plain decision is per thread: two loops instead of a branch per pixel
                 if (small_eps) {
 #pragma unroll UNR
-                    for (int j = 0; j < d.ncols; ++j) stencil4_pixel<true>(rp[j], xi, xi1, cc, cc2, cc3, lam[0], acc);
+                    for (int j = 0; j < d.ncols; ++j) stencil4_pixel<true>(tr, rp[j], xi, xi1, cc, cc2, cc3, lam[0], acc);
                 } else {
 #pragma unroll UNR
-                    for (int j = 0; j < d.ncols; ++j) stencil4_pixel<false>(rp[j], xi, xi1, cc, cc2, cc3, lam[0], acc);
+                    for (int j = 0; j < d.ncols; ++j) stencil4_pixel<false>(tr, rp[j], xi, xi1, cc, cc2, cc3, lam[0], acc);
                 }
                 rp += d.ncols;
                 continue;
@@ -337,12 +336,10 @@ __device__ __forceinline__ void interact_item(const InteractParams& p, double4 (
 #pragma unroll
                         for (int c = 0; c < 3; ++c) {
                             double n, cs;
-                            int sg;
-                            kernel_n_cos(lam[tt][c] * rr, n, cs, sg);
-                            const double wbs = flip_sign_if(wb[c], sg);
+                            kernel_n_cos(lam[tt][c] * rr, tr, n, cs);
                             const double e = fma(lam2[tt][c], cs, n * m3y2);
-                            const double gb = e * wbs;
-                            acc[4 * tt + 0][c] = fma(n, wbs, acc[4 * tt + 0][c]);
+                            const double gb = e * wb[c];
+                            acc[4 * tt + 0][c] = fma(n, wb[c], acc[4 * tt + 0][c]);
                             acc[4 * tt + 1][c] = fma(gb, dx, acc[4 * tt + 1][c]);
                             acc[4 * tt + 2][c] = fma(gb, dy, acc[4 * tt + 2][c]);
                             acc[4 * tt + 3][c] += gb;
@@ -358,14 +355,14 @@ __device__ __forceinline__ void interact_item(const InteractParams& p, double4 (
                     // the size of the rounding theta carries anyway; at most NT/2 <= 4 rotation steps from the middle trial.
                     // Needs lo >= 0 (no |.| fold inside the group): true for T >= 3 (dbie_solve rejects T < 4).
                     double sd, cd;
-                    sincos_pos(p.dlam * rr, sd, cd);
+                    sincos_pos(p.dlam * rr, tr, sd, cd);
                     const double wb[3] = {wx, wy, wz};
                     constexpr int TB = NT / 2;   // the full sincos is taken at the middle trial
 #pragma unroll
                     for (int c = 0; c < 3; ++c) {
                         const double thb = lam[TB][c] * rr;
                         double sb, cb;
-                        sincos_pos(thb, sb, cb);
+                        sincos_pos(thb, tr, sb, cb);
                         acc[TB][c] = fma(fma(thb, sb, cb), wb[c], acc[TB][c]);
                         double sn = sb, cs = cb;
 #pragma unroll
@@ -391,9 +388,9 @@ __device__ __forceinline__ void interact_item(const InteractParams& p, double4 (
                 }
 #pragma unroll
                 for (int tt = 0; tt < NT; ++tt) {
-                    acc[tt][0] = fma(kernel_n(lam[tt][0] * rr), wx, acc[tt][0]);
-                    acc[tt][1] = fma(kernel_n(lam[tt][1] * rr), wy, acc[tt][1]);
-                    acc[tt][2] = fma(kernel_n(lam[tt][2] * rr), wz, acc[tt][2]);
+                    acc[tt][0] = fma(kernel_n(lam[tt][0] * rr, tr), wx, acc[tt][0]);
+                    acc[tt][1] = fma(kernel_n(lam[tt][1] * rr, tr), wy, acc[tt][1]);
+                    acc[tt][2] = fma(kernel_n(lam[tt][2] * rr, tr), wz, acc[tt][2]);
                 }
             }
             rp += d.ncols;
@@ -409,6 +406,17 @@ __device__ __forceinline__ void interact_item(const InteractParams& p, double4 (
     }
 }
 
+// shared memory of interact64_kernel
+constexpr size_t kInteractSmem = kTrigTableBytes + sizeof(double4) * 2 * kTilePx + 64;
+
+// Every CTA copies the 4 KB angle table from global memory (L2-resident) into 8 interleaved copies at the start of
+// its dynamic shared memory; the caller's __syncthreads publishes it.  Returns the calling lane's copy.
+__device__ __forceinline__ TrigRef trig_fill(unsigned char* smem, int tid, int nthreads) {
+    TrigEntry* tab = reinterpret_cast<TrigEntry*>(smem);
+    for (int i = tid; i < kTrigEntries * kTrigCopies; i += nthreads) tab[i] = kTrigTabG[i / kTrigCopies];
+    return TrigRef{tab, (unsigned)(tid & (kTrigCopies - 1)) * (unsigned)sizeof(TrigEntry)};
+}
+
 // split of the chunk range of a launch with `nblk` position blocks (shared by the kernels and their launchers)
 __host__ __device__ inline int chunk_split(long long nblk, int target_items, int nchunks) {
     int nsplit = 1;
@@ -422,9 +430,11 @@ __host__ __device__ inline int chunk_split(long long nblk, int target_items, int
 template <int MODE, int NT, int THREADS, int MINB, int UNR>
 __global__ void __launch_bounds__(THREADS, MINB) interact64_kernel(const __grid_constant__ InteractParams p) {
     constexpr bool kGridLam = (MODE == MODE_GRID || MODE == MODE_GRID_ANALYTIC);
-    __shared__ alignas(128) double4 tile[2][kTilePx];
-    __shared__ alignas(8) uint64_t full[2];
-    __shared__ long long next_item;
+    // dynamic shared memory: [trig table, 8 copies, 32 KB][2 boundary tiles, 32 KB][mbarriers, work-item slot]
+    extern __shared__ __align__(128) unsigned char smem_raw[];
+    double4(*tile)[kTilePx] = reinterpret_cast<double4(*)[kTilePx]>(smem_raw + kTrigTableBytes);
+    uint64_t* full = reinterpret_cast<uint64_t*>(smem_raw + kTrigTableBytes + sizeof(double4) * 2 * kTilePx);
+    long long& next_item = *reinterpret_cast<long long*>(full + 2);
 
     const int tid = threadIdx.x;
     if (tid == 0) {
@@ -432,6 +442,7 @@ __global__ void __launch_bounds__(THREADS, MINB) interact64_kernel(const __grid_
         mbar_init(&full[1], 1);
         mbar_fence_init();
     }
+    const TrigRef tr = trig_fill(smem_raw, tid, THREADS);
     __syncthreads();
 
     if (blockIdx.x == 0 && tid == 0) {
@@ -463,7 +474,7 @@ __global__ void __launch_bounds__(THREADS, MINB) interact64_kernel(const __grid_
         const int c0 = (int)(((long long)sp * NCH) / nsplit);
         const int c1 = (int)(((long long)(sp + 1) * NCH) / nsplit);
         PartSink<MODE, NT> sink{p, nsplit, NCH, {0.0, 0.0, 0.0}};
-        interact_item<MODE, NT, THREADS, UNR>(p, tile, full, it, nitems, G, blk, c0, c1, sink);
+        interact_item<MODE, NT, THREADS, UNR>(p, tr, tile, full, it, nitems, G, blk, c0, c1, sink);
     }
 }
 

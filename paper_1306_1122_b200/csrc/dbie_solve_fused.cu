@@ -41,7 +41,8 @@ namespace dbie {
 constexpr int kFusedThreads = 128, kFusedMinB = 2;
 constexpr int kFusedWarps = kFusedThreads / 32;
 constexpr int kStageRow = 33;   // 32 pixels + 1 pad: the chain lanes' reads hit distinct banks
-constexpr size_t kFusedSmem = sizeof(double4) * 2 * kTilePx                          // boundary tiles
+constexpr size_t kFusedSmem = kTrigTableBytes                                        // angle table (dbie_math.cuh)
+                              + sizeof(double4) * 2 * kTilePx                        // boundary tiles
                               + sizeof(double) * kFusedWarps * 24 * kStageRow        // factor pairs of 32 pixels
                               + 64;                                                  // mbarriers, scalars
 
@@ -94,9 +95,9 @@ static __device__ bool nm_consume(const FusedParams& P, int id, const double (&S
 
 // The warp-per-point shape: warp w of the CTA owns slot grp*4 + w; lanes = 32 consecutive pixels of a row.
 template <int MODE>
-__device__ __forceinline__ void interact_item_warp(const InteractParams& p, double4 (*tile)[kTilePx], uint64_t* full,
-                                                   unsigned& it, double* stage, long long n, long long grp, int c0,
-                                                   int c1) {
+__device__ __forceinline__ void interact_item_warp(const InteractParams& p, const TrigRef& tr, double4 (*tile)[kTilePx],
+                                                   uint64_t* full, unsigned& it, double* stage, long long n,
+                                                   long long grp, int c0, int c1) {
     const int tid = threadIdx.x, lane = tid & 31, wib = tid >> 5;
     const BoundaryView& bd = p.bd;
     const long long slot0 = grp * kFusedWarps + wib;
@@ -147,10 +148,10 @@ __device__ __forceinline__ void interact_item_warp(const InteractParams& p, doub
                 if (j < d.ncols) {
                     double fa[4][3], fb[4][3];
                     if (MODE == MODE_STENCIL4) {
-                        if (small_eps) stencil4_terms<true>(rp[j], xi, xi1, cc, cc2, cc3, lam, fa, fb);
-                        else stencil4_terms<false>(rp[j], xi, xi1, cc, cc2, cc3, lam, fa, fb);
+                        if (small_eps) stencil4_terms<true>(tr, rp[j], xi, xi1, cc, cc2, cc3, lam, fa, fb);
+                        else stencil4_terms<false>(tr, rp[j], xi, xi1, cc, cc2, cc3, lam, fa, fb);
                     } else {
-                        analytic_terms(rp[j], xi, dy, cc, lam, lam2, fa, fb);
+                        analytic_terms(tr, rp[j], xi, dy, cc, lam, lam2, fa, fb);
                     }
 #pragma unroll
                     for (int kd = 0; kd < 4; ++kd)
@@ -184,8 +185,8 @@ __device__ __forceinline__ void interact_item_warp(const InteractParams& p, doub
 template <int MODE, int UNR>
 __global__ void __launch_bounds__(kFusedThreads, kFusedMinB) solve_nm_fused_kernel(const __grid_constant__ FusedParams P) {
     extern __shared__ __align__(128) unsigned char smem_raw[];
-    double4(*tile)[kTilePx] = reinterpret_cast<double4(*)[kTilePx]>(smem_raw);
-    double* stage = reinterpret_cast<double*>(smem_raw + sizeof(double4) * 2 * kTilePx);
+    double4(*tile)[kTilePx] = reinterpret_cast<double4(*)[kTilePx]>(smem_raw + kTrigTableBytes);
+    double* stage = reinterpret_cast<double*>(smem_raw + kTrigTableBytes + sizeof(double4) * 2 * kTilePx);
     uint64_t* full = reinterpret_cast<uint64_t*>(stage + kFusedWarps * 24 * kStageRow);
     long long* next_item = reinterpret_cast<long long*>(full + 2);
     int* is_last = reinterpret_cast<int*>(next_item + 1);
@@ -197,6 +198,7 @@ __global__ void __launch_bounds__(kFusedThreads, kFusedMinB) solve_nm_fused_kern
         mbar_init(&full[1], 1);
         mbar_fence_init();
     }
+    const TrigRef tr = trig_fill(smem_raw, tid, kFusedThreads);
     __syncthreads();
 
     const InteractParams& ip = P.ip;
@@ -253,7 +255,7 @@ __global__ void __launch_bounds__(kFusedThreads, kFusedMinB) solve_nm_fused_kern
                 const int c0 = (int)(((long long)sp * NCH) / nsplit);
                 const int c1 = (int)(((long long)(sp + 1) * NCH) / nsplit);
                 FusedSink sink{q, nsplit == 1, {}};
-                interact_item<MODE, 1, kFusedThreads, UNR>(q, tile, full, it, n, 1, blk, c0, c1, sink);
+                interact_item<MODE, 1, kFusedThreads, UNR>(q, tr, tile, full, it, n, 1, blk, c0, c1, sink);
                 const long long slot = blk * kFusedThreads + tid;
                 const bool live = slot < n;
                 if (nsplit > 1) {
@@ -296,7 +298,7 @@ __global__ void __launch_bounds__(kFusedThreads, kFusedMinB) solve_nm_fused_kern
                 if (w >= nwork) break;
                 const long long grp = w / NCH;
                 const int c0 = (int)(w % NCH);
-                interact_item_warp<MODE>(q, tile, full, it, stage, n, grp, c0, c0 + 1);
+                interact_item_warp<MODE>(q, tr, tile, full, it, stage, n, grp, c0, c0 + 1);
                 __threadfence();
                 __syncthreads();
                 if (tid == 0) {

@@ -1,15 +1,17 @@
-"""Generate the polynomial coefficients of the device sincos in trig_coeffs.h.
+"""Generate the polynomial coefficients and the angle table of the device sincos (trig_coeffs.h).
 
 The interaction kernel needs sin(theta) and cos(theta) for theta = lambda*r >= 0
-(Eq. 6 numerator theta*sin(theta) + cos(theta)).  After a 2-term
-Cody-Waite reduction theta = k*pi/2 + t, |t| <= pi/4, the kernel evaluates
+(Eq. 6 numerator theta*sin(theta) + cos(theta)).  fp64: after a one-step
+Cody-Waite reduction theta = k*(pi/128) + t, |t| <= pi/256, the kernel reads
+(sin, cos)(k pi/128) from a 256-entry table (one period) and evaluates
 
-    sin t = t + t*t^2 * S(t^2)          S of degree NS-1 in u = t^2
-    cos t = 1 + t^2 * C(t^2)            C of degree NC-1 in u = t^2
+    sin t = t + t*t^2 * S(t^2)          S of degree NS-1 in u = t^2   (NS = 2)
+    cos t = 1 + t^2 * C(t^2)            C of degree NC-1 in u = t^2   (NC = 3)
 
-This script computes S and C as weighted minimax polynomials (Remez exchange,
-mpmath, 60 digits), rounds them to double, reports the approximation error of
-the ROUNDED coefficients, and writes trig_coeffs.h.  Run:
+(fp32 variant: theta = k*pi/2 + t, |t| <= pi/4, no table.)  This script computes S and C as
+weighted minimax polynomials (Remez exchange, mpmath, 60 digits), rounds them to double, reports
+the approximation error of the ROUNDED coefficients, and writes trig_coeffs.h with the correctly
+rounded table.  Run:
 
     python paper_1306_1122_b200/csrc/gen_trig_coeffs.py [--check]
 
@@ -25,8 +27,15 @@ import mpmath as mp
 
 mp.mp.dps = 60
 HERE = os.path.dirname(os.path.abspath(__file__))
-A = (mp.pi / 4) * mp.mpf("1.0005")        # |t| bound with slack for the rounding of k
+TAB_N = 256                               # table entries over one period: step 2 pi / 256 = pi / 128
+A = (mp.pi / 4) * mp.mpf("1.0005")        # |t| bound with slack for the rounding of k (set per variant below)
 UA = A * A
+
+
+def set_interval(a):
+    global A, UA
+    A = a
+    UA = A * A
 
 
 def g_sin(u):
@@ -146,6 +155,7 @@ def hexbits32(f):
 def f32_header():
     """fp32 variant (dbie_eval_f32): degree-2 S and degree-3 C in u = t^2, coefficients rounded
     to float; pi/2 split into a 24-bit head and a float tail for the two-term reduction."""
+    set_interval((mp.pi / 4) * mp.mpf("1.0005"))
     S = [to_float(a) for a in remez(g_sin, 3, lambda u: u * mp.sqrt(u))]
     C = [to_float(a) for a in remez(g_cos, 4, lambda u: u)]
     es = report("sin", S, mp.sin, sin_from)
@@ -175,41 +185,52 @@ def f32_header():
 
 
 def main():
+    set_interval((mp.pi / TAB_N) * mp.mpf("1.0005"))
     out = {}
-    for ns in (5, 6):
+    for ns in (2, 3):
         c = remez(g_sin, ns, lambda u: u * mp.sqrt(u))      # error enters as t^3 * (S - g)
         cd = [to_double(a) for a in c]
         out[("S", ns)] = (cd, report("sin", cd, mp.sin, sin_from))
-    for nc in (6, 7):
+    for nc in (2, 3, 4):
         c = remez(g_cos, nc, lambda u: u)                   # error enters as t^2 * (C - g)
         cd = [to_double(a) for a in c]
         out[("C", nc)] = (cd, report("cos", cd, mp.cos, cos_from))
     for k, (cd, e) in out.items():
         print(k, "max abs approx error = %.3e (%.3f x 2^-53)" % (float(e), float(e * 2 ** 53)))
-    NS, NC = 6, 6
+    NS, NC = 2, 3
     S, C = out[("S", NS)][0], out[("C", NC)][0]
-    pio2_hi, pio2_lo = split_hi_lo(mp.pi / 2)
-    two_over_pi = float(2 / mp.pi)
+    step_hi, step_lo = split_hi_lo(2 * mp.pi / TAB_N)
+    inv_step = float(TAB_N / (2 * mp.pi))
     lines = [
         "// GENERATED by gen_trig_coeffs.py (weighted Remez, mpmath 60 digits) -- do not edit.",
-        "// sin t = t + t*t^2*S(t^2), cos t = 1 + t^2*C(t^2) on |t| <= pi/4 (1.0005 slack).",
+        "// theta = k (pi/128) + t: (sin, cos)(k pi/128) from DBIE_TRIG_TABLE (correctly rounded), and",
+        "// sin t = t + t*t^2*S(t^2), cos t = 1 + t^2*C(t^2) on |t| <= pi/256 (1.0005 slack).",
         "// approximation error of the rounded coefficients: sin %.2e, cos %.2e (absolute)."
         % (float(out[("S", NS)][1]), float(out[("C", NC)][1])),
         "#pragma once",
         "#define DBIE_TRIG_NS %d" % NS,
         "#define DBIE_TRIG_NC %d" % NC,
+        "#define DBIE_TRIG_ENTRIES %d" % TAB_N,
     ]
     for i, a in enumerate(S):
         lines.append("#define DBIE_SIN_S%d %s  /* %s */" % (i, repr(a), hexbits(a)))
     for i, a in enumerate(C):
         lines.append("#define DBIE_COS_C%d %s  /* %s */" % (i, repr(a), hexbits(a)))
     lines += [
-        "#define DBIE_TWO_OVER_PI %s  /* %s */" % (repr(two_over_pi), hexbits(two_over_pi)),
-        "#define DBIE_PIO2_HI %s  /* %s */" % (repr(pio2_hi), hexbits(pio2_hi)),
-        "#define DBIE_PIO2_LO %s  /* %s */" % (repr(pio2_lo), hexbits(pio2_lo)),
+        "#define DBIE_INV_STEP %s  /* 128/pi  %s */" % (repr(inv_step), hexbits(inv_step)),
+        "#define DBIE_STEP_HI %s  /* pi/128  %s */" % (repr(step_hi), hexbits(step_hi)),
+        "#define DBIE_STEP_LO %s  /* %s */" % (repr(step_lo), hexbits(step_lo)),
         "#define DBIE_ROUND_MAGIC 6755399441055744.0  /* 1.5 * 2^52 */",
-        "",
+        "// {sin, cos}(k pi/128), k = 0..255, each rounded to nearest",
+        "#define DBIE_TRIG_TABLE \\",
     ]
+    for k in range(TAB_N):
+        a = 2 * mp.pi * k / TAB_N
+        sv, cv = float(mp.sin(a)), float(mp.cos(a))
+        if k % (TAB_N // 4) == 0:                        # exact values at the multiples of pi/2
+            sv, cv = float(round(mp.sin(a))), float(round(mp.cos(a)))
+        lines.append("    {%s, %s}%s" % (repr(sv), repr(cv), ", \\" if k + 1 < TAB_N else ""))
+    lines.append("")
     text = "\n".join(lines)
     for name, body in (("trig_coeffs.h", text), ("trig_coeffs_f32.h", f32_header())):
         path = os.path.join(HERE, name)

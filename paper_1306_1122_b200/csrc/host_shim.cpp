@@ -8,13 +8,18 @@
 #include "dbie_math_f32.cuh"
 #include "dbie_nm.cuh"
 
+static const dbie::TrigRef kTr{dbie::kTrigTabHost, 0u};   // the same table the kernels copy into shared memory
+
 extern "C" {
 
 void shim_sincos(long n, const double* th, double* s, double* c) {
-    for (long i = 0; i < n; ++i) dbie::sincos_pos(th[i], s[i], c[i]);
+    for (long i = 0; i < n; ++i) dbie::sincos_pos(th[i], kTr, s[i], c[i]);
 }
 void shim_kernel_n(long n, const double* th, double* out) {
-    for (long i = 0; i < n; ++i) out[i] = dbie::kernel_n(th[i]);
+    for (long i = 0; i < n; ++i) out[i] = dbie::kernel_n(th[i], kTr);
+}
+void shim_kernel_n_cos(long n, const double* th, double* nv, double* cv) {
+    for (long i = 0; i < n; ++i) dbie::kernel_n_cos(th[i], kTr, nv[i], cv[i]);
 }
 void shim_rotate_small(long n, const double* s0, const double* c0, const double* eps, double* s, double* c) {
     for (long i = 0; i < n; ++i) dbie::rotate_small(s0[i], c0[i], eps[i], s[i], c[i]);
@@ -30,7 +35,7 @@ void shim_interaction(double dx, double dy, double z, const double lam[3], const
     const double y = dbie::rsqrt_full(r2);
     const double rr = r2 * y;
     const double w = (y * y) * y;
-    for (int p = 0; p < 3; ++p) out[p] = dbie::kernel_n(fabs(lam[p]) * rr) * (w * b0[p]);
+    for (int p = 0; p < 3; ++p) out[p] = dbie::kernel_n(fabs(lam[p]) * rr, kTr) * (w * b0[p]);
 }
 
 // fp32 kernel value n(theta) on the FMA-pipe polynomials (the SFU variant is device only)

@@ -79,29 +79,40 @@ def loops(body):
     return [l for l in inner if any(op.startswith("MUFU.RSQ") for _, op, _ in body[l[0]:l[1] + 1])]
 
 
-def main():
-    pats = sys.argv[1:] or ["interact"]
-    for name, body in kernels(LIB):
+def loop_table(lib: str = LIB, pats=("interact",)):
+    """[(demangled kernel name, [loop dict])] for every matching kernel; a loop dict has the instruction counts
+    by pipe and by opcode and `rsqrt`, the point-pixel distances per trip."""
+    out = []
+    for name, body in kernels(lib):
         d = demangle(name)
         if not any(p in d for p in pats):
             continue
-        ls = loops(body)
-        if not ls:
-            continue
-        print(f"== {d}")
-        for (i0, i1) in ls:
+        rows = []
+        for (i0, i1) in loops(body):
             seg = body[i0:i1 + 1]
             ops = collections.Counter(op for _, op, _ in seg)
             pipes = collections.Counter(pipe_of(op) for _, op, _ in seg)
-            rsq = sum(v for k, v in ops.items() if k.startswith("MUFU.RSQ"))
             base = collections.Counter()
             for k, v in ops.items():
                 base[k.split(".")[0]] += v
-            print(f"  loop 0x{seg[0][0]:04x}-0x{seg[-1][0]:04x}: {len(seg)} instructions, {rsq} rsqrt (point-pixel distances) per trip")
+            rows.append({"start": seg[0][0], "end": seg[-1][0], "n": len(seg), "pipes": pipes, "opcodes": base,
+                         "rsqrt": sum(v for k, v in ops.items() if k.startswith("MUFU.RSQ"))})
+        if rows:
+            out.append((d, rows))
+    return out
+
+
+def main():
+    pats = sys.argv[1:] or ["interact"]
+    for d, rows in loop_table(LIB, pats):
+        print(f"== {d}")
+        for r in rows:
+            pipes, rsq = r["pipes"], r["rsqrt"]
+            print(f"  loop 0x{r['start']:04x}-0x{r['end']:04x}: {r['n']} instructions, {rsq} rsqrt (point-pixel distances) per trip")
             print("    by pipe: " + ", ".join(f"{k} {v}" for k, v in sorted(pipes.items(), key=lambda kv: -kv[1])))
             print(f"    per distance: fp64 {pipes['fp64'] / rsq:.2f}, fp32 {pipes['fp32'] / rsq:.2f}, sfu {pipes['sfu'] / rsq:.2f}, "
-                  f"all {len(seg) / rsq:.2f}")
-            print("    opcodes: " + ", ".join(f"{k} {v}" for k, v in sorted(base.items(), key=lambda kv: -kv[1])))
+                  f"all {r['n'] / rsq:.2f}")
+            print("    opcodes: " + ", ".join(f"{k} {v}" for k, v in sorted(r["opcodes"].items(), key=lambda kv: -kv[1])))
 
 
 if __name__ == "__main__":

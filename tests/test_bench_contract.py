@@ -35,3 +35,33 @@ def test_rank_workloads_are_disjoint_and_equal_sized():
     s = bench.make_workload("cfg5")                     # config 5 defaults to a 16,384-point subset
     assert s.M == 16384 and (s.nx, s.ny) == (1024, 1024)
     assert bench.shard_info(100, 1, 4) == {"rank": 1, "world": 4, "points_per_rank": 100, "points_total": 400}
+
+
+def test_fp64_instruction_counts_match_the_built_library():
+    """bench.py's roofline multiplies interactions/s by the FP64-pipe instructions per interaction of each inner
+    loop.  Those figures are recounted here from the SASS of the library as built (cuobjdump, no GPU needed)."""
+    import importlib.util
+    sys.path.insert(0, ROOT)
+    import bench
+    from paper_1306_1122_b200 import build as b
+    b.build_lib()
+    spec = importlib.util.spec_from_file_location("sass_loops", os.path.join(b.CSRC, "sass_loops.py"))
+    sl = importlib.util.module_from_spec(spec)
+    spec.loader.exec_module(sl)
+    table = dict(sl.loop_table(b.LIB, ("interact64_kernel", "solve_nm_fused_kernel")))
+
+    def count(sub, which=0, per=1):
+        (name, rows), = [(k, v) for k, v in table.items() if sub in k]
+        r = rows[which]
+        return r["pipes"]["fp64"] / (r["rsqrt"] * per)
+
+    # kernel<MODE, NT, THREADS, MINB, UNR>: eval = mode 0 (loop 0: general lambda; loop 1: lambda = 0),
+    # Eq. 13 stencil = mode 5 (loop 0: small-angle rotation between the positions), GRID NT = 8 = mode 2,
+    # analytic gradient = mode 3, GRID on it (NT = 2) = mode 4
+    assert count("interact64_kernel<(int)0, (int)1,") == bench.FP64_INSTR["eval"]
+    assert count("interact64_kernel<(int)5, (int)1,") == bench.FP64_INSTR["nm"]
+    assert count("solve_nm_fused_kernel<(int)5,") == bench.FP64_INSTR["nm"]
+    assert count("interact64_kernel<(int)2, (int)8,", per=8) == bench.FP64_INSTR["grid"]
+    assert count("interact64_kernel<(int)3, (int)1,") == bench.FP64_INSTR["analytic"]
+    assert count("solve_nm_fused_kernel<(int)3,") == bench.FP64_INSTR["analytic"]
+    assert count("interact64_kernel<(int)4, (int)2,", per=2) == bench.FP64_INSTR["grid_analytic"]

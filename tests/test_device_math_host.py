@@ -86,7 +86,9 @@ def test_rsqrt_refinement(shim):
     shim.shim_rsqrt(C.c_long(a.size), _p(a), _p(out))
     mp.mp.dps = 50
     rel = [abs(mp.mpf(float(o)) * mp.sqrt(mp.mpf(float(x))) - 1) for x, o in zip(a, out)]
-    assert max(rel) <= 2.3e-16, float(max(rel))     # ~1 ulp
+    # the last step is y0 * (1 + e p) (two roundings: no FP64 instruction with three different register
+    # operands), so the bound is 1 ulp + the product's half ulp at worst
+    assert max(rel) <= 3.4e-16, float(max(rel))
 
 
 def test_single_interaction_term(shim):
@@ -219,13 +221,13 @@ def test_kernel_n_f32_polynomial_path(shim):
 
 
 def test_rotate_small_against_mpmath(shim):
-    """(sin, cos)(theta0 + eps) from (sin, cos)(theta0) for |eps| <= 4e-3 (the Eq. 13 stencil positions
+    """(sin, cos)(theta0 + eps) from (sin, cos)(theta0) for |eps| <= 1e-3 (the Eq. 13 stencil positions
     of one point): within 2 ulp-class of the exact values given exact inputs, and the DIFFERENCE to
     (s0, c0) - what the finite differences see - to a relative 1e-12."""
     rng = np.random.default_rng(6)
     n = 4000
     th0 = rng.uniform(0, 300, n)
-    eps = np.concatenate([rng.uniform(-4e-3, 4e-3, n // 2), rng.uniform(-1e-4, 1e-4, n // 2 - 2), [0.0, 4e-3]])
+    eps = np.concatenate([rng.uniform(-1e-3, 1e-3, n // 2), rng.uniform(-1e-4, 1e-4, n // 2 - 2), [0.0, 1e-3]])
     mp.mp.dps = 40
     s0 = np.array([float(mp.sin(mp.mpf(t))) for t in th0]); c0 = np.array([float(mp.cos(mp.mpf(t))) for t in th0])
     s = np.empty(n); c = np.empty(n)

@@ -256,7 +256,7 @@ def test_residual_matches_oracle(dbie, case):
 
 
 def test_residual_large_delta_takes_the_plain_stencil_path(dbie):
-    """MODE_STENCIL4 rotates sin/cos between the stencil positions only while lambda*delta <= 4e-3;
+    """MODE_STENCIL4 rotates sin/cos between the stencil positions only while lambda*delta <= 1e-3;
     with delta = 0.05 h and lambda up to 0.3/h (lambda*delta = 1.5e-2) most threads take the plain
     four-sincos path, the lambda = 0 points of the same warps the rotated one (divergent warps)."""
     import torch
