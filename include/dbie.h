@@ -77,6 +77,14 @@ typedef enum {
                               Needs nx, ny >= 3.  The sums then run over 3 ceil((nx-1)/2) x
                               3 ceil((ny-1)/2) weighted sources; everything else is unchanged.     */
 
+#define DBIE_EVAL_REDUCED_SINCOS 4u /* dbie_eval / dbie_eval_host (and the fixed-lambda field lines of dbie_trace,
+                              which call dbie_eval) only (reading A-12): sin and cos of the
+                              reduced argument from polynomials with one coefficient fewer each (55 instead of
+                              61 FP64 instructions per interaction).  Approximation error 3e-13 absolute on
+                              sin/cos; measured on BASELINE config 4: max |dB|/|B| = 2e-12 against the oracle
+                              (bound 1e-9).  dbie_residual, dbie_solve and the lambda-solving dbie_trace never
+                              use it: their finite differences need the full-accuracy kernel. */
+
 /* Boundary staging (Eq. 3, Eq. 16).
  * nx, ny: boundary grid, N = nx*ny, pixel k = iy*nx + ix (x fastest).
  * h: pixel size.  (x0, y0): coordinate of the CORNER of pixel (0,0); its centre is
@@ -208,6 +216,12 @@ dbie_status dbie_last_kernel_time(dbie_ctx* ctx, double* interact_ms, long long*
 /* Measured peak of the FP64 pipe: runs a register-only DFMA loop on every SM for about
  * `millis` ms and returns DFMA instructions (per lane) per second.  Synchronises. */
 dbie_status dbie_probe_dfma_rate(double millis, double* dfma_per_s, double* ffma_per_s);
+
+/* FP64 issue cost by operand pattern (the design rule of the interaction kernels):
+ * rates[0] = DFMA with two register operands and an immediate, rates[1] = DFMA reading three different,
+ * changing registers, rates[2] = DMUL, rates[3] = DFMA with one changing and two loop-invariant registers
+ * (operand-reuse cache); lane-instructions per second, about `millis` ms each.  Synchronises. */
+dbie_status dbie_probe_fp64_operands(double millis, double* rates /* host, 4 */);
 
 /* Tuning knob of dbie_eval_f32: bit p of mask set = component p takes sin/cos of the reduced
  * argument from the SFU (MUFU.SIN/COS) instead of the FMA-pipe polynomials, to balance the two

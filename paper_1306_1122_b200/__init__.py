@@ -25,6 +25,7 @@ _lib = None
 DBIE_OK, DBIE_EINVAL, DBIE_ENOMEM, DBIE_ECUDA, DBIE_ESTATE = range(5)
 DBIE_WITH_FP32 = 1
 DBIE_QUAD_9NODE = 2
+DBIE_EVAL_REDUCED_SINCOS = 4
 
 
 class DBIEError(RuntimeError):
@@ -87,6 +88,7 @@ def load() -> C.CDLL:
                                        C.POINTER(C.c_longlong)]
     lib.dbie_profile.argtypes = [_vp, C.c_int]
     lib.dbie_last_kernel_time.argtypes = [_vp, C.POINTER(C.c_double), C.POINTER(C.c_longlong)]
+    lib.dbie_probe_fp64_operands.argtypes = [C.c_double, C.POINTER(C.c_double)]
     lib.dbie_probe_dfma_rate.argtypes = [C.c_double, C.POINTER(C.c_double), C.POINTER(C.c_double)]
     lib.dbie_strerror.argtypes = [C.c_int]
     lib.dbie_strerror.restype = C.c_char_p
@@ -135,6 +137,15 @@ def probe_dfma_rate(millis: float = 200.0) -> tuple[float, float]:
     return d.value, f.value
 
 
+def probe_fp64_operands(millis: float = 100.0) -> dict:
+    """Measured FP64 lane-instruction rates by operand pattern (dbie_probe_fp64_operands)."""
+    r = (C.c_double * 4)()
+    st = load().dbie_probe_fp64_operands(float(millis), r)
+    if st != DBIE_OK:
+        raise DBIEError(st, load().dbie_last_cuda_error(None).decode())
+    return {"dfma_2reg_imm": r[0], "dfma_3reg": r[1], "dmul": r[2], "dfma_1reg_2reuse": r[3]}
+
+
 def _torch():
     import torch
     return torch
@@ -175,13 +186,14 @@ class DBIE:
     """One boundary magnetogram staged on the device (dbie_create / dbie_destroy)."""
 
     def __init__(self, nx: int, ny: int, h: float, x0: float, y0: float, bx, by, bz, fp32: bool = False,
-                 quad9: bool = False):
+                 quad9: bool = False, reduced_sincos: bool = False):
         lib = load()
         self._lib = lib
         self._h = _vp()
         self.nx, self.ny, self.h, self.x0, self.y0 = int(nx), int(ny), float(h), float(x0), float(y0)
         self.N = self.nx * self.ny
-        flags = (DBIE_WITH_FP32 if fp32 else 0) | (DBIE_QUAD_9NODE if quad9 else 0)
+        flags = ((DBIE_WITH_FP32 if fp32 else 0) | (DBIE_QUAD_9NODE if quad9 else 0)
+                 | (DBIE_EVAL_REDUCED_SINCOS if reduced_sincos else 0))
         if isinstance(bx, np.ndarray):
             b = [_host_f64(a, self.N, n) for a, n in ((bx, "bx"), (by, "by"), (bz, "bz"))]
             st = lib.dbie_create_host(C.byref(self._h), nx, ny, h, x0, y0, *[_vp(a.ctypes.data) for a in b],
@@ -194,10 +206,10 @@ class DBIE:
             raise DBIEError(st, f"{lib.dbie_strerror(st).decode()}: {lib.dbie_last_cuda_error(None).decode()}")
 
     @classmethod
-    def from_workload(cls, wl, device=None, fp32: bool = False) -> "DBIE":
+    def from_workload(cls, wl, device=None, fp32: bool = False, reduced_sincos: bool = False) -> "DBIE":
         """Stage the boundary of a workloads.Workload (host arrays) on the current device."""
         return cls(wl.nx, wl.ny, wl.h, wl.x0, wl.y0, np.asarray(wl.bx), np.asarray(wl.by),
-                   np.asarray(wl.bz), fp32=fp32, quad9=getattr(wl, "quad", 0) == 9)
+                   np.asarray(wl.bz), fp32=fp32, quad9=getattr(wl, "quad", 0) == 9, reduced_sincos=reduced_sincos)
 
     # -- lifetime
     def close(self):

@@ -38,6 +38,7 @@ struct dbie_ctx {
     int evals_on_device;                      // last call was a solve: read nevals back on demand
     int positions_per_eval;                   // evaluation positions per objective evaluation of that solve (4, or 1 analytic)
     int f32_sfu_mask;                         // dbie_eval_f32: components whose sincos use the SFU
+    bool eval_reduced;                        // DBIE_EVAL_REDUCED_SINCOS: dbie_eval uses the reduced-degree sincos
     long long batch_limit;                    // dbie_debug_set_batch_limit: points per internal batch (0: defaults)
     int profile;                              // record CUDA events around every interaction launch
     cudaEvent_t* ev;    int ev_cap, ev_n;     // event pairs of the last call (profile mode)
@@ -227,6 +228,7 @@ extern "C" dbie_status dbie_create(dbie_ctx** out, int nx, int ny, double h, dou
         }
         BoundaryView& b = ctx->bd;
         const bool q9 = (flags & DBIE_QUAD_9NODE) != 0;
+        ctx->eval_reduced = (flags & DBIE_EVAL_REDUCED_SINCOS) != 0;
         // 9-node elements: the sources are 3 Gauss abscissae per element and direction (O-6)
         const int sx = q9 ? 3 * (nx / 2) : nx, sy = q9 ? 3 * (ny / 2) : ny;
         ctx->win_nx = nx; ctx->win_ny = ny;
@@ -313,7 +315,7 @@ extern "C" dbie_status dbie_eval(dbie_ctx* ctx, long long M, const double* x, co
         p.part = ctx->part; p.cap = cap;
         prof_mark(ctx, st);
         int nparts = ctx->bd.nchunks;
-        CU(launch_interact_eval(p, ctx->sm_count, &nparts, st));
+        CU(launch_interact_eval(p, ctx->sm_count, ctx->eval_reduced, &nparts, st));
         prof_mark(ctx, st);
         CU(launch_eval_finalize(ctx->bd, nparts, off, cnt, M, z, lam, ctx->part, cap, B, st));
         launches += 2;
@@ -756,6 +758,16 @@ extern "C" dbie_status dbie_last_counters(dbie_ctx* ctx, double* interactions, l
     if (interactions) *interactions = ctx->last_interactions;
     if (launches) *launches = ctx->last_launches;
     if (objective_evals) *objective_evals = ctx->last_evals;
+    return DBIE_OK;
+}
+
+extern "C" dbie_status dbie_probe_fp64_operands(double millis, double* rates) {
+    dbie_ctx* ctx = nullptr;
+    if (!(millis > 0.0) || !rates) return DBIE_EINVAL;
+    int dev = 0, sms = 0;
+    CU(cudaGetDevice(&dev));
+    CU(cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, dev));
+    CU(launch_operand_probe(millis, sms, rates));
     return DBIE_OK;
 }
 

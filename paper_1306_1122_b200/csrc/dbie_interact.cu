@@ -150,9 +150,11 @@ static cudaError_t launch64(const InteractParams& p, int sm_count, int waves, cu
 
 // *nparts: how many chunk slots the launch fills per output (1 when every CTA covers all chunks and adds
 // them itself, else nchunks); the epilogue adds exactly that many, in chunk order.
-cudaError_t launch_interact_eval(const InteractParams& p, int sm_count, int* nparts, cudaStream_t st) {
+cudaError_t launch_interact_eval(const InteractParams& p, int sm_count, bool reduced_sincos, int* nparts,
+                                 cudaStream_t st) {
     const long long nblk = (p.count + kThreads64 - 1) / kThreads64;
     *nparts = (nblk >= 8LL * sm_count * kMinB64 || p.bd.nchunks == 1) ? 1 : p.bd.nchunks;
+    if (reduced_sincos) return launch64<MODE_EVAL_R, 1, 3>(p, sm_count, 8, st);
     return launch64<MODE_EVAL, 1, 3>(p, sm_count, 8, st);   // three pixels in flight (_work sweep: u1 .822, u2 .835, u3 .848, u4 .842)
 }
 
@@ -434,6 +436,72 @@ __global__ void __launch_bounds__(256) fma_probe_kernel(int iters, T seed, T* si
 #pragma unroll
     for (int i = 0; i < 8; ++i) s += a[i];
     if (s == (T)-1.2345) sink[0] = s;  // never true; keeps the chains alive
+}
+
+// FP64 operand patterns: KIND 0 = DFMA with two register operands and an immediate,
+// 1 = DFMA whose three operands are three different, changing registers, 2 = DMUL, 3 = DFMA with one changing and
+// two loop-invariant register operands (served by the operand-reuse cache).
+template <int KIND>
+__global__ void __launch_bounds__(256) fp64_operand_probe_kernel(int iters, double seed, double* sink) {
+    double a[8];
+#pragma unroll
+    for (int i = 0; i < 8; ++i) a[i] = seed + 1e-9 * (double)(threadIdx.x + i);
+    const double m = seed * 0.999999, c = seed * 1e-7;
+    for (int k = 0; k < iters; ++k) {
+#pragma unroll
+        for (int u = 0; u < 8; ++u) {
+#pragma unroll
+            for (int i = 0; i < 8; ++i) {
+                if (KIND == 0) a[i] = fma(a[i], m, 0.5);
+                if (KIND == 1) a[i] = fma(a[i], a[(i + 1) & 7], a[(i + 2) & 7]);
+                if (KIND == 2) a[i] = a[i] * m;
+                if (KIND == 3) a[i] = fma(a[i], m, c);
+            }
+        }
+    }
+    double s = 0;
+#pragma unroll
+    for (int i = 0; i < 8; ++i) s += a[i];
+    if (s == -1.2345) sink[0] = s;  // never true; keeps the chains alive
+}
+
+template <int KIND>
+static cudaError_t operand_probe_one(double millis, int sm_count, double* rate) {
+    double* sink = nullptr;
+    cudaError_t e = cudaMalloc(&sink, sizeof(double));
+    if (e != cudaSuccess) return e;
+    cudaEvent_t ev0, ev1;
+    cudaEventCreate(&ev0);
+    cudaEventCreate(&ev1);
+    const int grid = sm_count * 8, threads = 256;
+    int iters = 2000;
+    float ms = 0.f;
+    for (int attempt = 0; attempt < 8; ++attempt) {
+        fp64_operand_probe_kernel<KIND><<<grid, threads>>>(iters / 4 + 1, 1.0, sink);  // warm-up
+        cudaEventRecord(ev0);
+        fp64_operand_probe_kernel<KIND><<<grid, threads>>>(iters, 1.0, sink);
+        cudaEventRecord(ev1);
+        e = cudaEventSynchronize(ev1);
+        if (e != cudaSuccess) break;
+        cudaEventElapsedTime(&ms, ev0, ev1);
+        if (ms >= millis * 0.5 || iters > (1 << 28)) break;
+        const double scale = (ms > 0.01f) ? (millis / ms) * 1.1 : 16.0;
+        iters = (int)(iters * (scale > 16.0 ? 16.0 : scale)) + 1;
+    }
+    if (e == cudaSuccess) e = cudaGetLastError();
+    if (e == cudaSuccess) *rate = (double)grid * threads * 64.0 * (double)iters / (ms * 1e-3);
+    cudaEventDestroy(ev0);
+    cudaEventDestroy(ev1);
+    cudaFree(sink);
+    return e;
+}
+
+cudaError_t launch_operand_probe(double millis, int sm_count, double rates[4]) {
+    cudaError_t e = operand_probe_one<0>(millis, sm_count, &rates[0]);
+    if (e == cudaSuccess) e = operand_probe_one<1>(millis, sm_count, &rates[1]);
+    if (e == cudaSuccess) e = operand_probe_one<2>(millis, sm_count, &rates[2]);
+    if (e == cudaSuccess) e = operand_probe_one<3>(millis, sm_count, &rates[3]);
+    return e;
 }
 
 template <typename T>

@@ -37,11 +37,12 @@ namespace dbie {
 // one full sincos per component at r_i and a small-angle rotation (rotate_small) for the other three
 // positions; geometry (dx, dy, z terms) is shared where the offsets allow.  59 FP64 instructions per
 // interaction instead of 76.  Threads whose lambda delta exceeds kRotateSmallMax take the plain path.
-enum { MODE_EVAL = 0, MODE_GRID = 2, MODE_ANALYTIC = 3, MODE_GRID_ANALYTIC = 4, MODE_STENCIL4 = 5 };
+// MODE_EVAL_R: MODE_EVAL with the reduced-degree sincos of reading A-12 (DBIE_EVAL_REDUCED_SINCOS): 55 instructions.
+enum { MODE_EVAL = 0, MODE_GRID = 2, MODE_ANALYTIC = 3, MODE_GRID_ANALYTIC = 4, MODE_STENCIL4 = 5, MODE_EVAL_R = 6 };
 
 // items (threads' units of work) per slot
 __host__ __device__ inline long long items_per_slot(int mode, int G) {
-    if (mode == MODE_EVAL || mode == MODE_ANALYTIC || mode == MODE_STENCIL4) return 1;
+    if (mode == MODE_EVAL || mode == MODE_EVAL_R || mode == MODE_ANALYTIC || mode == MODE_STENCIL4) return 1;
     if (mode == MODE_GRID_ANALYTIC) return G;
     return (long long)kStencil * G;   // MODE_GRID: one item per stencil position and group of NT trials
 }
@@ -143,7 +144,7 @@ struct PartSink {
     __device__ __forceinline__ void operator()(const ItemCtx& ic, int c, const double (&acc)[NA][3]) {
         if (!ic.live) return;
         const long long slot = ic.slot;
-        if (MODE == MODE_EVAL) {
+        if (MODE == MODE_EVAL || MODE == MODE_EVAL_R) {
             if (nsplit == 1) {
                 // this CTA sees every chunk: add them here, in chunk order with the epilogue's own
                 // operation (bit-identical), and write one sum instead of nchunks partial sums
@@ -204,7 +205,7 @@ __device__ __forceinline__ void interact_item(const InteractParams& p, const Tri
     const long long jt = ic.live ? item : nitems - 1;
     int s = 0, g = 0;
     long long slot;
-    if (MODE == MODE_EVAL || MODE == MODE_ANALYTIC || MODE == MODE_STENCIL4) {
+    if (MODE == MODE_EVAL || MODE == MODE_EVAL_R || MODE == MODE_ANALYTIC || MODE == MODE_STENCIL4) {
         slot = jt;
     } else if (MODE == MODE_GRID_ANALYTIC) {
         g = (int)(jt % G);
@@ -220,7 +221,8 @@ __device__ __forceinline__ void interact_item(const InteractParams& p, const Tri
     ic.g = g;
     // the active list and the trial lambda may have been written earlier in the SAME launch by another SM
     // (fused solver): read them through L2
-    const long long id = (MODE == MODE_EVAL) ? p.slot0 + slot : (p.act ? (long long)__ldcg(p.act + slot) : slot);
+    constexpr bool kEval = (MODE == MODE_EVAL || MODE == MODE_EVAL_R);
+    const long long id = kEval ? p.slot0 + slot : (p.act ? (long long)__ldcg(p.act + slot) : slot);
     double xi = p.x[id], yi = p.y[id], zi = p.z[id];
     if (MODE == MODE_GRID) {   // Eq. 13: r_i, r_i + delta x, + delta y, + delta z
         if (s == 1) xi = __dadd_rn(xi, p.delta_abs);
@@ -298,7 +300,7 @@ __device__ __forceinline__ void interact_item(const InteractParams& p, const Tri
                 rp += d.ncols;
                 continue;
             }
-            if constexpr (MODE == MODE_EVAL) {
+            if constexpr (kEval) {
                 // lambda = 0 in all three components (the potential field, BASELINE config 1): n(0) = 1
                 // exactly, so the term is w B_p0 and the sum is bit-identical to the general loop's
                 // fma(1, w B, acc) at 16 instead of 76 FP64 instructions.  Per-thread decision.
@@ -388,9 +390,9 @@ __device__ __forceinline__ void interact_item(const InteractParams& p, const Tri
                 }
 #pragma unroll
                 for (int tt = 0; tt < NT; ++tt) {
-                    acc[tt][0] = fma(kernel_n(lam[tt][0] * rr, tr), wx, acc[tt][0]);
-                    acc[tt][1] = fma(kernel_n(lam[tt][1] * rr, tr), wy, acc[tt][1]);
-                    acc[tt][2] = fma(kernel_n(lam[tt][2] * rr, tr), wz, acc[tt][2]);
+                    acc[tt][0] = fma(kernel_n<MODE == MODE_EVAL_R>(lam[tt][0] * rr, tr), wx, acc[tt][0]);
+                    acc[tt][1] = fma(kernel_n<MODE == MODE_EVAL_R>(lam[tt][1] * rr, tr), wy, acc[tt][1]);
+                    acc[tt][2] = fma(kernel_n<MODE == MODE_EVAL_R>(lam[tt][2] * rr, tr), wz, acc[tt][2]);
                 }
             }
             rp += d.ncols;

@@ -168,7 +168,8 @@ cudaError_t launch_stage_boundary(int nx, int ny, double h, double x0, double y0
 cudaError_t launch_stage_q9(int nx, int ny, double h, double x0, double y0, const double* bx, const double* by,
                             const double* bz, int nsx, int nsy, double4* rec, double* yk, float4* rec32,
                             float* yk32, cudaStream_t st);
-cudaError_t launch_interact_eval(const InteractParams& p, int sm_count, int* nparts, cudaStream_t st);
+cudaError_t launch_interact_eval(const InteractParams& p, int sm_count, bool reduced_sincos, int* nparts,
+                                 cudaStream_t st);
 cudaError_t launch_interact_stencil(const InteractParams& p, int sm_count, cudaStream_t st);
 cudaError_t launch_interact_grid(const InteractParams& p, int sm_count, cudaStream_t st);
 cudaError_t launch_interact_analytic(const InteractParams& p, int sm_count, cudaStream_t st);
@@ -181,6 +182,7 @@ cudaError_t launch_eval_finalize_f32(const BoundaryView& bd, int nparts, long lo
                                      const float* z, const float* lam, const double* part, long long cap,
                                      float* B, cudaStream_t st);
 cudaError_t launch_probe(double millis, int sm_count, double* dfma_per_s, double* ffma_per_s);
+cudaError_t launch_operand_probe(double millis, int sm_count, double rates[4]);
 
 cudaError_t launch_solve_init(const SolveArrays& s, const NMConsts& k, long long M, long long ldo,
                               const double* x, const double* y, const double* z, double* B, double* lam,

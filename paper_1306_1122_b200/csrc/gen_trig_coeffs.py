@@ -199,6 +199,11 @@ def main():
         print(k, "max abs approx error = %.3e (%.3f x 2^-53)" % (float(e), float(e * 2 ** 53)))
     NS, NC = 2, 3
     S, C = out[("S", NS)][0], out[("C", NC)][0]
+    # eval-only reduced variant (reading A-12; DBIE_EVAL_REDUCED_SINCOS): one coefficient fewer in each
+    SR = [to_double(a) for a in remez(g_sin, 1, lambda u: u * mp.sqrt(u))]
+    ESR = report("sin", SR, mp.sin, sin_from)
+    CR, ECR = out[("C", 2)]
+    print("reduced: sin %.3e cos %.3e" % (float(ESR), float(ECR)))
     step_hi, step_lo = split_hi_lo(2 * mp.pi / TAB_N)
     inv_step = float(TAB_N / (2 * mp.pi))
     lines = [
@@ -216,6 +221,11 @@ def main():
         lines.append("#define DBIE_SIN_S%d %s  /* %s */" % (i, repr(a), hexbits(a)))
     for i, a in enumerate(C):
         lines.append("#define DBIE_COS_C%d %s  /* %s */" % (i, repr(a), hexbits(a)))
+    lines.append("// reduced variant: sin t = t + t*t^2*SR0, cos t = 1 + t^2*(CR0 + CR1 t^2); approximation error sin %.2e, cos %.2e"
+                 % (float(ESR), float(ECR)))
+    lines.append("#define DBIE_SINR_S0 %s  /* %s */" % (repr(SR[0]), hexbits(SR[0])))
+    for i, a in enumerate(CR):
+        lines.append("#define DBIE_COSR_C%d %s  /* %s */" % (i, repr(a), hexbits(a)))
     lines += [
         "#define DBIE_INV_STEP %s  /* 128/pi  %s */" % (repr(inv_step), hexbits(inv_step)),
         "#define DBIE_STEP_HI %s  /* pi/128  %s */" % (repr(step_hi), hexbits(step_hi)),

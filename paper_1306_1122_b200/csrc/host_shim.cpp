@@ -18,6 +18,9 @@ void shim_sincos(long n, const double* th, double* s, double* c) {
 void shim_kernel_n(long n, const double* th, double* out) {
     for (long i = 0; i < n; ++i) out[i] = dbie::kernel_n(th[i], kTr);
 }
+void shim_kernel_n_reduced(long n, const double* th, double* out) {   // reading A-12 (eval-only flag)
+    for (long i = 0; i < n; ++i) out[i] = dbie::kernel_n<true>(th[i], kTr);
+}
 void shim_kernel_n_cos(long n, const double* th, double* nv, double* cv) {
     for (long i = 0; i < n; ++i) dbie::kernel_n_cos(th[i], kTr, nv[i], cv[i]);
 }

@@ -71,6 +71,7 @@ def test_argument_errors_before_any_launch(lib):
     assert lib.dbie_eval(None, 1, p, p, p, p, p, None) == E
     assert lib.dbie_solve(None, 1, p, p, p, None, p, p, p, p, p, None) == E
     assert lib.dbie_probe_dfma_rate(0.0, None, None) == E
+    assert lib.dbie_probe_fp64_operands(C.c_double(0.0), None) == E
     lib.dbie_destroy(None)   # no-op
 
 

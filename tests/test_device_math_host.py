@@ -79,6 +79,57 @@ def test_kernel_n_matches_definition(shim):
     assert out[-4] == 1.0
 
 
+def test_kernel_n_reduced_sincos_error(shim):
+    """The eval-only reduced-degree variant (reading A-12; DBIE_EVAL_REDUCED_SINCOS): its error on n(theta) is the
+    sin polynomial's 3.0e-13 times theta (n = theta sin + cos), far inside what dbie_eval's 1e-9 on B allows."""
+    rng = np.random.default_rng(12)
+    th = np.concatenate([rng.uniform(0, 400, 6000), [0.0, 1e-9]])
+    out = np.empty_like(th)
+    full = np.empty_like(th)
+    shim.shim_kernel_n_reduced(C.c_long(th.size), _p(th), _p(out))
+    shim.shim_kernel_n(C.c_long(th.size), _p(th), _p(full))
+    mp.mp.dps = 40
+    worst = 0.0
+    for t, got in zip(th, out):
+        ex = mp.mpf(float(t)) * mp.sin(mp.mpf(float(t))) + mp.cos(mp.mpf(float(t)))
+        worst = max(worst, float(abs(mp.mpf(float(got)) - ex)) / (float(t) + 1.0))
+    assert 1e-14 < worst <= 3.5e-13, worst          # really the reduced polynomials, and within their bound
+    assert out[-2] == 1.0 and np.abs(out - full).max() > 0
+
+
+def test_kernel_n_cos_matches_definition(shim):
+    """kernel_n_cos (analytic-gradient mode, O-5): n(theta) as kernel_n, bit for bit, and cos(theta)."""
+    rng = np.random.default_rng(13)
+    th = rng.uniform(0, 300, 3000)
+    n = np.empty_like(th); c = np.empty_like(th); n0 = np.empty_like(th)
+    shim.shim_kernel_n_cos(C.c_long(th.size), _p(th), _p(n), _p(c))
+    shim.shim_kernel_n(C.c_long(th.size), _p(th), _p(n0))
+    assert np.array_equal(n, n0)
+    mp.mp.dps = 40
+    for t, got in zip(th, c):
+        assert abs(mp.mpf(float(got)) - mp.cos(mp.mpf(float(t)))) <= 3.5e-16 + 4e-17 * float(t)
+
+
+def test_trig_table_is_correctly_rounded():
+    """The 256-entry (sin, cos)(k pi/128) table of trig_coeffs.h: every entry is the double nearest to the exact
+    value (exact 0, +-1 at the multiples of pi/2)."""
+    import os
+    import re
+    path = os.path.join(os.path.dirname(dbuild.__file__), "csrc", "trig_coeffs.h")
+    text = open(path).read()
+    body = text[text.index("#define DBIE_TRIG_TABLE"):]
+    pairs = re.findall(r"\{([-+0-9.e]+), ([-+0-9.e]+)\}", body)
+    assert len(pairs) == 256
+    mp.mp.dps = 50
+    for k, (sv, cv) in enumerate(pairs):
+        a = 2 * mp.pi * k / 256
+        for got, ex in ((float(sv), mp.sin(a)), (float(cv), mp.cos(a))):
+            if k % 64 == 0:
+                assert got == float(round(ex))
+            else:
+                assert got == float(ex)             # mpmath -> float conversion rounds to nearest
+
+
 def test_rsqrt_refinement(shim):
     rng = np.random.default_rng(3)
     a = np.concatenate([10.0 ** rng.uniform(-6, 8, 5000), [1.0, 4.0, 2.0, 1e-30, 1e30]])

@@ -105,6 +105,32 @@ def test_eval_config4_full_size_sampled(dbie):
     assert err <= TOL_B, err
 
 
+def test_eval_reduced_sincos_flag_measured_error(dbie):
+    """DBIE_EVAL_REDUCED_SINCOS (reading A-12: eval only, never the solver): sin/cos of the reduced argument
+    with one coefficient fewer each (approximation error 3e-13).  Measured here on BASELINE configs[3]'s
+    boundary and on config 2's: B must stay within the same 1e-9 as the full kernel, the solver must be
+    untouched by the flag (bit-identical results), and the flag must really change the eval arithmetic."""
+    import torch
+    w = workloads.config4()
+    sub, _ = w.seeded_subset(1024, seed_offset=3)
+    ref = oracle.eval(sub)
+    with dbie.DBIE.from_workload(sub, reduced_sincos=True) as ctx:
+        dw = dbie.to_device(sub)
+        Br = ctx.eval(dw.x, dw.y, dw.z, dw.lam).cpu().numpy()
+    Bf = gpu_eval(dbie, sub)
+    err_r, _ = vec_relerr(Br, ref)
+    err_f, _ = vec_relerr(Bf, ref)
+    print(f"reduced sincos: max |dB|/|B| = {err_r:.2e} (full kernel: {err_f:.2e})")
+    assert err_r <= TOL_B and err_f <= TOL_B
+    assert not np.array_equal(Br, Bf)
+    w2, _ = workloads.config2().seeded_subset(64, seed_offset=11)
+    with dbie.DBIE.from_workload(w2, reduced_sincos=True) as c1, dbie.DBIE.from_workload(w2) as c0:
+        dw = dbie.to_device(w2)
+        s1, s0 = c1.solve(dw.x, dw.y, dw.z), c0.solve(dw.x, dw.y, dw.z)
+        for k in ("B", "lam", "resid", "iters", "status"):
+            assert torch.equal(s1[k], s0[k]), k
+
+
 def test_eval_edge_cases(dbie):
     import torch
     w = workloads.random_boundary(20, 12, seed=3, npts=9)
