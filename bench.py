@@ -50,7 +50,7 @@ MUFU_LANES_PER_SM = 16
 # DRAM bytes (dram__bytes_read.sum + dram__bytes_write.sum) of ONE launch of the dominant kernel, from the
 # committed `ncu --set full` captures; evidence that HBM is idle (the bound is the FP64 pipe).
 NCU_TRAFFIC = {
-    "eval": (60.2e6 + 5.8e6, "profiles/r01_ncu_full_interact64_eval_cfg4.md"),
+    "eval": (59.97e6 + 5.81e6, "profiles/r02_ncu_full_interact64_eval_cfg4.md"),
 }
 
 
@@ -329,10 +329,13 @@ def measure_f64(mode: Mode, steps: int, warmup: int, rank=0, world=1, local=0, d
         barrier()
         t0 = time.perf_counter()
         e2e_inter = 0.0
+        step_ms = []
         for k in range(steps):
+            ts = time.perf_counter()
             ctx, out = step_host()
             e2e_inter += ctx.counters()["interactions"]
             ctx.close()
+            step_ms.append((time.perf_counter() - ts) * 1e3)
         torch.cuda.synchronize()
         e2e_ms = (time.perf_counter() - t0) * 1e3
         barrier()
@@ -341,6 +344,10 @@ def measure_f64(mode: Mode, steps: int, warmup: int, rank=0, world=1, local=0, d
         d2h = (3 + 3 + 2) * wl.M * 8 + 2 * wl.M * 4 if is_solve else 3 * wl.M * 8
         e2e_line = {"value": e2e_inter / (e2e_ms * 1e-3), "unit": UNIT, "h2d_bytes_per_step": h2d,
                     "d2h_bytes_per_step": d2h, "ms_per_step": e2e_ms / steps,
+                    "ms_each_step": [round(t, 3) for t in step_ms],
+                    "ms_each_step_note": "host wall clock of every timed step on this rank (create, copies, kernels, "
+                                         "destroy); `value` uses their sum: a spread between steps is host-side jitter "
+                                         "(cudaMalloc/cudaFree, page faults of the output buffer) on a shared box",
                     "api": "dbie_create_host + dbie_solve_host" if is_solve else "dbie_create_host + dbie_eval_host"}
     if rank != 0:
         return {}

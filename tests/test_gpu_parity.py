@@ -127,7 +127,7 @@ def test_eval_reduced_sincos_flag_measured_error(dbie):
     with dbie.DBIE.from_workload(w2, reduced_sincos=True) as c1, dbie.DBIE.from_workload(w2) as c0:
         dw = dbie.to_device(w2)
         s1, s0 = c1.solve(dw.x, dw.y, dw.z), c0.solve(dw.x, dw.y, dw.z)
-        for k in ("B", "lam", "resid", "iters", "status"):
+        for k in ("B", "lam", "f", "g", "iters", "status"):
             assert torch.equal(s1[k], s0[k]), k
 
 
