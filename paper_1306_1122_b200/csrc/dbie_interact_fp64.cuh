@@ -76,9 +76,7 @@ __device__ __forceinline__ void stencil4_terms(const TrigRef& tr, const double4 
 #pragma unroll
             for (int q = 1; q < 4; ++q) {
                 const double thq = lam[c] * rs[q];
-                double sn, cs;
-                rotate_small(s0, c0, thq - th0, sn, cs);
-                nv[q][c] = fma(thq, sn, cs);
+                nv[q][c] = kernel_n_near(thq, s0, c0, thq - th0);
                 wb[q][c] = ws[q] * b0[c];
             }
         } else {
@@ -349,41 +347,45 @@ __device__ __forceinline__ void interact_item(const InteractParams& p, const Tri
                     continue;
                 }
                 if (MODE == MODE_GRID && NT > 1) {
-                    // The NT trial values of a component are equally spaced (lambda_t = lo + W t/(T-1)), so
-                    // theta advances by the same d_theta = W/(T-1) r for all three components: one full
-                    // sincos per component for the first trial, one for d_theta, and a plane rotation
-                    // (4 FP64 instructions) per further trial instead of a 17-instruction sincos.  The
-                    // rotated angle theta_0 + tt d_theta differs from fl(lambda_tt r) by a few ulp(theta),
-                    // the size of the rounding theta carries anyway; at most NT/2 <= 4 rotation steps from the middle trial.
+                    // The NT trial values of a component are equally spaced (lambda_t = lo + W t/(T-1)), so theta
+                    // advances by the same d_theta = W/(T-1) r for all three components.  With (s_j, c_j) =
+                    // (sin, cos)(j d_theta), j = 1..NT/2, formed ONCE per pixel (one full sincos, then angle doubling /
+                    // addition), and one full sincos per component at the middle trial,
+                    //   n(theta_m + j d) = s_m (theta c_j - s_j) + c_m (theta s_j + c_j),   theta = fl(lambda_t r):
+                    // 6 FP64 instructions per further trial and component instead of a 16-instruction kernel_n, every
+                    // trial independent of the others (no chained rotation).  theta_m + j d_theta differs from
+                    // fl(lambda_t r) by a few ulp(theta), the size of the rounding theta carries anyway.
                     // Needs lo >= 0 (no |.| fold inside the group): true for T >= 3 (dbie_solve rejects T < 4).
-                    double sd, cd;
-                    sincos_pos(p.dlam * rr, tr, sd, cd);
-                    const double wb[3] = {wx, wy, wz};
                     constexpr int TB = NT / 2;   // the full sincos is taken at the middle trial
+                    double sj[TB + 1], cj[TB + 1];
+                    sincos_pos(p.dlam * rr, tr, sj[1], cj[1]);
+#pragma unroll
+                    for (int j = 2; j <= TB; ++j) {
+                        if (j % 2 == 0) {   // doubling: sin 2a = 2 sin a cos a, cos 2a = 1 - 2 sin^2 a
+                            const double d2 = sj[j / 2] + sj[j / 2];
+                            sj[j] = d2 * cj[j / 2];
+                            cj[j] = fma(-d2, sj[j / 2], 1.0);
+                        } else {            // addition of one step
+                            sj[j] = fma(sj[j - 1], cj[1], cj[j - 1] * sj[1]);
+                            cj[j] = fma(cj[j - 1], cj[1], -(sj[j - 1] * sj[1]));
+                        }
+                    }
+                    const double wb[3] = {wx, wy, wz};
 #pragma unroll
                     for (int c = 0; c < 3; ++c) {
                         const double thb = lam[TB][c] * rr;
                         double sb, cb;
                         sincos_pos(thb, tr, sb, cb);
                         acc[TB][c] = fma(fma(thb, sb, cb), wb[c], acc[TB][c]);
-                        double sn = sb, cs = cb;
 #pragma unroll
-                        for (int tt = TB + 1; tt < NT; ++tt) {   // rotate by +d_theta
-                            const double s1 = fma(sn, cd, cs * sd);
-                            const double c1 = fma(cs, cd, -(sn * sd));
-                            sn = s1;
-                            cs = c1;
-                            acc[tt][c] = fma(fma(lam[tt][c] * rr, sn, cs), wb[c], acc[tt][c]);
-                        }
-                        sn = sb;
-                        cs = cb;
-#pragma unroll
-                        for (int tt = TB - 1; tt >= 0; --tt) {   // rotate by -d_theta
-                            const double s1 = fma(sn, cd, -(cs * sd));
-                            const double c1 = fma(cs, cd, sn * sd);
-                            sn = s1;
-                            cs = c1;
-                            acc[tt][c] = fma(fma(lam[tt][c] * rr, sn, cs), wb[c], acc[tt][c]);
+                        for (int tt = 0; tt < NT; ++tt) {
+                            if (tt == TB) continue;
+                            const int j = tt > TB ? tt - TB : TB - tt;
+                            const double th = lam[tt][c] * rr;
+                            // sin(+-j d) = +-s_j: the sign is an operand modifier
+                            const double pp = tt > TB ? fma(th, cj[j], -sj[j]) : fma(th, cj[j], sj[j]);
+                            const double qq = tt > TB ? fma(th, sj[j], cj[j]) : fma(th, -sj[j], cj[j]);
+                            acc[tt][c] = fma(fma(sb, pp, cb * qq), wb[c], acc[tt][c]);
                         }
                     }
                     continue;

@@ -177,16 +177,34 @@ DBIE_HD void kernel_n_cos(double th, const TrigRef& tr, double& n, double& c) {
     c = fma(e.c, cs, -(e.s * sn));
 }
 
-// (sin, cos)(theta0 + eps) from (s0, c0) = (sin, cos)(theta0) for |eps| <= 1e-3: the angle-addition
-// formulas with sin eps = eps - eps^3/6 (next term eps^5/120 <= 8e-18) and cos eps = 1 - eps^2/2 + eps^4/24
-// (next term eps^6/720 <= 1.4e-21).  10 FP64 instructions instead of the 15 of a full sincos; the
-// DIFFERENCE to (s0, c0), which is what Eq. 13's finite differences see, is formed without cancellation.
-DBIE_HD void rotate_small(double s0, double c0, double eps, double& s, double& c) {
+// (sin, cos)(eps) for |eps| <= 1e-3: sin eps = eps - eps^3/6 (next term eps^5/120 <= 8e-18), cos eps = 1 - eps^2/2 +
+// eps^4/24 (next term eps^6/720 <= 1.4e-21).  5 FP64 instructions.
+DBIE_HD void sincos_tiny(double eps, double& se, double& ce) {
     const double e2 = eps * eps;
-    const double ce = fma(e2, fma(e2, 1.0 / 24.0, -0.5), 1.0);
-    const double se = fma(eps * e2, -1.0 / 6.0, eps);
+    ce = fma(e2, fma(e2, 1.0 / 24.0, -0.5), 1.0);
+    se = fma(eps * e2, -1.0 / 6.0, eps);
+}
+
+// (sin, cos)(theta0 + eps) from (s0, c0) = (sin, cos)(theta0): the angle-addition formulas.  9 FP64 instructions
+// instead of the 15 of a full sincos; the DIFFERENCE to (s0, c0), which is what Eq. 13's finite differences see, is
+// formed without cancellation.
+DBIE_HD void rotate_small(double s0, double c0, double eps, double& s, double& c) {
+    double se, ce;
+    sincos_tiny(eps, se, ce);
     s = fma(s0, ce, c0 * se);
     c = fma(c0, ce, -(s0 * se));
+}
+
+// n(theta) = theta sin(theta) + cos(theta) at theta = theta0 + eps from (s0, c0) = (sin, cos)(theta0):
+//   n = s0 (theta cos eps - sin eps) + c0 (theta sin eps + cos eps).
+// 9 FP64 instructions (one fewer than rotate_small + the n form, and one three-register DFMA fewer); what the
+// Eq. 13 stencil uses for the three offset positions of a field point.
+DBIE_HD double kernel_n_near(double th, double s0, double c0, double eps) {
+    double se, ce;
+    sincos_tiny(eps, se, ce);
+    const double p = fma(th, ce, -se);
+    const double q = fma(th, se, ce);
+    return fma(s0, p, c0 * q);
 }
 constexpr double kRotateSmallMax = 1e-3;
 

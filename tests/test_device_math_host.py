@@ -289,3 +289,24 @@ def test_rotate_small_against_mpmath(shim):
         es, ec = S0 * mp.cos(e) + C0 * mp.sin(e), C0 * mp.cos(e) - S0 * mp.sin(e)
         assert abs(mp.mpf(float(s[i])) - es) <= 2.5e-16 and abs(mp.mpf(float(c[i])) - ec) <= 2.5e-16
     assert s[-2] == s0[-2] and c[-2] == c0[-2]                     # eps = 0 is the identity
+
+
+def test_kernel_n_near_against_mpmath(shim):
+    """n(theta0 + eps) from (sin, cos)(theta0), the form the Eq. 13 stencil uses for its three offset positions:
+    within a few ulp of theta for exact inputs, and the DIFFERENCE n(theta0 + eps) - n(theta0) - what the finite
+    differences divide by delta - to a relative 1e-11 of its own size (no cancellation between the positions)."""
+    rng = np.random.default_rng(16)
+    n = 3000
+    th0 = rng.uniform(0.5, 300, n)
+    eps = np.concatenate([rng.uniform(-1e-3, 1e-3, n // 2), rng.uniform(-1e-4, 1e-4, n // 2)])
+    mp.mp.dps = 40
+    s0 = np.array([float(mp.sin(mp.mpf(t))) for t in th0]); c0 = np.array([float(mp.cos(mp.mpf(t))) for t in th0])
+    th = th0 + eps
+    out = np.empty(n)
+    shim.shim_kernel_n_near(C.c_long(n), _p(th), _p(s0), _p(c0), _p(eps), _p(out))
+    for i in range(n):
+        e, T = mp.mpf(float(eps[i])), mp.mpf(float(th[i]))
+        S0, C0 = mp.mpf(float(s0[i])), mp.mpf(float(c0[i]))
+        S, Cc = S0 * mp.cos(e) + C0 * mp.sin(e), C0 * mp.cos(e) - S0 * mp.sin(e)    # exact rotation of the given pair
+        ex = T * S + Cc
+        assert abs(mp.mpf(float(out[i])) - ex) <= 3e-16 * (float(th[i]) + 1.0)
