@@ -179,6 +179,11 @@ def f32_header():
         "#define DBIE_F32_PIO2_HI %sf  /* %s */" % (repr(hi), hexbits32(hi)),
         "#define DBIE_F32_PIO2_LO %sf  /* %s */" % (repr(lo), hexbits32(lo)),
         "#define DBIE_F32_ROUND_MAGIC 12582912.0f  /* 1.5 * 2^23 */",
+        "// SFU path: theta = k 2 pi + t, |t| <= pi (MUFU.SIN/COS: 2^-21.4 absolute on [-pi, pi])",
+        "#define DBIE_F32_INV_TWOPI %sf  /* %s */" % (repr(to_float(1 / (2 * mp.pi))), hexbits32(to_float(1 / (2 * mp.pi)))),
+        "#define DBIE_F32_TWOPI_HI %sf  /* %s */" % (repr(to_float(2 * mp.pi)), hexbits32(to_float(2 * mp.pi))),
+        "#define DBIE_F32_TWOPI_LO %sf  /* %s */" % (repr(to_float(2 * mp.pi - mp.mpf(to_float(2 * mp.pi)))),
+                                                      hexbits32(to_float(2 * mp.pi - mp.mpf(to_float(2 * mp.pi))))),
         "",
     ]
     return "\n".join(lines)
