@@ -488,8 +488,8 @@ def measure_f32(steps: int, warmup: int, points: int = 0) -> dict:
                      "traffic": None, "traffic_source": "profiles/r01_ncu_full_interact_f32_eval_cfg4.md (that launch is split; "
                                                         "no per-launch figure)",
                      "mufu_per_interaction": MUFU_PER_INTERACTION,
-                     "note": "SFU-bound: 148 SM x 16 MUFU lanes x clocks.max.sm / 7 MUFU per interaction (the issue port, 55 "
-                             "instructions per interaction, allows 2 % more; the FP32 FMA pipe 60 % more)",
+                     "note": "SFU-bound: 148 SM x 16 MUFU lanes x clocks.max.sm / 7 MUFU per interaction (the issue port, 40 "
+                             "instructions per interaction, allows 40 % more; the FP32 FMA pipe 75 % more; profiles/r02_sass_loops.txt)",
                      "kernel_interactions_per_s": kern_ips, "kernel_ms_per_launch": kern_ms / max(kern_launches, 1),
                      "kernel_launches": kern_launches, "kernel_share_of_step": kern_ms / ms_total if ms_total else None,
                      "peak_measured_ffma_per_s": ffma_meas},
