@@ -579,6 +579,8 @@ def run_ours(args, mode: Mode) -> None:
             ls, lw = max(1, min(args.steps, 2)), max(1, min(args.warmup, 3))
             legs = {}
             legs["cfg2_nm"] = measure_f64(Mode("cfg2"), ls, lw)
+            # small-batch latency (what a line tracer calls): 48 points, the warp-per-point shape of the fused kernel
+            legs["cfg2_nm_48pts"] = measure_f64(Mode("cfg2", points=48), 5, 3)
             legs["cfg5_grid"] = measure_f64(Mode("cfg5", grid=True, points=8192), 1, 1)
             legs["cfg4_f32"] = measure_f32(ls, lw)
             legs["cfg4_f64_reduced_sincos"] = measure_f64(Mode("cfg4", reduced=True), ls, lw)

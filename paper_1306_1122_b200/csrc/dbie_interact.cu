@@ -115,7 +115,7 @@ cudaError_t launch_stage_q9(int nx, int ny, double h, double x0, double y0, cons
 }
 
 // ------------------------------------------------------------------ fp64 launchers --------
-// The kernel is dbie_interact_fp64.cuh.  Shapes measured on B200 (profiles/r01_variants.md):
+// The kernel is dbie_interact_fp64.cuh.  Shapes measured on B200 (profiles/r01_variants.md, re-checked in round 2):
 // 256 threads x 2 CTAs/SM (<= 128 registers), two pixels in flight per thread; GRID mode carries
 // 4 (else 2, else 1) trial lambda triples per thread on one geometry.
 constexpr int kThreads64 = 256, kMinB64 = 2;
@@ -169,7 +169,7 @@ cudaError_t launch_interact_analytic(const InteractParams& p, int sm_count, cuda
 }
 
 cudaError_t launch_interact_grid_analytic(const InteractParams& p, int sm_count, cudaStream_t st) {
-    // two trial triples per thread share the geometry (88 instead of 95 instructions per interaction);
+    // two trial triples per thread share the geometry (79 instead of 86 instructions per interaction);
     // 24 accumulators + 2 x 6 lambda, lambda^2: 128 threads x 2 CTAs/SM (10 % faster than x 3 at 168 registers)
     if (p.T < 2) return cudaErrorInvalidValue;
     if (p.T % 2 == 0) return launch64<MODE_GRID_ANALYTIC, 2, 1, 128, 2>(p, sm_count, 16, st);

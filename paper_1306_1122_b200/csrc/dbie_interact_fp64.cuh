@@ -10,9 +10,11 @@
 // or one stencil position with NT equally spaced trial lambda triples (GRID).  The boundary is
 // streamed through shared memory in 16 KB tiles by the TMA bulk-copy engine (cp.async.bulk +
 // mbarrier, double buffered) and every thread of the CTA reads the same pixel record as a broadcast
-// LDS.128 pair; UNR pixels are in flight per thread.  The bound is the FP64 pipe; the history of the
-// stencil launch over round 1 (14.17 -> 11.11 -> 9.04 -> 8.39 ms) is in profiles/r01_ncu_full_interact64_*_cfg2.md
-// and the shape sweep behind every THREADS x MINB x UNR choice in profiles/r01_variants.md.
+// LDS.128 pair; UNR pixels are in flight per thread.  sin/cos come from a 256-entry angle table that every CTA
+// keeps in shared memory (8 interleaved copies, dbie_math.cuh) plus short polynomials.  The bound is the FP64
+// pipe; the history of the stencil launch over round 1 (14.17 -> 11.11 -> 9.04 -> 8.39 ms) is in
+// profiles/r01_ncu_full_interact64_*_cfg2.md, the shape sweep behind the THREADS x MINB x UNR choices in
+// profiles/r01_variants.md, round 2's table kernel in profiles/r02_ncu_full_interact64_eval_cfg4.md.
 //
 // The body of one work item (a block of evaluation positions x a range of canonical chunks) is the
 // device function interact_item; what happens to a finished chunk sum is the caller's `sink`:
@@ -34,9 +36,9 @@ namespace dbie {
 // MODE_GRID_ANALYTIC: the same four sums for NT trial triples of GRID mode (item = slot * G + g).
 // MODE_STENCIL4: the Eq. 13 stencil with all 4 positions of a field point in ONE thread (item = slot).
 // The positions are delta = 1e-3 h apart, so theta_s = lambda r_s differs from theta_0 by eps <= lambda delta:
-// one full sincos per component at r_i and a small-angle rotation (rotate_small) for the other three
-// positions; geometry (dx, dy, z terms) is shared where the offsets allow.  59 FP64 instructions per
-// interaction instead of 76.  Threads whose lambda delta exceeds kRotateSmallMax take the plain path.
+// one full sincos per component at r_i and, for the other three positions, n(theta_0 + eps) from (sin, cos)(theta_0)
+// (kernel_n_near); geometry (dx, dy, z terms) is shared where the offsets allow.  52.25 FP64 instructions per
+// interaction instead of 61.  Threads whose lambda delta exceeds kRotateSmallMax take the plain path (60.5).
 // MODE_EVAL_R: MODE_EVAL with the reduced-degree sincos of reading A-12 (DBIE_EVAL_REDUCED_SINCOS): 55 instructions.
 enum { MODE_EVAL = 0, MODE_GRID = 2, MODE_ANALYTIC = 3, MODE_GRID_ANALYTIC = 4, MODE_STENCIL4 = 5, MODE_EVAL_R = 6 };
 
@@ -301,7 +303,7 @@ __device__ __forceinline__ void interact_item(const InteractParams& p, const Tri
             if constexpr (kEval) {
                 // lambda = 0 in all three components (the potential field, BASELINE config 1): n(0) = 1
                 // exactly, so the term is w B_p0 and the sum is bit-identical to the general loop's
-                // fma(1, w B, acc) at 16 instead of 76 FP64 instructions.  Per-thread decision.
+                // fma(1, w B, acc) at 15 instead of 61 FP64 instructions.  Per-thread decision.
                 if (lam_all_zero) {
 #pragma unroll 4
                     for (int j = 0; j < d.ncols; ++j) {

@@ -651,26 +651,74 @@ def test_analytic_grid_config5_large_batch_sampled(dbie):
 
 
 # ---------------------------------------------- the paper's own validation case --
-def test_lowlou_case2_figures_of_merit(dbie):
-    """PAPER.md:145-163 / Table 1: Low & Lou n = 3, m = 1, l = 0.3, Phi = 4 pi/5, 192x192 boundary
-    around the 64^3 region, "bottom boundary only".  The paper prints C_vec 0.99, C_cs 0.52,
-    E'_n 0.83, E'_m -0.53, eps 1.08 for its DBIE; with the readings of DESIGN.md section 3 (its
-    quadrature, thresholds, simplex and objective are not given) this build measures
-    C_vec 0.918, C_cs 0.25, E'_n -0.48, eps 1.40, so Table 1 is NOT reproduced and stays "parity
-    unpinned".  Gated here: the pipeline runs at the paper's size, the GPU field
-    matches the oracle on sampled points, and the figures stay where this build measured them."""
+PAPER_TABLE1 = {   # PAPER.md:145-159, Table 1 (printed values)
+    "paper: Present DBIE Method": (0.99, 0.52, 0.83, -0.53, 1.08),
+    "paper: Boundary Integral Method (no iteration)": (0.97, 0.41, -0.02, -14.0, 1.00),
+}
+
+
+def test_lowlou_case2_figures_of_merit(dbie, capsys):
+    """PAPER.md:145-163 / Table 1: Low & Lou n = 3, m = 1, l = 0.3, Phi = 4 pi/5, 192x192 boundary around the 64^3
+    region, "bottom boundary only".  Gated: the pipeline runs at the paper's size, the GPU results match the oracle
+    on sampled points (P-4), and the solved field is far more force-free than the potential field.  NOT gated: the
+    five figures of merit.  Table 1's "Present DBIE" row is not reproduced under the readings of DESIGN.md section 3
+    (parity unpinned); the table printed here (pytest -s) records what each open reading gives,
+    next to the paper's two rows, without freezing this build's own numbers into a test."""
+    import dataclasses
     import torch
     w = workloads.lowlou_case2()
-    Bex = np.array(w.extra["lowlou"].field(w.x, w.y, w.z)) * w.extra["scale"]
+    ll, scale = w.extra["lowlou"], w.extra["scale"]
+    exact = lambda wl: np.array(ll.field(wl.x, wl.y, wl.z)) * scale
+    rows = {}
+
+    def fom(name, wl, B):
+        m = workloads.figures_of_merit(exact(wl), B)
+        rows[name] = (m["C_vec"], m["C_cs"], m["E_n_prime"], m["E_m_prime"], m["eps"])
+
+    def gpu_eval_at(wl, lam):
+        with dbie.DBIE.from_workload(wl) as ctx:
+            dw = dbie.to_device(wl)
+            return ctx.eval(dw.x, dw.y, dw.z, torch.from_numpy(np.ascontiguousarray(lam)).cuda()).cpu().numpy()
+
+    def gpu_solve(wl, **kw):
+        with dbie.DBIE.from_workload(wl) as ctx:
+            dw = dbie.to_device(wl)
+            return {k: v.cpu().numpy() for k, v in ctx.solve(dw.x, dw.y, dw.z, dbie.default_opts(**kw)).items()}
+
+    # the gated part: one full-volume solve, sampled against the oracle
     (_, _, info), s = _solve_full_and_sample(dbie, w, 24, dict(analytic=1))
-    m = workloads.figures_of_merit(Bex, s["B"])
-    assert 0.88 < m["C_vec"] < 0.96 and 1.2 < m["eps"] < 1.6, m
+    fom("NM solve, defaults (analytic gradient)", w, s["B"])
+    pot = gpu_eval_at(w, np.zeros((3, w.M)))
+    fom("lambda = 0 (potential field of the window)", w, pot)
+    pot_res = None
     with dbie.DBIE.from_workload(w) as ctx:
         dw = dbie.to_device(w)
-        pot = ctx.eval(dw.x, dw.y, dw.z, torch.zeros((3, w.M), dtype=torch.float64, device="cuda")).cpu().numpy()
-    mp_ = workloads.figures_of_merit(Bex, pot)
-    assert 0.90 < mp_["C_vec"] < 0.97                      # lambda = 0 (potential) field, same window
-    assert float(np.mean(s["f"])) < 0.2                    # far more force-free than the potential field
+        pot_res = ctx.residual(dw.x, dw.y, dw.z, torch.zeros((3, w.M), dtype=torch.float64, device="cuda"),
+                               dbie.default_opts(analytic=1))["f"].cpu().numpy()
+    assert float(np.mean(s["f"])) < 0.5 * float(np.nanmean(pot_res))    # far more force-free than the potential field
+    assert float(np.mean(s["f"])) < 0.2
+
+    # the reported part: open readings, one at a time
+    al = np.abs(ll.alpha(w.x, w.y, w.z))
+    fom("lambda = the exact alpha of the model field, all three components", w, gpu_eval_at(w, np.tile(al, (3, 1))))
+    fom("NM solve, Eq. 13 finite differences", w, gpu_solve(w)["B"])
+    fom("NM solve, Phi = f only (w_g = 0)", w, gpu_solve(w, analytic=1, w_g=0.0)["B"])
+    fom("NM solve, Phi = f + 10 g", w, gpu_solve(w, analytic=1, w_g=10.0)["B"])
+    fom("NM solve, start and step 0.5 / h", w, gpu_solve(w, analytic=1, lam0=0.5, step=0.5)["B"])
+    w_half = dataclasses.replace(w, z=w.z - 0.5 * w.h)
+    fom("NM solve, layers at z = (k + 1/2) h", w_half, gpu_solve(w_half, analytic=1)["B"])
+    w9 = dataclasses.replace(w, quad=9)
+    fom("NM solve, 9-node element quadrature (O-6)", w9, gpu_solve(w9, analytic=1)["B"])
+    low = w.z <= 16.5 * w.h
+    m = workloads.figures_of_merit(exact(w)[:, low], s["B"][:, low])
+    rows["NM solve, defaults: metrics over the 16 lowest layers only"] = (m["C_vec"], m["C_cs"], m["E_n_prime"],
+                                                                         m["E_m_prime"], m["eps"])
+    with capsys.disabled():
+        print("\nLow & Lou Case II, figures of merit over the 64^3 region (C_vec, C_cs, E'_n, E'_m, eps):")
+        for name, v in list(PAPER_TABLE1.items()) + list(rows.items()):
+            print(f"  {name:68s} " + " ".join(f"{x:8.3f}" for x in v))
+    for v in rows.values():
+        assert all(np.isfinite(v))
 
 
 # ------------------------------------ 9-node element quadrature (SURVEY 8(f) f3, DESIGN.md O-6) -

@@ -754,3 +754,70 @@ def test_oracle_runs_clean_under_address_and_undefined_sanitizers(tmp_path):
                        env=dict(os.environ, ASAN_OPTIONS="detect_leaks=1", OMP_NUM_THREADS="2"))
     assert r.returncode == 0, r.stdout + r.stderr
     assert "sanitize_main ok" in r.stdout
+
+
+def test_k11_linear_force_free_field_is_recovered_with_lambda_equal_alpha():
+    """Pins the PHYSICS of Eq. 6 with lambda != 0: for a constant-alpha force-free field whose
+    boundary spectrum lies above alpha (every Fourier mode decays as exp(-sqrt(k^2 - alpha^2) z)), the boundary
+    integral with lambda_x = lambda_y = lambda_z = alpha reproduces all three components of the field above the
+    boundary, and lambda = 0 (the potential field of the same boundary) does not.  The reference is built here from
+    the textbook mode solution (Nakagawa & Raadu 1972 form, derived from B = curl curl (P z) + alpha curl (P z) with
+    (laplace + alpha^2) P = 0), checked to be force-free by finite differences, and evaluated by FFT; nothing of it
+    comes from the oracle."""
+    n, h, alpha = 512, 1.0, 0.3
+    k0, sig = 0.8, 20.0
+    c = (np.arange(n) - n // 2 + 0.5) * h                      # pixel centres, symmetric about 0
+    Y, X = np.meshgrid(c, c, indexing="ij")
+    bz0 = np.exp(-(X ** 2 + Y ** 2) / (2 * sig ** 2)) * (np.cos(k0 * X) + 0.5 * np.sin(0.9 * k0 * Y + 0.3 * k0 * X))
+    kx = 2 * np.pi * np.fft.fftfreq(n, h)
+    KY, KX = np.meshgrid(kx, kx, indexing="ij")
+    K2 = KX ** 2 + KY ** 2
+    Fz = np.fft.fft2(bz0)
+    live = np.abs(Fz) > 1e-13 * np.abs(Fz).max()
+    assert K2[live].min() > (1.2 * alpha) ** 2                 # every carried mode decays
+    K2s = np.where(K2 > 0, K2, 1.0)
+    L = np.sqrt(np.maximum(K2 - alpha ** 2, 0.0))
+    Fz = np.where(live, Fz, 0.0)
+    Fx = 1j * (alpha * KY - L * KX) / K2s * Fz
+    Fy = -1j * (alpha * KX + L * KY) / K2s * Fz
+
+    def at(z):
+        d = np.exp(-L * z)
+        return [np.real(np.fft.ifft2(F * d)) for F in (Fx, Fy, Fz)]
+
+    # the reference really is force-free with this alpha: curl B = alpha B by central differences at z = 4
+    e = 1e-3
+    Bm, B0, Bp = at(4.0 - e), at(4.0), at(4.0 + e)
+    ddz = [(p - m) / (2 * e) for p, m in zip(Bp, Bm)]
+    spec = lambda f, K: np.real(np.fft.ifft2(1j * K * np.fft.fft2(f)))
+    curl = [spec(B0[2], KY) - ddz[1], ddz[0] - spec(B0[2], KX), spec(B0[1], KX) - spec(B0[0], KY)]
+    sc = max(np.abs(b).max() for b in B0)
+    for cq, bq in zip(curl, B0):
+        assert np.abs(cq - alpha * bq).max() <= 1e-6 * sc
+
+    # boundary window: the central 256 x 256 pixels (the packet is 1e-9 of its peak at the window edge)
+    m, o = 256, (n - 256) // 2
+    win = (slice(o, o + m), slice(o, o + m))
+    B00 = at(0.0)
+    iy, ix = np.meshgrid(np.arange(o + 100, o + 156, 11), np.arange(o + 100, o + 156, 11), indexing="ij")
+    pts = []
+    ref = []
+    for z in (3.0, 6.0, 12.0):
+        Bz_ = at(z)
+        for a, b in zip(iy.ravel(), ix.ravel()):
+            pts.append((c[b], c[a], z))
+            ref.append([Bz_[0][a, b], Bz_[1][a, b], Bz_[2][a, b]])
+    pts = np.array(pts).T
+    ref = np.array(ref).T
+    w = Workload("lff_packet", m, m, h, c[o] - 0.5 * h, c[o] - 0.5 * h, B00[0][win].ravel(),
+                           B00[1][win].ravel(), B00[2][win].ravel(), pts[0].copy(), pts[1].copy(), pts[2].copy())
+    Ba = oracle.eval(w, lam=np.full((3, w.M), alpha))
+    Bp0 = oracle.eval(w, lam=np.zeros((3, w.M)))
+    scale = np.linalg.norm(ref, axis=0).max()
+    err_a = np.linalg.norm(Ba - ref, axis=0).max() / scale
+    err_0 = np.linalg.norm(Bp0 - ref, axis=0).max() / scale
+    assert err_a <= 2e-6, err_a                                # lambda = alpha: the field, to quadrature accuracy
+    assert err_0 >= 3e-2, err_0                                # lambda = 0: a different field
+    # and the sign of the sin term / of alpha matters: lambda = 2 alpha is wrong as well
+    err_2 = np.linalg.norm(oracle.eval(w, lam=np.full((3, w.M), 2 * alpha)) - ref, axis=0).max() / scale
+    assert err_2 >= 3e-2, err_2
