@@ -38,7 +38,7 @@ namespace dbie {
 // The positions are delta = 1e-3 h apart, so theta_s = lambda r_s differs from theta_0 by eps <= lambda delta:
 // one full sincos per component at r_i and, for the other three positions, n(theta_0 + eps) from (sin, cos)(theta_0)
 // (kernel_n_near); geometry (dx, dy, z terms) is shared where the offsets allow.  52.25 FP64 instructions per
-// interaction instead of 61.  Threads whose lambda delta exceeds kRotateSmallMax take the plain path (60.5).
+// interaction instead of 61.  Threads whose lambda delta exceeds kNearEpsMax take the plain path (60.5).
 // MODE_EVAL_R: MODE_EVAL with the reduced-degree sincos of reading A-12 (DBIE_EVAL_REDUCED_SINCOS): 55 instructions.
 enum { MODE_EVAL = 0, MODE_GRID = 2, MODE_ANALYTIC = 3, MODE_GRID_ANALYTIC = 4, MODE_STENCIL4 = 5, MODE_EVAL_R = 6 };
 
@@ -50,7 +50,7 @@ __host__ __device__ inline long long items_per_slot(int mode, int G) {
 }
 
 // One pixel of MODE_STENCIL4: the 4 stencil positions (x_i, x_i + delta | y, y + delta | z, z + delta share
-// dx / dy^2 + z^2 terms where they can).  FAST: one sincos per component at r_i, rotate_small for the rest.
+// dx / dy^2 + z^2 terms where they can).  FAST: one sincos per component at r_i, kernel_n_near for the rest.
 // The pixel's 12 terms are returned as factor pairs: the accumulation is acc[q][c] = fma(nv[q][c], wb[q][c], acc[q][c]),
 // in pixel order, whoever performs it (the owning thread, or a chain lane of the warp-per-point path).
 template <bool FAST>
@@ -257,7 +257,7 @@ __device__ __forceinline__ void interact_item(const InteractParams& p, const Tri
 #pragma unroll
     for (int tt = 0; tt < NA; ++tt) acc[tt][0] = acc[tt][1] = acc[tt][2] = 0.0;
     const bool lam_all_zero = (lam[0][0] == 0.0) && (lam[0][1] == 0.0) && (lam[0][2] == 0.0);   // MODE_EVAL
-    const bool small_eps = fmax(fmax(lam[0][0], lam[0][1]), lam[0][2]) * p.delta_abs <= kRotateSmallMax;
+    const bool small_eps = fmax(fmax(lam[0][0], lam[0][1]), lam[0][2]) * p.delta_abs <= kNearEpsMax;
     double lam2[NT][3];   // analytic modes: lambda^2
 #pragma unroll
     for (int tt = 0; tt < NT; ++tt)

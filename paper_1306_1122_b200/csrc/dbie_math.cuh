@@ -66,18 +66,6 @@ DBIE_HD int lo32(double v) {
 #endif
 }
 
-DBIE_HD double flip_sign_if(double v, int bit31) {  // bit31 is 0 or 0x80000000
-#if defined(__CUDA_ARCH__)
-    return __hiloint2double(__double2hiint(v) ^ bit31, __double2loint(v));
-#else
-    uint64_t b;
-    memcpy(&b, &v, 8);
-    b ^= (uint64_t)(uint32_t)bit31 << 32;
-    memcpy(&v, &b, 8);
-    return v;
-#endif
-}
-
 // Seed of 1/sqrt(a), relative error <= 2^-22 (MUFU.RSQ64H on the device).
 DBIE_HD double rsqrt_seed(double a) {
 #if defined(__CUDA_ARCH__)
@@ -185,19 +173,9 @@ DBIE_HD void sincos_tiny(double eps, double& se, double& ce) {
     se = fma(eps * e2, -1.0 / 6.0, eps);
 }
 
-// (sin, cos)(theta0 + eps) from (s0, c0) = (sin, cos)(theta0): the angle-addition formulas.  9 FP64 instructions
-// instead of the 15 of a full sincos; the DIFFERENCE to (s0, c0), which is what Eq. 13's finite differences see, is
-// formed without cancellation.
-DBIE_HD void rotate_small(double s0, double c0, double eps, double& s, double& c) {
-    double se, ce;
-    sincos_tiny(eps, se, ce);
-    s = fma(s0, ce, c0 * se);
-    c = fma(c0, ce, -(s0 * se));
-}
-
 // n(theta) = theta sin(theta) + cos(theta) at theta = theta0 + eps from (s0, c0) = (sin, cos)(theta0):
 //   n = s0 (theta cos eps - sin eps) + c0 (theta sin eps + cos eps).
-// 9 FP64 instructions (one fewer than rotate_small + the n form, and one three-register DFMA fewer); what the
+// 9 FP64 instructions instead of the 16 of a full kernel_n, formed without cancellation against n(theta0); what the
 // Eq. 13 stencil uses for the three offset positions of a field point.
 DBIE_HD double kernel_n_near(double th, double s0, double c0, double eps) {
     double se, ce;
@@ -206,7 +184,7 @@ DBIE_HD double kernel_n_near(double th, double s0, double c0, double eps) {
     const double q = fma(th, se, ce);
     return fma(s0, p, c0 * q);
 }
-constexpr double kRotateSmallMax = 1e-3;
+constexpr double kNearEpsMax = 1e-3;   // largest |lambda delta| for which the Eq. 13 stencil uses kernel_n_near
 
 // sin(theta) and cos(theta), theta >= 0: 15 FP64 instructions (stencil and GRID rotations start from these)
 DBIE_HD void sincos_pos(double th, const TrigRef& tr, double& s, double& c) {

@@ -114,7 +114,7 @@ __device__ __forceinline__ void interact_item_warp(const InteractParams& p, cons
         lam[c] = fabs(__ldcg(p.lam + c * p.ldlam + id));
         lam2[c] = lam[c] * lam[c];
     }
-    const bool small_eps = fmax(fmax(lam[0], lam[1]), lam[2]) * p.delta_abs <= kRotateSmallMax;
+    const bool small_eps = fmax(fmax(lam[0], lam[1]), lam[2]) * p.delta_abs <= kNearEpsMax;
     double* stA = stage + (size_t)wib * 24 * kStageRow;   // [12][33]
     double* stB = stA + 12 * kStageRow;
     double acc = 0.0;                                      // chain lane k < 12 owns sum k = kind*3 + component

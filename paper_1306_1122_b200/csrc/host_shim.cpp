@@ -24,9 +24,6 @@ void shim_kernel_n_reduced(long n, const double* th, double* out) {   // reading
 void shim_kernel_n_cos(long n, const double* th, double* nv, double* cv) {
     for (long i = 0; i < n; ++i) dbie::kernel_n_cos(th[i], kTr, nv[i], cv[i]);
 }
-void shim_rotate_small(long n, const double* s0, const double* c0, const double* eps, double* s, double* c) {
-    for (long i = 0; i < n; ++i) dbie::rotate_small(s0[i], c0[i], eps[i], s[i], c[i]);
-}
 void shim_kernel_n_near(long n, const double* th, const double* s0, const double* c0, const double* eps, double* out) {
     for (long i = 0; i < n; ++i) out[i] = dbie::kernel_n_near(th[i], s0[i], c0[i], eps[i]);
 }

@@ -271,26 +271,6 @@ def test_kernel_n_f32_polynomial_path(shim):
     assert worst <= 1.0, worst
 
 
-def test_rotate_small_against_mpmath(shim):
-    """(sin, cos)(theta0 + eps) from (sin, cos)(theta0) for |eps| <= 1e-3 (the Eq. 13 stencil positions
-    of one point): within 2 ulp-class of the exact values given exact inputs, and the DIFFERENCE to
-    (s0, c0) - what the finite differences see - to a relative 1e-12."""
-    rng = np.random.default_rng(6)
-    n = 4000
-    th0 = rng.uniform(0, 300, n)
-    eps = np.concatenate([rng.uniform(-1e-3, 1e-3, n // 2), rng.uniform(-1e-4, 1e-4, n // 2 - 2), [0.0, 1e-3]])
-    mp.mp.dps = 40
-    s0 = np.array([float(mp.sin(mp.mpf(t))) for t in th0]); c0 = np.array([float(mp.cos(mp.mpf(t))) for t in th0])
-    s = np.empty(n); c = np.empty(n)
-    shim.shim_rotate_small(C.c_long(n), _p(s0), _p(c0), _p(eps), _p(s), _p(c))
-    for i in range(n):
-        e = mp.mpf(float(eps[i]))
-        S0, C0 = mp.mpf(float(s0[i])), mp.mpf(float(c0[i]))       # exact rotation of the given (s0, c0)
-        es, ec = S0 * mp.cos(e) + C0 * mp.sin(e), C0 * mp.cos(e) - S0 * mp.sin(e)
-        assert abs(mp.mpf(float(s[i])) - es) <= 2.5e-16 and abs(mp.mpf(float(c[i])) - ec) <= 2.5e-16
-    assert s[-2] == s0[-2] and c[-2] == c0[-2]                     # eps = 0 is the identity
-
-
 def test_kernel_n_near_against_mpmath(shim):
     """n(theta0 + eps) from (sin, cos)(theta0), the form the Eq. 13 stencil uses for its three offset positions:
     within a few ulp of theta for exact inputs, and the DIFFERENCE n(theta0 + eps) - n(theta0) - what the finite

@@ -650,6 +650,17 @@ def test_analytic_grid_config5_large_batch_sampled(dbie):
     _solve_full_and_sample(dbie, w, 6, dict(method=1, analytic=1, n_level=3))
 
 
+def test_fp64_operand_probe_shows_the_three_register_penalty(dbie):
+    """dbie_probe_fp64_operands (the measurement behind DESIGN.md section 6): two-register FP64 instructions run at
+    the FP64 pipe's rate, a DFMA reading three different registers at about two thirds of it."""
+    r = dbie.probe_fp64_operands(30.0)
+    peak = 148 * 64 * 1.965e9
+    assert 0.5 * peak < r["dfma_2reg_imm"] < 1.05 * peak           # loose: the SM clock is the box's business
+    assert abs(r["dmul"] / r["dfma_2reg_imm"] - 1.0) < 0.05
+    assert 0.55 * r["dfma_2reg_imm"] < r["dfma_3reg"] < 0.8 * r["dfma_2reg_imm"]
+    assert r["dfma_3reg"] < r["dfma_1reg_2reuse"] <= 1.02 * r["dfma_2reg_imm"]
+
+
 # ---------------------------------------------- the paper's own validation case (SURVEY f2) --
 PAPER_TABLE1 = {   # PAPER.md:145-159, Table 1 (printed values)
     "paper: Present DBIE Method": (0.99, 0.52, 0.83, -0.53, 1.08),
