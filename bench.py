@@ -301,6 +301,7 @@ def measure_f64(mode: Mode, steps: int, warmup: int, rank=0, world=1, local=0, d
     barrier()
     ms_total = inter_total = kern_ms = 0.0
     launches = kern_launches = evals = 0
+    pass_trace = None
     for k in range(steps):
         flush_buf.zero_()                       # L2 flush, outside the event pair
         e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
@@ -316,6 +317,8 @@ def measure_f64(mode: Mode, steps: int, warmup: int, rank=0, world=1, local=0, d
         evals += c["objective_evals"]
         kern_ms += kt["interact_ms"]
         kern_launches += kt["interact_launches"]
+        if is_solve and not mode.grid and k == steps - 1:
+            pass_trace = ctx.pass_trace()
         ctx.close()
     barrier()
     clocks = sampler.stop() if sampler else None
@@ -396,6 +399,23 @@ def measure_f64(mode: Mode, steps: int, warmup: int, rank=0, world=1, local=0, d
         "peak_measured_dfma_per_s": dfma_meas, "peak_measured_ffma_per_s": ffma_meas,
         "frac_of_measured_dfma": (achieved_slots / dfma_meas) if dfma_meas else None,
     }
+    if pass_trace is not None and pass_trace["npass"] > 0:
+        # the pass timeline of the last timed solve (dbie_last_pass_trace): where the fused kernel's time goes
+        act, pms = pass_trace["active"].astype(np.float64), pass_trace["ms"]
+        per_eval = (1.0 if mode.analytic else 4.0) * wl.N
+        bins = []
+        grid_pts = SM_COUNT * 2 * 128                      # one round of the persistent grid: 296 CTAs x 128 points
+        for lo, hi, label in ((0, 512, "<= 512"), (512, 4096, "513 - 4,096"), (4096, grid_pts // 2, "4,097 - half a round"),
+                              (grid_pts // 2, grid_pts, "half a round - one round (37,888)"),
+                              (grid_pts, 2 * grid_pts, "one - two rounds"), (2 * grid_pts, 1e18, "> two rounds")):
+            m = (act > lo) & (act <= hi)
+            if m.any():
+                bins.append({"active_points": label, "passes": int(m.sum()), "ms": float(pms[m].sum()),
+                             "interactions_per_s": float(act[m].sum() * per_eval / (pms[m].sum() * 1e-3))})
+        roofline["passes"] = {"count": int(pass_trace["npass"]), "ms_total": float(pms.sum()), "by_active_points": bins,
+                              "note": "one pass = one objective evaluation of every still-active point, ended by a grid-wide "
+                                      "barrier; a work item cannot be smaller than one canonical chunk of 128 points, so passes "
+                                      "that fill less than a round of the 296 CTAs run below the inner loop's rate"}
     if operand_probe:
         roofline["fp64_operand_probe_per_s"] = operand_probe
         roofline["fp64_operand_probe_note"] = (

@@ -213,6 +213,12 @@ dbie_status dbie_last_counters(dbie_ctx* ctx, double* interactions, long long* l
 dbie_status dbie_profile(dbie_ctx* ctx, int enable);
 dbie_status dbie_last_kernel_time(dbie_ctx* ctx, double* interact_ms, long long* interact_launches);
 
+/* Profile mode, Nelder-Mead solve: the pass timeline of the LAST fused launch of the last dbie_solve call (its last
+ * batch).  active[i] = points still searching at the start of pass i, ms[i] = duration of pass i on the device
+ * (%globaltimer of CTA 0 at consecutive pass starts).  cap: capacity of the two host arrays; *npass = passes of the
+ * launch (may exceed cap; 0 if nothing was recorded).  Synchronises the device. */
+dbie_status dbie_last_pass_trace(dbie_ctx* ctx, int cap, long long* active, double* ms, int* npass);
+
 /* Measured peak of the FP64 pipe: runs a register-only DFMA loop on every SM for about
  * `millis` ms and returns DFMA instructions (per lane) per second.  Synchronises. */
 dbie_status dbie_probe_dfma_rate(double millis, double* dfma_per_s, double* ffma_per_s);
@@ -224,9 +230,10 @@ dbie_status dbie_probe_dfma_rate(double millis, double* dfma_per_s, double* ffma
 dbie_status dbie_probe_fp64_operands(double millis, double* rates /* host, 4 */);
 
 /* Tuning knob of dbie_eval_f32: bit p of mask set = component p takes sin/cos of the reduced
- * argument from the SFU (MUFU.SIN/COS) instead of the FMA-pipe polynomials, to balance the two
- * pipes.  Allowed masks: 0, 1, 3, 7 (default: all three from the SFU, the fastest measured).  Results
- * differ at the 1e-6 level between masks; all meet the 2e-4 target. */
+ * argument from the SFU (MUFU.SIN/COS after a reduction by 2 pi); bit clear = from the fp32 angle table in
+ * shared memory (the fp64 kernel's scheme in fp32, no MUFU).  Allowed masks: 0, 1, 3, 7 (default: all three
+ * from the SFU, the fastest measured: 5.6e11 interactions/s against 5.4e11 / 5.0e11 / 4.6e11 for 3 / 1 / 0).
+ * Results differ at the 1e-6 level between masks; all meet the 2e-4 target (measured 4e-5). */
 dbie_status dbie_set_f32_sfu_mask(dbie_ctx* ctx, int mask);
 
 /* Test knob: process eval / residual / solve in internal batches of at most `points` points

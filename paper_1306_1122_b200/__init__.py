@@ -88,6 +88,8 @@ def load() -> C.CDLL:
                                        C.POINTER(C.c_longlong)]
     lib.dbie_profile.argtypes = [_vp, C.c_int]
     lib.dbie_last_kernel_time.argtypes = [_vp, C.POINTER(C.c_double), C.POINTER(C.c_longlong)]
+    lib.dbie_last_pass_trace.argtypes = [_vp, C.c_int, C.POINTER(C.c_longlong), C.POINTER(C.c_double),
+                                         C.POINTER(C.c_int)]
     lib.dbie_probe_fp64_operands.argtypes = [C.c_double, C.POINTER(C.c_double)]
     lib.dbie_probe_dfma_rate.argtypes = [C.c_double, C.POINTER(C.c_double), C.POINTER(C.c_double)]
     lib.dbie_strerror.argtypes = [C.c_int]
@@ -350,6 +352,15 @@ class DBIE:
         a, b = C.c_double(), C.c_longlong()
         self._check(self._lib.dbie_last_kernel_time(self._h, C.byref(a), C.byref(b)))
         return {"interact_ms": a.value, "interact_launches": b.value}
+
+    def pass_trace(self, cap: int = 4096) -> dict:
+        """dbie_last_pass_trace (profile mode): active points and device ms of every pass of the last fused NM launch."""
+        act = (C.c_longlong * cap)()
+        ms = (C.c_double * cap)()
+        n = C.c_int()
+        self._check(self._lib.dbie_last_pass_trace(self._h, cap, act, ms, C.byref(n)))
+        k = min(n.value, cap)
+        return {"npass": n.value, "active": np.array(act[:k], dtype=np.int64), "ms": np.array(ms[:k])}
 
     def counters(self) -> dict:
         """dbie_last_counters: interactions, launches, objective evaluations of the last call."""

@@ -41,6 +41,8 @@ struct dbie_ctx {
     bool eval_reduced;                        // DBIE_EVAL_REDUCED_SINCOS: dbie_eval uses the reduced-degree sincos
     long long batch_limit;                    // dbie_debug_set_batch_limit: points per internal batch (0: defaults)
     int profile;                              // record CUDA events around every interaction launch
+    unsigned long long* pass_trace;           // profile mode: pass timeline of the last fused Nelder-Mead launch
+    int pass_trace_cap;
     cudaEvent_t* ev;    int ev_cap, ev_n;     // event pairs of the last call (profile mode)
     char err[256];
 };
@@ -136,6 +138,31 @@ extern "C" dbie_status dbie_last_kernel_time(dbie_ctx* ctx, double* interact_ms,
     return DBIE_OK;
 }
 
+extern "C" dbie_status dbie_last_pass_trace(dbie_ctx* ctx, int cap, long long* active, double* ms, int* npass) {
+    if (!ctx || cap < 0 || !npass || (cap > 0 && (!active || !ms))) return DBIE_EINVAL;
+    GUARD_DEVICE();
+    *npass = 0;
+    if (!ctx->pass_trace) return DBIE_OK;
+    CU(cudaDeviceSynchronize());
+    const int n = ctx->pass_trace_cap;
+    unsigned long long* h = (unsigned long long*)malloc(sizeof(unsigned long long) * 2 * n);
+    if (!h) return DBIE_ENOMEM;
+    const cudaError_t e = cudaMemcpy(h, ctx->pass_trace, sizeof(unsigned long long) * 2 * n, cudaMemcpyDeviceToHost);
+    if (e != cudaSuccess) { free(h); return fail_cuda(ctx, e, "dbie_last_pass_trace"); }
+    // passes are the entries before the first stamp with no active point (the stamp of the search's end)
+    int np = 0;
+    while (np < n && h[2 * np] != 0ull) ++np;
+    const bool have_end = np < n && h[2 * np + 1] != 0ull;
+    const int full = have_end ? np : (np > 0 ? np - 1 : 0);   // passes with both a start and an end stamp
+    for (int i = 0; i < full && i < cap; ++i) {
+        active[i] = (long long)h[2 * i];
+        ms[i] = (double)(h[2 * i + 3] - h[2 * i + 1]) * 1e-6;
+    }
+    *npass = full;
+    free(h);
+    return DBIE_OK;
+}
+
 extern "C" const char* dbie_strerror(dbie_status s) {
     switch (s) {
         case DBIE_OK: return "ok";
@@ -198,6 +225,7 @@ extern "C" void dbie_destroy(dbie_ctx* ctx) {
     cudaFree(ctx->state);
     cudaFree(ctx->io);
     cudaFree(ctx->trace);
+    cudaFree(ctx->pass_trace);
     cudaFree(ctx->counters);
     if (ctx->own_stream) cudaStreamDestroy(ctx->own_stream);
     for (int i = 0; i < ctx->ev_cap; ++i) cudaEventDestroy(ctx->ev[i]);
@@ -610,6 +638,17 @@ extern "C" dbie_status dbie_solve(dbie_ctx* ctx, long long M, const double* x, c
         f.work3 = ctx->counters + 8;
         f.done = done;
         f.maxpass = 4 + 5 * k.maxiter + 1;
+        if (ctx->profile) {   // diagnostic: (active points, time stamp) of every pass of this launch
+            const int need = f.maxpass + 1;
+            if (ctx->pass_trace_cap < need) {
+                cudaFree(ctx->pass_trace);
+                ctx->pass_trace = nullptr; ctx->pass_trace_cap = 0;
+                CU(cudaMalloc(&ctx->pass_trace, sizeof(unsigned long long) * 2 * need));
+                ctx->pass_trace_cap = need;
+            }
+            CU(cudaMemsetAsync(ctx->pass_trace, 0, sizeof(unsigned long long) * 2 * need, st));
+            f.trace = ctx->pass_trace; f.trace_cap = need;
+        }
         prof_mark(ctx, st);
         int nl = 0;
         CU(launch_solve_nm_fused(f, ctx->sm_count, &nl, st));

@@ -189,13 +189,15 @@ cudaError_t launch_interact_grid(const InteractParams& p, int sm_count, cudaStre
 // ------------------------------------------------------------------ fp32 eval kernel ------
 // dbie_eval_f32 (BASELINE.json config 4, fp32 leg): geometry, theta, sincos and products in fp32;
 // a row segment (<= 512 pixels) is summed in fp32, row sums are carried in fp64.
-// SFU_MASK bit p set: component p takes sin/cos of the reduced argument from MUFU.SIN/COS instead
-// of the FMA-pipe polynomials, to balance the FP32 and SFU pipes (SURVEY 8(d) "fp32 variant").
+// SFU_MASK bit p set: component p takes sin/cos of the reduced argument from MUFU.SIN/COS, else from the
+// angle table in shared memory (dbie_math_f32.cuh), to balance the SFU against the issue port (SURVEY 8(d)
+// "fp32 variant").  Shared memory (dynamic): [fp32 angle table, 16 copies, 32 KB][2 tiles, 16 KB][mbarriers].
 template <int R, int THREADS, int MINB, int SFU_MASK>
 __global__ void __launch_bounds__(THREADS, MINB) interact_f32_kernel(const __grid_constant__ InteractParamsF32 p) {
     constexpr int SPB = THREADS * R;
-    __shared__ alignas(128) float4 tile[2][kTilePx];
-    __shared__ alignas(8) uint64_t full[2];
+    extern __shared__ __align__(128) unsigned char smem_raw[];
+    float4(*tile)[kTilePx] = reinterpret_cast<float4(*)[kTilePx]>(smem_raw + kTrigTableBytesF);
+    uint64_t* full = reinterpret_cast<uint64_t*>(smem_raw + kTrigTableBytesF + sizeof(float4) * 2 * kTilePx);
 
     const int tid = threadIdx.x;
     if (tid == 0) {
@@ -203,6 +205,11 @@ __global__ void __launch_bounds__(THREADS, MINB) interact_f32_kernel(const __gri
         mbar_init(&full[1], 1);
         mbar_fence_init();
     }
+    TrigEntryF* tab = reinterpret_cast<TrigEntryF*>(smem_raw);
+    if (SFU_MASK != 7) {   // some component reads the table
+        for (int i = tid; i < DBIE_TRIG_ENTRIES * kTrigCopiesF; i += THREADS) tab[i] = kTrigTabGF[i / kTrigCopiesF];
+    }
+    const TrigRefF tr{tab, (unsigned)(tid & (kTrigCopiesF - 1)) * (unsigned)sizeof(TrigEntryF)};
     __syncthreads();
 
     const long long count = p.count;
@@ -277,9 +284,9 @@ __global__ void __launch_bounds__(THREADS, MINB) interact_f32_kernel(const __gri
                         const float y = rsqrt_f32(r2);
                         const float rr = r2 * y;
                         const float wgt = (y * y) * y;
-                        a32[r][0] = fmaf(kernel_n_f32<(SFU_MASK & 1) != 0>(lam[r][0] * rr), wgt * px.y, a32[r][0]);
-                        a32[r][1] = fmaf(kernel_n_f32<(SFU_MASK & 2) != 0>(lam[r][1] * rr), wgt * px.z, a32[r][1]);
-                        a32[r][2] = fmaf(kernel_n_f32<(SFU_MASK & 4) != 0>(lam[r][2] * rr), wgt * px.w, a32[r][2]);
+                        a32[r][0] = fmaf(kernel_n_f32<(SFU_MASK & 1) != 0>(lam[r][0] * rr, tr), wgt * px.y, a32[r][0]);
+                        a32[r][1] = fmaf(kernel_n_f32<(SFU_MASK & 2) != 0>(lam[r][1] * rr, tr), wgt * px.z, a32[r][1]);
+                        a32[r][2] = fmaf(kernel_n_f32<(SFU_MASK & 4) != 0>(lam[r][2] * rr, tr), wgt * px.w, a32[r][2]);
                     }
                 }
 #pragma unroll
@@ -324,7 +331,11 @@ constexpr int kF32R = 4, kF32Threads = 128, kF32MinB = 4;
 
 template <int MASK>
 static cudaError_t launch_f32_variant(const InteractParamsF32& q, unsigned grid, cudaStream_t st) {
-    interact_f32_kernel<kF32R, kF32Threads, kF32MinB, MASK><<<grid, kF32Threads, 0, st>>>(q);
+    auto kern = interact_f32_kernel<kF32R, kF32Threads, kF32MinB, MASK>;
+    constexpr size_t smem = kTrigTableBytesF + sizeof(float4) * 2 * kTilePx + 64;
+    cudaError_t e = cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
+    if (e != cudaSuccess) return e;
+    kern<<<grid, kF32Threads, smem, st>>>(q);
     return cudaGetLastError();
 }
 

@@ -131,6 +131,8 @@ struct FusedParams {
     unsigned* done;             // [cap/4 + 2] arrivals per point block (thread mode) / point group (warp mode)
     int maxpass;
     int warp_items_max;         // warp-per-point path when ceil(n/4) * nchunks <= this
+    unsigned long long* trace;  // profile mode: [2*(trace_cap)] (active points, %globaltimer ns) at the start of every
+    int trace_cap;              //   pass and at the end of the search; nullptr otherwise
 };
 
 struct GridArrays {             // per-point GRID state (O-4), structure-of-arrays by point id

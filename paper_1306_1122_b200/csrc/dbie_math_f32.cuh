@@ -3,17 +3,20 @@
 //   geometry  r^2 -> 1/r (MUFU.RSQ, 2^-22), r, 1/r^3
 //   kernel    n(theta) = theta sin(theta) + cos(theta), theta = |lambda| r >= 0
 // Two ways to get (sin, cos), chosen per component at compile time:
-//   POLY: two-term Cody-Waite reduction by pi/2 (exact first step while k < 2^7 ... see below)
-//         + minimax polynomials on the FMA pipe (trig_coeffs_f32.h);
 //   SFU : two-term reduction by 2 pi, then MUFU.SIN / MUFU.COS of the REDUCED argument (|t| <= pi,
 //         where their absolute error is 2^-21.4), so the error does not grow with theta and no quadrant
-//         logic is needed.
-// __host__ __device__ so the host shim can check POLY against mpmath (the SFU path is device only).
+//         logic is needed: 10 FP32-pipe instructions + 2 MUFU per component;
+//   TAB : the fp64 kernel's scheme in fp32 — theta = k pi/128 + t, (sin, cos)(k pi/128) from the 256-entry table
+//         (float copy, 16 interleaved copies in shared memory so that the LDS.64 of a half-warp never conflicts),
+//         sin t = t - t^3/6, cos t = 1 - t^2/2 on |t| <= pi/256: 15 FP32-pipe instructions, no MUFU.
+// Mixing them balances the SFU (16 lanes/clk/SM) against the issue port.
+// __host__ __device__ so the host shim can check TAB against mpmath (the SFU path is device only).
 #pragma once
 #include <math.h>
 #include <stdint.h>
 #include <string.h>
 
+#include "trig_coeffs.h"
 #include "trig_coeffs_f32.h"
 
 #if defined(__CUDACC__)
@@ -53,37 +56,38 @@ DBIE_HD32 float rsqrt_f32(float a) {
 #endif
 }
 
-// theta = k pi/2 + t.  k = rint(theta 2/pi) through the magic-number sum (its low mantissa
-// bits are k, no F2I).  fma(-k, PIO2_HI, theta) is exact: both are multiples of 2^-23 and the
-// difference is below 1 (theta < 2^16 keeps k's product within the FMA's exact range).
-DBIE_HD32 float reduce_pio2_f32(float th, int& q) {
-    const float kf = fmaf(th, DBIE_F32_TWO_OVER_PI, DBIE_F32_ROUND_MAGIC);
-    q = f32_bits(kf);
-    const float kd = kf - DBIE_F32_ROUND_MAGIC;
-    float t = fmaf(-kd, DBIE_F32_PIO2_HI, th);
-    t = fmaf(-kd, DBIE_F32_PIO2_LO, t);
-    return t;
-}
+struct TrigEntryF {
+    float s, c;
+};
+constexpr int kTrigCopiesF = 16;
+constexpr int kTrigTableBytesF = DBIE_TRIG_ENTRIES * kTrigCopiesF * (int)sizeof(TrigEntryF);   // 32 KB
+#if !defined(__CUDA_ARCH__)
+static const TrigEntryF kTrigTabHostF[DBIE_TRIG_ENTRIES] = {DBIE_TRIG_TABLE};   // the fp64 table, rounded to float
+#endif
+#if defined(__CUDACC__)
+static __device__ const TrigEntryF kTrigTabGF[DBIE_TRIG_ENTRIES] = {DBIE_TRIG_TABLE};
+#endif
+struct TrigRefF {
+    const TrigEntryF* e;   // host: the table; device: the CTA's shared-memory table (copy 0)
+    unsigned lane_off;     // device: byte offset of this lane's copy, (lane & 15) * 8
+};
 
-DBIE_HD32 void sincos_reduced_f32(float t, float& sn, float& cs) {
-    const float u = t * t;
-    float s = DBIE_F32_SIN_S2;
-    s = fmaf(s, u, DBIE_F32_SIN_S1);
-    s = fmaf(s, u, DBIE_F32_SIN_S0);
-    float c = DBIE_F32_COS_C3;
-    c = fmaf(c, u, DBIE_F32_COS_C2);
-    c = fmaf(c, u, DBIE_F32_COS_C1);
-    c = fmaf(c, u, DBIE_F32_COS_C0);
-    sn = fmaf(t * u, s, t);
-    cs = fmaf(u, c, 1.0f);
+DBIE_HD32 TrigEntryF trig_entry_f32(const TrigRefF& tr, int k) {
+#if defined(__CUDA_ARCH__)
+    const unsigned off = (((unsigned)k << 7) & (unsigned)((DBIE_TRIG_ENTRIES - 1) << 7)) | tr.lane_off;
+    const float2 v = *reinterpret_cast<const float2*>(reinterpret_cast<const unsigned char*>(tr.e) + off);   // LDS.64
+    return TrigEntryF{v.x, v.y};
+#else
+    return tr.e[k & (DBIE_TRIG_ENTRIES - 1)];
+#endif
 }
 
 template <bool SFU>
-DBIE_HD32 float kernel_n_f32(float th) {
+DBIE_HD32 float kernel_n_f32(float th, const TrigRefF& tr) {
 #if defined(__CUDA_ARCH__)
     if (SFU) {
         // theta = k 2 pi + t, |t| <= pi, where MUFU.SIN / MUFU.COS are good to 2^-21.4 absolute: no quadrant
-        // logic at all, n = theta sin t + cos t.  7 FP32-pipe instructions + 2 MUFU per component.
+        // logic at all, n = theta sin t + cos t.
         const float kf = fmaf(th, DBIE_F32_INV_TWOPI, DBIE_F32_ROUND_MAGIC);
         const float kd = kf - DBIE_F32_ROUND_MAGIC;
         float t = fmaf(-kd, DBIE_F32_TWOPI_HI, th);
@@ -91,16 +95,19 @@ DBIE_HD32 float kernel_n_f32(float th) {
         return fmaf(th, __sinf(t), __cosf(t));
     }
 #endif
-    int q;
-    const float t = reduce_pio2_f32(th, q);
-    float sn, cs;
-    sincos_reduced_f32(t, sn, cs);
-    // both quadrant forms, one selected (as in the fp64 kernel_n): the kernel is issue-bound, and this
-    // trades one FSEL + two LOP3/SHF per component for one FFMA
-    const float ne = fmaf(th, sn, cs);
-    const float no = fmaf(th, cs, -sn);
-    const float n = (q & 1) ? no : ne;
-    return f32_from_bits(f32_bits(n) ^ ((q << 30) & (int)0x80000000));
+    // theta = k pi/128 + t: k from the low mantissa bits of the magic-number sum (no F2I), two-term Cody-Waite
+    const float kf = fmaf(th, DBIE_F32_INV_STEP, DBIE_F32_ROUND_MAGIC);
+    const int k = f32_bits(kf);
+    const float kd = kf - DBIE_F32_ROUND_MAGIC;
+    float t = fmaf(-kd, DBIE_F32_STEP_HI, th);
+    t = fmaf(-kd, DBIE_F32_STEP_LO, t);
+    const TrigEntryF e = trig_entry_f32(tr, k);
+    const float u = t * t;
+    const float sn = fmaf(t * u, -1.0f / 6.0f, t);
+    const float cs = fmaf(u, -0.5f, 1.0f);
+    const float a = fmaf(th, e.s, e.c);
+    const float b = fmaf(th, e.c, -e.s);
+    return fmaf(cs, a, sn * b);
 }
 
 }  // namespace dbie

@@ -207,6 +207,12 @@ __global__ void __launch_bounds__(kFusedThreads, kFusedMinB) solve_nm_fused_kern
     for (int pass = 0; pass < P.maxpass; ++pass) {
         const int cur = pass & 1, r0 = pass % 3, r1 = (pass + 1) % 3, r2 = (pass + 2) % 3;
         const long long n = (long long)*(volatile const unsigned*)(P.nact3 + r0);
+        if (P.trace && blockIdx.x == 0 && tid == 0 && pass < P.trace_cap) {   // diagnostic (dbie_profile): pass timeline
+            unsigned long long now;
+            asm volatile("mov.u64 %0, %%globaltimer;" : "=l"(now));
+            P.trace[2 * pass] = (unsigned long long)n;
+            P.trace[2 * pass + 1] = now;
+        }
         if (n == 0) break;   // the same value in every CTA: nobody writes slot r0 during this pass
         if (blockIdx.x == 0 && tid == 0) {
             P.nact3[r2] = 0u;

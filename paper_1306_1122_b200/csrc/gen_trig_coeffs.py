@@ -8,7 +8,7 @@ Cody-Waite reduction theta = k*(pi/128) + t, |t| <= pi/256, the kernel reads
     sin t = t + t*t^2 * S(t^2)          S of degree NS-1 in u = t^2   (NS = 2)
     cos t = 1 + t^2 * C(t^2)            C of degree NC-1 in u = t^2   (NC = 3)
 
-(fp32 variant: theta = k*pi/2 + t, |t| <= pi/4, no table.)  This script computes S and C as
+(fp32 variant: the same table rounded to float with two-term polynomials, or MUFU.SIN/COS after a reduction by 2 pi.)  This script computes S and C as
 weighted minimax polynomials (Remez exchange, mpmath, 60 digits), rounds them to double, reports
 the approximation error of the ROUNDED coefficients, and writes trig_coeffs.h with the correctly
 rounded table.  Run:
@@ -153,37 +153,25 @@ def hexbits32(f):
 
 
 def f32_header():
-    """fp32 variant (dbie_eval_f32): degree-2 S and degree-3 C in u = t^2, coefficients rounded
-    to float; pi/2 split into a 24-bit head and a float tail for the two-term reduction."""
-    set_interval((mp.pi / 4) * mp.mpf("1.0005"))
-    S = [to_float(a) for a in remez(g_sin, 3, lambda u: u * mp.sqrt(u))]
-    C = [to_float(a) for a in remez(g_cos, 4, lambda u: u)]
-    es = report("sin", S, mp.sin, sin_from)
-    ec = report("cos", C, mp.cos, cos_from)
-    hi = to_float(mp.pi / 2)
-    lo = to_float(mp.pi / 2 - mp.mpf(hi))
+    """fp32 variant (dbie_eval_f32): reduction constants of its two sincos paths.  The table path uses the fp64
+    header's DBIE_TRIG_TABLE rounded to float, with sin t = t - t^3/6, cos t = 1 - t^2/2 on |t| <= pi/256."""
+    step = 2 * mp.pi / TAB_N
+    shi = to_float(step)
+    slo = to_float(step - mp.mpf(shi))
+    tp = to_float(2 * mp.pi)
     lines = [
-        "// GENERATED by gen_trig_coeffs.py (weighted Remez, mpmath 60 digits) -- do not edit.",
-        "// fp32: sin t = t + t*t^2*S(t^2), cos t = 1 + t^2*C(t^2) on |t| <= pi/4 (1.0005 slack).",
-        "// approximation error of the rounded coefficients: sin %.2e, cos %.2e (absolute)."
-        % (float(es), float(ec)),
+        "// GENERATED by gen_trig_coeffs.py -- do not edit.",
         "#pragma once",
-    ]
-    for i, a in enumerate(S):
-        lines.append("#define DBIE_F32_SIN_S%d %sf  /* %s */" % (i, repr(a), hexbits32(a)))
-    for i, a in enumerate(C):
-        lines.append("#define DBIE_F32_COS_C%d %sf  /* %s */" % (i, repr(a), hexbits32(a)))
-    t = to_float(2 / mp.pi)
-    lines += [
-        "#define DBIE_F32_TWO_OVER_PI %sf  /* %s */" % (repr(t), hexbits32(t)),
-        "#define DBIE_F32_PIO2_HI %sf  /* %s */" % (repr(hi), hexbits32(hi)),
-        "#define DBIE_F32_PIO2_LO %sf  /* %s */" % (repr(lo), hexbits32(lo)),
         "#define DBIE_F32_ROUND_MAGIC 12582912.0f  /* 1.5 * 2^23 */",
+        "// table path: theta = k (pi/128) + t, |t| <= pi/256; truncation of sin t = t - t^3/6: 2.3e-12, of cos t = 1 - t^2/2: 9.5e-10",
+        "#define DBIE_F32_INV_STEP %sf  /* 128/pi  %s */" % (repr(to_float(1 / step)), hexbits32(to_float(1 / step))),
+        "#define DBIE_F32_STEP_HI %sf  /* pi/128  %s */" % (repr(shi), hexbits32(shi)),
+        "#define DBIE_F32_STEP_LO %sf  /* %s */" % (repr(slo), hexbits32(slo)),
         "// SFU path: theta = k 2 pi + t, |t| <= pi (MUFU.SIN/COS: 2^-21.4 absolute on [-pi, pi])",
         "#define DBIE_F32_INV_TWOPI %sf  /* %s */" % (repr(to_float(1 / (2 * mp.pi))), hexbits32(to_float(1 / (2 * mp.pi)))),
-        "#define DBIE_F32_TWOPI_HI %sf  /* %s */" % (repr(to_float(2 * mp.pi)), hexbits32(to_float(2 * mp.pi))),
-        "#define DBIE_F32_TWOPI_LO %sf  /* %s */" % (repr(to_float(2 * mp.pi - mp.mpf(to_float(2 * mp.pi)))),
-                                                      hexbits32(to_float(2 * mp.pi - mp.mpf(to_float(2 * mp.pi))))),
+        "#define DBIE_F32_TWOPI_HI %sf  /* %s */" % (repr(tp), hexbits32(tp)),
+        "#define DBIE_F32_TWOPI_LO %sf  /* %s */" % (repr(to_float(2 * mp.pi - mp.mpf(tp))),
+                                                      hexbits32(to_float(2 * mp.pi - mp.mpf(tp)))),
         "",
     ]
     return "\n".join(lines)

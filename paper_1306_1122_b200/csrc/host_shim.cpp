@@ -41,9 +41,10 @@ void shim_interaction(double dx, double dy, double z, const double lam[3], const
     for (int p = 0; p < 3; ++p) out[p] = dbie::kernel_n(fabs(lam[p]) * rr, kTr) * (w * b0[p]);
 }
 
-// fp32 kernel value n(theta) on the FMA-pipe polynomials (the SFU variant is device only)
+// fp32 kernel value n(theta) on the table path (the SFU variant is device only)
 void shim_kernel_n_f32(long n, const float* th, float* out) {
-    for (long i = 0; i < n; ++i) out[i] = dbie::kernel_n_f32<false>(th[i]);
+    static const dbie::TrigRefF trf{dbie::kTrigTabHostF, 0u};
+    for (long i = 0; i < n; ++i) out[i] = dbie::kernel_n_f32<false>(th[i], trf);
 }
 
 typedef double (*shim_objective)(const double*);

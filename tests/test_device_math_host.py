@@ -251,8 +251,8 @@ def test_nm_maxiter_and_shrink_paths(shim):
     assert np.array_equal(mine["simplex"][0], res.x)
 
 
-def test_kernel_n_f32_polynomial_path(shim):
-    """fp32 n(theta) = theta sin theta + cos theta of dbie_math_f32.cuh (FMA-pipe path) against
+def test_kernel_n_f32_table_path(shim):
+    """fp32 n(theta) = theta sin theta + cos theta of dbie_math_f32.cuh (angle-table path, no MUFU) against
     mpmath at the float inputs: |error| <= 4 ulp_f32(theta) + 2e-7 for theta up to 400 rad
     (config 4 reaches ~155).  The dominant term is theta * (error of sin) ~ theta * 6e-8."""
     rng = np.random.default_rng(5)

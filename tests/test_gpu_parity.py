@@ -950,3 +950,22 @@ def test_trace_analytic_gradient_and_options(dbie):
         for bad in (dict(ds=0.0), dict(direction=0), dict(max_steps=-1), dict(z_min=2.0, z_max=1.0)):
             with pytest.raises(dbie.DBIEError):
                 ctx.trace(t(seeds[0]), t(seeds[1]), t(seeds[2]), dbie.default_trace_opts(**bad))
+
+
+def test_pass_trace_of_the_fused_solve(dbie):
+    """dbie_last_pass_trace (profile mode): one entry per pass of the fused Nelder-Mead launch; the active counts
+    start at M, never grow, and their sum is the number of objective evaluations the counters report."""
+    w, _ = workloads.config2().seeded_subset(3000, seed_offset=5)
+    with dbie.DBIE.from_workload(w) as ctx:
+        dw = dbie.to_device(w)
+        assert ctx.pass_trace()["npass"] == 0                  # nothing recorded without profile mode
+        ctx.solve(dw.x, dw.y, dw.z)
+        assert ctx.pass_trace()["npass"] == 0
+        ctx.profile(True)
+        s = ctx.solve(dw.x, dw.y, dw.z)
+        t = ctx.pass_trace()
+        c = ctx.counters()
+    assert t["npass"] == len(t["active"]) > 50
+    assert t["active"][0] == w.M and np.all(np.diff(t["active"]) <= 0) and t["active"][-1] > 0
+    assert int(t["active"].sum()) == c["objective_evals"]
+    assert np.all(t["ms"] > 0) and t["ms"].sum() < 1e4
