@@ -195,6 +195,9 @@ def cpu_baseline(wl, mode: Mode, target_s: float = 15.0) -> dict:
             "cpu": cpu_model(),
             "sample": f"oracle.{kind} on {r['points']} seeded points of {wl.name} "
                       f"({r['interactions']:.3e} interactions in {r['seconds']:.1f} s)",
+            "speedup_over_one_core": (r["interactions"] / r["seconds"]) / (r1["interactions"] / r1["seconds"]),
+            "speedup_note": "all-threads rate / one-thread rate: well below `cores` when the box exposes more cores than "
+                            "its CPU quota delivers",
             "one_core": {"value": r1["interactions"] / r1["seconds"], "cores": 1,
                          "sample": f"{r1['points']} points ({r1['interactions']:.3e} interactions in {r1['seconds']:.1f} s)"}}
 
