@@ -51,6 +51,10 @@ MUFU_LANES_PER_SM = 16
 # committed `ncu --set full` captures; evidence that HBM is idle (the bound is the FP64 pipe).
 NCU_TRAFFIC = {
     "eval": (59.97e6 + 5.81e6, "profiles/r02_ncu_full_interact64_eval_cfg4.md"),
+    # the fused Nelder-Mead launch = the whole config-2 search (375 passes): the optimiser state of every active point
+    # (48 doubles) is written back once per pass
+    "nm": (0.826e9 + 9.520e9, "profiles/r02_ncu_full_interact64_fused_nm_cfg2.md"),
+    "analytic": (1.113e9 + 9.607e9, "profiles/r02_ncu_full_interact64_fused_analytic_cfg2.md"),
 }
 
 
@@ -372,7 +376,8 @@ def measure_f64(mode: Mode, steps: int, warmup: int, rank=0, world=1, local=0, d
     kern_ips = inter_total / (kern_ms * 1e-3) if kern_ms > 0 else 0.0
     per_inter = FP64_INSTR[kind]
     achieved_slots = kern_ips * per_inter
-    traffic = NCU_TRAFFIC.get(kind) if (mode.points == 0 and mode.workload in ("cfg4", "cfg2")) else None
+    traffic = NCU_TRAFFIC.get(kind) if (mode.points == 0 and not mode.reduced and
+                                        mode.workload == ("cfg4" if not is_solve else "cfg2")) else None
     kernel_name = ("dbie::interact64_kernel (fp64 point-pixel sums)" if (not is_solve or mode.grid) else
                    "dbie::solve_nm_fused_kernel (whole Nelder-Mead search in one cooperative launch: point-pixel sums "
                    "+ residual + simplex step + list compaction)")
@@ -508,8 +513,9 @@ def measure_f32(steps: int, warmup: int, points: int = 0) -> dict:
         "gpu_launches": launches,
         "roofline": {"bound": "alu", "kernel": "dbie::interact_f32_kernel (fp32 point-pixel sums, SFU sincos of the reduced argument)",
                      "achieved": 1e-12 * ach, "peak": 1e-12 * peak, "unit": "T MUFU lane-op/s", "frac": ach / peak,
-                     "traffic": None, "traffic_source": "profiles/r01_ncu_full_interact_f32_eval_cfg4.md (that launch is split; "
-                                                        "no per-launch figure)",
+                     "traffic": 51.65e6 + 359.04e6,
+                     "traffic_source": "profiles/r02_ncu_full_interact_f32_eval_cfg4.md (the launch is split over chunk "
+                                       "ranges: 403 MB of fp64 partial sums; algorithmic bytes 36 M + 16 N = 42 MB)",
                      "mufu_per_interaction": MUFU_PER_INTERACTION,
                      "note": "SFU-bound: 148 SM x 16 MUFU lanes x clocks.max.sm / 7 MUFU per interaction (the issue port, 40 "
                              "instructions per interaction, allows 40 % more; the FP32 FMA pipe 75 % more; profiles/r02_sass_loops.txt)",
