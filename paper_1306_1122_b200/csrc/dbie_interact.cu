@@ -159,7 +159,7 @@ cudaError_t launch_interact_eval(const InteractParams& p, int sm_count, bool red
 }
 
 cudaError_t launch_interact_stencil(const InteractParams& p, int sm_count, cudaStream_t st) {
-    // all 4 stencil positions of a point in one thread (small-angle rotation between them), two pixels in
+    // all 4 stencil positions of a point in one thread (one sincos per component, kernel_n_near for the offsets), two pixels in
     // flight: 128 threads x 2 CTAs/SM; +35 % over one position per thread (MODE_STENCIL, profiles/r01_variants.md)
     return launch64<MODE_STENCIL4, 1, 2, 128, 2>(p, sm_count, 16, st);
 }
@@ -178,7 +178,7 @@ cudaError_t launch_interact_grid_analytic(const InteractParams& p, int sm_count,
 
 cudaError_t launch_interact_grid(const InteractParams& p, int sm_count, cudaStream_t st) {
     if (p.T < 2) return cudaErrorInvalidValue;
-    // NT > 1 uses the rotation recurrence, which needs window starts lo >= 0: not guaranteed for T = 2
+    // NT > 1 shares (sin, cos)(j d_theta) between the trials, which needs window starts lo >= 0: not guaranteed for T = 2
     // 8 trial triples per thread need 234 registers: 128 threads x 2 CTAs/SM (profiles/r01_variants.md)
     if (p.T % 8 == 0) return launch64<MODE_GRID, 8, 1, 128, 2>(p, sm_count, 16, st);
     if (p.T % 4 == 0) return launch64<MODE_GRID, 4, 1, 128, 3>(p, sm_count, 16, st);

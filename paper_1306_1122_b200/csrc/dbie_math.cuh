@@ -186,7 +186,7 @@ DBIE_HD double kernel_n_near(double th, double s0, double c0, double eps) {
 }
 constexpr double kNearEpsMax = 1e-3;   // largest |lambda delta| for which the Eq. 13 stencil uses kernel_n_near
 
-// sin(theta) and cos(theta), theta >= 0: 15 FP64 instructions (stencil and GRID rotations start from these)
+// sin(theta) and cos(theta), theta >= 0: 15 FP64 instructions (the Eq. 13 stencil and the GRID trials start from these)
 DBIE_HD void sincos_pos(double th, const TrigRef& tr, double& s, double& c) {
     int k;
     const double t = reduce_step(th, k);

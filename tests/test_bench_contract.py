@@ -56,7 +56,7 @@ def test_fp64_instruction_counts_match_the_built_library():
         return r["pipes"]["fp64"] / (r["rsqrt"] * per)
 
     # kernel<MODE, NT, THREADS, MINB, UNR>: eval = mode 0 (loop 0: general lambda; loop 1: lambda = 0),
-    # Eq. 13 stencil = mode 5 (loop 0: small-angle rotation between the positions), GRID NT = 8 = mode 2,
+    # Eq. 13 stencil = mode 5 (loop 0: one sincos per component, kernel_n_near for the three offset positions), GRID NT = 8 = mode 2,
     # analytic gradient = mode 3, GRID on it (NT = 2) = mode 4
     assert count("interact64_kernel<(int)0, (int)1,") == bench.FP64_INSTR["eval"]
     assert count("interact64_kernel<(int)5, (int)1,") == bench.FP64_INSTR["nm"]

@@ -41,7 +41,7 @@ def test_trig_coefficients_header_is_current():
 
 def test_sincos_accuracy_against_mpmath(shim):
     """|theta| up to 1000 rad (config 4 reaches ~155): error <= 1.5 ulp of the result + the reduced
-    argument's rounding + the one-step Cody-Waite tail theta*(pi/2 - fl(pi/2))/(pi/2) = 3.9e-17 theta,
+    argument's rounding + the one-step Cody-Waite tail theta*(pi/128 - fl(pi/128))/(pi/128) = 3.9e-17 theta,
     which stays below the half-ulp rounding 1.1e-16 theta that theta = |lambda| r itself carries
     (dbie_math.cuh reduce_pio2)."""
     rng = np.random.default_rng(1)
@@ -54,8 +54,8 @@ def test_sincos_accuracy_against_mpmath(shim):
     worst = 0.0
     for t, si, ci in zip(th, s, c):
         es, ec = mp.sin(mp.mpf(float(t))), mp.cos(mp.mpf(float(t)))
-        # error budget: 1.5 ulp of the value + the reduced argument's own rounding (2^-53 relative of
-        # t <= pi/4 -> 1.2e-16 absolute)
+        # error budget: 1.5 ulp of the value + the roundings of the table entries and of the two products that
+        # combine them with (sin t, cos t) (1.2e-16 absolute)
         for got, ex in ((si, es), (ci, ec)):
             err = abs(mp.mpf(float(got)) - ex)
             tol = 1.5 * float(_ulp(float(ex))) + 1.2e-16 + 4.0e-17 * float(t)

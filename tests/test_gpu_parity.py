@@ -282,9 +282,9 @@ def test_residual_matches_oracle(dbie, case):
 
 
 def test_residual_large_delta_takes_the_plain_stencil_path(dbie):
-    """MODE_STENCIL4 rotates sin/cos between the stencil positions only while lambda*delta <= 1e-3;
+    """MODE_STENCIL4 derives the offset positions from one sincos per component only while lambda*delta <= 1e-3;
     with delta = 0.05 h and lambda up to 0.3/h (lambda*delta = 1.5e-2) most threads take the plain
-    four-sincos path, the lambda = 0 points of the same warps the rotated one (divergent warps)."""
+    four-sincos path, the lambda = 0 points of the same warps the shared-sincos one (divergent warps)."""
     import torch
     w = workloads.random_boundary(48, 40, seed=15, npts=200, h=0.25)
     lam = np.random.default_rng(4).uniform(0.0, 0.3, (3, w.M)) / w.h
@@ -850,7 +850,7 @@ def test_internal_batches_do_not_change_a_bit(dbie):
 @pytest.mark.parametrize("theta", [1e3, 1e4, 1e5])
 def test_eval_large_theta_against_oracle(dbie, theta):
     """include/dbie.h: theta = |lambda| r < 2^20.  The kernel's one-step Cody-Waite reduction leaves
-    k (pi/2 - fl(pi/2)) = 3.9e-17 theta, and theta = lambda r itself carries half an ulp (1.1e-16 theta) on
+    k (pi/128 - fl(pi/128)) = 3.9e-17 theta, and theta = lambda r itself carries half an ulp (1.1e-16 theta) on
     both sides, r possibly one more: each term n(theta) w b is then off by about |theta| * ulp(theta), i.e.
     2^-52 theta relative to its own amplitude.  Gate: |dB| <= 8 * 2^-52 * theta_max * sum |terms|."""
     w = workloads.random_boundary(40, 24, seed=77, npts=64, zmin=2.0, zmax=9.0)
