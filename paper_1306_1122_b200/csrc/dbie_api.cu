@@ -211,7 +211,8 @@ static void setup_tiling(BoundaryView& b) {
         b.seg_w += b.seg_w & 1;
         b.ntiles = b.ny * b.segs_per_row;
     }
-    b.nchunks = b.ntiles < kMaxChunks ? b.ntiles : kMaxChunks;
+    b.nunits = b.ny * b.segs_per_row;
+    b.nchunks = b.nunits < kMaxChunks ? b.nunits : kMaxChunks;
 }
 
 extern "C" void dbie_destroy(dbie_ctx* ctx) {

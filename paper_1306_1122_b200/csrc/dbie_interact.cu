@@ -154,8 +154,9 @@ cudaError_t launch_interact_eval(const InteractParams& p, int sm_count, bool red
                                  cudaStream_t st) {
     const long long nblk = (p.count + kThreads64 - 1) / kThreads64;
     *nparts = (nblk >= 8LL * sm_count * kMinB64 || p.bd.nchunks == 1) ? 1 : p.bd.nchunks;
-    if (reduced_sincos) return launch64<MODE_EVAL_R, 1, 3>(p, sm_count, 8, st);
-    return launch64<MODE_EVAL, 1, 3>(p, sm_count, 8, st);   // three pixels in flight (_work sweep: u1 .822, u2 .835, u3 .848, u4 .842)
+    // four pixels in flight (developer sweep at 512 x 512, M = 1,048,576: u1 1098 ms, u2 1081, u3 1088, u4 1071)
+    if (reduced_sincos) return launch64<MODE_EVAL_R, 1, 4>(p, sm_count, 8, st);
+    return launch64<MODE_EVAL, 1, 4>(p, sm_count, 8, st);
 }
 
 cudaError_t launch_interact_stencil(const InteractParams& p, int sm_count, cudaStream_t st) {
@@ -247,9 +248,10 @@ __global__ void __launch_bounds__(THREADS, MINB) interact_f32_kernel(const __gri
 #pragma unroll
         for (int r = 0; r < R; ++r) acc[r][0] = acc[r][1] = acc[r][2] = 0.0;
 
-        const int t0 = chunk_first_tile(bd, c0), t1 = chunk_first_tile(bd, c1);
+        const int u0 = chunk_first_unit(bd, c0), u1 = chunk_first_unit(bd, c1);   // as in the fp64 interact_item
+        const int t0 = unit_tile(bd, u0), t1 = unit_tile(bd, u1 - 1) + 1;
         int c = c0;
-        int t_chunk_end = chunk_first_tile(bd, c + 1);
+        int u_chunk_end = chunk_first_unit(bd, c + 1);
         if (tid == 0) {
             const TileDesc d = tile_desc(bd, t0);
             mbar_expect_tx(&full[it & 1], (unsigned)d.npx * 16u);
@@ -265,7 +267,9 @@ __global__ void __launch_bounds__(THREADS, MINB) interact_f32_kernel(const __gri
             const TileDesc d = tile_desc(bd, t);
             mbar_wait(&full[it & 1], (it >> 1) & 1);
             const float4* __restrict__ rp = &tile[it & 1][0];
-            for (int row = 0; row < d.nrows; ++row) {
+            for (int row = 0; row < d.nrows; ++row, rp += d.ncols) {
+                const int unit = (bd.segs_per_row == 1) ? d.row0 + row : t;
+                if (unit < u0 || unit >= u1) continue;   // a row of a neighbouring chunk in a shared tile
                 const float yk = __ldg(bd.yk32 + d.row0 + row);
                 float cc[R], a32[R][3];
 #pragma unroll
@@ -293,9 +297,7 @@ __global__ void __launch_bounds__(THREADS, MINB) interact_f32_kernel(const __gri
                 for (int r = 0; r < R; ++r)
 #pragma unroll
                     for (int q = 0; q < 3; ++q) acc[r][q] += (double)a32[r][q];
-                rp += d.ncols;
-            }
-            if (t + 1 == t_chunk_end) {
+                if (unit + 1 != u_chunk_end) continue;
                 if (nsplit == 1) {   // unsplit launch: add the chunk sums here, in chunk order (as the epilogue would)
 #pragma unroll
                     for (int r = 0; r < R; ++r)
@@ -320,7 +322,7 @@ __global__ void __launch_bounds__(THREADS, MINB) interact_f32_kernel(const __gri
 #pragma unroll
                 for (int r = 0; r < R; ++r) acc[r][0] = acc[r][1] = acc[r][2] = 0.0;
                 ++c;
-                t_chunk_end = chunk_first_tile(bd, c + 1);
+                u_chunk_end = chunk_first_unit(bd, c + 1);
             }
             __syncthreads();
         }

@@ -264,9 +264,12 @@ __device__ __forceinline__ void interact_item(const InteractParams& p, const Tri
 #pragma unroll
         for (int c = 0; c < 3; ++c) lam2[tt][c] = lam[tt][c] * lam[tt][c];
 
-    const int t0 = chunk_first_tile(bd, c0), t1 = chunk_first_tile(bd, c1);
+    // the item's canonical chunks [c0, c1) = units [u0, u1); the tiles that hold them (the first and the last tile may
+    // also hold rows of neighbouring chunks, which are skipped)
+    const int u0 = chunk_first_unit(bd, c0), u1 = chunk_first_unit(bd, c1);
+    const int t0 = unit_tile(bd, u0), t1 = unit_tile(bd, u1 - 1) + 1;
     int c = c0;
-    int t_chunk_end = chunk_first_tile(bd, c + 1);
+    int u_chunk_end = chunk_first_unit(bd, c + 1);
     if (tid == 0) {
         const TileDesc d = tile_desc(bd, t0);
         mbar_expect_tx(&full[it & 1], (unsigned)d.npx * 32u);
@@ -282,12 +285,15 @@ __device__ __forceinline__ void interact_item(const InteractParams& p, const Tri
         const TileDesc d = tile_desc(bd, t);
         mbar_wait(&full[it & 1], (it >> 1) & 1);
         const double4* __restrict__ rp = &tile[it & 1][0];
-        for (int row = 0; row < d.nrows; ++row) {
+        for (int row = 0; row < d.nrows; ++row, rp += d.ncols) {
+            const int unit = (bd.segs_per_row == 1) ? d.row0 + row : t;
+            if (unit < u0 || unit >= u1) continue;   // a row of a neighbouring chunk in a shared tile
             const double yk = __ldg(bd.yk + d.row0 + row);
             const double dy = yk - yi;
             const double cc = fma(dy, dy, z2);
             const double dy2 = yk - yi2;
             const double cc2 = fma(dy2, dy2, z2), cc3 = fma(dy, dy, z23);   // MODE_STENCIL4
+            bool row_done = false;
             if constexpr (MODE == MODE_STENCIL4) {
                 // the small-angle / plain decision is per thread: two loops instead of a branch per pixel
                 if (small_eps) {
@@ -297,8 +303,7 @@ __device__ __forceinline__ void interact_item(const InteractParams& p, const Tri
 #pragma unroll UNR
                     for (int j = 0; j < d.ncols; ++j) stencil4_pixel<false>(tr, rp[j], xi, xi1, cc, cc2, cc3, lam[0], acc);
                 }
-                rp += d.ncols;
-                continue;
+                row_done = true;
             }
             if constexpr (kEval) {
                 // lambda = 0 in all three components (the potential field, BASELINE config 1): n(0) = 1
@@ -316,10 +321,10 @@ __device__ __forceinline__ void interact_item(const InteractParams& p, const Tri
                         acc[0][1] = __dadd_rn(acc[0][1], __dmul_rn(wgt, px.z));   // roundings as fma(1, w B, acc)
                         acc[0][2] = __dadd_rn(acc[0][2], __dmul_rn(wgt, px.w));
                     }
-                    rp += d.ncols;
-                    continue;
+                    row_done = true;
                 }
             }
+            if (!row_done) {
 #pragma unroll UNR
             for (int j = 0; j < d.ncols; ++j) {
                 const double4 px = rp[j];  // {x_k, Bx0, By0, Bz0}: two broadcast LDS.128
@@ -399,14 +404,14 @@ __device__ __forceinline__ void interact_item(const InteractParams& p, const Tri
                     acc[tt][2] = fma(kernel_n<MODE == MODE_EVAL_R>(lam[tt][2] * rr, tr), wz, acc[tt][2]);
                 }
             }
-            rp += d.ncols;
-        }
-        if (t + 1 == t_chunk_end) {  // A4: one partial sum per chunk, added in chunk order later
-            sink(ic, c, acc);
+            }
+            if (unit + 1 == u_chunk_end) {  // A4: one partial sum per chunk, added in chunk order later
+                sink(ic, c, acc);
 #pragma unroll
-            for (int tt = 0; tt < NA; ++tt) acc[tt][0] = acc[tt][1] = acc[tt][2] = 0.0;
-            ++c;
-            t_chunk_end = chunk_first_tile(bd, c + 1);
+                for (int tt = 0; tt < NA; ++tt) acc[tt][0] = acc[tt][1] = acc[tt][2] = 0.0;
+                ++c;
+                u_chunk_end = chunk_first_unit(bd, c + 1);
+            }
         }
         __syncthreads();  // everyone is done with stage it&1 before it is refilled
     }

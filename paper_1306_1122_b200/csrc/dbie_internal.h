@@ -27,9 +27,11 @@ struct BoundaryView {
     const float4* rec32;   // fp32 copy {x_k, Bx0, By0, Bz0} or nullptr
     const float* yk32;
     // tiling: a tile is `tile_rows` full rows (nx <= kTilePx) or one row segment of
-    // `seg_w` columns (nx > kTilePx); a chunk is a run of consecutive tiles.
+    // `seg_w` columns (nx > kTilePx); a chunk is a run of consecutive UNITS, a unit being one row
+    // (or one row segment): nunits = ny * segs_per_row.  Chunk boundaries may fall inside a tile
+    // (small boundaries: 64 x 64 has 8 tiles of 8 rows and 16 chunks of 4 rows).
     int tile_rows, segs_per_row, seg_w;
-    int ntiles, nchunks;
+    int ntiles, nunits, nchunks;
 };
 
 struct TileDesc {
@@ -56,8 +58,13 @@ __host__ __device__ inline TileDesc tile_desc(const BoundaryView& b, int t) {
     return d;
 }
 
-__host__ __device__ inline int chunk_first_tile(const BoundaryView& b, int c) {
-    return (int)(((long long)c * b.ntiles) / b.nchunks);
+// first unit (row, or row segment when nx > kTilePx) of canonical chunk c; chunk nchunks starts at nunits
+__host__ __device__ inline int chunk_first_unit(const BoundaryView& b, int c) {
+    return (int)(((long long)c * b.nunits) / b.nchunks);
+}
+// the tile that holds unit u
+__host__ __device__ inline int unit_tile(const BoundaryView& b, int u) {
+    return (b.segs_per_row == 1) ? u / b.tile_rows : u;
 }
 
 // One launch of the interaction kernel.

@@ -119,9 +119,10 @@ __device__ __forceinline__ void interact_item_warp(const InteractParams& p, cons
     double* stB = stA + 12 * kStageRow;
     double acc = 0.0;                                      // chain lane k < 12 owns sum k = kind*3 + component
 
-    const int t0 = chunk_first_tile(bd, c0), t1 = chunk_first_tile(bd, c1);
+    const int u0 = chunk_first_unit(bd, c0), u1 = chunk_first_unit(bd, c1);   // as in interact_item
+    const int t0 = unit_tile(bd, u0), t1 = unit_tile(bd, u1 - 1) + 1;
     int c = c0;
-    int t_chunk_end = chunk_first_tile(bd, c + 1);
+    int u_chunk_end = chunk_first_unit(bd, c + 1);
     if (tid == 0) {
         const TileDesc d = tile_desc(bd, t0);
         mbar_expect_tx(&full[it & 1], (unsigned)d.npx * 32u);
@@ -137,7 +138,9 @@ __device__ __forceinline__ void interact_item_warp(const InteractParams& p, cons
         const TileDesc d = tile_desc(bd, t);
         mbar_wait(&full[it & 1], (it >> 1) & 1);
         const double4* __restrict__ rp = &tile[it & 1][0];
-        for (int row = 0; row < d.nrows; ++row) {
+        for (int row = 0; row < d.nrows; ++row, rp += d.ncols) {
+            const int unit = (bd.segs_per_row == 1) ? d.row0 + row : t;
+            if (unit < u0 || unit >= u1) continue;   // a row of a neighbouring chunk in a shared tile
             const double yk = __ldg(bd.yk + d.row0 + row);
             const double dy = yk - yi;
             const double cc = fma(dy, dy, z2);
@@ -170,13 +173,12 @@ __device__ __forceinline__ void interact_item_warp(const InteractParams& p, cons
                 }
                 __syncwarp();
             }
-            rp += d.ncols;
-        }
-        if (t + 1 == t_chunk_end) {
-            if (live && lane < 12) p.part[((long long)c * 12 + lane) * p.cap + slot] = acc;
-            acc = 0.0;
-            ++c;
-            t_chunk_end = chunk_first_tile(bd, c + 1);
+            if (unit + 1 == u_chunk_end) {
+                if (live && lane < 12) p.part[((long long)c * 12 + lane) * p.cap + slot] = acc;
+                acc = 0.0;
+                ++c;
+                u_chunk_end = chunk_first_unit(bd, c + 1);
+            }
         }
         __syncthreads();
     }
