@@ -50,10 +50,10 @@ MUFU_LANES_PER_SM = 16
 # DRAM bytes (dram__bytes_read.sum + dram__bytes_write.sum) of ONE launch of the dominant kernel, from the
 # committed `ncu --set full` captures; evidence that HBM is idle (the bound is the FP64 pipe).
 NCU_TRAFFIC = {
-    "eval": (59.97e6 + 5.81e6, "profiles/r02_ncu_full_interact64_eval_cfg4.md"),
+    "eval": (60.12e6 + 5.77e6, "profiles/r02_ncu_full_interact64_eval_cfg4.md"),
     # the fused Nelder-Mead launch = the whole config-2 search (375 passes): the optimiser state of every active point
-    # (48 doubles) is written back once per pass
-    "nm": (0.826e9 + 9.520e9, "profiles/r02_ncu_full_interact64_fused_nm_cfg2.md"),
+    # (48 doubles) is written back once per pass, plus the chunk partial sums of the split items
+    "nm": (2.214e9 + 14.692e9, "profiles/r02_ncu_full_interact64_fused_nm_cfg2.md"),
     "analytic": (1.113e9 + 9.607e9, "profiles/r02_ncu_full_interact64_fused_analytic_cfg2.md"),
 }
 
