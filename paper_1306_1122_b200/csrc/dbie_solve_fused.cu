@@ -21,7 +21,7 @@
 //          n) never writes the partial sums at all.
 //          grid-wide barrier.
 //
-// The decisions are those of solve_step_kernel of round 1 (dbie_nm.cuh, separately rounded IEEE operations);
+// The decisions are those of the resumable state machine nm_advance (dbie_nm.cuh, separately rounded IEEE operations);
 // results do not depend on the batch, the shape or the CTA that happened to finish last.
 // This unit is compiled like dbie_interact.cu (FMA contraction on): the interaction arithmetic must be the
 // same instruction sequence as in dbie_residual; the search itself uses __dmul_rn / __dadd_rn throughout.
