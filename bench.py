@@ -41,7 +41,7 @@ METRIC = "point-pixel DBIE interactions/sec (fp64)"
 UNIT = "interactions/s"
 # FP64-pipe instructions per interaction of each inner loop, counted from the SASS of the built library by
 # paper_1306_1122_b200/csrc/sass_loops.py (profiles/r02_sass_loops.txt); DESIGN.md section 6 derives them.
-FP64_INSTR = {"eval": 61.0, "eval_reduced": 55.0, "nm": 418 / 8, "analytic": 86.0, "grid": 215 / 8, "grid_analytic": 158 / 2}
+FP64_INSTR = {"eval": 61.0, "eval_reduced": 55.0, "nm": 418 / 8, "analytic": 86.0, "grid": 200 / 8, "grid_analytic": 158 / 2}
 FP64_INSTR_SURVEY = 82               # SURVEY.md 8(d) canonical count
 SM_COUNT, FP64_LANES_PER_SM = 148, 64   # B200: 148 SMs, 64 FP64 lanes per SM per clock
 MUFU_PER_INTERACTION = 7             # dbie_eval_f32 default (SFU sincos): 1 rsqrt + 3 x (sin, cos)
@@ -396,7 +396,7 @@ def measure_f64(mode: Mode, steps: int, warmup: int, rank=0, world=1, local=0, d
         "traffic_note": "DRAM bytes of one launch.  Algorithmic bytes: eval 72 M + 32 N (cfg4: 84 MB); solve: 24 M of "
                         "point data + 480 M of optimiser state per pass through L2.  HBM is idle either way (bound: FP64 pipe)",
         "note": "FP64-pipe bound (no HBM/tensor step): achieved = interactions/s of the kernel x FP64 lane-instructions per "
-                "interaction (eval 61, 55 with DBIE_EVAL_REDUCED_SINCOS; Eq. 13 stencil 52.25; GRID T=8 26.875; analytic gradient 86; GRID on it 79; "
+                "interaction (eval 61, 55 with DBIE_EVAL_REDUCED_SINCOS; Eq. 13 stencil 52.25; GRID T=8 25; analytic gradient 86; GRID on it 79; "
                 "profiles/r02_sass_loops.txt) x 2; peak = 148 SM x 64 FP64 lanes x clocks.max.sm (derived, DESIGN.md s7)",
         "kernel_interactions_per_s": kern_ips, "kernel_ms_per_launch": kern_ms / max(kern_launches, 1),
         "kernel_launches": kern_launches, "kernel_share_of_step": kern_ms / ms_total if ms_total else None,

@@ -359,7 +359,7 @@ __device__ __forceinline__ void interact_item(const InteractParams& p, const Tri
                     // (sin, cos)(j d_theta), j = 1..NT/2, formed ONCE per pixel (one full sincos, then angle doubling /
                     // addition), and one full sincos per component at the middle trial,
                     //   n(theta_m + j d) = s_m (theta c_j - s_j) + c_m (theta s_j + c_j),   theta = fl(lambda_t r):
-                    // 6 FP64 instructions per further trial and component instead of a 16-instruction kernel_n, every
+                    // 5 FP64 instructions per further trial and component instead of a 16-instruction kernel_n, every
                     // trial independent of the others (no chained rotation).  theta_m + j d_theta differs from
                     // fl(lambda_t r) by a few ulp(theta), the size of the rounding theta carries anyway.
                     // Needs lo >= 0 (no |.| fold inside the group): true for T >= 3 (dbie_solve rejects T < 4).
@@ -384,6 +384,9 @@ __device__ __forceinline__ void interact_item(const InteractParams& p, const Tri
                         double sb, cb;
                         sincos_pos(thb, tr, sb, cb);
                         acc[TB][c] = fma(fma(thb, sb, cb), wb[c], acc[TB][c]);
+                        // the weight w B_p0 is folded into (sin, cos)(theta_m) once per component, so a further
+                        // trial costs theta, P, Q and two accumulating FMAs: 5 instructions
+                        const double sbw = sb * wb[c], cbw = cb * wb[c];
 #pragma unroll
                         for (int tt = 0; tt < NT; ++tt) {
                             if (tt == TB) continue;
@@ -392,7 +395,7 @@ __device__ __forceinline__ void interact_item(const InteractParams& p, const Tri
                             // sin(+-j d) = +-s_j: the sign is an operand modifier
                             const double pp = tt > TB ? fma(th, cj[j], -sj[j]) : fma(th, cj[j], sj[j]);
                             const double qq = tt > TB ? fma(th, sj[j], cj[j]) : fma(th, -sj[j], cj[j]);
-                            acc[tt][c] = fma(fma(sb, pp, cb * qq), wb[c], acc[tt][c]);
+                            acc[tt][c] = fma(sbw, pp, fma(cbw, qq, acc[tt][c]));
                         }
                     }
                     continue;
