@@ -115,6 +115,43 @@ dbie_status dbie_eval_host(dbie_ctx* ctx, long long M, const double* x, const do
 dbie_status dbie_eval_f32(dbie_ctx* ctx, long long M, const float* x, const float* y,
                           const float* z, const float* lam, float* B, void* cuda_stream);
 
+/* dbie_eval for callers that must not allocate device memory.
+ *
+ * Who needs it: dbie_eval keeps its per-chunk partial sums (Eq. 16's sum is split into up to 16 row
+ * chunks, added in chunk order) in a buffer the context obtains with cudaMalloc on first use and
+ * regrows when M grows.  Some hosts cannot tolerate that: a program that hands the whole of HBM to its
+ * own pool at start-up, so that a later cudaMalloc fails; a real-time or in-situ loop (field
+ * extrapolation next to an MHD step) in which cudaMalloc / cudaFree, which may synchronise the whole
+ * device, must never run; code that holds a lock other threads' allocations wait on.  For them this
+ * entry point computes exactly what dbie_eval computes (same kernels, same summation order: the two
+ * results are bit-identical) with the partial sums in a fixed array that is part of the library image.
+ *
+ * The limit: M <= DBIE_NOALLOC_MAX_POINTS (16,384 points per call; loop over larger sets).  The array is
+ * 16 chunks x 3 components x 16,384 points x 8 B = 6 MiB of device memory on every GPU that loads the
+ * library, held until the process exits whether or not this function is ever called.  A larger M returns
+ * DBIE_EINVAL before anything is launched, and dbie_last_cuda_error(ctx) then names the limit.
+ *
+ * What the call does not do: no cudaMalloc, cudaFree, event or stream creation, and nothing is grown or
+ * cached in the context (profile mode is ignored, dbie_last_kernel_time keeps the previous call's events).
+ * x, y, z, lam, B are caller-allocated DEVICE arrays as in dbie_eval.  The context must exist already:
+ * dbie_create does allocate (the staged boundary), so create contexts during start-up.
+ *
+ * First call per device: the first call on a given GPU looks up the device address of the array
+ * (cudaGetSymbolAddress, done once per device and remembered) and, like any first launch, lets the CUDA
+ * runtime load the kernels.  Make that first call during set-up, before any stream capture is begun.
+ *
+ * Sharing: there is ONE array per GPU, shared by every context, stream and host thread of the process.
+ * Two dbie_eval_noalloc calls whose kernels may overlap on the GPU (different streams, or different host
+ * threads) race on it and give wrong results; run them on one stream or order them with events.  The
+ * array keeps the previous call's partial sums; nothing in it has to start at zero, because every element
+ * the epilogue reads is written by the same call's interaction kernel first, so the call clears nothing.
+ * Asynchronous on the stream, like dbie_eval.  M = 0 is a no-op. */
+#define DBIE_NOALLOC_MAX_POINTS 16384
+dbie_status dbie_eval_noalloc(dbie_ctx* ctx, long long M, const double* x, const double* y,
+                              const double* z, const double* lam, double* B, void* cuda_stream);
+/* DBIE_NOALLOC_MAX_POINTS of the loaded library (for bindings that cannot read the macro). */
+long long dbie_noalloc_max_points(void);
+
 /* Options of dbie_solve.  Fill with dbie_solve_default_opts, then change fields. */
 typedef struct {
     int method;       /* 0 = NM: Downhill Simplex; 1 = GRID (O-4)     */

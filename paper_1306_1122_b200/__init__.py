@@ -70,6 +70,9 @@ def load() -> C.CDLL:
     lib.dbie_eval.argtypes = [_vp, C.c_longlong, _vp, _vp, _vp, _vp, _vp, _vp]
     lib.dbie_eval_host.argtypes = [_vp, C.c_longlong, _vp, _vp, _vp, _vp, _vp]
     lib.dbie_eval_f32.argtypes = [_vp, C.c_longlong, _vp, _vp, _vp, _vp, _vp, _vp]
+    lib.dbie_eval_noalloc.argtypes = [_vp, C.c_longlong, _vp, _vp, _vp, _vp, _vp, _vp]
+    lib.dbie_noalloc_max_points.argtypes = []
+    lib.dbie_noalloc_max_points.restype = C.c_longlong
     lib.dbie_set_f32_sfu_mask.argtypes = [_vp, C.c_int]
     lib.dbie_debug_set_batch_limit.argtypes = [_vp, C.c_longlong]
     lib.dbie_solve_default_opts.argtypes = [C.POINTER(SolveOpts)]
@@ -128,6 +131,11 @@ def default_trace_opts(**kw) -> TraceOpts:
 
 def version() -> str:
     return load().dbie_version().decode()
+
+
+def noalloc_max_points() -> int:
+    """DBIE_NOALLOC_MAX_POINTS of the loaded library: the most points one eval_noalloc call takes."""
+    return int(load().dbie_noalloc_max_points())
 
 
 def probe_dfma_rate(millis: float = 200.0) -> tuple[float, float]:
@@ -258,6 +266,19 @@ class DBIE:
         self._check(self._lib.dbie_eval_host(self._h, M, _vp(x.ctypes.data), _vp(y.ctypes.data),
                                              _vp(z.ctypes.data), _vp(lam.ctypes.data), _vp(B.ctypes.data)))
         return B
+
+    # -- dbie_eval_noalloc
+    def eval_noalloc(self, x, y, z, lam, out, stream=None):
+        """dbie_eval_noalloc: dbie_eval for callers that must not allocate device memory (their own pool owns
+        the GPU's memory, or cudaMalloc's device-wide synchronisation is not allowed where they run).  The
+        partial sums go to a fixed 6 MiB array inside the library, so M <= noalloc_max_points() (16,384) per
+        call, and `out` (3, M) must be passed in: this method creates no tensor.  Bit-identical to eval().
+        Calls that may overlap on the GPU share that array and race; keep them on one stream."""
+        M = x.numel()
+        self._check(self._lib.dbie_eval_noalloc(self._h, M, _dev_f64(x, M, "x"), _dev_f64(y, M, "y"),
+                                                _dev_f64(z, M, "z"), _dev_f64(lam, 3 * M, "lam"),
+                                                _dev_f64(out, 3 * M, "out"), _stream_ptr(stream)))
+        return out
 
     # -- dbie_eval_f32
     def eval_f32(self, x, y, z, lam, out=None, stream=None):

@@ -6,6 +6,8 @@
 #include <stdlib.h>
 #include <string.h>
 
+#include <mutex>
+
 #include <nvtx3/nvToolsExt.h>   // header-only; ranges show up in Nsight tools, a no-op otherwise
 
 #include "dbie_internal.h"
@@ -378,6 +380,75 @@ extern "C" dbie_status dbie_eval_host(dbie_ctx* ctx, long long M, const double* 
     if (s != DBIE_OK) return s;
     CU(cudaMemcpyAsync(B, d + 6 * M, 3 * m, cudaMemcpyDeviceToHost, st));
     CU(cudaStreamSynchronize(st));
+    return DBIE_OK;
+}
+
+// ------------------------------------------------------------------ eval, no allocation ---
+// dbie_eval for callers that cannot allocate device memory (a process whose own pool owns all of HBM, a
+// real-time loop that must never hit the device-wide synchronisation of cudaMalloc / cudaFree): the chunk
+// partial sums live in this fixed array instead of the context's lazily grown buffer.  It is part of the
+// library image, so every GPU that loads the library holds these 6 MiB until the process exits.
+static const long long kNoAllocMaxPoints = DBIE_NOALLOC_MAX_POINTS;
+static __device__ __align__(256) double g_noalloc_part[(size_t)kMaxChunks * 3 * DBIE_NOALLOC_MAX_POINTS];
+
+// In host code `g_noalloc_part` is only a handle for the runtime, not a device address: the address a kernel
+// may use comes from cudaGetSymbolAddress, asked once per device with that device current and kept here.
+static const int kNoAllocMaxDevices = 64;
+static double* g_noalloc_addr[kNoAllocMaxDevices];   // zero-initialised: "not looked up yet"
+static std::mutex g_noalloc_mutex;
+
+static dbie_status noalloc_scratch(dbie_ctx* ctx, double** out) {   // ctx's device is current
+    const int dev = ctx->device;
+    std::lock_guard<std::mutex> lock(g_noalloc_mutex);
+    if (dev >= 0 && dev < kNoAllocMaxDevices && g_noalloc_addr[dev]) {
+        *out = g_noalloc_addr[dev];
+        return DBIE_OK;
+    }
+    double* ptr = nullptr;
+    CU(cudaGetSymbolAddress((void**)&ptr, g_noalloc_part));
+    if (!ptr) {
+        snprintf(ctx->err, 256, "dbie_eval_noalloc: cudaGetSymbolAddress returned a null address");
+        return DBIE_ECUDA;
+    }
+    if (dev >= 0 && dev < kNoAllocMaxDevices) g_noalloc_addr[dev] = ptr;   // beyond the table: asked again every call
+    *out = ptr;
+    return DBIE_OK;
+}
+
+extern "C" long long dbie_noalloc_max_points(void) { return kNoAllocMaxPoints; }
+
+extern "C" dbie_status dbie_eval_noalloc(dbie_ctx* ctx, long long M, const double* x, const double* y,
+                                         const double* z, const double* lam, double* B, void* cuda_stream) {
+    if (!ctx || M < 0) return DBIE_EINVAL;
+    if (M == 0) return DBIE_OK;
+    if (!x || !y || !z || !lam || !B) return DBIE_EINVAL;
+    if (M > kNoAllocMaxPoints) {
+        snprintf(ctx->err, 256, "dbie_eval_noalloc: M = %lld exceeds DBIE_NOALLOC_MAX_POINTS = %lld (the fixed "
+                 "scratch array holds no more; split the points over several calls)", M, kNoAllocMaxPoints);
+        return DBIE_EINVAL;
+    }
+    GUARD_DEVICE();
+    NvtxRange nvtx_("dbie_eval_noalloc");
+    double* part = nullptr;
+    const dbie_status s = noalloc_scratch(ctx, &part);   // the first call on this device looks the address up
+    if (s != DBIE_OK) return s;
+    cudaStream_t st = (cudaStream_t)cuda_stream;
+    // One batch (M <= the limit), laid out as dbie_eval lays out a batch of M points: part[(c*3 + q)*M + slot].
+    // Every element the epilogue reads is written by the interaction launch before it, so the previous
+    // call's contents are never read and nothing is cleared.
+    InteractParams p;
+    memset(&p, 0, sizeof p);
+    p.bd = ctx->bd;
+    p.x = x; p.y = y; p.z = z; p.lam = lam; p.ldlam = M;
+    p.count = M; p.slot0 = 0;
+    p.part = part; p.cap = M;
+    int nparts = ctx->bd.nchunks;
+    CU(launch_interact_eval(p, ctx->sm_count, ctx->eval_reduced, &nparts, st));
+    CU(launch_eval_finalize(ctx->bd, nparts, 0, M, M, z, lam, part, M, B, st));
+    ctx->last_interactions = (double)M * (double)ctx->bd.N;
+    ctx->last_launches = 2;
+    ctx->last_evals = 0;
+    ctx->evals_on_device = 0;
     return DBIE_OK;
 }
 
