@@ -3,7 +3,7 @@
 
     python bench.py [--gpus N] [--steps K] [--warmup W] [--impl ours|reference]
                     [--workload cfg4|cfg2|cfg3|cfg5] [--method nm|grid] [--gradient fd|analytic]
-                    [--dtype f64|f32] [--points P] [--slabs] [--no-legs]
+                    [--dtype f64|f32] [--points P] [--slabs] [--legs] [--detail FILE]
 
 The metric is BASELINE.json's: point-pixel DBIE interactions/s in fp64 and the fraction of the FP64
 roofline.  One interaction = one (evaluation point, pixel) pair, all three components; in the solver
@@ -12,15 +12,19 @@ every stencil position and every objective evaluation counts.
 Default (no flags, one GPU): the HEADLINE line is BASELINE configs[3] ("cfg4": 512x512 boundary,
 M = 1,048,576 random points, per-component lambda, fp64) — the configuration the metric's "interactions/s
 and roofline fraction" are quoted on.  A step is one pass of the hot path over that batch: stage the
-boundary (dbie_create) and evaluate Eq. 6/16 at every point (dbie_eval).  The same run then times three
-more legs, each with its own value / roofline / clocks, under "legs":
-    cfg2_nm    BASELINE configs[1]: full per-point Nelder-Mead lambda solve of the 64x64x32 Low & Lou volume
-    cfg5_grid  BASELINE configs[4]: GRID solve (T = 8, 10 levels) of a seeded 8,192-point subset at 1024x1024
-    cfg4_f32   BASELINE configs[3], fp32 leg: dbie_eval_f32
+boundary (dbie_create) and evaluate Eq. 6/16 at every point (dbie_eval).  The same run also times BASELINE
+configs[1] ("cfg2": the full per-point Nelder-Mead solve of the 64x64x32 Low & Lou volume) for two steps and
+reports it under "also", so that both workloads stay comparable from round to round ("vs_previous_round").
 `value` is measured with the inputs resident in HBM; `e2e` goes through the host-pointer C-ABI calls with
 the copies inside the timed region.  `roofline` is for the dominant kernel, timed live with CUDA-event pairs
 around each of its launches.  `cpu_baseline` times the oracle, as it stands, on the host cores (all cores and
-one core) over a bounded sample.  One JSON line on stdout (rank 0).
+one core) over a bounded sample.
+
+Output: the LAST line of stdout (rank 0) is ONE compact JSON line of fewer than 2,000 bytes (`headline`): the
+contract keys only, no prose.  What each field means is in DESIGN.md section 7.  `--detail FILE` also writes the
+full record (every diagnostic field, the pass timeline, the operand probe) to FILE; `--legs` times four more
+legs (48-point latency, config 5 GRID, fp32, reduced sincos) and puts their full records into that file
+(default gpurun_out/bench_detail.json when --legs is given) and their values into "also".
 """
 from __future__ import annotations
 
@@ -40,22 +44,28 @@ sys.path.insert(0, ROOT)
 METRIC = "point-pixel DBIE interactions/sec (fp64)"
 UNIT = "interactions/s"
 # FP64-pipe instructions per interaction of each inner loop, counted from the SASS of the built library by
-# paper_1306_1122_b200/csrc/sass_loops.py (profiles/r02_sass_loops.txt); DESIGN.md section 6 derives them.
+# tests/sass_loops.py (profiles/r02_sass_loops.txt); DESIGN.md section 6 derives them.
 FP64_INSTR = {"eval": 61.0, "eval_reduced": 55.0, "nm": 418 / 8, "analytic": 86.0, "grid": 200 / 8, "grid_analytic": 158 / 2}
 FP64_INSTR_SURVEY = 82               # SURVEY.md 8(d) canonical count
 SM_COUNT, FP64_LANES_PER_SM = 148, 64   # B200: 148 SMs, 64 FP64 lanes per SM per clock
 MUFU_PER_INTERACTION = 7             # dbie_eval_f32 default (SFU sincos): 1 rsqrt + 3 x (sin, cos)
 MUFU_LANES_PER_SM = 16
 
-# DRAM bytes (dram__bytes_read.sum + dram__bytes_write.sum) of ONE launch of the dominant kernel, from the
-# committed `ncu --set full` captures; evidence that HBM is idle (the bound is the FP64 pipe).
-NCU_TRAFFIC = {
-    "eval": (60.12e6 + 5.77e6, "profiles/r02_ncu_full_interact64_eval_cfg4.md"),
-    # the fused Nelder-Mead launch = the whole config-2 search (375 passes): the optimiser state of every active point
-    # (48 doubles) is written back once per pass, plus the chunk partial sums of the split items
-    "nm": (2.214e9 + 14.692e9, "profiles/r02_ncu_full_interact64_fused_nm_cfg2.md"),
-    "analytic": (1.113e9 + 9.607e9, "profiles/r02_ncu_full_interact64_fused_analytic_cfg2.md"),
-}
+# Results of the previous round's final runs (profiles/r02_bench_default.json.txt, r02_bench_cfg2_solve.json.txt):
+# the default line reports this round's value over these, workload by workload.
+PREVIOUS_ROUND = {"cfg4_eval": 2.56e11, "cfg2_nm": 2.79e11}
+HEADLINE_MAX_BYTES = 2000            # the driver keeps about 3 KB of stdout: the last line must fit with room to spare
+
+
+def ncu_traffic() -> dict:
+    """DRAM bytes (dram__bytes_read.sum + dram__bytes_write.sum) of ONE launch of the dominant kernel, from the
+    committed `ncu --set full` captures named in profiles/traffic.json (kind -> bytes, capture file, date), so
+    that a stale figure is visible next to its source; evidence that HBM is idle (the bound is the FP64 pipe)."""
+    try:
+        with open(os.path.join(ROOT, "profiles", "traffic.json")) as f:
+            return json.load(f)["kernels"]
+    except (OSError, ValueError, KeyError):
+        return {}
 
 
 def make_workload(name: str, rank: int = 0, world: int = 1, points: int = 0):
@@ -71,6 +81,9 @@ def make_workload(name: str, rank: int = 0, world: int = 1, points: int = 0):
     if world > 1:
         wl.z = wl.z + rank * wl.h / world
     return wl
+
+
+SHARDING = "points, boundary replicated, no data-path collective"
 
 
 def shard_info(M: int, rank: int, world: int) -> dict:
@@ -199,6 +212,7 @@ def cpu_baseline(wl, mode: Mode, target_s: float = 15.0) -> dict:
             "cpu": cpu_model(),
             "sample": f"oracle.{kind} on {r['points']} seeded points of {wl.name} "
                       f"({r['interactions']:.3e} interactions in {r['seconds']:.1f} s)",
+            "cores_delivered": (r["interactions"] / r["seconds"]) / (r1["interactions"] / r1["seconds"]),
             "speedup_over_one_core": (r["interactions"] / r["seconds"]) / (r1["interactions"] / r1["seconds"]),
             "speedup_note": "all-threads rate / one-thread rate: well below `cores` when the box exposes more cores than "
                             "its CPU quota delivers",
@@ -235,7 +249,8 @@ def run_reference(args, mode: Mode) -> None:
                          "sample": f"each step: oracle on {n} seeded points of {wl.name}"},
         "e2e": {"value": value, "unit": UNIT, "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0},
     }
-    print(json.dumps(line), flush=True)
+    line["cpu_baseline"]["value"] = line["e2e"]["value"] = _sig(value)   # the line's own value, digit for digit
+    print(headline(line), flush=True)
 
 
 def workload_config(wl, mode: Mode, n_points_per_step=None) -> dict:
@@ -255,6 +270,70 @@ def workload_config(wl, mode: Mode, n_points_per_step=None) -> dict:
     return {"workload": desc, "boundary": [wl.nx, wl.ny], "points": wl.M if n_points_per_step is None
             else n_points_per_step, "step": "dbie_create + dbie_solve" if wl.lam is None else "dbie_create + dbie_eval",
             "l2": "flushed between timed steps (256 MiB write)"}
+
+
+# --------------------------------------------------------------------------- the line ------
+def _sig(v, digits=6):
+    """Floats to `digits` significant digits (the line is read by a parser with a 3 KB window)."""
+    if isinstance(v, float):
+        return float(f"{v:.{digits}g}")
+    if isinstance(v, dict):
+        return {k: _sig(x, digits) for k, x in v.items()}
+    if isinstance(v, (list, tuple)):
+        return [_sig(x, digits) for x in v]
+    return v
+
+
+def _pick(d, keys):
+    return None if d is None else {k: d[k] for k in keys if k in d}
+
+
+HEADLINE_KEYS = ("impl", "metric", "value", "unit", "n_gpus", "steps", "warmup", "ms_per_step", "higher_is_better",
+                 "scaling", "vs_baseline", "dtype", "data", "gpu_launches")
+HEADLINE_SUB = {
+    "config": ("workload", "boundary", "points", "step", "l2", "sharding", "points_total"),
+    "clocks": ("sm_mhz", "sm_max_mhz", "power_w_max", "reasons"),
+    "e2e": ("value", "unit", "h2d_bytes_per_step", "d2h_bytes_per_step", "ms_per_step", "api"),
+    "roofline": ("bound", "kernel", "achieved", "peak", "unit", "frac", "frac_survey82", "frac_of_measured_dfma",
+                 "traffic", "kernel_ms_per_launch", "kernel_share_of_step", "fp64_instr_per_interaction",
+                 "mufu_per_interaction"),
+    "cpu_baseline": ("value", "unit", "cores", "cores_delivered", "kind", "sample"),
+}
+
+
+def headline(full: dict) -> str:
+    """The ONE line bench.py ends with: the contract keys of `full`, numbers at 6 significant digits, no prose
+    (field meanings: DESIGN.md section 7).  Always shorter than HEADLINE_MAX_BYTES: optional parts are dropped,
+    least important first, if a record would not fit (it does not happen with the records this file builds;
+    tests/test_bench_contract.py pins the size on canned numbers)."""
+    line = {k: full[k] for k in HEADLINE_KEYS if k in full}
+    for name, keys in HEADLINE_SUB.items():
+        if name in full:
+            line[name] = _pick(full[name], keys)
+    for k in ("also", "vs_previous_round", "detail"):
+        if full.get(k) is not None:
+            line[k] = full[k]
+    line = _sig(line)
+    for drop in (None, "detail", "also", "vs_previous_round"):
+        if drop:
+            line.pop(drop, None)
+        text = json.dumps(line, separators=(",", ":"))
+        if len(text) < HEADLINE_MAX_BYTES:
+            return text
+    raise RuntimeError(f"bench.py: the headline line has {len(text)} bytes (limit {HEADLINE_MAX_BYTES})")
+
+
+def emit(full: dict, detail_path: str = "") -> None:
+    """Write the full record to `detail_path` (if given), then print the headline as the last stdout line."""
+    if detail_path:
+        try:
+            os.makedirs(os.path.dirname(os.path.abspath(detail_path)), exist_ok=True)
+            with open(detail_path, "w") as f:
+                json.dump(full, f, indent=1)
+            full = dict(full, detail=detail_path)
+        except OSError as e:
+            print(f"bench.py: could not write {detail_path}: {e}", file=sys.stderr)
+    print(headline(full), flush=True)
 
 
 # --------------------------------------------------------------------------- our arm -------
@@ -376,16 +455,18 @@ def measure_f64(mode: Mode, steps: int, warmup: int, rank=0, world=1, local=0, d
     kern_ips = inter_total / (kern_ms * 1e-3) if kern_ms > 0 else 0.0
     per_inter = FP64_INSTR[kind]
     achieved_slots = kern_ips * per_inter
-    traffic = NCU_TRAFFIC.get(kind) if (mode.points == 0 and not mode.reduced and
-                                        mode.workload == ("cfg4" if not is_solve else "cfg2")) else None
-    kernel_name = ("dbie::interact64_kernel (fp64 point-pixel sums)" if (not is_solve or mode.grid) else
-                   "dbie::solve_nm_fused_kernel (whole Nelder-Mead search in one cooperative launch: point-pixel sums "
-                   "+ residual + simplex step + list compaction)")
+    traffic = ncu_traffic().get(kind) if (mode.points == 0 and not mode.reduced and
+                                          mode.workload == ("cfg4" if not is_solve else "cfg2")) else None
+    traffic = (traffic["dram_bytes_per_launch"], f"{traffic['capture']} ({traffic['date']})") if traffic else None
+    kernel_name = "dbie::interact64_kernel" if (not is_solve or mode.grid) else "dbie::solve_nm_fused_kernel"
+    kernel_what = ("fp64 point-pixel sums" if (not is_solve or mode.grid) else
+                   "whole Nelder-Mead search in one cooperative launch: point-pixel sums + residual + simplex step + "
+                   "list compaction")
     # independent-geometry rate: objective evaluations x N, without the x4 stencil or xT trial multipliers
     pos = 1.0 if (not is_solve or mode.analytic) else 4.0
     indep = (inter_total / pos / (8.0 if mode.grid else 1.0)) / (ms_total * 1e-3)
     roofline = {
-        "bound": "alu", "kernel": kernel_name,
+        "bound": "alu", "kernel": kernel_name, "kernel_what": kernel_what,
         "achieved": 2e-12 * achieved_slots, "peak": 2e-12 * peak_slots, "unit": "TFLOP/s",
         "frac": achieved_slots / peak_slots,
         "unit_note": "achieved and peak count every FP64-pipe lane-instruction (DFMA, DMUL, DADD alike) as 2 flop: "
@@ -433,7 +514,7 @@ def measure_f64(mode: Mode, steps: int, warmup: int, rank=0, world=1, local=0, d
         "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": steps,
         "warmup": warmup, "ms_per_step": ms_max / steps, "higher_is_better": True,
         "scaling": "weak", "vs_baseline": None, "dtype": "f64", "data": "synthetic",
-        "config": dict(workload_config(wl, mode), **shard_info(wl.M, rank, world),
+        "config": dict(workload_config(wl, mode), **shard_info(wl.M, rank, world), sharding=SHARDING,
                        objective_evals_per_step=evals / steps),
         "clocks": clocks,
         "e2e": e2e_line,
@@ -511,11 +592,11 @@ def measure_f32(steps: int, warmup: int, points: int = 0) -> dict:
                 "h2d_bytes_per_step": 3 * wl.N * 8 + 6 * wl.M * 4, "d2h_bytes_per_step": 3 * wl.M * 4,
                 "ms_per_step": e2e_ms / steps, "api": "DBIE(host boundary, fp32=True) + eval_f32 on pinned host points"},
         "gpu_launches": launches,
-        "roofline": {"bound": "alu", "kernel": "dbie::interact_f32_kernel (fp32 point-pixel sums, SFU sincos of the reduced argument)",
+        "roofline": {"bound": "alu", "kernel": "dbie::interact_f32_kernel",
+                     "kernel_what": "fp32 point-pixel sums, SFU sincos of the reduced argument",
                      "achieved": 1e-12 * ach, "peak": 1e-12 * peak, "unit": "T MUFU lane-op/s", "frac": ach / peak,
-                     "traffic": 51.65e6 + 359.04e6,
-                     "traffic_source": "profiles/r02_ncu_full_interact_f32_eval_cfg4.md (the launch is split over chunk "
-                                       "ranges: 403 MB of fp64 partial sums; algorithmic bytes 36 M + 16 N = 42 MB)",
+                     "traffic": (ncu_traffic().get("f32") or {}).get("dram_bytes_per_launch") if points == 0 else None,
+                     "traffic_source": (ncu_traffic().get("f32") or {}).get("capture"),
                      "mufu_per_interaction": MUFU_PER_INTERACTION,
                      "note": "SFU-bound: 148 SM x 16 MUFU lanes x clocks.max.sm / 7 MUFU per interaction (the issue port, 40 "
                              "instructions per interaction, allows 40 % more; the FP32 FMA pipe 75 % more; profiles/r02_sass_loops.txt)",
@@ -542,6 +623,7 @@ def measure_slabs(steps: int) -> dict:
     ctx.profile(True)
     sopts = dbie.default_opts(method=1)
     out = []
+    sampler = ClockSampler(0)
     for layer in (0, 31, 127):                      # z = 1, 32, 128 pixels
         idx = np.arange(layer * per, (layer + 1) * per)
         sub = full.subset(idx)
@@ -561,12 +643,14 @@ def measure_slabs(steps: int) -> dict:
                    "mean_f": float(s["f"].mean().item()), "mean_g": float(s["g"].mean().item())}
             if best is None or rec["ms"] < best["ms"]:
                 best = rec
-        peak = SM_COUNT * FP64_LANES_PER_SM * 1965e6
-        best["roofline_frac_kernel"] = best["interactions"] / (best["kernel_ms"] * 1e-3) * FP64_INSTR["grid"] / peak
         out.append(best)
     ctx.close()
+    clocks = sampler.stop()
+    peak = SM_COUNT * FP64_LANES_PER_SM * ((clocks or {}).get("sm_max_mhz") or 1965.0) * 1e6   # the sampled clocks.max.sm
+    for rec in out:
+        rec["roofline_frac_kernel"] = rec["interactions"] / (rec["kernel_ms"] * 1e-3) * FP64_INSTR["grid"] / peak
     mean_ms = float(np.mean([r["ms"] for r in out]))
-    return {"workload": "BASELINE configs[4] z-slabs: 256x256 points at z = 1, 32, 128 px, 1024x1024 boundary, GRID T=8, 10 levels",
+    return {"clocks": clocks, "workload": "BASELINE configs[4] z-slabs: 256x256 points at z = 1, 32, 128 px, 1024x1024 boundary, GRID T=8, 10 levels",
             "slabs": out, "projected_full_volume_s": mean_ms * 1e-3 * nlay,
             "note": "full volume (128 slabs, 8,388,608 points) NOT run: projected = mean slab time x 128"}
 
@@ -581,19 +665,23 @@ def run_ours(args, mode: Mode) -> None:
     if world > 1:
         import torch.distributed as dist
         os.environ.setdefault("MASTER_ADDR", "127.0.0.1")
+        # the communicator lines (rank / nranks) of NCCL's start-up let a reader of the log check the world size
+        os.environ.setdefault("NCCL_DEBUG", "INFO")
+        os.environ.setdefault("NCCL_DEBUG_SUBSYS", "INIT")
         dist.init_process_group("nccl", device_id=torch.device("cuda", local))
     if not torch.cuda.is_available():
         raise SystemExit("bench.py: no CUDA device (the CUDA path has no CPU fallback)")
     torch.cuda.set_device(local)
     dbie.load()
 
+    detail = args.detail or ("gpurun_out/bench_detail.json" if args.legs else "")
     if args.dtype == "f32":
         if rank == 0:
-            print(json.dumps(measure_f32(args.steps, args.warmup, args.points)), flush=True)
+            emit(measure_f32(args.steps, args.warmup, args.points), detail)
         return
     if args.slabs:
         if rank == 0:
-            print(json.dumps(measure_slabs(args.steps)), flush=True)
+            print(json.dumps(_sig(measure_slabs(args.steps))), flush=True)
         return
 
     line = measure_f64(mode, args.steps, args.warmup, rank, world, local, dist)
@@ -603,20 +691,30 @@ def run_ours(args, mode: Mode) -> None:
         line["cpu_baseline"] = base
         if base:
             line["gpu_over_cpu_baseline"] = line["value"] / base["value"]
-        if world == 1 and args.legs:
-            # the other legs of the same run: fewer steps each so that the default run stays within a few minutes
+        headline_default = mode.workload == "cfg4" and mode.points == 0 and not mode.analytic
+        if headline_default:
+            line["vs_previous_round"] = {"cfg4_eval": line["value"] / PREVIOUS_ROUND["cfg4_eval"]}
+        if world == 1 and headline_default and args.also:
+            # BASELINE configs[1] in the same run (two steps): the Nelder-Mead solve stays comparable round over round
             ls, lw = max(1, min(args.steps, 2)), max(1, min(args.warmup, 3))
-            legs = {}
-            legs["cfg2_nm"] = measure_f64(Mode("cfg2"), ls, lw)
-            # small-batch latency (what a line tracer calls): 48 points, the warp-per-point shape of the fused kernel
-            legs["cfg2_nm_48pts"] = measure_f64(Mode("cfg2", points=48), 5, 3)
-            legs["cfg5_grid"] = measure_f64(Mode("cfg5", grid=True, points=8192), 1, 1)
-            legs["cfg4_f32"] = measure_f32(ls, lw)
-            legs["cfg4_f64_reduced_sincos"] = measure_f64(Mode("cfg4", reduced=True), ls, lw)
+            legs = {"cfg2_nm": measure_f64(Mode("cfg2"), ls, lw, e2e=False)}
+            if args.legs:
+                # small-batch latency (what a line tracer calls): 48 points, the warp-per-point shape of the fused kernel
+                legs["cfg2_nm_48pts"] = measure_f64(Mode("cfg2", points=48), 5, 3)
+                legs["cfg5_grid"] = measure_f64(Mode("cfg5", grid=True, points=8192), 1, 1)
+                legs["cfg4_f32"] = measure_f32(ls, lw)
+                legs["cfg4_f64_reduced_sincos"] = measure_f64(Mode("cfg4", reduced=True), ls, lw)
             line["legs"] = legs
-        print(json.dumps(line), flush=True)
+            line["also"] = {k: {"value": v["value"], "ms_per_step": v["ms_per_step"], "frac": v["roofline"]["frac"]}
+                            for k, v in legs.items()}
+            line["vs_previous_round"]["cfg2_nm"] = legs["cfg2_nm"]["value"] / PREVIOUS_ROUND["cfg2_nm"]
     if dist is not None:
+        dist.barrier()
         dist.destroy_process_group()
+        if rank == 0:
+            time.sleep(1.0)      # NCCL's INFO lines of the other ranks' teardown come first: the headline stays the LAST line
+    if rank == 0:
+        emit(line, detail)
 
 
 def main():
@@ -636,13 +734,19 @@ def main():
                     help="solve/eval a seeded subset of this many points (0: the whole volume; cfg5: 16384)")
     ap.add_argument("--slabs", action="store_true",
                     help="config 5 as SURVEY 8(d) asks: GRID solve of three 65,536-point z-slabs + projected full-volume time")
-    ap.add_argument("--no-legs", dest="legs", action="store_false",
-                    help="only the headline workload (legs run by default for --workload cfg4 on one GPU)")
+    ap.add_argument("--legs", action="store_true",
+                    help="default workload on one GPU: also time the 48-point latency, config-5 GRID, fp32 and reduced-sincos "
+                         "legs; their full records go to the --detail file, their values into the line's `also`")
+    ap.add_argument("--no-also", dest="also", action="store_false",
+                    help="default workload: skip the two-step config-2 Nelder-Mead leg reported under `also`")
+    ap.add_argument("--detail", default="",
+                    help="also write the full record (every diagnostic field) to this file")
     ap.add_argument("--cpu-seconds", type=float, default=15.0,
                     help="target CPU time of the cpu_baseline leg (0 disables it)")
     args = ap.parse_args()
     if args.workload != "cfg4":
         args.legs = False
+        args.also = False
     mode = Mode(args.workload, grid=(args.method == "grid") or (args.method is None and args.workload == "cfg5"),
                 analytic=args.gradient == "analytic", points=args.points)
     if args.impl == "reference":
