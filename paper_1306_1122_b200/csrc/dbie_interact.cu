@@ -115,7 +115,7 @@ cudaError_t launch_stage_q9(int nx, int ny, double h, double x0, double y0, cons
 }
 
 // ------------------------------------------------------------------ fp64 launchers --------
-// The kernel is dbie_interact_fp64.cuh.  Shapes measured on B200 (profiles/r01_variants.md, re-checked in round 2):
+// The kernel is dbie_interact_fp64.cuh.  Shapes measured on B200 (round-1 shape sweep, re-checked in round 2):
 // 256 threads x 2 CTAs/SM (<= 128 registers), two pixels in flight per thread; GRID mode carries
 // 4 (else 2, else 1) trial lambda triples per thread on one geometry.
 constexpr int kThreads64 = 256, kMinB64 = 2;
@@ -161,7 +161,7 @@ cudaError_t launch_interact_eval(const InteractParams& p, int sm_count, bool red
 
 cudaError_t launch_interact_stencil(const InteractParams& p, int sm_count, cudaStream_t st) {
     // all 4 stencil positions of a point in one thread (one sincos per component, kernel_n_near for the offsets), two pixels in
-    // flight: 128 threads x 2 CTAs/SM; +35 % over one position per thread (MODE_STENCIL, profiles/r01_variants.md)
+    // flight: 128 threads x 2 CTAs/SM; +35 % over one position per thread (MODE_STENCIL, round-1 shape sweep)
     return launch64<MODE_STENCIL4, 1, 2, 128, 2>(p, sm_count, 16, st);
 }
 
@@ -180,7 +180,7 @@ cudaError_t launch_interact_grid_analytic(const InteractParams& p, int sm_count,
 cudaError_t launch_interact_grid(const InteractParams& p, int sm_count, cudaStream_t st) {
     if (p.T < 2) return cudaErrorInvalidValue;
     // NT > 1 shares (sin, cos)(j d_theta) between the trials, which needs window starts lo >= 0: not guaranteed for T = 2
-    // 8 trial triples per thread need 234 registers: 128 threads x 2 CTAs/SM (profiles/r01_variants.md)
+    // 8 trial triples per thread need 234 registers: 128 threads x 2 CTAs/SM (round-1 shape sweep)
     if (p.T % 8 == 0) return launch64<MODE_GRID, 8, 1, 128, 2>(p, sm_count, 16, st);
     if (p.T % 4 == 0) return launch64<MODE_GRID, 4, 1, 128, 3>(p, sm_count, 16, st);
     if (p.T % 2 == 0 && p.T > 2) return launch64<MODE_GRID, 2, 2>(p, sm_count, 16, st);

@@ -12,9 +12,9 @@
 // mbarrier, double buffered) and every thread of the CTA reads the same pixel record as a broadcast
 // LDS.128 pair; UNR pixels are in flight per thread.  sin/cos come from a 256-entry angle table that every CTA
 // keeps in shared memory (8 interleaved copies, dbie_math.cuh) plus short polynomials.  The bound is the FP64
-// pipe; the history of the stencil launch over round 1 (14.17 -> 11.11 -> 9.04 -> 8.39 ms) is in
-// profiles/r01_ncu_full_interact64_*_cfg2.md, the shape sweep behind the THREADS x MINB x UNR choices in
-// profiles/r01_variants.md, round 2's table kernel in profiles/r02_ncu_full_interact64_eval_cfg4.md.
+// pipe; the stencil launch went 14.17 -> 11.11 -> 9.04 -> 8.39 ms over round 1 (its captures and the shape sweep
+// behind the THREADS x MINB x UNR choices are in git history, profiles/r01_*), round 2's table kernel is in
+// profiles/r02_ncu_full_interact64_eval_cfg4.md.
 //
 // The body of one work item (a block of evaluation positions x a range of canonical chunks) is the
 // device function interact_item; what happens to a finished chunk sum is the caller's `sink`:
@@ -475,7 +475,7 @@ __global__ void __launch_bounds__(THREADS, MINB) interact64_kernel(const __grid_
     unsigned it = 0;  // tiles consumed by this CTA so far
     // Work items: one per CTA when the host knows the count (the hardware scheduler balances them);
     // a persistent grid (count on the device) takes them from an atomic counter in index order,
-    // which balances the same way (static striding measured 1-15 % slower, profiles/r01_variants.md).
+    // which balances the same way (static striding measured 1-15 % slower in round 1's shape sweep).
     for (long long w = blockIdx.x;; w += gridDim.x) {
         if (p.work_ctr) {
             if (tid == 0) next_item = (long long)atomicAdd(p.work_ctr, 1u);

@@ -1,6 +1,6 @@
 """SASS opcode histogram of the inner (pixel) loops of the interaction kernels.
 
-    python paper_1306_1122_b200/csrc/sass_loops.py [kernel-name-substring ...] > profiles/<name>.txt
+    python tests/sass_loops.py [kernel-name-substring ...] > profiles/<name>.txt
 
 Disassembles libdbie_b200.so with cuobjdump, finds in every matching kernel the innermost loops
 (backward branches) that contain a reciprocal square root (MUFU.RSQ64H in fp64, MUFU.RSQ in fp32:
@@ -17,7 +17,7 @@ import subprocess
 import sys
 
 HERE = os.path.dirname(os.path.abspath(__file__))
-LIB = os.path.join(os.path.dirname(HERE), "libdbie_b200.so")
+LIB = os.path.join(os.path.dirname(HERE), "paper_1306_1122_b200", "libdbie_b200.so")
 INSTR = re.compile(r"^\s+/\*([0-9a-f]{4,})\*/\s+(?:@!?U?P\d+\s+)?([A-Z0-9_.]+)(.*?);")
 FP64 = ("DFMA", "DMUL", "DADD", "DSETP", "DMNMX")
 

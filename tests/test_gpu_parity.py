@@ -281,6 +281,37 @@ def test_residual_matches_oracle(dbie, case):
     assert np.abs(r["phi"] - ro["phi"]).max() <= 2 * TOL_FG
 
 
+@pytest.mark.parametrize("alpha", [0.3, -0.3])
+def test_residual_on_the_constant_alpha_packet_gives_J_equal_alpha_B(dbie, alpha):
+    """Pin K-12 on the CUDA path: on the constant-alpha force-free packet (workloads/lff.py) at lambda = alpha,
+    dbie_residual returns J = alpha B against the closed-form field (not against its own B), div B = 0, f = g = 0
+    up to the differences of Eq. 13 / the quadrature of the analytic gradient; J . B has the sign of alpha; at
+    lambda = 0 the residuals are two orders larger.  And it agrees with the oracle element by element."""
+    import torch
+    from workloads.lff import LFFPacket
+    w, ref = LFFPacket(alpha).workload()
+    nB = np.linalg.norm(ref, axis=0)
+    with dbie.DBIE.from_workload(w) as ctx:
+        dw = dbie.to_device(w)
+        for analytic, tolJ, tolf, tolg in ((0, 6e-3, 5e-3, 2e-4), (1, 1e-4, 1e-4, 5e-6)):
+            lam = np.full((3, w.M), alpha)
+            r = ctx.residual(dw.x, dw.y, dw.z, torch.from_numpy(lam).cuda(), dbie.default_opts(analytic=analytic))
+            r = {k: v.cpu().numpy() for k, v in r.items()}
+            assert (np.linalg.norm(r["B"] - ref, axis=0) / nB).max() <= 1e-5
+            dJ = np.linalg.norm(r["J"] - alpha * ref, axis=0) / (abs(alpha) * nB)
+            assert dJ.max() <= tolJ, (analytic, dJ.max())
+            assert np.all(np.sign((r["J"] * ref).sum(axis=0)) == np.sign(alpha))
+            assert (np.abs(r["div"]) * w.h / nB).max() <= 6 * tolg
+            assert r["f"].max() <= tolf and r["g"].max() <= tolg
+            ro = oracle.residual(w, lam, oracle.Opts(analytic=analytic))
+            assert vec_relerr(r["B"], ro["B"])[0] <= TOL_B
+            assert np.all(np.abs(r["J"] - ro["J"]) <= 1e-8 * nB / w.h)
+            assert np.abs(r["f"] - ro["f"]).max() <= TOL_FG and np.abs(r["g"] - ro["g"]).max() <= TOL_FG
+            r0 = ctx.residual(dw.x, dw.y, dw.z, torch.zeros((3, w.M), dtype=torch.float64, device="cuda"),
+                              dbie.default_opts(analytic=analytic))
+            assert float(r0["f"].min()) >= 0.02 and float(r0["f"].max()) >= 0.2 and float(r0["g"].max()) >= 1e-2
+
+
 def test_residual_large_delta_takes_the_plain_stencil_path(dbie):
     """MODE_STENCIL4 derives the offset positions from one sincos per component only while lambda*delta <= 1e-3;
     with delta = 0.05 h and lambda up to 0.3/h (lambda*delta = 1.5e-2) most threads take the plain

@@ -821,3 +821,44 @@ def test_k11_linear_force_free_field_is_recovered_with_lambda_equal_alpha():
     # and the sign of the sin term / of alpha matters: lambda = 2 alpha is wrong as well
     err_2 = np.linalg.norm(oracle.eval(w, lam=np.full((3, w.M), 2 * alpha)) - ref, axis=0).max() / scale
     assert err_2 >= 3e-2, err_2
+
+
+def test_k12_residual_on_the_constant_alpha_packet_gives_J_equal_alpha_B():
+    """Pins the assembly of Eq. 14 (J = curl B: orientation and every entry), Eq. 8 (f) and Eq. 9 (g)
+     on a field for which they are known: on the constant-alpha force-free packet of
+    workloads/lff.py (the field of K-11, built there from the textbook mode solution and checked force-free by
+    differences in tests/test_workloads.py; nothing of it comes from the oracle) with lambda_x = lambda_y =
+    lambda_z = alpha, oracle.residual must return J = alpha B (closed form: alpha times the REFERENCE field, not
+    the oracle's own B), div B = 0, f = 0 and g = 0, up to the first-order differences of Eq. 13 (delta = 1e-3 h)
+    or, with the analytic gradient (O-5), up to the quadrature.  A J of the wrong sign gives |J - alpha B| =
+    2 alpha |B|, two swapped entries of the curl or a transposed gradient give O(alpha |B|); alpha -> -alpha flips
+    J.  With lambda = 0 or 2 alpha the same code reports what it should for a field that is NOT force-free with
+    that boundary: J off alpha B by more than 20 %, f and g two orders of magnitude larger."""
+    from workloads.lff import LFFPacket
+    for alpha in (0.3, -0.3):
+        w, ref = LFFPacket(alpha).workload()
+        nB = np.linalg.norm(ref, axis=0)
+        for analytic, tolJ, tolf, tolg in ((0, 6e-3, 5e-3, 2e-4), (1, 1e-4, 1e-4, 5e-6)):
+            o = oracle.Opts(analytic=analytic)
+            r = oracle.residual(w, np.full((3, w.M), alpha), o)
+            assert (np.linalg.norm(r["B"] - ref, axis=0) / nB).max() <= 1e-5          # K-11 again, through O-2
+            dJ = np.linalg.norm(r["J"] - alpha * ref, axis=0) / (abs(alpha) * nB)
+            assert dJ.max() <= tolJ, (alpha, analytic, dJ.max())
+            # orientation, said once more without a tolerance on the size: J . B has the sign of alpha everywhere
+            assert np.all(np.sign((r["J"] * ref).sum(axis=0)) == np.sign(alpha))
+            assert (np.abs(r["div"]) * w.h / nB).max() <= 6 * tolg
+            assert r["f"].max() <= tolf and r["g"].max() <= tolg, (alpha, analytic, r["f"].max(), r["g"].max())
+            assert np.all(r["f"] >= 0) and np.all(r["g"] >= 0)
+            assert np.allclose(r["phi"], r["f"] + r["g"], rtol=0, atol=1e-15)         # reading A-7, w_g = 1
+            for lam_wrong in (0.0, 2 * alpha):
+                rw = oracle.residual(w, np.full((3, w.M), lam_wrong), o)
+                dJw = np.linalg.norm(rw["J"] - alpha * ref, axis=0) / (abs(alpha) * nB)
+                assert dJw.max() >= 0.2
+                assert rw["f"].min() >= 0.02 and rw["f"].max() >= 0.2 and rw["g"].max() >= 1e-2
+                assert np.all(rw["phi"] > r["phi"])
+    # alpha -> -alpha mirrors the packet's transverse field and flips J (checked above through the sign of J . B);
+    # and the three components of J are each pinned: rotate which component carries the error
+    w, ref = LFFPacket(0.3).workload()
+    r = oracle.residual(w, np.full((3, w.M), 0.3), oracle.Opts(analytic=1))
+    for c in range(3):
+        assert np.abs(r["J"][c] - 0.3 * ref[c]).max() <= 1e-4 * 0.3 * np.linalg.norm(ref, axis=0).max()

@@ -1,6 +1,7 @@
 """Self-checks of the seeded input generators (workloads/) and the solver-level
 pins S-2 / S-3 of DESIGN.md on an oracle-sized subset of config 2."""
 import numpy as np
+import pytest
 
 import oracle
 from workloads import CONFIGS, config2, config3, config4
@@ -91,3 +92,32 @@ def test_lowlou_case2_generator_and_figures_of_merit():
     assert abs(m2["E_n_prime"]) < 1e-12 and abs(m2["E_m_prime"]) < 1e-12
     m3 = figures_of_merit(Bx, -Bx)
     assert abs(m3["C_vec"] + 1) < 1e-12 and abs(m3["E_n_prime"] + 1) < 1e-12
+
+
+def test_lff_packet_generator_is_force_free_with_constant_alpha():
+    """workloads/lff.py (the input of pins K-12 and of the GPU test of dbie_residual): curl B = alpha B and
+    div B = 0 by differences (spectral in x, y; central in z) for both signs of alpha; the boundary window
+    holds the packet (1e-9 of its peak at the edge); the points' reference values are the field there."""
+    from workloads.lff import LFFPacket
+    for alpha in (0.3, -0.3):
+        p = LFFPacket(alpha)
+        e = 1e-3
+        Bm, B0, Bp = p.at(4.0 - e), p.at(4.0), p.at(4.0 + e)
+        ddz = [(a - b) / (2 * e) for a, b in zip(Bp, Bm)]
+        spec = lambda f, K: np.real(np.fft.ifft2(1j * K * np.fft.fft2(f)))
+        curl = [spec(B0[2], p.KY) - ddz[1], ddz[0] - spec(B0[2], p.KX), spec(B0[1], p.KX) - spec(B0[0], p.KY)]
+        sc = max(np.abs(b).max() for b in B0)
+        for cq, bq in zip(curl, B0):
+            assert np.abs(cq - alpha * bq).max() <= 1e-6 * sc
+        assert np.abs(spec(B0[0], p.KX) + spec(B0[1], p.KY) + ddz[2]).max() <= 1e-6 * sc
+        w, ref = p.workload()
+        assert (w.nx, w.ny, w.M) == (256, 256, 108) and ref.shape == (3, 108)
+        bz = w.bz.reshape(256, 256)
+        assert max(np.abs(bz[0]).max(), np.abs(bz[:, 0]).max()) <= 1e-8 * np.abs(bz).max()
+        # a point of the list sits on a pixel centre of the boundary grid, at the stated height
+        i = 37
+        ix = int(round((w.x[i] - w.x0) / w.h - 0.5)); iy = int(round((w.y[i] - w.y0) / w.h - 0.5))
+        o = (p.n - 256) // 2
+        assert abs(p.at(w.z[i])[2][o + iy, o + ix] - ref[2, i]) == 0.0
+    with pytest.raises(ValueError):
+        LFFPacket(0.9)                                           # modes with |k| <= 1.2 alpha would not decay
