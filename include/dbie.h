@@ -41,6 +41,10 @@
  *  - Devices: a context belongs to the CUDA device that was current in dbie_create.  Every later
  *    entry point makes that device current for the duration of the call and restores the caller's
  *    device before returning; the arrays and the stream passed in must belong to the context's device.
+ *    The Nelder-Mead dbie_solve (and a lambda-solving dbie_trace) runs as ONE cooperative launch: the device must
+ *    support cooperative launches (else DBIE_ESTATE; the GRID method does not need them), and the grid must be
+ *    co-resident.  Where the context may use only part of the SMs (MPS active-thread percentage, green contexts) the
+ *    launch is retried with smaller grids; results do not depend on the grid.
  *  - Range of lambda: theta = |lambda| r must stay below 2^20 (about 1e6 rad) for every point-pixel
  *    pair; the one-step argument reduction of the kernel is exact up to theta * 4e-17 there (relative
  *    to theta: the same size as the rounding of theta itself).  Beyond that the result is unspecified
@@ -114,6 +118,10 @@ dbie_status dbie_eval_host(dbie_ctx* ctx, long long M, const double* x, const do
  * (north_star): relative vector error <= 2e-4 against the fp64 definition. */
 dbie_status dbie_eval_f32(dbie_ctx* ctx, long long M, const float* x, const float* y,
                           const float* z, const float* lam, float* B, void* cuda_stream);
+/* Same with HOST arrays (BASELINE.json config 4 "fp64 and fp32": the end-to-end leg of the fp32 variant): the
+ * copies in and out are inside the call, which returns when B is in the host array. */
+dbie_status dbie_eval_f32_host(dbie_ctx* ctx, long long M, const float* x, const float* y,
+                               const float* z, const float* lam, float* B);
 
 /* dbie_eval for callers that must not allocate device memory.
  *
@@ -164,7 +172,7 @@ typedef struct {
     double step;      /*   0.05, 0.05 (reading A-9)                                           */
     double xtol;      /* NM stop: max |V_j - V_0| <= xtol/h and max |Phi_j - Phi_0| <= ftol;  */
     double ftol;      /*   1e-4, 1e-6                                                         */
-    int maxiter;      /* NM iteration cap; 200                                                */
+    int maxiter;      /* NM iteration cap; 200 (0 <= maxiter <= 2^24, else DBIE_EINVAL)                 */
     int n_trial;      /* GRID: T trial lambda per component per level, 4 <= T <= 32 (else
                          DBIE_EINVAL: below 4 the refined window 2W/(T-1) does not shrink); 8.
                          Multiples of 8 (then 4, then 2) run fastest.                            */
@@ -239,7 +247,9 @@ dbie_status dbie_trace(dbie_ctx* ctx, long long L, const double* x0, const doubl
 /* Counters of the last eval/solve/residual call on this context (host values, valid after
  * the stream has been synchronised): point-pixel interactions evaluated (one interaction =
  * one (evaluation point, pixel) pair, all three components), kernel launches enqueued, and
- * objective evaluations.  Any pointer may be NULL. */
+ * objective evaluations.  Any pointer may be NULL.  After dbie_trace the interactions and evaluations cover the
+ * eval / residual calls of the trace only: the lambda searches of a lambda-solving trace are NOT included (each inner
+ * solve restarts the device counter), so treat them as undefined there. */
 dbie_status dbie_last_counters(dbie_ctx* ctx, double* interactions, long long* launches,
                                long long* objective_evals);
 
@@ -253,7 +263,9 @@ dbie_status dbie_last_kernel_time(dbie_ctx* ctx, double* interact_ms, long long*
 /* Profile mode, Nelder-Mead solve: the pass timeline of the LAST fused launch of the last dbie_solve call (its last
  * batch).  active[i] = points still searching at the start of pass i, ms[i] = duration of pass i on the device
  * (%globaltimer of CTA 0 at consecutive pass starts).  cap: capacity of the two host arrays; *npass = passes of the
- * launch (may exceed cap; 0 if nothing was recorded).  Synchronises the device. */
+ * launch (may exceed cap; 0 if nothing was recorded, and 0 whenever the context's LAST call was anything but a
+ * profiled Nelder-Mead dbie_solve: an eval, residual, GRID solve or trace in between invalidates the timeline).  At
+ * most the first 65,536 passes of a launch are recorded.  Synchronises the device. */
 dbie_status dbie_last_pass_trace(dbie_ctx* ctx, int cap, long long* active, double* ms, int* npass);
 
 /* Measured peak of the FP64 pipe: runs a register-only DFMA loop on every SM for about

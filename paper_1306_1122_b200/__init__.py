@@ -70,6 +70,7 @@ def load() -> C.CDLL:
     lib.dbie_eval.argtypes = [_vp, C.c_longlong, _vp, _vp, _vp, _vp, _vp, _vp]
     lib.dbie_eval_host.argtypes = [_vp, C.c_longlong, _vp, _vp, _vp, _vp, _vp]
     lib.dbie_eval_f32.argtypes = [_vp, C.c_longlong, _vp, _vp, _vp, _vp, _vp, _vp]
+    lib.dbie_eval_f32_host.argtypes = [_vp, C.c_longlong, _vp, _vp, _vp, _vp, _vp]
     lib.dbie_eval_noalloc.argtypes = [_vp, C.c_longlong, _vp, _vp, _vp, _vp, _vp, _vp]
     lib.dbie_noalloc_max_points.argtypes = []
     lib.dbie_noalloc_max_points.restype = C.c_longlong
@@ -291,6 +292,19 @@ class DBIE:
                                             _dev_f32(z, M, "z"), _dev_f32(lam, 3 * M, "lam"),
                                             _dev_f32(out, 3 * M, "out"), _stream_ptr(stream)))
         return out
+
+    def eval_f32_host(self, x, y, z, lam) -> np.ndarray:
+        """dbie_eval_f32_host: float32 numpy in, (3, M) float32 numpy out; the copies are inside the call."""
+        x = np.ascontiguousarray(x, dtype=np.float32)
+        M = x.size
+        y, z = (np.ascontiguousarray(a, dtype=np.float32) for a in (y, z))
+        lam = np.ascontiguousarray(lam, dtype=np.float32)
+        if y.size != M or z.size != M or lam.size != 3 * M:
+            raise ValueError("eval_f32_host: y, z need M elements and lam 3 M")
+        B = np.empty((3, M), dtype=np.float32)
+        self._check(self._lib.dbie_eval_f32_host(self._h, M, _vp(x.ctypes.data), _vp(y.ctypes.data),
+                                                 _vp(z.ctypes.data), _vp(lam.ctypes.data), _vp(B.ctypes.data)))
+        return B
 
     def set_f32_sfu_mask(self, mask: int):
         """dbie_set_f32_sfu_mask: which components take sin/cos from the SFU (0, 1, 3 or 7)."""

@@ -45,12 +45,16 @@ struct dbie_ctx {
     int profile;                              // record CUDA events around every interaction launch
     unsigned long long* pass_trace;           // profile mode: pass timeline of the last fused Nelder-Mead launch
     int pass_trace_cap;
+    bool pass_trace_valid;                    // the buffer holds the timeline of the LAST call (a profiled NM solve); any other call clears it
+    int coop_launch;                          // cudaDevAttrCooperativeLaunch of the device (the Nelder-Mead solve needs it)
     cudaEvent_t* ev;    int ev_cap, ev_n;     // event pairs of the last call (profile mode)
     char err[256];
 };
 
 static char g_err[256] = "no error";
 static const size_t kCounterBytes = 128;   // device counters: list lengths [0..2], objective evaluations (u64) at +16 B, work items at +32 B
+static const int kMaxIter = 1 << 24;       // dbie_solve_opts.maxiter above this is refused (the pass bound 5 maxiter + 5 stays far inside int)
+static const int kPassTraceMax = 1 << 16;  // profile mode records at most this many passes of a fused launch (1 MiB)
 static const int kDefaultF32SfuMask = 7;   // sin/cos of the reduced argument from the SFU for all three components:
                                            // measured fastest (4.90e11 vs 4.26e11 interactions/s with polynomials), same accuracy
 
@@ -144,7 +148,7 @@ extern "C" dbie_status dbie_last_pass_trace(dbie_ctx* ctx, int cap, long long* a
     if (!ctx || cap < 0 || !npass || (cap > 0 && (!active || !ms))) return DBIE_EINVAL;
     GUARD_DEVICE();
     *npass = 0;
-    if (!ctx->pass_trace) return DBIE_OK;
+    if (!ctx->pass_trace || !ctx->pass_trace_valid) return DBIE_OK;   // the last call was not a profiled Nelder-Mead solve
     CU(cudaDeviceSynchronize());
     const int n = ctx->pass_trace_cap;
     unsigned long long* h = (unsigned long long*)malloc(sizeof(unsigned long long) * 2 * n);
@@ -257,6 +261,9 @@ extern "C" dbie_status dbie_create(dbie_ctx** out, int nx, int ny, double h, dou
         if ((e = cudaDeviceGetAttribute(&ctx->sm_count, cudaDevAttrMultiProcessorCount, ctx->device)) != cudaSuccess) {
             st = fail_cuda(ctx, e, "cudaDeviceGetAttribute"); break;
         }
+        if ((e = cudaDeviceGetAttribute(&ctx->coop_launch, cudaDevAttrCooperativeLaunch, ctx->device)) != cudaSuccess) {
+            st = fail_cuda(ctx, e, "cudaDeviceGetAttribute(cooperative launch)"); break;
+        }
         BoundaryView& b = ctx->bd;
         const bool q9 = (flags & DBIE_QUAD_9NODE) != 0;
         ctx->eval_reduced = (flags & DBIE_EVAL_REDUCED_SINCOS) != 0;
@@ -355,6 +362,7 @@ extern "C" dbie_status dbie_eval(dbie_ctx* ctx, long long M, const double* x, co
     ctx->last_launches = launches;
     ctx->last_evals = 0;
     ctx->evals_on_device = 0;
+    ctx->pass_trace_valid = false;
     return DBIE_OK;
 }
 
@@ -449,6 +457,7 @@ extern "C" dbie_status dbie_eval_noalloc(dbie_ctx* ctx, long long M, const doubl
     ctx->last_launches = 2;
     ctx->last_evals = 0;
     ctx->evals_on_device = 0;
+    ctx->pass_trace_valid = false;
     return DBIE_OK;
 }
 
@@ -489,6 +498,34 @@ extern "C" dbie_status dbie_eval_f32(dbie_ctx* ctx, long long M, const float* x,
     ctx->last_launches = launches;
     ctx->last_evals = 0;
     ctx->evals_on_device = 0;
+    ctx->pass_trace_valid = false;
+    return DBIE_OK;
+}
+
+extern "C" dbie_status dbie_eval_f32_host(dbie_ctx* ctx, long long M, const float* x, const float* y, const float* z,
+                                          const float* lam, float* B) {
+    if (!ctx || M < 0) return DBIE_EINVAL;
+    if (!ctx->rec32) {
+        snprintf(ctx->err, 256, "dbie_eval_f32_host: the context was created without DBIE_WITH_FP32");
+        return DBIE_ESTATE;
+    }
+    if (M == 0) return DBIE_OK;
+    if (!x || !y || !z || !lam || !B) return DBIE_EINVAL;
+    GUARD_DEVICE();
+    const size_t m = (size_t)M * sizeof(float);
+    CU(cudaDeviceSynchronize());   // earlier work on this context may be in flight on another stream
+    dbie_status s = io_reserve(ctx, 9 * m);
+    if (s != DBIE_OK) return s;
+    float* d = (float*)ctx->io;   // x, y, z, lam[3], B[3]
+    cudaStream_t st = ctx->own_stream;
+    CU(cudaMemcpyAsync(d, x, m, cudaMemcpyHostToDevice, st));
+    CU(cudaMemcpyAsync(d + M, y, m, cudaMemcpyHostToDevice, st));
+    CU(cudaMemcpyAsync(d + 2 * M, z, m, cudaMemcpyHostToDevice, st));
+    CU(cudaMemcpyAsync(d + 3 * M, lam, 3 * m, cudaMemcpyHostToDevice, st));
+    s = dbie_eval_f32(ctx, M, d, d + M, d + 2 * M, d + 3 * M, d + 6 * M, st);
+    if (s != DBIE_OK) return s;
+    CU(cudaMemcpyAsync(B, d + 6 * M, 3 * m, cudaMemcpyDeviceToHost, st));
+    CU(cudaStreamSynchronize(st));
     return DBIE_OK;
 }
 
@@ -503,7 +540,7 @@ static dbie_status make_consts(const dbie_ctx* ctx, const dbie_solve_opts* o, NM
     dbie_solve_opts d;
     if (!o) { dbie_solve_default_opts(&d); o = &d; }
     const double h = ctx->bd.h;
-    if (!(o->delta > 0.0) || !(o->cell > 0.0) || !isfinite(o->w_g) || o->maxiter < 0 || !(o->xtol >= 0.0) ||
+    if (!(o->delta > 0.0) || !(o->cell > 0.0) || !isfinite(o->w_g) || o->maxiter < 0 || o->maxiter > kMaxIter || !(o->xtol >= 0.0) ||
         !(o->ftol >= 0.0) || !isfinite(o->lam0) || !isfinite(o->step) || o->step == 0.0)
         return DBIE_EINVAL;
     k->delta_abs = o->delta * h;
@@ -559,6 +596,7 @@ extern "C" dbie_status dbie_residual(dbie_ctx* ctx, long long M, const double* x
     ctx->last_launches = launches;
     ctx->last_evals = M;
     ctx->evals_on_device = 0;
+    ctx->pass_trace_valid = false;
     return DBIE_OK;
 }
 
@@ -569,6 +607,7 @@ static size_t align256(size_t v) { return (v + 255) & ~(size_t)255; }
 static dbie_status solve_grid(dbie_ctx* ctx, long long M, const double* x, const double* y, const double* z,
                               const dbie_solve_opts* opts, const NMConsts& k, double* B, double* lam, double* resid,
                               int* iters, int* status, void* cuda_stream) {
+    ctx->pass_trace_valid = false;
     const int T = opts->n_trial, L = opts->n_level;
     // T < 4: the refined window 2W/(T-1) would not shrink (T = 3) or would grow (T = 2)
     if (T < 4 || T > kGridMaxTrials || L < 1 || !(opts->lam_max > 0.0) || !isfinite(opts->lam_max)) return DBIE_EINVAL;
@@ -655,6 +694,12 @@ extern "C" dbie_status dbie_solve(dbie_ctx* ctx, long long M, const double* x, c
     if (s != DBIE_OK) return s;
     if (opts && opts->method == 1) return solve_grid(ctx, M, x, y, z, opts, k, B, lam, resid, iters, status, cuda_stream);
     if (opts && opts->method != 0) return DBIE_EINVAL;
+    ctx->pass_trace_valid = false;
+    if (!ctx->coop_launch) {
+        snprintf(ctx->err, 256, "dbie_solve: the Nelder-Mead search is one cooperative launch and this device does not "
+                 "support cooperative launches (cudaDevAttrCooperativeLaunch = 0); method = 1 (GRID) does not need them");
+        return DBIE_ESTATE;
+    }
     cudaStream_t st = (cudaStream_t)cuda_stream;
     const long long cap = M < stencil_batch(ctx) ? M : stencil_batch(ctx);
     s = ensure(ctx, (void**)&ctx->part, &ctx->part_bytes, (size_t)ctx->bd.nchunks * 12 * cap * sizeof(double));
@@ -709,17 +754,18 @@ extern "C" dbie_status dbie_solve(dbie_ctx* ctx, long long M, const double* x, c
         f.nact3 = ctx->counters;
         f.work3 = ctx->counters + 8;
         f.done = done;
-        f.maxpass = 4 + 5 * k.maxiter + 1;
-        if (ctx->profile) {   // diagnostic: (active points, time stamp) of every pass of this launch
-            const int need = f.maxpass + 1;
+        f.maxpass = 4 + 5 * k.maxiter + 1;   // 4 initial evaluations + at most 5 per iteration; maxiter <= kMaxIter, so no overflow
+        if (ctx->profile) {   // diagnostic: (active points, time stamp) of every pass of this launch, the first kPassTraceMax of them
+            const int need = (f.maxpass < kPassTraceMax ? f.maxpass : kPassTraceMax) + 1;
             if (ctx->pass_trace_cap < need) {
-                cudaFree(ctx->pass_trace);
+                if (ctx->pass_trace) CU(cudaFree(ctx->pass_trace));
                 ctx->pass_trace = nullptr; ctx->pass_trace_cap = 0;
                 CU(cudaMalloc(&ctx->pass_trace, sizeof(unsigned long long) * 2 * need));
                 ctx->pass_trace_cap = need;
             }
             CU(cudaMemsetAsync(ctx->pass_trace, 0, sizeof(unsigned long long) * 2 * need, st));
             f.trace = ctx->pass_trace; f.trace_cap = need;
+            ctx->pass_trace_valid = true;
         }
         prof_mark(ctx, st);
         int nl = 0;

@@ -179,7 +179,7 @@ cudaError_t launch_interact_grid_analytic(const InteractParams& p, int sm_count,
 
 cudaError_t launch_interact_grid(const InteractParams& p, int sm_count, cudaStream_t st) {
     if (p.T < 2) return cudaErrorInvalidValue;
-    // NT > 1 shares (sin, cos)(j d_theta) between the trials, which needs window starts lo >= 0: not guaranteed for T = 2
+    // NT > 1 shares (sin, cos)(j d_theta) between the trials, which needs window starts lo >= 0 (dbie_solve accepts T >= 4 only)
     // 8 trial triples per thread need 234 registers: 128 threads x 2 CTAs/SM (round-1 shape sweep)
     if (p.T % 8 == 0) return launch64<MODE_GRID, 8, 1, 128, 2>(p, sm_count, 16, st);
     if (p.T % 4 == 0) return launch64<MODE_GRID, 4, 1, 128, 3>(p, sm_count, 16, st);

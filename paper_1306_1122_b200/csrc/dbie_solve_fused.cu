@@ -353,10 +353,20 @@ static cudaError_t launch_fused(const FusedParams& p, int sm_count, cudaStream_t
     if (blocks_per_sm < 1) return cudaErrorLaunchOutOfResources;
     if (blocks_per_sm > kFusedMinB) blocks_per_sm = kFusedMinB;
     FusedParams q = p;
-    const int grid = sm_count * blocks_per_sm;
-    q.warp_items_max = 11 * grid;   // warp shape while its items fit ~11 rounds of the grid (one item costs ~1/11 of a thread-shape item)
-    void* args[] = {(void*)&q};
-    return cudaLaunchCooperativeKernel((const void*)kern, dim3(grid), dim3(kFusedThreads), args, kFusedSmem, st);
+    // The grid must be co-resident.  sm_count is the device's; a context that may use only part of the SMs (MPS with
+    // an active-thread percentage, a green context, a profiler holding SMs back) refuses that grid with
+    // cudaErrorCooperativeLaunchTooLarge: shrink it by an eighth of the device at a time until it is accepted.  Work
+    // items come from an atomic counter and sums are added in canonical chunk order, so any grid gives the same bits.
+    const int full = sm_count * blocks_per_sm;
+    const int dec = full / 8 > 0 ? full / 8 : 1;
+    for (int grid = full; grid >= 1; grid -= dec) {
+        q.warp_items_max = 11 * grid;   // warp shape while its items fit ~11 rounds of the grid (one item costs ~1/11 of a thread-shape item)
+        void* args[] = {(void*)&q};
+        e = cudaLaunchCooperativeKernel((const void*)kern, dim3(grid), dim3(kFusedThreads), args, kFusedSmem, st);
+        if (e != cudaErrorCooperativeLaunchTooLarge) return e;
+        (void)cudaGetLastError();       // not sticky: try a smaller grid
+    }
+    return cudaErrorCooperativeLaunchTooLarge;
 }
 
 cudaError_t launch_solve_nm_fused(const FusedParams& p, int sm_count, int* launches, cudaStream_t st) {

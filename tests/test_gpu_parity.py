@@ -1,8 +1,9 @@
 """GPU parity: the CUDA path (through the C ABI, libdbie_b200.so) against the CPU oracle on the
 same seeded inputs.  Tolerances (BASELINE.json north_star; derivation in DESIGN.md section 8):
   B      : max_i ||dB_i|| / ||B_i||  <= 1e-9 over points with ||B_i|| >= 1e-6 max ||B||
-  lambda : | |lam|_gpu - |lam|_orc | * h <= 1e-6 with identical status and iteration count on >= 95 %
-           of the valid points of every solve batch; the rest must be explained forks (protocol P-4)
+  lambda : | |lam|_gpu - |lam|_orc | * h <= 1e-6 with identical status and iteration count on >= 99 %
+           of the valid points of every solve batch (measured: 100 %; samples below 150 points may hold one
+           fork); every other point must be an explained fork: oracle margin < 1e-7 (protocol P-4)
   f, g   : 1e-6 absolute
 """
 import numpy as np
@@ -236,6 +237,25 @@ def test_eval_f32_ragged_boundaries(dbie, nx, ny):
     assert err <= TOL_B_F32, err
 
 
+def test_eval_f32_host_entry_matches_the_device_entry(dbie):
+    """dbie_eval_f32_host (host float arrays, copies inside the call) returns the bits of dbie_eval_f32; it needs the
+    fp32 copy of the boundary like the device entry, and M = 0 is a no-op."""
+    w = _f32_inputs(workloads.random_boundary(70, 33, seed=8, npts=1111, h=0.5))
+    f = lambda a: np.ascontiguousarray(a, dtype=np.float32)
+    with dbie.DBIE.from_workload(w, fp32=True) as ctx:
+        Bh = ctx.eval_f32_host(f(w.x), f(w.y), f(w.z), f(w.lam))
+        assert Bh.dtype == np.float32 and Bh.shape == (3, w.M)
+        assert ctx.eval_f32_host(f(w.x[:0]), f(w.y[:0]), f(w.z[:0]), f(w.lam[:, :0])).shape == (3, 0)
+    Bd = gpu_eval_f32(dbie, w, mask=7)
+    assert np.array_equal(Bh.astype(np.float64), Bd)
+    err, _ = vec_relerr(Bd, oracle.eval(w), floor=1e-3)
+    assert err <= TOL_B_F32
+    with dbie.DBIE.from_workload(w) as ctx:          # no DBIE_WITH_FP32
+        with pytest.raises(dbie.DBIEError) as ei:
+            ctx.eval_f32_host(f(w.x), f(w.y), f(w.z), f(w.lam))
+        assert ei.value.status == dbie.DBIE_ESTATE
+
+
 def test_eval_f32_needs_the_fp32_copy_and_handles_invalid_points(dbie):
     import torch
     w = _f32_inputs(workloads.random_boundary(20, 12, seed=3, npts=9))
@@ -337,7 +357,7 @@ def test_residual_large_delta_takes_the_plain_stencil_path(dbie):
 
 
 # ---------------------------------------------------------------------------- solve --------
-def _check_solve_parity(dbie, wl, opts_kw=None, gpu=None, min_same=0.95):
+def _check_solve_parity(dbie, wl, opts_kw=None, gpu=None, min_same=0.99):
     """Protocol P-4; opts_kw["method"] = 1 selects GRID on both sides.
     `gpu`: results already computed on the GPU for exactly the points of `wl` (a sample of a
     larger launch); otherwise the points of `wl` are solved here.
@@ -592,7 +612,7 @@ def test_solve_config3_whole_volume_sampled(dbie):
     w = workloads.config3()
     assert w.M == 1048576
     (_, _, info), s = _solve_full_and_sample(dbie, w, 64)
-    assert info["same_frac"] >= 0.95
+    assert info["forked"] <= 1
     assert 0.005 < float(np.mean(s["f"])) < 0.5
 
 
@@ -614,6 +634,44 @@ def test_grid_config5_large_batch_sampled(dbie):
     re-solved by the oracle."""
     w, _ = workloads.config5().seeded_subset(16384, seed_offset=900)
     _solve_full_and_sample(dbie, w, 6, dict(method=1, n_level=3))
+
+
+def test_grid_config5_z_slab_at_the_timed_shape(dbie):
+    """BASELINE configs[4] at the launch shape `bench.py --slabs` times and projects the full volume from: ONE
+    z-slab of 256 x 256 = 65,536 points (z = 32 px) of the 256x256x128 volume, 1024x1024 boundary, GRID with
+    T = 8 and all 10 levels, in one dbie_solve call.  8 seeded points of the slab are re-solved by
+    orc_solve_grid (2.7e9 oracle interactions) and solved again alone on the GPU (bit-identical)."""
+    full = workloads.config5()
+    per = full.M // 128
+    assert per == 65536
+    slab = full.subset(np.arange(31 * per, 32 * per))
+    assert np.all(slab.z == slab.z[0]) and abs(slab.z[0] / full.h - 32.0) < 1e-9
+    (_, so, info), s = _solve_full_and_sample(dbie, slab, 8, dict(method=1))
+    assert np.all(so["iters"][so["status"] == 1] == 10)
+    assert np.isin(s["iters"], np.arange(1, 11)).all()
+
+
+def test_eval_f32_config4_full_size_sampled(dbie):
+    """BASELINE configs[3], fp32 leg, in the launch configuration bench.py times: the full M = 1,048,576 launch
+    of dbie_eval_f32 (unsplit work items, fp64 chunk sums); 192 seeded outputs recomputed one by one by the fp64
+    oracle (<= 2e-4 relative vector error), and the launch is bitwise reproducible."""
+    import torch
+    w = _f32_inputs(workloads.config4())
+    t = lambda a: torch.from_numpy(np.ascontiguousarray(a, dtype=np.float32)).cuda()
+    with dbie.DBIE.from_workload(w, fp32=True) as ctx:
+        x, y, z, lam = t(w.x), t(w.y), t(w.z), t(w.lam)
+        B = ctx.eval_f32(x, y, z, lam)
+        B2 = ctx.eval_f32(x, y, z, lam)
+        assert torch.equal(B, B2) and bool(torch.isfinite(B).all())
+        assert ctx.counters()["interactions"] == float(w.M) * w.N
+        # a result does not depend on the batch it was computed in (chunk sums in canonical order)
+        idx = torch.arange(70000, 70000 + 1500, device="cuda")
+        Bs = ctx.eval_f32(x[idx].contiguous(), y[idx].contiguous(), z[idx].contiguous(), lam[:, idx].contiguous())
+        assert torch.equal(Bs, B[:, idx])
+        B = B.cpu().numpy().astype(np.float64)
+    sub, idx = w.seeded_subset(192)
+    err, dropped = vec_relerr(B[:, idx], oracle.eval(sub))
+    assert err <= TOL_B_F32 and dropped == 0, err
 
 
 # ------------------------------------------- analytic gradient (SURVEY 8(f) f1, DESIGN.md O-5) -
@@ -1004,7 +1062,47 @@ def test_pass_trace_of_the_fused_solve(dbie):
         s = ctx.solve(dw.x, dw.y, dw.z)
         t = ctx.pass_trace()
         c = ctx.counters()
+        # the timeline belongs to the LAST call only: an unprofiled solve, a GRID solve, an eval or a residual after
+        # the profiled solve invalidates it (it used to keep reporting the old launch)
+        import torch
+        lam0 = torch.zeros((3, w.M), dtype=torch.float64, device="cuda")
+        for other in (lambda: ctx.eval(dw.x, dw.y, dw.z, lam0), lambda: ctx.residual(dw.x, dw.y, dw.z, lam0),
+                      lambda: ctx.solve(dw.x[:64].contiguous(), dw.y[:64].contiguous(), dw.z[:64].contiguous(),
+                                        dbie.default_opts(method=1, n_level=2))):
+            ctx.solve(dw.x, dw.y, dw.z)
+            assert ctx.pass_trace()["npass"] == t["npass"]
+            other()
+            assert ctx.pass_trace()["npass"] == 0
+        ctx.profile(False)
+        ctx.solve(dw.x, dw.y, dw.z)
+        assert ctx.pass_trace()["npass"] == 0
     assert t["npass"] == len(t["active"]) > 50
     assert t["active"][0] == w.M and np.all(np.diff(t["active"]) <= 0) and t["active"][-1] > 0
     assert int(t["active"].sum()) == c["objective_evals"]
     assert np.all(t["ms"] > 0) and t["ms"].sum() < 1e4
+
+
+def test_maxiter_is_bounded_and_a_capped_search_reports_status_2(dbie):
+    """dbie_solve_opts.maxiter above 2^24 is refused (5 maxiter + 5 passes would overflow int near 4.3e8 and the
+    fused kernel would then run zero passes and return DBIE_OK with nothing written); maxiter = 0 and 1 are legal
+    and every valid point then ends with status 2 (or an earlier stop) and finite outputs."""
+    w, _ = workloads.config2().seeded_subset(64, seed_offset=11)
+    with dbie.DBIE.from_workload(w) as ctx:
+        dw = dbie.to_device(w)
+        for bad in ((1 << 24) + 1, 500_000_000, 2 ** 31 - 1, -1):
+            with pytest.raises(dbie.DBIEError) as ei:
+                ctx.solve(dw.x, dw.y, dw.z, dbie.default_opts(maxiter=bad))
+            assert ei.value.status == dbie.DBIE_EINVAL
+        ctx.profile(True)                                       # the pass-trace buffer is capped too, not sized from maxiter
+        big = ctx.solve(dw.x, dw.y, dw.z, dbie.default_opts(maxiter=1 << 24))
+        ref = ctx.solve(dw.x, dw.y, dw.z)
+        import torch
+        npass_ref = ctx.pass_trace()["npass"]
+        m = ref["status"] != 2                                  # points the default cap of 200 did not cut short
+        assert int(m.sum()) > 0 and torch.equal(big["lam"][:, m], ref["lam"][:, m]) and torch.equal(big["B"][:, m], ref["B"][:, m])
+        assert int((big["status"] == 2).sum()) == 0 and 0 < npass_ref <= 65536
+        for mi in (0, 1):
+            s = ctx.solve(dw.x, dw.y, dw.z, dbie.default_opts(maxiter=mi))
+            st = s["status"].cpu().numpy()
+            assert np.all((st == 2) | (st == 0) | (st == 1)) and (st == 2).sum() > 0
+            assert bool(torch.isfinite(s["B"]).all()) and int(s["iters"].max()) <= mi
