@@ -161,6 +161,39 @@ def test_eval_edge_cases(dbie):
     assert np.isnan(oracle.eval(wb)[:, 2]).all()
 
 
+def test_blocks_of_invalid_points_are_skipped_without_changing_the_others(dbie):
+    """dbie_eval / dbie_residual skip the pixel loop of a 256- (128-) point block whose every point is invalid (what
+    dbie_trace hands over for stopped lines: z = -1): those outputs are NaN as before, and every other point keeps its
+    bits, whether its block holds invalid neighbours or not."""
+    import torch
+    w = workloads.random_boundary(96, 80, seed=21, npts=1500, h=0.7)
+    dead = np.zeros(w.M, dtype=bool)
+    dead[256:1024] = True                       # three whole eval blocks (six residual blocks)
+    dead[[3, 1100, 1499]] = True                # and stragglers inside live blocks
+    z = w.z.copy(); z[dead] = -1.0; z[300] = np.nan; z[301] = 0.0
+    with dbie.DBIE.from_workload(w) as ctx:
+        d = dbie.to_device(w)
+        dz = torch.from_numpy(z).cuda()
+        ref = ctx.eval(d.x, d.y, d.z, d.lam)
+        B = ctx.eval(d.x, d.y, dz, d.lam)
+        assert bool(torch.isnan(B[:, dead]).all()) and torch.equal(B[:, ~dead], ref[:, ~dead])
+        rref = ctx.residual(d.x, d.y, d.z, d.lam)
+        for an in (0, 1):
+            o = dbie.default_opts(analytic=an)
+            rr = ctx.residual(d.x, d.y, d.z, d.lam, o)
+            r = ctx.residual(d.x, d.y, dz, d.lam, o)
+            for k in ("B", "J"):
+                assert bool(torch.isnan(r[k][:, dead]).all()) and torch.equal(r[k][:, ~dead], rr[k][:, ~dead])
+            for k in ("f", "g", "div", "phi"):
+                assert bool(torch.isnan(r[k][dead]).all()) and torch.equal(r[k][~dead], rr[k][~dead])
+        # everything invalid: nothing to sum at all
+        allbad = ctx.eval(d.x, d.y, -d.z, d.lam)
+        assert bool(torch.isnan(allbad).all())
+        out = torch.empty_like(ref)
+        ctx.eval_noalloc(d.x, d.y, dz, d.lam, out)
+        assert torch.equal(out[:, ~dead], ref[:, ~dead]) and bool(torch.isnan(out[:, dead]).all())
+
+
 def test_eval_potential_field_fast_path_is_bit_identical(dbie):
     """Points with lambda = 0 in all three components take a loop without sincos (n(0) = 1 exactly).  Their
     result must equal, bit for bit, what the general loop gives: lambda = 1e-300 r underflows theta to a
