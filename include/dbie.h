@@ -234,9 +234,9 @@ void dbie_trace_default_opts(dbie_trace_opts* opts);
  * path: out, 3*(S+1)*L doubles, point k of line i at path[(c*(S+1) + k)*L + i], c = 0, 1, 2; NaN beyond a
  * line's last point.  npts: out L, points stored (0 if the seed is outside the region).  status: out L:
  * 0 = max_steps reached, 1 = left the region (a stage point or the new point), 2 = v zero or not finite at
- * a stage point.  Asynchronous on the stream; 4 S field evaluations of L points are enqueued; lines that
- * have stopped cost nothing in the lambda search, and with a fixed lambda / for current lines the sum is skipped
- * for every block of 256 (128) consecutive lines that have all stopped. */
+ * a stage point.  Asynchronous on the stream; 4 S field evaluations of L points are enqueued, lines that
+ * have stopped cost nothing in the lambda search (with a fixed lambda, and for current lines, a stopped line still
+ * pays its sums: they are evaluated for all L lines at every stage). */
 dbie_status dbie_trace(dbie_ctx* ctx, long long L, const double* x0, const double* y0, const double* z0,
                        const dbie_solve_opts* sopts, const dbie_trace_opts* topts, double* path, int* npts,
                        int* status, void* cuda_stream);

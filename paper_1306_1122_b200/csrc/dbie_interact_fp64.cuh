@@ -137,7 +137,6 @@ struct ItemCtx {      // what a sink needs to know about the calling thread's wo
 // The sink of interact64_kernel: chunk sums go to the scratch, part[(c*Q + q)*cap + slot] (A4).
 template <int MODE, int NT>
 struct PartSink {
-    static constexpr bool kSkipDeadBlocks = true;   // nobody counts this sink's calls: a block of invalid points may be skipped
     const InteractParams& p;
     int nsplit, nch;
     double run[3];   // MODE_EVAL, unsplit launch: running sum of the chunk sums
@@ -229,12 +228,6 @@ __device__ __forceinline__ void interact_item(const InteractParams& p, const Tri
         if (s == 1) xi = __dadd_rn(xi, p.delta_abs);
         if (s == 2) yi = __dadd_rn(yi, p.delta_abs);
         if (s == 3) zi = __dadd_rn(zi, p.delta_abs);
-    }
-    if constexpr (Sink::kSkipDeadBlocks && (kEval || MODE == MODE_STENCIL4 || MODE == MODE_ANALYTIC)) {
-        // dbie_eval / dbie_residual: a block whose every point is invalid (z <= 0 or NaN; dbie_trace hands stopped lines
-        // over as z = -1) skips the pixel loop.  The epilogues write NaN for such points whatever the scratch holds.
-        // Before any tile is requested, so the mbarrier phases stay in step; the vote is uniform over the CTA.
-        if (!__syncthreads_or(ic.live && zi > 0.0)) return;
     }
     const double z2 = zi * zi;
     // MODE_STENCIL4: the offset coordinates of positions 1 (x), 2 (y), 3 (z)

@@ -48,7 +48,6 @@ constexpr size_t kFusedSmem = kTrigTableBytes                                   
 
 // chunk sums of a thread that covered every chunk itself stay in registers; otherwise they go to the scratch
 struct FusedSink {
-    static constexpr bool kSkipDeadBlocks = false;  // the arrivals of every item are counted; invalid points never enter the lists
     const InteractParams& p;
     bool whole;
     double run[12];

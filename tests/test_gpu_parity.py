@@ -161,10 +161,10 @@ def test_eval_edge_cases(dbie):
     assert np.isnan(oracle.eval(wb)[:, 2]).all()
 
 
-def test_blocks_of_invalid_points_are_skipped_without_changing_the_others(dbie):
-    """dbie_eval / dbie_residual skip the pixel loop of a 256- (128-) point block whose every point is invalid (what
-    dbie_trace hands over for stopped lines: z = -1): those outputs are NaN as before, and every other point keeps its
-    bits, whether its block holds invalid neighbours or not."""
+def test_blocks_of_invalid_points_do_not_change_the_others(dbie):
+    """Whole 256- (128-) point blocks of invalid points (what dbie_trace hands over for stopped lines: z = -1) and
+    invalid stragglers inside live blocks: those outputs are NaN, and every other point keeps its bits, in dbie_eval,
+    dbie_eval_noalloc and dbie_residual (both gradients)."""
     import torch
     w = workloads.random_boundary(96, 80, seed=21, npts=1500, h=0.7)
     dead = np.zeros(w.M, dtype=bool)
